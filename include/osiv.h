@@ -1,0 +1,152 @@
+/*
+ * osiv.h -- C ABI of libosiv: ordered-subset, TV-regularised statistical iterative
+ * reconstruction (OS-TV) of 2-D fan-beam MVCT slices on one NVIDIA B200 (sm_100a).
+ *
+ * Method: arxiv 1903.10088, "Technical Note: Fast Statistical Iterative Reconstruction for
+ * MVCT in TomoTherapy".  Citations "PAPER.md:N" are lines of the extracted paper text;
+ * "C1..C12" are the readings adopted where the paper is silent (SURVEY.md section 8(c),
+ * restated in DESIGN.md section 3).
+ *
+ * Problem statement: geometry + measured Poisson counts + TV weight
+ * beta + ordered subsets + iterations -> attenuation image.  Every step of the iteration runs
+ * in hand-written CUDA kernels; this library has no CPU fallback and every entry point that
+ * needs the GPU returns OSIV_ERR_CUDA when none is usable.
+ *
+ * Conventions
+ *   - Pointers named d_* are DEVICE pointers, h_* are HOST pointers.  All are owned by the
+ *     caller, contiguous, and are neither freed nor retained beyond the call (asynchronous work
+ *     enqueued on `cuda_stream` still reads/writes them until the stream reaches that point).
+ *   - Images are float32 [batch][ny][nx], row-major, img[iy*nx+ix]; pixel (ix,iy) has its centre
+ *     at ((ix-(nx-1)/2)*pixel_mm, (iy-(ny-1)/2)*pixel_mm).  Attenuation in 1/mm.
+ *   - Sinograms are float32 [batch][V_S][C] (compact: the views v = m, m+M, m+2M, ... of subset
+ *     m of M in that order; V_S = n_views/M, or all n_views when subset < 0).  Line integrals
+ *     are dimensionless (mm * 1/mm).
+ *   - Counts are float32 [batch][n_views][n_channels] (all views; integers < 2^24 are exact).
+ *   - `cuda_stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).
+ *   - Every function returns 0 (OSIV_OK) or a negative osiv_status; nothing throws, aborts or
+ *     prints.
+ */
+#ifndef OSIV_H
+#define OSIV_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+    OSIV_OK              =  0,
+    OSIV_ERR_INVALID_ARG = -1,  /* null pointer, non-positive size, n_views % n_subsets != 0,
+                                   batch > max_batch, source inside the grid's circumscribed circle */
+    OSIV_ERR_CUDA        = -2,  /* a CUDA runtime call failed (no device, out of memory, launch error) */
+    OSIV_ERR_NOT_FINITE  = -3   /* the monitor D became NaN/Inf for at least one slice */
+} osiv_status;
+
+/* Scan geometry (reading C1; the paper prints none, BASELINE.json supplies SAD/SDD/channels).
+ * Lengths in mm, angles in rad.  Source of view v: SAD*(cos th_v, sin th_v), th_v = theta0 + 2*pi*v/V.
+ * Ray (v,c): the zero-width line from the source in direction -(cos(th_v+ga_c), sin(th_v+ga_c)),
+ * ga_c = (c - (C-1)/2 + channel_offset) * dgamma. */
+typedef struct {
+    int32_t nx, ny;          /* image size in pixels */
+    double  pixel_mm;        /* square pixel side */
+    int32_t n_views;         /* V, equally spaced over 360 degrees */
+    int32_t n_channels;      /* C, equiangular */
+    double  sad_mm;          /* source to isocentre */
+    double  sdd_mm;          /* source to detector; informational only (line integrals do not use it) */
+    double  dgamma_rad;      /* channel pitch; <= 0 selects 2*asin(R_FOV/SAD)/C, R_FOV = min(nx,ny)*pixel/2 */
+    double  channel_offset;  /* in channels */
+    double  theta0_rad;
+} osiv_geometry;
+
+/* Iteration parameters.  osiv_default_params() fills the paper's values. */
+typedef struct {
+    double  beta;            /* TV weight against the blank-normalised log-likelihood (C6,C7); the
+                                subset update uses beta/M ("multiplied by the thinning parameter") */
+    int32_t n_subsets;       /* M; subset m holds views {v : v mod M == m}; M must divide n_views */
+    int32_t n_iters;         /* number of SUBSET updates */
+    double  mu0;             /* homogeneous initial image, default 0.005 /mm = 0.05 /cm */
+    double  lambda0;         /* 0.01 */
+    double  lambda_up;       /* 1e-4   (Eq. 4) */
+    double  lambda_down;     /* 2e-4   (Eq. 5) */
+    double  lambda_min;      /* floor of lambda, 1e-4 (C10) */
+    double  kappa;           /* step scale, 100 (C6): tau_S = kappa*SAD*dgamma/(V_S*max(nx,ny)*pixel^3) */
+    double  tv_eps;          /* TV smoothing, 1e-5 /mm (C9) */
+    int32_t return_best;     /* 0: final iterate; 1: iterate with the smallest monitor D */
+    int32_t reserved;        /* must be 0 */
+    const double* forced_lambda;  /* HOST pointer: NULL, or n_iters values used instead of Eq. 4-5 */
+} osiv_params;
+
+typedef struct osiv_handle osiv_handle;
+
+/* Library version (major*10000 + minor*100 + patch). */
+int osiv_version(void);
+
+/* Text for a status code; never NULL; static storage. */
+const char* osiv_strerror(int status);
+
+/* Fill *p with the defaults listed above (beta = 0.005, n_subsets = 1, n_iters = 1). */
+int osiv_default_params(osiv_params* p);
+
+/* Create a reconstruction context on CUDA device `device` for up to `max_batch` slices per call:
+ * builds the per-ray geometry tables in float64 on the host, stores them as float32 in HBM, and
+ * allocates the per-slice workspace lazily.  The handle is not thread-safe; use one per thread. */
+int osiv_create(const osiv_geometry* geom, int32_t max_batch, int32_t device, osiv_handle** out);
+
+/* Release everything the handle owns (synchronises the device).  NULL is accepted. */
+int osiv_destroy(osiv_handle* h);
+
+/* Resolved channel pitch (after the dgamma_rad <= 0 rule) and step constant tau_S for M subsets. */
+int osiv_get_dgamma(const osiv_handle* h, double* dgamma_rad);
+int osiv_get_tau(const osiv_handle* h, int32_t n_subsets, double kappa, double* tau);
+
+/* Number of CUDA kernels this handle has launched since osiv_create (for launch accounting). */
+int64_t osiv_launch_count(const osiv_handle* h);
+
+/* Forward projection ("reprojection"):  l_i = sum_r a(i,r) mu_r  for the rays of
+ * subset `subset` of `n_subsets` (subset < 0: all views; then n_subsets is ignored), where a(i,r) is
+ * the exact length of ray i inside square pixel r (C2).
+ * d_img [batch][ny][nx] -> d_sino [batch][V_S][C].  Asynchronous on cuda_stream. */
+int osiv_forward(osiv_handle* h, const float* d_img, float* d_sino, int32_t batch,
+                 int32_t subset, int32_t n_subsets, void* cuda_stream);
+
+/* Matched backprojection ("estimation"):  g_r = sum_{i in S} a(i,r) s_i  with the same
+ * a(i,r), computed as an atomic-free gather per pixel (C3).
+ * d_sino [batch][V_S][C] -> d_img [batch][ny][nx].  Asynchronous on cuda_stream. */
+int osiv_backward(osiv_handle* h, const float* d_sino, float* d_img, int32_t batch,
+                  int32_t subset, int32_t n_subsets, void* cuda_stream);
+
+/* Gradient of the smoothed isotropic total variation (C8):  d_grad[b] = dTV_eps/dmu (d_img[b]).
+ * Both [batch][ny][nx].  Asynchronous on cuda_stream. */
+int osiv_tv_gradient(osiv_handle* h, const float* d_img, float* d_grad, int32_t batch, double tv_eps,
+                     void* cuda_stream);
+
+/* The ordered-subset iteration (PAPER.md:74 Eq. 3, :100-108 Eq. 4-5, :114, :118, :63, :140):
+ *   mu(0) = mu0;  for n = 0 .. n_iters-1, m = n mod M:
+ *     l = A_m mu(n);  ybar = b exp(-l);  r = (ybar - y)/b_ref;  D(n) = sum_i (l_i - ln(b_i/max(y_i,1)))^2
+ *     lambda(n) by Eq. 4-5 on D(n) vs D(n-1) (lambda(0) = lambda0; floor lambda_min)
+ *     mu(n+1) = max(mu(n) + lambda(n) tau_S (A_m^T r - (beta/M) dTV_eps(mu(n))), 0)
+ * for `batch` independent slices that share geometry and subset order but own lambda, D and best image.
+ *   d_counts    [batch][V][C] measured counts y
+ *   d_blank     [C] blank-scan counts b per channel, or NULL to use blank_scalar for every channel;
+ *               b_ref = mean_c b_c
+ *   d_img_out   [batch][ny][nx] result
+ *   h_trace     HOST pointer: NULL, or [batch][n_iters][2] doubles receiving (D(n), lambda(n)).
+ * All work is enqueued on cuda_stream with no host round-trip inside the loop.  If h_trace is NULL the
+ * call returns without synchronising; otherwise it synchronises the stream, fills h_trace and returns
+ * OSIV_ERR_NOT_FINITE if any slice's monitor was not finite. */
+int osiv_reconstruct(osiv_handle* h, const float* d_counts, const float* d_blank, float blank_scalar,
+                     const osiv_params* params, int32_t batch, float* d_img_out, double* h_trace,
+                     void* cuda_stream);
+
+/* Same reconstruction with HOST buffers (the end-to-end call): copies h_counts (and h_blank) to the
+ * device, runs osiv_reconstruct, copies the images back to h_img_out and synchronises the stream.
+ * Pinned host memory makes the copies asynchronous but is not required. */
+int osiv_reconstruct_host(osiv_handle* h, const float* h_counts, const float* h_blank, float blank_scalar,
+                          const osiv_params* params, int32_t batch, float* h_img_out, double* h_trace,
+                          void* cuda_stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* OSIV_H */

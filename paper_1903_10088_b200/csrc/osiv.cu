@@ -1,0 +1,409 @@
+// osiv.cu -- host side of libosiv: the C ABI of include/osiv.h over the kernels in osiv_kernels.cuh.
+// Build: nvcc -O3 -lineinfo -gencode arch=compute_100a,code=sm_100a -shared -Xcompiler -fPIC
+// (paper_1903_10088_b200/build.py).  No CPU fallback exists: without a usable device every
+// compute entry point returns OSIV_ERR_CUDA.
+#include "../../include/osiv.h"
+#include "osiv_kernels.cuh"
+
+#include <cmath>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+#include <vector>
+
+using namespace osiv;
+
+struct osiv_handle {
+    osiv_geometry geom;
+    double dgamma;
+    int device;
+    int max_batch;
+    DevGeom dg;
+    float4* d_rays = nullptr;
+    float2* d_views = nullptr;
+    // per-slice workspace, grown lazily
+    int ws_batch = 0;
+    float *d_imgA = nullptr, *d_imgB = nullptr, *d_imgTA = nullptr, *d_imgTB = nullptr;
+    float* d_best = nullptr;
+    size_t rec_elems = 0;       float4* d_rec = nullptr;
+    size_t partial_elems = 0;   double* d_partials = nullptr;
+    SliceState* d_state = nullptr;
+    float* d_inv_bref = nullptr;
+    size_t trace_elems = 0;     double* d_trace = nullptr;
+    size_t forced_elems = 0;    double* d_forced = nullptr;
+    // staging for osiv_reconstruct_host
+    size_t hc_elems = 0;        float* d_hcounts = nullptr;
+    float* d_hblank = nullptr;
+    size_t hi_elems = 0;        float* d_himg = nullptr;
+    int64_t launches = 0;
+};
+
+namespace {
+
+struct DeviceGuard {
+    int prev = -1;
+    bool ok = true;
+    explicit DeviceGuard(int dev) {
+        if (cudaGetDevice(&prev) != cudaSuccess) { ok = false; prev = -1; return; }
+        if (prev != dev && cudaSetDevice(dev) != cudaSuccess) ok = false;
+    }
+    ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
+};
+
+#define OSIV_CUDA(call) do { if ((call) != cudaSuccess) { cudaGetLastError(); return OSIV_ERR_CUDA; } } while (0)
+
+template <class T>
+int grow(T** p, size_t* have, size_t want) {
+    if (*have >= want && *p) return OSIV_OK;
+    if (*p) { OSIV_CUDA(cudaFree(*p)); *p = nullptr; *have = 0; }
+    OSIV_CUDA(cudaMalloc((void**)p, want * sizeof(T)));
+    *have = want;
+    return OSIV_OK;
+}
+
+double resolve_dgamma(const osiv_geometry& g) {
+    if (g.dgamma_rad > 0.0) return g.dgamma_rad;
+    const int nmin = g.nx < g.ny ? g.nx : g.ny;
+    return 2.0 * std::asin(0.5 * nmin * g.pixel_mm / g.sad_mm) / g.n_channels;
+}
+
+// A0: per-ray coefficients {alpha, beta, g0, h} in float64, stored float32 (header of osiv_kernels.cuh).
+// Ray (v,c): direction d = -(cos phi, sin phi), phi = th_v + ga_c; signed distance of the point
+// D*(xc,yc) from it: p = D*(xc*dy - yc*dx) + SAD*sin(ga_c).
+void build_tables(const osiv_geometry& g, double dgamma, std::vector<float4>& rays, std::vector<float2>& views) {
+    const int V = g.n_views, C = g.n_channels;
+    const double D = g.pixel_mm, tiny = 1e-9;
+    rays.resize((size_t)V * C);
+    views.resize(V);
+    for (int v = 0; v < V; ++v) {
+        const double th = g.theta0_rad + 2.0 * M_PI * (double)v / (double)V;
+        views[v] = make_float2((float)std::cos(th), (float)std::sin(th));
+        for (int c = 0; c < C; ++c) {
+            const double ga = ((double)c - 0.5 * (C - 1) + g.channel_offset) * dgamma;
+            double dx = -std::cos(th + ga), dy = -std::sin(th + ga);
+            const double S = g.sad_mm * std::sin(ga);
+            float4 r;
+            if (std::fabs(dy) >= std::fabs(dx)) {          // crosses every row once: in-line coordinate is x
+                if (std::fabs(dx) < tiny) dx = dx < 0 ? -tiny : tiny;
+                r.x = (float)(-dy / dx);                   // p / (-D dx)
+                r.y = 1.f;
+                r.z = (float)(-S / (D * dx));
+                r.w = (float)(D / std::fabs(dy));
+            } else {                                       // crosses every column once: in-line coordinate is y
+                if (std::fabs(dy) < tiny) dy = dy < 0 ? -tiny : tiny;
+                r.x = 1.f;                                 // p / (D dy)
+                r.y = (float)(-dx / dy);
+                r.z = (float)(S / (D * dy));
+                r.w = (float)(D / std::fabs(dx));
+            }
+            rays[(size_t)v * C + c] = r;
+        }
+    }
+}
+
+int subset_views(const osiv_handle* h, int subset, int n_subsets) {
+    return subset < 0 ? h->geom.n_views : h->geom.n_views / n_subsets;
+}
+
+int check_subset(const osiv_handle* h, int subset, int n_subsets) {
+    if (subset < 0) return OSIV_OK;
+    if (n_subsets <= 0 || h->geom.n_views % n_subsets != 0 || subset >= n_subsets) return OSIV_ERR_INVALID_ARG;
+    return OSIV_OK;
+}
+
+// padded image buffers for `batch` slices (pads are zeroed once and never written again)
+int ensure_images(osiv_handle* h, int batch, cudaStream_t st) {
+    if (h->ws_batch >= batch) return OSIV_OK;
+    float** bufs[4] = {&h->d_imgA, &h->d_imgB, &h->d_imgTA, &h->d_imgTB};
+    for (auto b : bufs) if (*b) { OSIV_CUDA(cudaFree(*b)); *b = nullptr; }
+    if (h->d_best) { OSIV_CUDA(cudaFree(h->d_best)); h->d_best = nullptr; }
+    h->ws_batch = 0;
+    const size_t ne = (size_t)h->dg.img_elems * batch, nt = (size_t)h->dg.imgT_elems * batch;
+    OSIV_CUDA(cudaMalloc((void**)&h->d_imgA, ne * sizeof(float)));
+    OSIV_CUDA(cudaMalloc((void**)&h->d_imgB, ne * sizeof(float)));
+    OSIV_CUDA(cudaMalloc((void**)&h->d_imgTA, nt * sizeof(float)));
+    OSIV_CUDA(cudaMalloc((void**)&h->d_imgTB, nt * sizeof(float)));
+    OSIV_CUDA(cudaMalloc((void**)&h->d_best, (size_t)h->geom.nx * h->geom.ny * batch * sizeof(float)));
+    OSIV_CUDA(cudaMemsetAsync(h->d_imgA, 0, ne * sizeof(float), st));
+    OSIV_CUDA(cudaMemsetAsync(h->d_imgB, 0, ne * sizeof(float), st));
+    OSIV_CUDA(cudaMemsetAsync(h->d_imgTA, 0, nt * sizeof(float), st));
+    OSIV_CUDA(cudaMemsetAsync(h->d_imgTB, 0, nt * sizeof(float), st));
+    h->ws_batch = batch;
+    return OSIV_OK;
+}
+
+dim3 fwd_grid(const osiv_handle* h, int VS, int batch) { return dim3((h->geom.n_channels + 31) / 32, VS, batch); }
+dim3 back_grid(const osiv_handle* h, int batch) {
+    return dim3((h->geom.nx + BK_BLOCK_PX_X - 1) / BK_BLOCK_PX_X, (h->geom.ny + BK_BLOCK_PX_Y - 1) / BK_BLOCK_PX_Y, batch);
+}
+dim3 px_grid(const osiv_handle* h, int batch) { return dim3((h->geom.nx + 31) / 32, (h->geom.ny + 7) / 8, batch); }
+
+int launch_check(osiv_handle* h, int n) {
+    h->launches += n;
+    OSIV_CUDA(cudaGetLastError());
+    return OSIV_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int osiv_version(void) { return 100; }
+
+const char* osiv_strerror(int status) {
+    switch (status) {
+        case OSIV_OK: return "ok";
+        case OSIV_ERR_INVALID_ARG: return "invalid argument";
+        case OSIV_ERR_CUDA: return "CUDA error (no usable device, out of memory or launch failure)";
+        case OSIV_ERR_NOT_FINITE: return "monitor D became non-finite";
+        default: return "unknown status";
+    }
+}
+
+int osiv_default_params(osiv_params* p) {
+    if (!p) return OSIV_ERR_INVALID_ARG;
+    std::memset(p, 0, sizeof(*p));
+    p->beta = 0.005; p->n_subsets = 1; p->n_iters = 1;
+    p->mu0 = 0.005;                                     // PAPER.md:140 (0.05 /cm)
+    p->lambda0 = 0.01; p->lambda_up = 1e-4; p->lambda_down = 2e-4;
+    p->lambda_min = 1e-4; p->kappa = 100.0; p->tv_eps = 1e-5;
+    p->return_best = 0; p->reserved = 0; p->forced_lambda = nullptr;
+    return OSIV_OK;
+}
+
+int osiv_create(const osiv_geometry* geom, int32_t max_batch, int32_t device, osiv_handle** out) {
+    if (out) *out = nullptr;
+    if (!geom || !out || max_batch <= 0 || device < 0) return OSIV_ERR_INVALID_ARG;
+    const osiv_geometry& g = *geom;
+    if (g.nx <= 0 || g.ny <= 0 || g.n_views <= 0 || g.n_channels <= 0 || g.nx > 16384 || g.ny > 16384)
+        return OSIV_ERR_INVALID_ARG;
+    if (!(g.pixel_mm > 0.0) || !(g.sad_mm > 0.0) || !std::isfinite(g.pixel_mm) || !std::isfinite(g.sad_mm) ||
+        !std::isfinite(g.dgamma_rad) || !std::isfinite(g.channel_offset) || !std::isfinite(g.theta0_rad))
+        return OSIV_ERR_INVALID_ARG;
+    const double rmax = 0.5 * g.pixel_mm * std::sqrt((double)g.nx * g.nx + (double)g.ny * g.ny);
+    if (!(g.sad_mm > rmax * 1.0001)) return OSIV_ERR_INVALID_ARG;      // source must be outside the grid
+    if (g.dgamma_rad <= 0.0 && 0.5 * (g.nx < g.ny ? g.nx : g.ny) * g.pixel_mm >= g.sad_mm) return OSIV_ERR_INVALID_ARG;
+    const double dgamma = resolve_dgamma(g);
+    if (!(dgamma > 0.0) || dgamma * g.n_channels >= M_PI) return OSIV_ERR_INVALID_ARG;
+
+    DeviceGuard guard(device);
+    if (!guard.ok) { cudaGetLastError(); return OSIV_ERR_CUDA; }
+
+    osiv_handle* h = new (std::nothrow) osiv_handle();
+    if (!h) return OSIV_ERR_CUDA;
+    h->geom = g; h->dgamma = dgamma; h->device = device; h->max_batch = max_batch;
+
+    std::vector<float4> rays;
+    std::vector<float2> views;
+    build_tables(g, dgamma, rays, views);
+    if (cudaMalloc((void**)&h->d_rays, rays.size() * sizeof(float4)) != cudaSuccess ||
+        cudaMalloc((void**)&h->d_views, views.size() * sizeof(float2)) != cudaSuccess ||
+        cudaMalloc((void**)&h->d_state, (size_t)max_batch * sizeof(SliceState)) != cudaSuccess ||
+        cudaMalloc((void**)&h->d_inv_bref, sizeof(float)) != cudaSuccess ||
+        cudaMemcpy(h->d_rays, rays.data(), rays.size() * sizeof(float4), cudaMemcpyHostToDevice) != cudaSuccess ||
+        cudaMemcpy(h->d_views, views.data(), views.size() * sizeof(float2), cudaMemcpyHostToDevice) != cudaSuccess) {
+        cudaGetLastError();
+        osiv_destroy(h);
+        return OSIV_ERR_CUDA;
+    }
+
+    DevGeom& d = h->dg;
+    d.nx = g.nx; d.ny = g.ny; d.V = g.n_views; d.C = g.n_channels;
+    d.pitch = g.nx + 2 * PAD; d.pitchT = g.ny + 2 * PAD;
+    d.img_elems = (long long)(g.ny + 2 * PADR) * d.pitch;
+    d.imgT_elems = (long long)(g.nx + 2 * PADR) * d.pitchT;
+    d.cx = 0.5f * (g.nx - 1); d.cy = 0.5f * (g.ny - 1);
+    d.pixel = (float)g.pixel_mm; d.sad = (float)g.sad_mm;
+    d.inv_dgamma = (float)(1.0 / dgamma);
+    d.c_center = (float)(0.5 * (g.n_channels - 1) - g.channel_offset);
+    d.hw_scale = (float)(g.pixel_mm / dgamma);
+    // short odd series for atan: error < z^9/9; demand < 0.01 channel, else fall back to atanf
+    const double zmax = rmax / (g.sad_mm - rmax);
+    d.use_atanf = (std::pow(zmax, 9) / 9.0 / dgamma > 0.01) ? 1 : 0;
+    d.rays = h->d_rays; d.views = h->d_views;
+    *out = h;
+    return OSIV_OK;
+}
+
+int osiv_destroy(osiv_handle* h) {
+    if (!h) return OSIV_OK;
+    DeviceGuard guard(h->device);
+    if (guard.ok) {
+        cudaDeviceSynchronize();
+        void* ptrs[] = {h->d_rays, h->d_views, h->d_imgA, h->d_imgB, h->d_imgTA, h->d_imgTB, h->d_best, h->d_rec,
+                        h->d_partials, h->d_state, h->d_inv_bref, h->d_trace, h->d_forced, h->d_hcounts, h->d_hblank,
+                        h->d_himg};
+        for (void* p : ptrs) if (p) cudaFree(p);
+        cudaGetLastError();
+    }
+    delete h;
+    return OSIV_OK;
+}
+
+int osiv_get_dgamma(const osiv_handle* h, double* dgamma_rad) {
+    if (!h || !dgamma_rad) return OSIV_ERR_INVALID_ARG;
+    *dgamma_rad = h->dgamma;
+    return OSIV_OK;
+}
+
+int osiv_get_tau(const osiv_handle* h, int32_t n_subsets, double kappa, double* tau) {
+    if (!h || !tau || n_subsets <= 0 || h->geom.n_views % n_subsets != 0) return OSIV_ERR_INVALID_ARG;
+    const osiv_geometry& g = h->geom;
+    const int N = g.nx > g.ny ? g.nx : g.ny;
+    const double vs = (double)(g.n_views / n_subsets), d = g.pixel_mm;
+    *tau = kappa * g.sad_mm * h->dgamma / (vs * N * d * d * d);       // C6
+    return OSIV_OK;
+}
+
+int64_t osiv_launch_count(const osiv_handle* h) { return h ? h->launches : 0; }
+
+int osiv_forward(osiv_handle* h, const float* d_img, float* d_sino, int32_t batch, int32_t subset,
+                 int32_t n_subsets, void* cuda_stream) {
+    if (!h || !d_img || !d_sino || batch <= 0 || batch > h->max_batch) return OSIV_ERR_INVALID_ARG;
+    if (check_subset(h, subset, n_subsets) != OSIV_OK) return OSIV_ERR_INVALID_ARG;
+    DeviceGuard guard(h->device);
+    if (!guard.ok) { cudaGetLastError(); return OSIV_ERR_CUDA; }
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    int rc = ensure_images(h, batch, st);
+    if (rc != OSIV_OK) return rc;
+    const int VS = subset_views(h, subset, n_subsets);
+    k_pad_transpose<<<dim3((h->geom.nx + 31) / 32, (h->geom.ny + 31) / 32, batch), 256, 0, st>>>(h->dg, d_img, h->d_imgA,
+                                                                                             h->d_imgTA);
+    FwdArgs a{};
+    a.g = h->dg; a.img = h->d_imgA; a.imgT = h->d_imgTA;
+    a.subset = subset; a.M = subset < 0 ? 1 : n_subsets; a.VS = VS; a.sino = d_sino;
+    k_forward<0><<<fwd_grid(h, VS, batch), FWD_THREADS, 0, st>>>(a);
+    return launch_check(h, 2);
+}
+
+int osiv_backward(osiv_handle* h, const float* d_sino, float* d_img, int32_t batch, int32_t subset,
+                  int32_t n_subsets, void* cuda_stream) {
+    if (!h || !d_img || !d_sino || batch <= 0 || batch > h->max_batch) return OSIV_ERR_INVALID_ARG;
+    if (check_subset(h, subset, n_subsets) != OSIV_OK) return OSIV_ERR_INVALID_ARG;
+    DeviceGuard guard(h->device);
+    if (!guard.ok) { cudaGetLastError(); return OSIV_ERR_CUDA; }
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const int VS = subset_views(h, subset, n_subsets), M = subset < 0 ? 1 : n_subsets;
+    int rc = grow(&h->d_rec, &h->rec_elems, (size_t)batch * VS * h->geom.n_channels);
+    if (rc != OSIV_OK) return rc;
+    k_make_rec<<<dim3((h->geom.n_channels + 255) / 256, VS, batch), 256, 0, st>>>(h->dg, d_sino, h->d_rec, subset, M, VS);
+    BackArgs b{};
+    b.g = h->dg; b.rec = h->d_rec; b.subset = subset; b.M = M; b.VS = VS; b.out = d_img;
+    k_back<0><<<back_grid(h, batch), BK_THREADS, 0, st>>>(b);
+    return launch_check(h, 2);
+}
+
+int osiv_tv_gradient(osiv_handle* h, const float* d_img, float* d_grad, int32_t batch, double tv_eps,
+                     void* cuda_stream) {
+    if (!h || !d_img || !d_grad || batch <= 0 || batch > h->max_batch || !(tv_eps >= 0.0)) return OSIV_ERR_INVALID_ARG;
+    DeviceGuard guard(h->device);
+    if (!guard.ok) { cudaGetLastError(); return OSIV_ERR_CUDA; }
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    int rc = ensure_images(h, batch, st);
+    if (rc != OSIV_OK) return rc;
+    k_pad_transpose<<<dim3((h->geom.nx + 31) / 32, (h->geom.ny + 31) / 32, batch), 256, 0, st>>>(h->dg, d_img, h->d_imgA,
+                                                                                             h->d_imgTA);
+    k_tv<<<back_grid(h, batch), BK_THREADS, 0, st>>>(h->dg, h->d_imgA, (float)(tv_eps * tv_eps), d_grad);
+    return launch_check(h, 2);
+}
+
+int osiv_reconstruct(osiv_handle* h, const float* d_counts, const float* d_blank, float blank_scalar,
+                     const osiv_params* prm, int32_t batch, float* d_img_out, double* h_trace, void* cuda_stream) {
+    if (!h || !d_counts || !prm || !d_img_out || batch <= 0 || batch > h->max_batch) return OSIV_ERR_INVALID_ARG;
+    const int M = prm->n_subsets, N = prm->n_iters;
+    if (M <= 0 || N < 0 || h->geom.n_views % M != 0 || prm->reserved != 0) return OSIV_ERR_INVALID_ARG;
+    if (!d_blank && !(blank_scalar > 0.f)) return OSIV_ERR_INVALID_ARG;
+    if (!(prm->tv_eps >= 0.0) || !std::isfinite(prm->beta) || !std::isfinite(prm->mu0) || !(prm->kappa > 0.0))
+        return OSIV_ERR_INVALID_ARG;
+    DeviceGuard guard(h->device);
+    if (!guard.ok) { cudaGetLastError(); return OSIV_ERR_CUDA; }
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+
+    const int VS = h->geom.n_views / M, C = h->geom.n_channels;
+    int rc = ensure_images(h, batch, st);
+    if (rc != OSIV_OK) return rc;
+    if ((rc = grow(&h->d_rec, &h->rec_elems, (size_t)batch * VS * C)) != OSIV_OK) return rc;
+    const dim3 fg = fwd_grid(h, VS, batch);
+    if ((rc = grow(&h->d_partials, &h->partial_elems, (size_t)batch * fg.x * fg.y)) != OSIV_OK) return rc;
+    if (h_trace && N > 0 && (rc = grow(&h->d_trace, &h->trace_elems, (size_t)batch * N * 2)) != OSIV_OK) return rc;
+    if (prm->forced_lambda && N > 0) {
+        if ((rc = grow(&h->d_forced, &h->forced_elems, (size_t)N)) != OSIV_OK) return rc;
+        OSIV_CUDA(cudaMemcpyAsync(h->d_forced, prm->forced_lambda, (size_t)N * sizeof(double), cudaMemcpyHostToDevice, st));
+    }
+    double tau;
+    osiv_get_tau(h, M, prm->kappa, &tau);
+
+    float* best = prm->return_best ? h->d_best : nullptr;
+    k_init_state<<<1, 32, 0, st>>>(h->d_state, batch, prm->lambda0, d_blank, blank_scalar, C, h->d_inv_bref);
+    k_fill<<<px_grid(h, batch), 256, 0, st>>>(h->dg, (float)prm->mu0, h->d_imgA, h->d_imgTA, best);
+    h->launches += 2;
+
+    FwdArgs f{};
+    f.g = h->dg; f.M = M; f.VS = VS;
+    f.counts = d_counts; f.blank = d_blank; f.blank_scalar = blank_scalar; f.inv_bref = h->d_inv_bref;
+    f.rec = h->d_rec; f.partials = h->d_partials; f.state = h->d_state;
+    f.ip.lambda0 = prm->lambda0; f.ip.up = prm->lambda_up; f.ip.down = prm->lambda_down; f.ip.lmin = prm->lambda_min;
+    f.ip.forced = (prm->forced_lambda && N > 0) ? h->d_forced : nullptr;
+    f.ip.trace = (h_trace && N > 0) ? h->d_trace : nullptr;
+    f.ip.n_iters = N; f.ip.return_best = prm->return_best;
+    BackArgs b{};
+    b.g = h->dg; b.rec = h->d_rec; b.M = M; b.VS = VS; b.best = best; b.state = h->d_state;
+    b.tau = tau; b.beta_over_M = (float)(prm->beta / M); b.eps2 = (float)(prm->tv_eps * prm->tv_eps);
+
+    float *cur = h->d_imgA, *curT = h->d_imgTA, *nxt = h->d_imgB, *nxtT = h->d_imgTB;
+    const dim3 bg = back_grid(h, batch);
+    for (int n = 0; n < N; ++n) {
+        const int m = n % M;                               // PAPER.md:118, C11
+        f.img = cur; f.imgT = curT; f.subset = m; f.monitor_only = 0;
+        k_forward<1><<<fg, FWD_THREADS, 0, st>>>(f);
+        b.img = cur; b.img_new = nxt; b.imgT_new = nxtT; b.subset = m;
+        k_back<1><<<bg, BK_THREADS, 0, st>>>(b);
+        float* t;
+        t = cur; cur = nxt; nxt = t;
+        t = curT; curT = nxtT; nxtT = t;
+    }
+    h->launches += 2 * (int64_t)N;
+    if (prm->return_best) {
+        // the final iterate competes too, judged on the subset that would come next (C12)
+        f.img = cur; f.imgT = curT; f.subset = N % M; f.monitor_only = 1;
+        k_forward<1><<<fg, FWD_THREADS, 0, st>>>(f);
+        h->launches += 1;
+    }
+    k_unpad<<<px_grid(h, batch), 256, 0, st>>>(h->dg, cur, best, h->d_state, d_img_out);
+    rc = launch_check(h, 1);
+    if (rc != OSIV_OK) return rc;
+
+    if (h_trace) {
+        std::vector<SliceState> hs(batch);
+        if (N > 0)
+            OSIV_CUDA(cudaMemcpyAsync(h_trace, h->d_trace, (size_t)batch * N * 2 * sizeof(double), cudaMemcpyDeviceToHost, st));
+        OSIV_CUDA(cudaMemcpyAsync(hs.data(), h->d_state, (size_t)batch * sizeof(SliceState), cudaMemcpyDeviceToHost, st));
+        OSIV_CUDA(cudaStreamSynchronize(st));
+        for (int s = 0; s < batch; ++s) if (hs[s].not_finite) return OSIV_ERR_NOT_FINITE;
+    }
+    return OSIV_OK;
+}
+
+int osiv_reconstruct_host(osiv_handle* h, const float* h_counts, const float* h_blank, float blank_scalar,
+                          const osiv_params* prm, int32_t batch, float* h_img_out, double* h_trace, void* cuda_stream) {
+    if (!h || !h_counts || !prm || !h_img_out || batch <= 0 || batch > h->max_batch) return OSIV_ERR_INVALID_ARG;
+    DeviceGuard guard(h->device);
+    if (!guard.ok) { cudaGetLastError(); return OSIV_ERR_CUDA; }
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const size_t nc = (size_t)batch * h->geom.n_views * h->geom.n_channels;
+    const size_t ni = (size_t)batch * h->geom.nx * h->geom.ny;
+    int rc;
+    if ((rc = grow(&h->d_hcounts, &h->hc_elems, nc)) != OSIV_OK) return rc;
+    if ((rc = grow(&h->d_himg, &h->hi_elems, ni)) != OSIV_OK) return rc;
+    if (h_blank && !h->d_hblank) OSIV_CUDA(cudaMalloc((void**)&h->d_hblank, (size_t)h->geom.n_channels * sizeof(float)));
+    OSIV_CUDA(cudaMemcpyAsync(h->d_hcounts, h_counts, nc * sizeof(float), cudaMemcpyHostToDevice, st));
+    if (h_blank)
+        OSIV_CUDA(cudaMemcpyAsync(h->d_hblank, h_blank, (size_t)h->geom.n_channels * sizeof(float), cudaMemcpyHostToDevice, st));
+    rc = osiv_reconstruct(h, h->d_hcounts, h_blank ? h->d_hblank : nullptr, blank_scalar, prm, batch, h->d_himg, h_trace, st);
+    if (rc != OSIV_OK && rc != OSIV_ERR_NOT_FINITE) return rc;
+    OSIV_CUDA(cudaMemcpyAsync(h_img_out, h->d_himg, ni * sizeof(float), cudaMemcpyDeviceToHost, st));
+    OSIV_CUDA(cudaStreamSynchronize(st));
+    return rc;
+}
+
+}  // extern "C"

@@ -1,0 +1,479 @@
+// osiv_kernels.cuh -- sm_100a device code of libosiv (see include/osiv.h).
+//
+// Hot path of arxiv 1903.10088: per ordered-subset iteration
+//   K1  k_forward<1>  ray-driven reprojection l = A_S mu, fused Poisson residual, monitor D (fp64,
+//                     fixed-order reduction) and the adaptive-step rule Eq. 4-5 in the last block
+//   K2  k_back<1>     matched atomic-free gather backprojection g = A_S^T r, fused TV gradient,
+//                     Eq. 3 update, mu > 0 clamp, best-image copy; double-buffered image
+//
+// System matrix (reading C2): a(i,r) = length of the zero-width ray i inside square pixel r.  With
+// p the signed distance of the pixel centre from the ray, the chord is the trapezoid
+//   a = h * sat((hi - |p|) / (hi - lo)),  h = D/max(|dx|,|dy|), hi = D(|dx|+|dy|)/2, hi-lo = D*min(|dx|,|dy|).
+// p is affine in the centred pixel indices (xc, yc), so after dividing by (hi-lo) every ray carries
+// four floats {alpha, beta, g0, h} with
+//   a(i; xc,yc) = h * sat( (|alpha|+|beta|)/2 - |alpha*xc + beta*yc + g0| ),
+// one of alpha,beta being exactly +1 and the other |k| >= 1.  Forward and back evaluate this same
+// expression, so the pair is matched by construction.  Nothing here is a dense contraction: no
+// tensor cores; the work is FP32 FMA/ALU issue plus L1/L2 gathers.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace osiv {
+
+constexpr int PAD = 4;                     // zero columns left and right of every padded image line
+constexpr int PADR = 1;                    // zero rows above and below a padded image
+constexpr int FWD_SEGS = 8;                // a ray is split into this many segments (one warp each)
+constexpr int FWD_THREADS = 32 * FWD_SEGS;
+constexpr int BK_TX = 2, BK_TY = 2;        // pixels per thread in the backprojector
+constexpr int BK_THREADS = 128;            // 4 warps as 2x2; a warp covers 8x4 tiles = 16x8 pixels
+constexpr int BK_BLOCK_PX_X = 2 * 8 * BK_TX;
+constexpr int BK_BLOCK_PX_Y = 2 * 4 * BK_TY;
+
+struct DevGeom {
+    int nx, ny, V, C;
+    int pitch, pitchT;                     // floats per padded line of img ([ny+2][nx+8]) and imgT ([nx+2][ny+8])
+    long long img_elems, imgT_elems;       // padded floats per slice
+    float cx, cy;                          // (nx-1)/2, (ny-1)/2
+    float pixel, sad, inv_dgamma, c_center;   // c_center = (C-1)/2 - channel_offset
+    float hw_scale;                        // pixel / dgamma
+    int use_atanf;                         // fan too wide for the short atan series
+    const float4* rays;                    // [V][C] {alpha, beta, g0, h}
+    const float2* views;                   // [V] {cos th_v, sin th_v}
+};
+
+struct SliceState {
+    double lambda, D_prev, D_best, D_last;
+    int n;                                 // subset updates done = next trace row
+    int improved;                          // last monitor value beat D_best (return_best)
+    int not_finite;
+    unsigned int ticket;
+};
+
+struct IterParams {
+    double lambda0, up, down, lmin;
+    const double* forced;                  // device, [n_iters] or null
+    double* trace;                         // device, [batch][n_iters][2] or null
+    int n_iters;
+    int return_best;
+};
+
+struct FwdArgs {
+    DevGeom g;
+    const float* img;                      // padded mu, slice stride g.img_elems
+    const float* imgT;                     // padded transpose, slice stride g.imgT_elems
+    int subset, M, VS;
+    float* sino;                           // MODE 0: [batch][VS][C]
+    const float* counts;                   // MODE 1: [batch][V][C]
+    const float* blank;                    // [C] or null
+    float blank_scalar;
+    const float* inv_bref;                 // device scalar 1/b_ref
+    float4* rec;                           // [batch][VS][C] {alpha, beta, g0, h*r}
+    double* partials;                      // [batch][blocks per slice]
+    SliceState* state;                     // [batch]
+    IterParams ip;
+    int monitor_only;
+};
+
+struct BackArgs {
+    DevGeom g;
+    const float4* rec;                     // [batch][VS][C]
+    int subset, M, VS;
+    float* out;                            // MODE 0: [batch][ny][nx]
+    const float* img;                      // MODE 1: padded mu(n)
+    float* img_new;                        // padded mu(n+1)
+    float* imgT_new;
+    float* best;                           // [batch][ny][nx] or null
+    const SliceState* state;
+    double tau;
+    float beta_over_M, eps2;
+};
+
+__device__ __forceinline__ size_t pad_off(const DevGeom& g, int iy, int ix) {
+    return (size_t)(iy + PADR) * g.pitch + PAD + ix;
+}
+__device__ __forceinline__ size_t padT_off(const DevGeom& g, int ix, int iy) {
+    return (size_t)(ix + PADR) * g.pitchT + PAD + iy;
+}
+
+// ------------------------------------------------------------------------------------------------
+// K1: forward projection (+ residual, monitor, step rule when MODE == 1).
+// grid (ceil(C/32), V_S, batch), block 32 x FWD_SEGS: lane = channel, warp = segment of the ray.
+// A ray marches over the image lines of its major axis (rows of img when |dy| >= |dx|, else rows of
+// the transposed copy imgT) and touches at most two adjacent pixels per line.
+// ------------------------------------------------------------------------------------------------
+template <int MODE>
+__global__ void __launch_bounds__(FWD_THREADS) k_forward(const FwdArgs a) {
+    const DevGeom& g = a.g;
+    const int lane = threadIdx.x & 31, seg = threadIdx.x >> 5;
+    const int c = blockIdx.x * 32 + lane, j = blockIdx.y, s = blockIdx.z;
+    const int v = a.subset < 0 ? j : a.subset + j * a.M;
+    __shared__ float part[FWD_SEGS][32];
+
+    float acc = 0.f;
+    float4 ray = make_float4(0.f, 0.f, 0.f, 0.f);
+    if (c < g.C) {
+        ray = __ldg(&g.rays[(size_t)v * g.C + c]);
+        const bool rowmaj = fabsf(ray.x) >= fabsf(ray.y);
+        const float kk = rowmaj ? ray.x : ray.y;          // coefficient of the in-line coordinate, |kk| >= 1
+        const float uu = rowmaj ? ray.y : ray.x;          // coefficient of the marching coordinate, +-1
+        const float* base = rowmaj ? a.img + (size_t)s * g.img_elems : a.imgT + (size_t)s * g.imgT_elems;
+        const int pitch = rowmaj ? g.pitch : g.pitchT;
+        const int na = rowmaj ? g.nx : g.ny, nb = rowmaj ? g.ny : g.nx;
+        const float ca = rowmaj ? g.cx : g.cy, cb = rowmaj ? g.cy : g.cx;
+        const float invk = 1.0f / kk;
+        const float hk = 0.5f * (fabsf(ray.x) + fabsf(ray.y));
+        // lines where the crossing lies within half a pixel of the image: |uu*b + g0| < |kk|*(na/2 + 1/2)
+        const float A = fabsf(kk) * (0.5f * na + 0.5f);
+        const float b1 = uu * (-ray.z - A), b2 = uu * (-ray.z + A);
+        const float flo = fminf(fmaxf(ceilf(fminf(b1, b2) + cb) - 1.f, 0.f), (float)nb);
+        const float fhi = fminf(fmaxf(floorf(fmaxf(b1, b2) + cb) + 1.f, -1.f), (float)(nb - 1));
+        const int jlo = (int)flo, jhi = (int)fhi;
+        const int nsteps = jhi - jlo + 1;
+        if (nsteps > 0) {
+            const int len = (nsteps + FWD_SEGS - 1) / FWD_SEGS;
+            const int j0 = jlo + seg * len;
+            const int j1 = min(j0 + len, jhi + 1);
+            const float* line = base + (size_t)(j0 + PADR) * pitch + PAD;
+            const int imax = na + PAD - 2;
+#pragma unroll 4
+            for (int jj = j0; jj < j1; ++jj, line += pitch) {
+                const float b = (float)jj - cb;
+                const float bg = fmaf(uu, b, ray.z);
+                const float fa = floorf(fmaf(-bg, invk, ca));     // index of the pixel left of the crossing
+                const float a0 = fa - ca;
+                const float q0 = fmaf(kk, a0, bg);
+                const float q1 = q0 + kk;
+                const float w0 = __saturatef(hk - fabsf(q0));
+                const float w1 = __saturatef(hk - fabsf(q1));
+                const int i0 = min(max((int)fa, -PAD), imax);
+                acc = fmaf(w0, __ldg(line + i0), acc);
+                acc = fmaf(w1, __ldg(line + i0 + 1), acc);
+            }
+        }
+    }
+    part[seg][lane] = acc;
+    __syncthreads();
+    if (seg != 0) return;
+
+    float t = 0.f;
+#pragma unroll
+    for (int k = 0; k < FWD_SEGS; ++k) t += part[k][lane];    // fixed order
+    const float l = ray.w * t;
+
+    if (MODE == 0) {
+        if (c < g.C) a.sino[((size_t)s * a.VS + j) * g.C + c] = l;
+        return;
+    }
+
+    // ---- A2: Poisson residual r = (b exp(-l) - y)/b_ref and monitor D = sum (l - ln(b/max(y,1)))^2 ----
+    double d2 = 0.0;
+    if (c < g.C) {
+        const float y = __ldg(&a.counts[((size_t)s * g.V + v) * g.C + c]);
+        const float b = a.blank ? __ldg(&a.blank[c]) : a.blank_scalar;
+        const float ybar = b * expf(-l);
+        const float r = (ybar - y) * __ldg(a.inv_bref);
+        if (!a.monitor_only)
+            a.rec[((size_t)s * a.VS + j) * g.C + c] = make_float4(ray.x, ray.y, ray.z, ray.w * r);
+        const float p = logf(b / fmaxf(y, 1.f));
+        const double d = (double)l - (double)p;
+        d2 = d * d;
+    }
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) d2 += __shfl_down_sync(0xffffffffu, d2, off);
+
+    const unsigned nblk = gridDim.x * gridDim.y;
+    const unsigned blk = blockIdx.y * gridDim.x + blockIdx.x;
+    double* partials = a.partials + (size_t)s * nblk;
+    SliceState* st = a.state + s;
+    unsigned ticket = 0;
+    if (lane == 0) {
+        partials[blk] = d2;
+        __threadfence();
+        ticket = atomicAdd(&st->ticket, 1u);
+    }
+    ticket = __shfl_sync(0xffffffffu, ticket, 0);
+    if (ticket != nblk - 1) return;
+
+    // ---- last block of this slice: D in a fixed order, then A3 (Eq. 4-5) ----
+    __threadfence();
+    double D = 0.0;
+    for (unsigned i = lane; i < nblk; i += 32) D += __ldcg(&partials[i]);
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) D += __shfl_down_sync(0xffffffffu, D, off);
+    if (lane != 0) return;
+    if (!isfinite(D)) st->not_finite = 1;
+    st->D_last = D;
+    if (a.monitor_only) {
+        st->improved = D < st->D_best;
+    } else {
+        const int n = st->n;
+        double lam;
+        if (a.ip.forced)        lam = a.ip.forced[n];
+        else if (n == 0)        lam = a.ip.lambda0;
+        else if (D < st->D_prev) lam = st->lambda + a.ip.up;
+        else                    lam = fmax(st->lambda - a.ip.down, a.ip.lmin);
+        st->lambda = lam;
+        st->D_prev = D;
+        if (a.ip.trace) {
+            double* tr = a.ip.trace + ((size_t)s * a.ip.n_iters + n) * 2;
+            tr[0] = D;
+            tr[1] = lam;
+        }
+        const int imp = a.ip.return_best && D < st->D_best;
+        if (imp) st->D_best = D;
+        st->improved = imp;
+        st->n = n + 1;
+    }
+    st->ticket = 0;
+}
+
+// ------------------------------------------------------------------------------------------------
+// Smoothed isotropic TV gradient (reading C8) of the 2x2 tile whose 4x4 neighbourhood is m:
+//   m[r][c] = mu(y0-1+r, x0-1+c).  Differences across the image border are 0, terms whose
+// neighbour is outside are dropped.
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ void tv_grad_tile(const float (&m)[4][4], int x0, int y0, int nx, int ny,
+                                             float eps2, float (&out)[2][2]) {
+    // it[r][c] = 1/t at (y0-1+r, x0-1+c) for r,c in 0..2
+    float it[3][3];
+#pragma unroll
+    for (int r = 0; r < 3; ++r)
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            const int x = x0 - 1 + c, y = y0 - 1 + r;
+            const float dxv = (x + 1 < nx) ? m[r][c + 1] - m[r][c] : 0.f;
+            const float dyv = (y + 1 < ny) ? m[r + 1][c] - m[r][c] : 0.f;
+            it[r][c] = rsqrtf(eps2 + dxv * dxv + dyv * dyv);
+        }
+#pragma unroll
+    for (int ty = 0; ty < 2; ++ty)
+#pragma unroll
+        for (int tx = 0; tx < 2; ++tx) {
+            const int x = x0 + tx, y = y0 + ty, r = ty + 1, c = tx + 1;
+            const float cv = m[r][c];
+            float sgrad = 0.f;
+            if (x > 0) sgrad += (cv - m[r][c - 1]) * it[r][c - 1];
+            if (y > 0) sgrad += (cv - m[r - 1][c]) * it[r - 1][c];
+            const float dxv = (x + 1 < nx) ? m[r][c + 1] - cv : 0.f;
+            const float dyv = (y + 1 < ny) ? m[r + 1][c] - cv : 0.f;
+            sgrad -= (dxv + dyv) * it[r][c];
+            out[ty][tx] = sgrad;
+        }
+}
+
+__device__ __forceinline__ void load_nbhd(const DevGeom& g, const float* img, int x0, int y0, float (&m)[4][4]) {
+#pragma unroll
+    for (int r = 0; r < 4; ++r) {
+        const int y = min(max(y0 - 1 + r, -PADR), g.ny + PADR - 1);
+        const float* row = img + (size_t)(y + PADR) * g.pitch + PAD;
+#pragma unroll
+        for (int c = 0; c < 4; ++c) {
+            const int x = min(x0 - 1 + c, g.nx + PAD - 1);
+            m[r][c] = __ldg(row + x);
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// K2: matched gather backprojection of the records written by K1 (+ TV gradient, Eq. 3 update,
+// positivity clamp, best-image copy when MODE == 1).
+// grid (ceil(nx/32), ceil(ny/16), batch), block 128: each thread owns a 2x2 pixel tile.  For every
+// view the channels whose ray can cross the tile form the interval |c - c*| < hw around the channel
+// coordinate c* of the tile centre; each candidate costs one 16-byte record load.
+// ------------------------------------------------------------------------------------------------
+template <int MODE>
+__global__ void __launch_bounds__(BK_THREADS) k_back(const BackArgs a) {
+    const DevGeom& g = a.g;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int tile_x = blockIdx.x * 16 + (warp & 1) * 8 + (lane & 7);
+    const int tile_y = blockIdx.y * 8 + (warp >> 1) * 4 + (lane >> 3);
+    const int x0 = tile_x * BK_TX, y0 = tile_y * BK_TY, s = blockIdx.z;
+    if (x0 >= g.nx || y0 >= g.ny) return;
+
+    const float xc0 = (float)x0 - g.cx, yc0 = (float)y0 - g.cy;
+    const float X = (xc0 + 0.5f * (BK_TX - 1)) * g.pixel, Y = (yc0 + 0.5f * (BK_TY - 1)) * g.pixel;
+    const float4* rec = a.rec + (size_t)s * a.VS * g.C;
+
+    float acc00 = 0.f, acc01 = 0.f, acc10 = 0.f, acc11 = 0.f;     // acc[ty][tx]
+    for (int jj = 0; jj < a.VS; ++jj, rec += g.C) {
+        const int v = a.subset < 0 ? jj : a.subset + jj * a.M;
+        const float2 cs = __ldg(&g.views[v]);
+        // fan angle of the tile centre: tan(gamma*) = perp/along
+        const float along = g.sad - fmaf(X, cs.x, Y * cs.y);
+        const float perp = fmaf(X, cs.y, -Y * cs.x);
+        const float z = __fdividef(perp, along);
+        float gam;
+        if (g.use_atanf) {
+            gam = atanf(z);
+        } else {
+            const float z2 = z * z;
+            gam = z * fmaf(z2, fmaf(z2, fmaf(z2, -1.f / 7.f, 0.2f), -1.f / 3.f), 1.f);
+        }
+        const float cstar = fmaf(gam, g.inv_dgamma, g.c_center);
+        // half-width of the tile seen from the source, in channels (+2 % and 0.05 channel of slack)
+        const float adX = fabsf(fmaf(-g.sad, cs.x, X)), adY = fabsf(fmaf(-g.sad, cs.y, Y));
+        const float L2 = fmaf(along, along, perp * perp);
+        const float hw = __fdividef(g.hw_scale * 0.5f * (BK_TX * adY + BK_TY * adX), L2) * 1.02f + 0.05f;
+        const int c_lo = max(0, (int)ceilf(cstar - hw));
+        const int c_hi = min(g.C - 1, (int)floorf(cstar + hw));
+        for (int c = c_lo; c <= c_hi; ++c) {
+            const float4 r = __ldg(&rec[c]);
+            const float hk = 0.5f * (fabsf(r.x) + fabsf(r.y));
+            const float q00 = fmaf(r.x, xc0, fmaf(r.y, yc0, r.z));
+            const float q01 = q00 + r.x;          // (ty=0, tx=1)
+            const float q10 = q00 + r.y;          // (ty=1, tx=0)
+            const float q11 = q10 + r.x;
+            acc00 = fmaf(__saturatef(hk - fabsf(q00)), r.w, acc00);
+            acc01 = fmaf(__saturatef(hk - fabsf(q01)), r.w, acc01);
+            acc10 = fmaf(__saturatef(hk - fabsf(q10)), r.w, acc10);
+            acc11 = fmaf(__saturatef(hk - fabsf(q11)), r.w, acc11);
+        }
+    }
+
+    const bool vx1 = x0 + 1 < g.nx, vy1 = y0 + 1 < g.ny;
+    if (MODE == 0) {
+        float* out = a.out + (size_t)s * g.nx * g.ny;
+        out[(size_t)y0 * g.nx + x0] = acc00;
+        if (vx1) out[(size_t)y0 * g.nx + x0 + 1] = acc01;
+        if (vy1) out[(size_t)(y0 + 1) * g.nx + x0] = acc10;
+        if (vx1 && vy1) out[(size_t)(y0 + 1) * g.nx + x0 + 1] = acc11;
+        return;
+    }
+
+    // ---- A5 TV gradient of mu(n), A6 update (Eq. 3) with mu > 0, A7 best copy ----
+    const float* img = a.img + (size_t)s * g.img_elems;
+    float m[4][4], tv[2][2];
+    load_nbhd(g, img, x0, y0, m);
+    tv_grad_tile(m, x0, y0, g.nx, g.ny, a.eps2, tv);
+    const SliceState* st = a.state + s;
+    const float step = (float)(st->lambda * a.tau);
+    const float u00 = fmaxf(fmaf(step, acc00 - a.beta_over_M * tv[0][0], m[1][1]), 0.f);
+    const float u01 = fmaxf(fmaf(step, acc01 - a.beta_over_M * tv[0][1], m[1][2]), 0.f);
+    const float u10 = fmaxf(fmaf(step, acc10 - a.beta_over_M * tv[1][0], m[2][1]), 0.f);
+    const float u11 = fmaxf(fmaf(step, acc11 - a.beta_over_M * tv[1][1], m[2][2]), 0.f);
+
+    float* nimg = a.img_new + (size_t)s * g.img_elems;
+    float* nimgT = a.imgT_new + (size_t)s * g.imgT_elems;
+    nimg[pad_off(g, y0, x0)] = u00;
+    nimgT[padT_off(g, x0, y0)] = u00;
+    if (vx1) { nimg[pad_off(g, y0, x0 + 1)] = u01; nimgT[padT_off(g, x0 + 1, y0)] = u01; }
+    if (vy1) { nimg[pad_off(g, y0 + 1, x0)] = u10; nimgT[padT_off(g, x0, y0 + 1)] = u10; }
+    if (vx1 && vy1) { nimg[pad_off(g, y0 + 1, x0 + 1)] = u11; nimgT[padT_off(g, x0 + 1, y0 + 1)] = u11; }
+
+    if (a.best && st->improved) {
+        float* best = a.best + (size_t)s * g.nx * g.ny;
+        best[(size_t)y0 * g.nx + x0] = m[1][1];
+        if (vx1) best[(size_t)y0 * g.nx + x0 + 1] = m[1][2];
+        if (vy1) best[(size_t)(y0 + 1) * g.nx + x0] = m[2][1];
+        if (vx1 && vy1) best[(size_t)(y0 + 1) * g.nx + x0 + 1] = m[2][2];
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// Small helpers around the two hot kernels
+// ------------------------------------------------------------------------------------------------
+
+// [batch][ny][nx] -> padded img and padded transpose imgT (32x32 tiles through shared memory)
+__global__ void __launch_bounds__(256) k_pad_transpose(DevGeom g, const float* __restrict__ src,
+                                                       float* __restrict__ img, float* __restrict__ imgT) {
+    __shared__ float tile[32][33];
+    const int s = blockIdx.z;
+    const int bx = blockIdx.x * 32, by = blockIdx.y * 32;
+    const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;       // 32 x 8
+    src += (size_t)s * g.nx * g.ny;
+    img += (size_t)s * g.img_elems;
+    imgT += (size_t)s * g.imgT_elems;
+    for (int r = ty; r < 32; r += 8) {
+        const int x = bx + tx, y = by + r;
+        float v = 0.f;
+        if (x < g.nx && y < g.ny) {
+            v = src[(size_t)y * g.nx + x];
+            img[pad_off(g, y, x)] = v;
+        }
+        tile[r][tx] = v;
+    }
+    __syncthreads();
+    for (int r = ty; r < 32; r += 8) {
+        const int x = bx + r, y = by + tx;
+        if (x < g.nx && y < g.ny) imgT[padT_off(g, x, y)] = tile[tx][r];
+    }
+}
+
+// padded img -> [batch][ny][nx]; with best != null picks per slice: improved ? img : best   (C12)
+__global__ void __launch_bounds__(256) k_unpad(DevGeom g, const float* __restrict__ img,
+                                               const float* __restrict__ best, const SliceState* __restrict__ state,
+                                               float* __restrict__ out) {
+    const int s = blockIdx.z;
+    const int x = blockIdx.x * 32 + (threadIdx.x & 31);
+    const int y = blockIdx.y * 8 + (threadIdx.x >> 5);
+    if (x >= g.nx || y >= g.ny) return;
+    const size_t o = (size_t)s * g.nx * g.ny + (size_t)y * g.nx + x;
+    if (best && !state[s].improved) out[o] = best[o];
+    else out[o] = img[(size_t)s * g.img_elems + pad_off(g, y, x)];
+}
+
+// homogeneous initial image into both padded layouts, and into best
+__global__ void __launch_bounds__(256) k_fill(DevGeom g, float mu0, float* __restrict__ img,
+                                              float* __restrict__ imgT, float* __restrict__ best) {
+    const int s = blockIdx.z;
+    const int x = blockIdx.x * 32 + (threadIdx.x & 31);
+    const int y = blockIdx.y * 8 + (threadIdx.x >> 5);
+    if (x >= g.nx || y >= g.ny) return;
+    img[(size_t)s * g.img_elems + pad_off(g, y, x)] = mu0;
+    imgT[(size_t)s * g.imgT_elems + padT_off(g, x, y)] = mu0;
+    if (best) best[(size_t)s * g.nx * g.ny + (size_t)y * g.nx + x] = mu0;
+}
+
+// per-slice state reset and 1/b_ref, b_ref = mean_c b_c (one warp, fixed order)
+__global__ void k_init_state(SliceState* state, int batch, double lambda0, const float* blank, float blank_scalar,
+                             int C, float* inv_bref) {
+    const int lane = threadIdx.x;
+    for (int s = lane; s < batch; s += 32) {
+        SliceState st;
+        st.lambda = lambda0; st.D_prev = 0.0; st.D_best = __longlong_as_double(0x7ff0000000000000LL);
+        st.D_last = 0.0; st.n = 0; st.improved = 0; st.not_finite = 0; st.ticket = 0;
+        state[s] = st;
+    }
+    double sum = 0.0;
+    if (blank) {
+        for (int c = lane; c < C; c += 32) sum += (double)blank[c];
+        for (int off = 16; off > 0; off >>= 1) sum += __shfl_down_sync(0xffffffffu, sum, off);
+        sum /= (double)C;
+    } else {
+        sum = (double)blank_scalar;
+    }
+    if (lane == 0) *inv_bref = (float)(1.0 / sum);
+}
+
+// sinogram [batch][VS][C] -> records {alpha, beta, g0, h*s} for the standalone backprojection
+__global__ void __launch_bounds__(256) k_make_rec(DevGeom g, const float* __restrict__ sino, float4* __restrict__ rec,
+                                                  int subset, int M, int VS) {
+    const int c = blockIdx.x * 256 + threadIdx.x, j = blockIdx.y, s = blockIdx.z;
+    if (c >= g.C) return;
+    const int v = subset < 0 ? j : subset + j * M;
+    const float4 ray = __ldg(&g.rays[(size_t)v * g.C + c]);
+    const size_t o = ((size_t)s * VS + j) * g.C + c;
+    rec[o] = make_float4(ray.x, ray.y, ray.z, ray.w * sino[o]);
+}
+
+// standalone TV gradient: [batch][ny][nx] -> [batch][ny][nx] through the padded workspace
+__global__ void __launch_bounds__(BK_THREADS) k_tv(DevGeom g, const float* __restrict__ img, float eps2,
+                                                   float* __restrict__ out) {
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int x0 = (blockIdx.x * 16 + (warp & 1) * 8 + (lane & 7)) * 2;
+    const int y0 = (blockIdx.y * 8 + (warp >> 1) * 4 + (lane >> 3)) * 2;
+    const int s = blockIdx.z;
+    if (x0 >= g.nx || y0 >= g.ny) return;
+    float m[4][4], tv[2][2];
+    load_nbhd(g, img + (size_t)s * g.img_elems, x0, y0, m);
+    tv_grad_tile(m, x0, y0, g.nx, g.ny, eps2, tv);
+    out += (size_t)s * g.nx * g.ny;
+    const bool vx1 = x0 + 1 < g.nx, vy1 = y0 + 1 < g.ny;
+    out[(size_t)y0 * g.nx + x0] = tv[0][0];
+    if (vx1) out[(size_t)y0 * g.nx + x0 + 1] = tv[0][1];
+    if (vy1) out[(size_t)(y0 + 1) * g.nx + x0] = tv[1][0];
+    if (vx1 && vy1) out[(size_t)(y0 + 1) * g.nx + x0 + 1] = tv[1][1];
+}
+
+}  // namespace osiv
