@@ -96,6 +96,13 @@ int osiv_create(const osiv_geometry* geom, int32_t max_batch, int32_t device, os
 /* Release everything the handle owns (synchronises the device).  NULL is accepted. */
 int osiv_destroy(osiv_handle* h);
 
+/* A0 setup, host only (no GPU needed): the per-ray coefficients the kernels use.  Writes, for every ray
+ * (v,c), four floats {alpha, beta, g0, h} to h_rays [V][C][4] and {cos th_v, sin th_v} to h_views [V][2]
+ * (either may be NULL), such that the chord of reading C2 is
+ *   a(v,c; ix,iy) = h * clamp( (|alpha|+|beta|)/2 - |alpha*(ix-(nx-1)/2) + beta*(iy-(ny-1)/2) + g0|, 0, 1 ).
+ * Computed in float64, rounded once to float32. */
+int osiv_ray_table(const osiv_geometry* geom, float* h_rays, float* h_views);
+
 /* Resolved channel pitch (after the dgamma_rad <= 0 rule) and step constant tau_S for M subsets. */
 int osiv_get_dgamma(const osiv_handle* h, double* dgamma_rad);
 int osiv_get_tau(const osiv_handle* h, int32_t n_subsets, double kappa, double* tau);

@@ -16,7 +16,7 @@ from . import build as _build
 OSIV_OK, OSIV_ERR_INVALID_ARG, OSIV_ERR_CUDA, OSIV_ERR_NOT_FINITE = 0, -1, -2, -3
 
 EXPORTED_SYMBOLS = (
-    "osiv_version", "osiv_strerror", "osiv_default_params", "osiv_create", "osiv_destroy", "osiv_get_dgamma",
+    "osiv_version", "osiv_strerror", "osiv_default_params", "osiv_create", "osiv_destroy", "osiv_ray_table", "osiv_get_dgamma",
     "osiv_get_tau", "osiv_launch_count", "osiv_forward", "osiv_backward", "osiv_tv_gradient", "osiv_reconstruct",
     "osiv_reconstruct_host",
 )
@@ -95,6 +95,7 @@ def lib():
         L.osiv_default_params.argtypes = [C.POINTER(_CParams)]
         L.osiv_create.argtypes = [C.POINTER(_CGeometry), ip, ip, C.POINTER(vp)]
         L.osiv_destroy.argtypes = [vp]
+        L.osiv_ray_table.argtypes = [C.POINTER(_CGeometry), vp, vp]
         L.osiv_get_dgamma.argtypes = [vp, C.POINTER(C.c_double)]
         L.osiv_get_tau.argtypes = [vp, ip, C.c_double, C.POINTER(C.c_double)]
         L.osiv_launch_count.restype = C.c_int64
@@ -122,6 +123,15 @@ def default_params() -> Params:
     return Params(beta=cp.beta, n_subsets=cp.n_subsets, n_iters=cp.n_iters, mu0=cp.mu0, lambda0=cp.lambda0,
                   lambda_up=cp.lambda_up, lambda_down=cp.lambda_down, lambda_min=cp.lambda_min, kappa=cp.kappa,
                   tv_eps=cp.tv_eps, return_best=cp.return_best)
+
+
+def ray_table(geom: "Geometry"):
+    """A0 setup on the host (no GPU): (rays [V][C][4] = {alpha, beta, g0, h}, views [V][2]) float32."""
+    rays = np.zeros((geom.n_views, geom.n_channels, 4), dtype=np.float32)
+    views = np.zeros((geom.n_views, 2), dtype=np.float32)
+    cg = geom.c()
+    _check(lib().osiv_ray_table(C.byref(cg), rays.ctypes.data, views.ctypes.data), "osiv_ray_table")
+    return rays, views
 
 
 def _check(status: int, where: str) -> None:

@@ -171,10 +171,7 @@ int osiv_default_params(osiv_params* p) {
     return OSIV_OK;
 }
 
-int osiv_create(const osiv_geometry* geom, int32_t max_batch, int32_t device, osiv_handle** out) {
-    if (out) *out = nullptr;
-    if (!geom || !out || max_batch <= 0 || device < 0) return OSIV_ERR_INVALID_ARG;
-    const osiv_geometry& g = *geom;
+static int check_geometry(const osiv_geometry& g) {
     if (g.nx <= 0 || g.ny <= 0 || g.n_views <= 0 || g.n_channels <= 0 || g.nx > 16384 || g.ny > 16384)
         return OSIV_ERR_INVALID_ARG;
     if (!(g.pixel_mm > 0.0) || !(g.sad_mm > 0.0) || !std::isfinite(g.pixel_mm) || !std::isfinite(g.sad_mm) ||
@@ -185,6 +182,26 @@ int osiv_create(const osiv_geometry* geom, int32_t max_batch, int32_t device, os
     if (g.dgamma_rad <= 0.0 && 0.5 * (g.nx < g.ny ? g.nx : g.ny) * g.pixel_mm >= g.sad_mm) return OSIV_ERR_INVALID_ARG;
     const double dgamma = resolve_dgamma(g);
     if (!(dgamma > 0.0) || dgamma * g.n_channels >= M_PI) return OSIV_ERR_INVALID_ARG;
+    return OSIV_OK;
+}
+
+int osiv_ray_table(const osiv_geometry* geom, float* h_rays, float* h_views) {
+    if (!geom || check_geometry(*geom) != OSIV_OK) return OSIV_ERR_INVALID_ARG;
+    std::vector<float4> rays;
+    std::vector<float2> views;
+    build_tables(*geom, resolve_dgamma(*geom), rays, views);
+    if (h_rays) std::memcpy(h_rays, rays.data(), rays.size() * sizeof(float4));
+    if (h_views) std::memcpy(h_views, views.data(), views.size() * sizeof(float2));
+    return OSIV_OK;
+}
+
+int osiv_create(const osiv_geometry* geom, int32_t max_batch, int32_t device, osiv_handle** out) {
+    if (out) *out = nullptr;
+    if (!geom || !out || max_batch <= 0 || device < 0) return OSIV_ERR_INVALID_ARG;
+    const osiv_geometry& g = *geom;
+    if (check_geometry(g) != OSIV_OK) return OSIV_ERR_INVALID_ARG;
+    const double rmax = 0.5 * g.pixel_mm * std::sqrt((double)g.nx * g.nx + (double)g.ny * g.ny);
+    const double dgamma = resolve_dgamma(g);
 
     DeviceGuard guard(device);
     if (!guard.ok) { cudaGetLastError(); return OSIV_ERR_CUDA; }
@@ -220,6 +237,8 @@ int osiv_create(const osiv_geometry* geom, int32_t max_batch, int32_t device, os
     // short odd series for atan: error < z^9/9; demand < 0.01 channel, else fall back to atanf
     const double zmax = rmax / (g.sad_mm - rmax);
     d.use_atanf = (std::pow(zmax, 9) / 9.0 / dgamma > 0.01) ? 1 : 0;
+    d.tile_r = (float)(0.5 * g.pixel_mm * std::sqrt((double)(BK_TX * BK_TX + BK_TY * BK_TY)));
+    d.wide = (d.tile_r / (g.sad_mm - rmax) > 0.015 || d.use_atanf) ? 1 : 0;
     d.rays = h->d_rays; d.views = h->d_views;
     *out = h;
     return OSIV_OK;

@@ -38,6 +38,8 @@ struct DevGeom {
     float pixel, sad, inv_dgamma, c_center;   // c_center = (C-1)/2 - channel_offset
     float hw_scale;                        // pixel / dgamma
     int use_atanf;                         // fan too wide for the short atan series
+    int wide;                              // tiles subtend a large angle: use the enclosing-circle candidate bound
+    float tile_r;                          // half-diagonal of a backprojector tile [mm]
     const float4* rays;                    // [V][C] {alpha, beta, g0, h}
     const float2* views;                   // [V] {cos th_v, sin th_v}
 };
@@ -314,7 +316,12 @@ __global__ void __launch_bounds__(BK_THREADS) k_back(const BackArgs a) {
         // half-width of the tile seen from the source, in channels (+2 % and 0.05 channel of slack)
         const float adX = fabsf(fmaf(-g.sad, cs.x, X)), adY = fabsf(fmaf(-g.sad, cs.y, Y));
         const float L2 = fmaf(along, along, perp * perp);
-        const float hw = __fdividef(g.hw_scale * 0.5f * (BK_TX * adY + BK_TY * adX), L2) * 1.02f + 0.05f;
+        float hw;
+        if (g.wide) {                      // every ray through the tile lies within asin(R/L) of its centre
+            hw = asinf(fminf(g.tile_r * rsqrtf(L2), 1.f)) * g.inv_dgamma * 1.001f + 0.05f;
+        } else {                           // tight: projected half-width / (L dgamma), direction error < R/L <= 1.5 %
+            hw = __fdividef(g.hw_scale * 0.5f * (BK_TX * adY + BK_TY * adX), L2) * 1.02f + 0.05f;
+        }
         const int c_lo = max(0, (int)ceilf(cstar - hw));
         const int c_hi = min(g.C - 1, (int)floorf(cstar + hw));
         for (int c = c_lo; c <= c_hi; ++c) {
