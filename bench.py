@@ -1,0 +1,307 @@
+#!/usr/bin/env python
+"""bench.py -- headline measurement of the OS-TV hot path (BASELINE.json metric) on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload 3|2|1]
+
+A "step" is one pass of the whole hot path over one batch of synthetic input: one complete
+reconstruction of the workload (config 3 by default: 512x512, 800 x 738, 20 ordered subsets, 500
+subset iterations, beta = 0.005) = 500 x (K1 forward+residual+monitor+step rule, K2 back+TV+update).
+`value` = subset iterations per second over the whole job, inputs resident in HBM; `e2e` = the same
+through osiv_reconstruct_host (host buffers, H2D + D2H inside the timed region).  With N > 1 (torchrun)
+every rank reconstructs its own slice (weak scaling, no data-path collective); time = max over ranks.
+
+`--impl reference` times the float64 CPU oracle (oracle/) as it stands on the host cores, one bounded
+sample of the same workload per step; only that leg and `cpu_baseline` execute anything under oracle/.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import synth_inputs as si  # noqa: E402
+
+METRIC = "os_tv_iterations_per_s"
+UNIT = "iterations/s"
+FP32_FLOP_PER_NNZ = 6          # q (FMA, 2) + half-width minus |q| (1) + clamp (1) + accumulate (FMA, 2)
+NNZ_PER_RAY_PER_N = 1.193      # measured non-zeros per ray / N when the fan spans the inscribed circle
+SM_COUNT, FP32_LANES_PER_SM = 148, 128
+
+
+def load_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return d, "measured"
+    return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0}, "fallback"
+
+
+def workload_desc(cfg, beta, batch):
+    return {"workload": f"config{cfg.name}: {cfg.nx}x{cfg.ny} image, {cfg.n_views}x{cfg.n_channels} fan sinogram, "
+                        f"{cfg.n_subsets} ordered subsets, {cfg.n_iters} subset iterations, beta={beta}, "
+                        f"Poisson(I0={cfg.i0:g}) counts of a seeded {cfg.n_ellipses}-ellipse phantom",
+            "slices_per_gpu": batch, "image": [cfg.ny, cfg.nx], "views": cfg.n_views, "channels": cfg.n_channels,
+            "subsets": cfg.n_subsets, "iterations_per_step": cfg.n_iters, "beta": beta,
+            "l2": "flushed between steps (256 MiB memset, outside the per-step events)",
+            "parallelism": "one slice per GPU, no collective"}
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md recipe)."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index: int):
+        self.gpu = gpu_index
+        self.proc = None
+        self.path = None
+
+    def start(self):
+        try:
+            fd, self.path = tempfile.mkstemp(suffix=".csv")
+            os.close(fd)
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.gpu), f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=open(self.path, "w"), stderr=subprocess.DEVNULL)
+        except Exception:
+            self.proc = None
+
+    def stop(self):
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        if self.proc is None:
+            return out
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        try:
+            for line in open(self.path):
+                f = [x.strip() for x in line.split(",")]
+                if len(f) < 9:
+                    continue
+                try:
+                    sm.append(float(f[1]))
+                    mx.append(float(f[2]))
+                except ValueError:
+                    continue
+                for name, val in zip(names, f[5:9]):
+                    if val.lower().startswith("active"):
+                        reasons.add(name)
+            os.unlink(self.path)
+        except Exception:
+            pass
+        if sm:
+            out.update(sm_mhz=float(np.median(sm)), sm_max_mhz=float(max(mx)), samples=len(sm))
+        out["reasons"] = sorted(reasons)
+        return out
+
+
+def oracle_sample(cfg, beta, counts, n_iters):
+    """Time the oracle, as it stands, on the first n_iters subset iterations of the workload."""
+    import oracle
+    og = oracle.Geometry(cfg.nx, cfg.ny, cfg.pixel_mm, cfg.n_views, cfg.n_channels, cfg.sad_mm, cfg.dgamma_rad,
+                         cfg.channel_offset, cfg.theta0_rad)
+    prm = oracle.Params(beta=beta, n_subsets=cfg.n_subsets, n_iters=n_iters)
+    t0 = time.perf_counter()
+    img, trace, status = oracle.reconstruct(og, counts, cfg.i0, prm)
+    dt = time.perf_counter() - t0
+    return dt, oracle.num_threads(), img
+
+
+def run_reference(args, cfg, beta):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    _, _, counts = si.make_case(cfg)
+    n_sample = min(cfg.n_iters, cfg.n_subsets)            # one pass over all subsets per step
+    for _ in range(args.warmup):
+        oracle_sample(cfg, beta, counts, n_sample)
+    t = 0.0
+    cores = 1
+    for _ in range(args.steps):
+        dt, cores, _ = oracle_sample(cfg, beta, counts, n_sample)
+        t += dt
+    value = n_sample * args.steps / t
+    sample = f"first {n_sample} of {cfg.n_iters} subset iterations of the workload per step (float64 oracle, OpenMP)"
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * t / args.steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": workload_desc(cfg, beta, 1),
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+    return 0
+
+
+def run_ours(args, cfg, beta):
+    import torch
+    import torch.distributed as dist
+    import paper_1903_10088_b200 as osiv
+    from paper_1903_10088_b200 import sharding
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device -- the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    osiv.lib()
+
+    geom = osiv.Geometry(cfg.nx, cfg.ny, cfg.pixel_mm, cfg.n_views, cfg.n_channels, cfg.sad_mm, cfg.sdd_mm,
+                         cfg.dgamma_rad, cfg.channel_offset, cfg.theta0_rad)
+    batch = 1
+    lo, hi = sharding.slice_range(rank, world, world * batch)     # weak scaling: `batch` slices per rank
+    counts_np = np.stack([si.make_case(cfg, slice_index=s)[2] for s in range(lo, hi)])
+    prm = osiv.Params(beta=beta, n_subsets=cfg.n_subsets, n_iters=cfg.n_iters)
+    h = osiv.Handle(geom, max_batch=batch, device=local)
+    counts = torch.from_numpy(counts_np).to(dev)
+    out = torch.empty((batch, cfg.ny, cfg.nx), dtype=torch.float32, device=dev)
+    flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device=dev)
+    pin_counts = torch.from_numpy(counts_np).pin_memory()
+    pin_out = torch.empty((batch, cfg.ny, cfg.nx), dtype=torch.float32).pin_memory()
+
+    def step():
+        h.reconstruct(counts, cfg.i0, prm, out=out)
+
+    def step_e2e():
+        h.reconstruct_host(pin_counts, cfg.i0, prm, out=pin_out)
+
+    for _ in range(max(args.warmup, 3)):
+        step()
+    step_e2e()
+    torch.cuda.synchronize()
+
+    # ---- timed region: K steps, device events per step, L2 flushed in between ----
+    sampler = ClockSampler(local)
+    sampler.start()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    sharding.barrier()
+    torch.cuda.synchronize()
+    n0 = h.launch_count()
+    wall0 = time.perf_counter()
+    for a, b in ev:
+        flush.zero_()
+        a.record()
+        step()
+        b.record()
+    torch.cuda.synchronize()
+    sharding.barrier()
+    wall = time.perf_counter() - wall0
+    launches = h.launch_count() - n0
+    t_dev = sum(a.elapsed_time(b) for a, b in ev) * 1e-3
+    t_dev = sharding.max_over_ranks(t_dev, dev)
+    clocks = sampler.stop()
+
+    # ---- end-to-end: host buffers through osiv_reconstruct_host ----
+    sharding.barrier()
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        step_e2e()
+    torch.cuda.synchronize()
+    t_e2e = sharding.max_over_ranks(time.perf_counter() - t0, dev)
+
+    # ---- per-kernel durations for the roofline (2 extra profiled steps; events around every launch) ----
+    h.set_profiling(True)
+    for _ in range(2):
+        flush.zero_()
+        step()
+    ms_f, n_f, ms_b, n_b = h.get_profile()
+    h.set_profiling(False)
+
+    total_iters = world * batch * cfg.n_iters * args.steps
+    value = total_iters / t_dev
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return 0
+
+    peaks, peak_kind = load_peaks()
+    sm_mhz_peak = float(peaks.get("sm_max_mhz", 1965.0))
+    alu_peak_tflops = SM_COUNT * FP32_LANES_PER_SM * 2 * sm_mhz_peak * 1e6 / 1e12
+    vs = cfg.n_views // cfg.n_subsets
+    nnz = NNZ_PER_RAY_PER_N * max(cfg.nx, cfg.ny) * vs * cfg.n_channels * batch       # per launch, fwd = back
+    kernels = {}
+    for name, ms, n in (("k_forward<1>", ms_f, n_f), ("k_back<1>", ms_b, n_b)):
+        us = 1e3 * ms / max(n, 1)
+        tf = nnz * FP32_FLOP_PER_NNZ / (us * 1e-6) / 1e12
+        kernels[name] = {"avg_us": us, "achieved_tflops": tf, "frac": tf / alu_peak_tflops, "launches": n}
+    dom = max(kernels, key=lambda k: kernels[k]["avg_us"])
+    # compulsory HBM bytes per launch: everything is L2-resident, so this is a floor
+    hbm_bytes = {"k_forward<1>": (cfg.nx * cfg.ny * 4 + 2 * vs * cfg.n_channels * 4 + vs * cfg.n_channels * 32) * batch,
+                 "k_back<1>": (cfg.nx * cfg.ny * 4 * 3 + vs * cfg.n_channels * 16) * batch}
+    roof = {"bound": "alu", "kernel": dom, "achieved": kernels[dom]["achieved_tflops"], "peak": alu_peak_tflops,
+            "unit": "TFLOP/s", "frac": kernels[dom]["frac"], "traffic": None,
+            "peak_source": f"148 SMs x 128 FP32 lanes x 2 flop x {sm_mhz_peak:.0f} MHz ({peak_kind} sm_max_mhz)",
+            "algorithmic_flop_per_launch": nnz * FP32_FLOP_PER_NNZ, "nnz_per_launch": nnz,
+            "timing": "CUDA events around every launch on the launching stream, 2 extra steps after the timed region",
+            "kernels": kernels,
+            "hbm": {"compulsory_bytes_per_launch": hbm_bytes[dom],
+                    "achieved_gbs": hbm_bytes[dom] / (kernels[dom]["avg_us"] * 1e-6) / 1e9,
+                    "peak_gbs": float(peaks["hbm_gbs"]), "peak_kind": peak_kind,
+                    "frac": hbm_bytes[dom] / (kernels[dom]["avg_us"] * 1e-6) / 1e9 / float(peaks["hbm_gbs"])}}
+
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": max(args.warmup, 3), "ms_per_step": 1e3 * t_dev / args.steps, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": workload_desc(cfg, beta, batch),
+            "seconds_per_500_iter_recon": (t_dev / args.steps) * 500.0 / cfg.n_iters,
+            "wall_ms_per_step_incl_flush": 1e3 * wall / args.steps,
+            "paper_context": {"gtx1080ti_s_per_slice_thinning_1_20": 3.71, "iterations_per_s": 134.8,
+                              "source": "PAPER.md:156,164 Table I (other hardware, real data; context only)"},
+            "clocks": clocks,
+            "e2e": {"value": world * batch * cfg.n_iters * args.steps / t_e2e, "unit": UNIT,
+                    "h2d_bytes_per_step": int(pin_counts.numel() * 4), "d2h_bytes_per_step": int(pin_out.numel() * 4),
+                    "ms_per_step": 1e3 * t_e2e / args.steps},
+            "gpu_launches": int(launches),
+            "roofline": roof}
+
+    if not args.no_cpu_baseline:
+        n_sample = min(cfg.n_iters, 5 * cfg.n_subsets)
+        dt, cores, _ = oracle_sample(cfg, beta, counts_np[0], n_sample)
+        line["cpu_baseline"] = {"value": n_sample / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
+                                "sample": f"first {n_sample} of {cfg.n_iters} subset iterations of slice 0 "
+                                          f"({dt:.1f} s, float64 oracle with OpenMP)"}
+    print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="3", choices=["1", "2", "3"])
+    ap.add_argument("--beta", type=float, default=None)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    cfg = si.scan_config(args.workload)
+    beta = args.beta if args.beta is not None else (0.005 if args.workload == "3" else cfg.betas[0])
+    if args.impl == "reference":
+        return run_reference(args, cfg, beta)
+    return run_ours(args, cfg, beta)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -110,6 +110,14 @@ int osiv_get_tau(const osiv_handle* h, int32_t n_subsets, double kappa, double* 
 /* Number of CUDA kernels this handle has launched since osiv_create (for launch accounting). */
 int64_t osiv_launch_count(const osiv_handle* h);
 
+/* Per-kernel device timing for the roofline report.  While enabled (enable != 0), osiv_reconstruct records a
+ * CUDA event on cuda_stream before and after every K1 (forward + residual + monitor + step rule) and K2
+ * (backprojection + TV + update) launch and synchronises the stream at the end of the call to accumulate the
+ * elapsed times; use it on extra steps, not on the steps whose throughput is reported.
+ * osiv_get_profile returns the sums since the last osiv_set_profiling call: milliseconds and launch counts. */
+int osiv_set_profiling(osiv_handle* h, int32_t enable);
+int osiv_get_profile(const osiv_handle* h, double* ms_forward, int64_t* n_forward, double* ms_back, int64_t* n_back);
+
 /* Forward projection ("reprojection"):  l_i = sum_r a(i,r) mu_r  for the rays of
  * subset `subset` of `n_subsets` (subset < 0: all views; then n_subsets is ignored), where a(i,r) is
  * the exact length of ray i inside square pixel r (C2).

@@ -17,7 +17,7 @@ OSIV_OK, OSIV_ERR_INVALID_ARG, OSIV_ERR_CUDA, OSIV_ERR_NOT_FINITE = 0, -1, -2, -
 
 EXPORTED_SYMBOLS = (
     "osiv_version", "osiv_strerror", "osiv_default_params", "osiv_create", "osiv_destroy", "osiv_ray_table", "osiv_get_dgamma",
-    "osiv_get_tau", "osiv_launch_count", "osiv_forward", "osiv_backward", "osiv_tv_gradient", "osiv_reconstruct",
+    "osiv_get_tau", "osiv_launch_count", "osiv_set_profiling", "osiv_get_profile", "osiv_forward", "osiv_backward", "osiv_tv_gradient", "osiv_reconstruct",
     "osiv_reconstruct_host",
 )
 
@@ -100,6 +100,9 @@ def lib():
         L.osiv_get_tau.argtypes = [vp, ip, C.c_double, C.POINTER(C.c_double)]
         L.osiv_launch_count.restype = C.c_int64
         L.osiv_launch_count.argtypes = [vp]
+        L.osiv_set_profiling.argtypes = [vp, ip]
+        L.osiv_get_profile.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_int64), C.POINTER(C.c_double),
+                                       C.POINTER(C.c_int64)]
         L.osiv_forward.argtypes = [vp, vp, vp, ip, ip, ip, vp]
         L.osiv_backward.argtypes = [vp, vp, vp, ip, ip, ip, vp]
         L.osiv_tv_gradient.argtypes = [vp, vp, vp, ip, C.c_double, vp]
@@ -207,6 +210,16 @@ class Handle:
 
     def launch_count(self) -> int:
         return int(lib().osiv_launch_count(self._h))
+
+    def set_profiling(self, enable: bool) -> None:
+        _check(lib().osiv_set_profiling(self._h, 1 if enable else 0), "osiv_set_profiling")
+
+    def get_profile(self):
+        """(ms_forward, n_forward, ms_back, n_back) accumulated by profiled osiv_reconstruct calls"""
+        a, b = C.c_double(), C.c_double()
+        na, nb = C.c_int64(), C.c_int64()
+        _check(lib().osiv_get_profile(self._h, C.byref(a), C.byref(na), C.byref(b), C.byref(nb)), "osiv_get_profile")
+        return a.value, na.value, b.value, nb.value
 
     def n_subset_views(self, subset: int, n_subsets: int) -> int:
         return self.geom.n_views if subset < 0 else self.geom.n_views // n_subsets

@@ -36,6 +36,11 @@ struct osiv_handle {
     float* d_hblank = nullptr;
     size_t hi_elems = 0;        float* d_himg = nullptr;
     int64_t launches = 0;
+    // per-kernel event timing (osiv_set_profiling)
+    bool profiling = false;
+    std::vector<cudaEvent_t> events;
+    double prof_ms_fwd = 0.0, prof_ms_back = 0.0;
+    int64_t prof_n_fwd = 0, prof_n_back = 0;
 };
 
 namespace {
@@ -253,6 +258,7 @@ int osiv_destroy(osiv_handle* h) {
                         h->d_partials, h->d_state, h->d_inv_bref, h->d_trace, h->d_forced, h->d_hcounts, h->d_hblank,
                         h->d_himg};
         for (void* p : ptrs) if (p) cudaFree(p);
+        for (cudaEvent_t e : h->events) cudaEventDestroy(e);
         cudaGetLastError();
     }
     delete h;
@@ -275,6 +281,23 @@ int osiv_get_tau(const osiv_handle* h, int32_t n_subsets, double kappa, double* 
 }
 
 int64_t osiv_launch_count(const osiv_handle* h) { return h ? h->launches : 0; }
+
+int osiv_set_profiling(osiv_handle* h, int32_t enable) {
+    if (!h) return OSIV_ERR_INVALID_ARG;
+    h->profiling = enable != 0;
+    h->prof_ms_fwd = h->prof_ms_back = 0.0;
+    h->prof_n_fwd = h->prof_n_back = 0;
+    return OSIV_OK;
+}
+
+int osiv_get_profile(const osiv_handle* h, double* ms_forward, int64_t* n_forward, double* ms_back, int64_t* n_back) {
+    if (!h) return OSIV_ERR_INVALID_ARG;
+    if (ms_forward) *ms_forward = h->prof_ms_fwd;
+    if (n_forward) *n_forward = h->prof_n_fwd;
+    if (ms_back) *ms_back = h->prof_ms_back;
+    if (n_back) *n_back = h->prof_n_back;
+    return OSIV_OK;
+}
 
 int osiv_forward(osiv_handle* h, const float* d_img, float* d_sino, int32_t batch, int32_t subset,
                  int32_t n_subsets, void* cuda_stream) {
@@ -371,17 +394,38 @@ int osiv_reconstruct(osiv_handle* h, const float* d_counts, const float* d_blank
 
     float *cur = h->d_imgA, *curT = h->d_imgTA, *nxt = h->d_imgB, *nxtT = h->d_imgTB;
     const dim3 bg = back_grid(h, batch);
+    const bool prof = h->profiling && N > 0;
+    if (prof) {
+        while (h->events.size() < (size_t)2 * N + 1) {
+            cudaEvent_t e;
+            OSIV_CUDA(cudaEventCreate(&e));
+            h->events.push_back(e);
+        }
+        OSIV_CUDA(cudaEventRecord(h->events[0], st));
+    }
     for (int n = 0; n < N; ++n) {
         const int m = n % M;                               // PAPER.md:118, C11
         f.img = cur; f.imgT = curT; f.subset = m; f.monitor_only = 0;
         k_forward<1><<<fg, FWD_THREADS, 0, st>>>(f);
+        if (prof) cudaEventRecord(h->events[2 * n + 1], st);
         b.img = cur; b.img_new = nxt; b.imgT_new = nxtT; b.subset = m;
         k_back<1><<<bg, BK_THREADS, 0, st>>>(b);
+        if (prof) cudaEventRecord(h->events[2 * n + 2], st);
         float* t;
         t = cur; cur = nxt; nxt = t;
         t = curT; curT = nxtT; nxtT = t;
     }
     h->launches += 2 * (int64_t)N;
+    if (prof) {
+        OSIV_CUDA(cudaStreamSynchronize(st));
+        for (int n = 0; n < N; ++n) {
+            float a = 0.f, c = 0.f;
+            OSIV_CUDA(cudaEventElapsedTime(&a, h->events[2 * n], h->events[2 * n + 1]));
+            OSIV_CUDA(cudaEventElapsedTime(&c, h->events[2 * n + 1], h->events[2 * n + 2]));
+            h->prof_ms_fwd += a; h->prof_ms_back += c;
+        }
+        h->prof_n_fwd += N; h->prof_n_back += N;
+    }
     if (prm->return_best) {
         // the final iterate competes too, judged on the subset that would come next (C12)
         f.img = cur; f.imgT = curT; f.subset = N % M; f.monitor_only = 1;
