@@ -110,9 +110,20 @@ int osiv_get_tau(const osiv_handle* h, int32_t n_subsets, double kappa, double* 
 /* Number of CUDA kernels this handle has launched since osiv_create (for launch accounting). */
 int64_t osiv_launch_count(const osiv_handle* h);
 
+/* Quarter-turn symmetry.  When the grid is square with nx % 4 == 0, n_views % 4 == 0 and a subset holds whole
+ * orbits {v, v+V/4, v+V/2, v+3V/4} (V_S % 4 == 0), the kernels evaluate each chord weight once for the four
+ * rotated (ray, pixel) pairs.  It is on by default wherever it applies; enable = 0 forces
+ * the general kernels (used by the tests to compare the two paths).  Results differ only by rounding. */
+int osiv_set_symmetry(osiv_handle* h, int32_t enable);
+
+/* Launch plan osiv_reconstruct would use for `n_subsets` subsets (<= 0: all views) and `batch` slices:
+ * out8 = {K1 orbit size (1 or 4), K1 blocks per ray group, K1 blocks, K1 threads per block,
+ *         K2 orbit size, K2 warps per block, K2 blocks, K2 threads per block}.  Host only. */
+int osiv_get_plan(const osiv_handle* h, int32_t n_subsets, int32_t batch, int32_t* out8);
+
 /* Per-kernel device timing for the roofline report.  While enabled (enable != 0), osiv_reconstruct records a
- * CUDA event on cuda_stream before and after every K1 (forward + residual + monitor + step rule) and K2
- * (backprojection + TV + update) launch and synchronises the stream at the end of the call to accumulate the
+ * CUDA event on cuda_stream before and after every K1 (forward + residual + monitor partials) and K2
+ * (step rule + backprojection + TV + update) launch and synchronises the stream at the end of the call to accumulate the
  * elapsed times; use it on extra steps, not on the steps whose throughput is reported.
  * osiv_get_profile returns the sums since the last osiv_set_profiling call: milliseconds and launch counts. */
 int osiv_set_profiling(osiv_handle* h, int32_t enable);

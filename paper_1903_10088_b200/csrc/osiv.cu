@@ -5,6 +5,7 @@
 #include "../../include/osiv.h"
 #include "osiv_kernels.cuh"
 
+#include <algorithm>
 #include <cmath>
 #include <cstdlib>
 #include <cstring>
@@ -25,10 +26,15 @@ struct osiv_handle {
     int ws_batch = 0;
     float *d_imgA = nullptr, *d_imgB = nullptr, *d_imgTA = nullptr, *d_imgTB = nullptr;
     float* d_best = nullptr;
-    size_t rec_elems = 0;       float4* d_rec = nullptr;
-    size_t partial_elems = 0;   double* d_partials = nullptr;
-    SliceState* d_state = nullptr;
+    size_t res_elems = 0;       float* d_res = nullptr;
+    size_t fpart_elems = 0;     float* d_fpart = nullptr;
+    size_t ticket_elems = 0;    unsigned int* d_tickets = nullptr;
+    size_t dpart_elems = 0;     double* d_dparts = nullptr;
+    SliceState* d_state = nullptr;      // [2][max_batch], ping-pong between iterations
+    int* d_not_finite = nullptr;        // [max_batch]
     float* d_inv_bref = nullptr;
+    int num_sms = 148;
+    int occ_fwd[2][2] = {{0, 0}, {0, 0}};   // resident K1 blocks per SM, [MODE][NS == 4]
     size_t trace_elems = 0;     double* d_trace = nullptr;
     size_t forced_elems = 0;    double* d_forced = nullptr;
     // staging for osiv_reconstruct_host
@@ -36,6 +42,7 @@ struct osiv_handle {
     float* d_hblank = nullptr;
     size_t hi_elems = 0;        float* d_himg = nullptr;
     int64_t launches = 0;
+    int force_ns1 = 0;                  // osiv_set_symmetry(h, 0): always take the general path
     // per-kernel event timing (osiv_set_profiling)
     bool profiling = false;
     std::vector<cudaEvent_t> events;
@@ -75,14 +82,25 @@ double resolve_dgamma(const osiv_geometry& g) {
 // A0: per-ray coefficients {alpha, beta, g0, h} in float64, stored float32 (header of osiv_kernels.cuh).
 // Ray (v,c): direction d = -(cos phi, sin phi), phi = th_v + ga_c; signed distance of the point
 // D*(xc,yc) from it: p = D*(xc*dy - yc*dx) + SAD*sin(ga_c).
+// With V % 4 == 0 the views of the second to fourth quarter turn are written as the exact rotations
+// (alpha,beta,g0,h) -> (-beta,alpha,g0,h) of the first quarter's (the same numbers up to the last bit of the
+// float64 cosines), which is what lets both kernels share one weight across a quarter-turn orbit.
 void build_tables(const osiv_geometry& g, double dgamma, std::vector<float4>& rays, std::vector<float2>& views) {
     const int V = g.n_views, C = g.n_channels;
     const double D = g.pixel_mm, tiny = 1e-9;
     rays.resize((size_t)V * C);
     views.resize(V);
+    const int Vq = (V % 4 == 0) ? V / 4 : V;
     for (int v = 0; v < V; ++v) {
         const double th = g.theta0_rad + 2.0 * M_PI * (double)v / (double)V;
         views[v] = make_float2((float)std::cos(th), (float)std::sin(th));
+        if (v >= Vq) {
+            for (int c = 0; c < C; ++c) {
+                const float4 q = rays[(size_t)(v - Vq) * C + c];
+                rays[(size_t)v * C + c] = make_float4(-q.y, q.x, q.z, q.w);
+            }
+            continue;
+        }
         for (int c = 0; c < C; ++c) {
             const double ga = ((double)c - 0.5 * (C - 1) + g.channel_offset) * dgamma;
             double dx = -std::cos(th + ga), dy = -std::sin(th + ga);
@@ -137,10 +155,70 @@ int ensure_images(osiv_handle* h, int batch, cudaStream_t st) {
     return OSIV_OK;
 }
 
-dim3 fwd_grid(const osiv_handle* h, int VS, int batch) { return dim3((h->geom.n_channels + 31) / 32, VS, batch); }
-dim3 back_grid(const osiv_handle* h, int batch) {
-    return dim3((h->geom.nx + BK_BLOCK_PX_X - 1) / BK_BLOCK_PX_X, (h->geom.ny + BK_BLOCK_PX_Y - 1) / BK_BLOCK_PX_Y, batch);
+// ---- launch plans -------------------------------------------------------------------------------------
+// NS = 4 (quarter-turn orbits share one weight) needs a square grid with nx % 4 == 0, V % 4 == 0 and a subset
+// made of whole orbits (V_S % 4 == 0); everything else takes the general NS = 1 kernels.
+int pick_ns(const osiv_handle* h, int VS) { return (h->dg.sym4 && !h->force_ns1 && VS % 4 == 0) ? 4 : 1; }
+
+struct FwdPlan { dim3 grid; int nsplit, groups, ns; };
+struct BackPlan { dim3 grid; int nsplit, ns; };
+
+// K1: one block per (32 channels, base view, share of the line segments); the shares are sized so that the
+// whole grid is resident in one wave.
+FwdPlan plan_forward(const osiv_handle* h, int mode, int VS, int batch) {
+    FwdPlan p;
+    p.ns = pick_ns(h, VS);
+    const int cg = (h->geom.n_channels + 31) / 32, vb = VS / p.ns;
+    p.groups = cg * vb;
+    const long long slots = (long long)h->num_sms * std::max(1, h->occ_fwd[mode][p.ns == 4]);
+    long long ns = slots / ((long long)p.groups * batch);
+    const int nmax = std::max(h->geom.nx, h->geom.ny);
+    ns = std::min<long long>(ns, std::max(1, nmax / (FWD_SEGS * 4)));      // keep >= 4 image lines per warp
+    p.nsplit = (int)std::max<long long>(1, std::min<long long>(ns, FWD_MAX_SPLIT));
+    p.grid = dim3(cg, vb * p.nsplit, batch);
+    return p;
 }
+
+// K2: one block per 16 x 8 pixel region of base tiles; its warps share the subset's views.
+BackPlan plan_back(const osiv_handle* h, int VS, int batch) {
+    BackPlan p;
+    p.ns = pick_ns(h, VS);
+    const int tx = p.ns == 4 ? h->geom.nx / 4 : (h->geom.nx + BK_TX - 1) / BK_TX;
+    const int ty = p.ns == 4 ? h->geom.ny / 4 : (h->geom.ny + BK_TY - 1) / BK_TY;
+    p.grid = dim3((tx + BK_WX - 1) / BK_WX, (ty + BK_WY - 1) / BK_WY, batch);
+    const long long blocks = (long long)p.grid.x * p.grid.y * batch;
+    long long want = ((long long)h->num_sms * 40 + blocks - 1) / blocks;      // about 40 resident warps per SM
+    want = std::max<long long>(1, std::min<long long>(want, std::min(BK_MAX_SPLIT, VS)));
+    int best = (int)want;
+    for (int d = (int)want; d >= 1; --d) if (VS % d == 0) { if (2 * d > want) best = d; break; }
+    p.nsplit = best;
+    return p;
+}
+
+template <int MODE>
+void launch_forward(const FwdPlan& p, const FwdArgs& a, cudaStream_t st) {
+    if (p.ns == 4) k_forward<MODE, 4><<<p.grid, FWD_THREADS, 0, st>>>(a);
+    else           k_forward<MODE, 1><<<p.grid, FWD_THREADS, 0, st>>>(a);
+}
+
+template <int MODE>
+void launch_back(const BackPlan& p, const BackArgs& a, cudaStream_t st) {
+    if (p.ns == 4) k_back<MODE, 4><<<p.grid, 32 * p.nsplit, 0, st>>>(a);
+    else           k_back<MODE, 1><<<p.grid, 32 * p.nsplit, 0, st>>>(a);
+}
+
+int ensure_forward_ws(osiv_handle* h, const FwdPlan& p, int batch, cudaStream_t st) {
+    int rc;
+    if (p.nsplit > 1 &&
+        (rc = grow(&h->d_fpart, &h->fpart_elems, (size_t)batch * p.groups * p.nsplit * p.ns * 32)) != OSIV_OK) return rc;
+    const size_t nt = (size_t)batch * p.groups;
+    if (h->ticket_elems < nt || !h->d_tickets) {
+        if ((rc = grow(&h->d_tickets, &h->ticket_elems, nt)) != OSIV_OK) return rc;
+        OSIV_CUDA(cudaMemsetAsync(h->d_tickets, 0, h->ticket_elems * sizeof(unsigned int), st));
+    }
+    return grow(&h->d_dparts, &h->dpart_elems, nt);
+}
+
 dim3 px_grid(const osiv_handle* h, int batch) { return dim3((h->geom.nx + 31) / 32, (h->geom.ny + 7) / 8, batch); }
 
 int launch_check(osiv_handle* h, int n) {
@@ -153,7 +231,7 @@ int launch_check(osiv_handle* h, int n) {
 
 extern "C" {
 
-int osiv_version(void) { return 100; }
+int osiv_version(void) { return 200; }
 
 const char* osiv_strerror(int status) {
     switch (status) {
@@ -220,10 +298,16 @@ int osiv_create(const osiv_geometry* geom, int32_t max_batch, int32_t device, os
     build_tables(g, dgamma, rays, views);
     if (cudaMalloc((void**)&h->d_rays, rays.size() * sizeof(float4)) != cudaSuccess ||
         cudaMalloc((void**)&h->d_views, views.size() * sizeof(float2)) != cudaSuccess ||
-        cudaMalloc((void**)&h->d_state, (size_t)max_batch * sizeof(SliceState)) != cudaSuccess ||
+        cudaMalloc((void**)&h->d_state, (size_t)2 * max_batch * sizeof(SliceState)) != cudaSuccess ||
+        cudaMalloc((void**)&h->d_not_finite, (size_t)max_batch * sizeof(int)) != cudaSuccess ||
         cudaMalloc((void**)&h->d_inv_bref, sizeof(float)) != cudaSuccess ||
         cudaMemcpy(h->d_rays, rays.data(), rays.size() * sizeof(float4), cudaMemcpyHostToDevice) != cudaSuccess ||
-        cudaMemcpy(h->d_views, views.data(), views.size() * sizeof(float2), cudaMemcpyHostToDevice) != cudaSuccess) {
+        cudaMemcpy(h->d_views, views.data(), views.size() * sizeof(float2), cudaMemcpyHostToDevice) != cudaSuccess ||
+        cudaDeviceGetAttribute(&h->num_sms, cudaDevAttrMultiProcessorCount, device) != cudaSuccess ||
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&h->occ_fwd[0][0], k_forward<0, 1>, FWD_THREADS, 0) != cudaSuccess ||
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&h->occ_fwd[0][1], k_forward<0, 4>, FWD_THREADS, 0) != cudaSuccess ||
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&h->occ_fwd[1][0], k_forward<1, 1>, FWD_THREADS, 0) != cudaSuccess ||
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&h->occ_fwd[1][1], k_forward<1, 4>, FWD_THREADS, 0) != cudaSuccess) {
         cudaGetLastError();
         osiv_destroy(h);
         return OSIV_ERR_CUDA;
@@ -238,12 +322,15 @@ int osiv_create(const osiv_geometry* geom, int32_t max_batch, int32_t device, os
     d.pixel = (float)g.pixel_mm; d.sad = (float)g.sad_mm;
     d.inv_dgamma = (float)(1.0 / dgamma);
     d.c_center = (float)(0.5 * (g.n_channels - 1) - g.channel_offset);
-    d.hw_scale = (float)(g.pixel_mm / dgamma);
-    // short odd series for atan: error < z^9/9; demand < 0.01 channel, else fall back to atanf
+    // K2 candidate bound: every ray through a tile passes within its half-diagonal r of the tile centre, so its fan
+    // angle is within asin(r/L) <= f*r/along of the centre's, f = asin(x)/x at the largest possible x = r/(SAD-r_max)
+    const double tile_r = 0.5 * g.pixel_mm * std::sqrt((double)(BK_TX * BK_TX + BK_TY * BK_TY));
+    const double xm = std::min(tile_r / (g.sad_mm - rmax), 1.0);
+    d.tile_hw = (float)(std::asin(xm) / xm * tile_r / dgamma * 1.0005);
+    // atan_small: |z| <= 0.75, error 3e-7 rad; demand < 0.01 channel, else atanf
     const double zmax = rmax / (g.sad_mm - rmax);
-    d.use_atanf = (std::pow(zmax, 9) / 9.0 / dgamma > 0.01) ? 1 : 0;
-    d.tile_r = (float)(0.5 * g.pixel_mm * std::sqrt((double)(BK_TX * BK_TX + BK_TY * BK_TY)));
-    d.wide = (d.tile_r / (g.sad_mm - rmax) > 0.015 || d.use_atanf) ? 1 : 0;
+    d.use_atanf = (zmax > 0.75 || 3e-7 / dgamma > 0.01) ? 1 : 0;
+    d.sym4 = (g.nx == g.ny && g.nx % 4 == 0 && g.n_views % 4 == 0) ? 1 : 0;
     d.rays = h->d_rays; d.views = h->d_views;
     *out = h;
     return OSIV_OK;
@@ -254,9 +341,9 @@ int osiv_destroy(osiv_handle* h) {
     DeviceGuard guard(h->device);
     if (guard.ok) {
         cudaDeviceSynchronize();
-        void* ptrs[] = {h->d_rays, h->d_views, h->d_imgA, h->d_imgB, h->d_imgTA, h->d_imgTB, h->d_best, h->d_rec,
-                        h->d_partials, h->d_state, h->d_inv_bref, h->d_trace, h->d_forced, h->d_hcounts, h->d_hblank,
-                        h->d_himg};
+        void* ptrs[] = {h->d_rays, h->d_views, h->d_imgA, h->d_imgB, h->d_imgTA, h->d_imgTB, h->d_best, h->d_res,
+                        h->d_fpart, h->d_tickets, h->d_dparts, h->d_state, h->d_not_finite, h->d_inv_bref, h->d_trace,
+                        h->d_forced, h->d_hcounts, h->d_hblank, h->d_himg};
         for (void* p : ptrs) if (p) cudaFree(p);
         for (cudaEvent_t e : h->events) cudaEventDestroy(e);
         cudaGetLastError();
@@ -281,6 +368,22 @@ int osiv_get_tau(const osiv_handle* h, int32_t n_subsets, double kappa, double* 
 }
 
 int64_t osiv_launch_count(const osiv_handle* h) { return h ? h->launches : 0; }
+
+int osiv_set_symmetry(osiv_handle* h, int32_t enable) {
+    if (!h) return OSIV_ERR_INVALID_ARG;
+    h->force_ns1 = enable ? 0 : 1;
+    return OSIV_OK;
+}
+
+int osiv_get_plan(const osiv_handle* h, int32_t n_subsets, int32_t batch, int32_t* out8) {
+    if (!h || !out8 || batch <= 0 || (n_subsets > 0 && h->geom.n_views % n_subsets != 0)) return OSIV_ERR_INVALID_ARG;
+    const int VS = n_subsets > 0 ? h->geom.n_views / n_subsets : h->geom.n_views;
+    const FwdPlan f = plan_forward(h, 1, VS, batch);
+    const BackPlan b = plan_back(h, VS, batch);
+    out8[0] = f.ns; out8[1] = f.nsplit; out8[2] = (int)(f.grid.x * f.grid.y * f.grid.z); out8[3] = FWD_THREADS;
+    out8[4] = b.ns; out8[5] = b.nsplit; out8[6] = (int)(b.grid.x * b.grid.y * b.grid.z); out8[7] = 32 * b.nsplit;
+    return OSIV_OK;
+}
 
 int osiv_set_profiling(osiv_handle* h, int32_t enable) {
     if (!h) return OSIV_ERR_INVALID_ARG;
@@ -309,12 +412,15 @@ int osiv_forward(osiv_handle* h, const float* d_img, float* d_sino, int32_t batc
     int rc = ensure_images(h, batch, st);
     if (rc != OSIV_OK) return rc;
     const int VS = subset_views(h, subset, n_subsets);
+    const FwdPlan p = plan_forward(h, 0, VS, batch);
+    if ((rc = ensure_forward_ws(h, p, batch, st)) != OSIV_OK) return rc;
     k_pad_transpose<<<dim3((h->geom.nx + 31) / 32, (h->geom.ny + 31) / 32, batch), 256, 0, st>>>(h->dg, d_img, h->d_imgA,
                                                                                              h->d_imgTA);
     FwdArgs a{};
     a.g = h->dg; a.img = h->d_imgA; a.imgT = h->d_imgTA;
-    a.subset = subset; a.M = subset < 0 ? 1 : n_subsets; a.VS = VS; a.sino = d_sino;
-    k_forward<0><<<fwd_grid(h, VS, batch), FWD_THREADS, 0, st>>>(a);
+    a.subset = subset; a.M = subset < 0 ? 1 : n_subsets; a.VS = VS; a.nsplit = p.nsplit; a.sino = d_sino;
+    a.fpart = h->d_fpart; a.tickets = h->d_tickets;
+    launch_forward<0>(p, a, st);
     return launch_check(h, 2);
 }
 
@@ -326,12 +432,13 @@ int osiv_backward(osiv_handle* h, const float* d_sino, float* d_img, int32_t bat
     if (!guard.ok) { cudaGetLastError(); return OSIV_ERR_CUDA; }
     cudaStream_t st = (cudaStream_t)cuda_stream;
     const int VS = subset_views(h, subset, n_subsets), M = subset < 0 ? 1 : n_subsets;
-    int rc = grow(&h->d_rec, &h->rec_elems, (size_t)batch * VS * h->geom.n_channels);
+    int rc = grow(&h->d_res, &h->res_elems, (size_t)batch * VS * h->geom.n_channels);
     if (rc != OSIV_OK) return rc;
-    k_make_rec<<<dim3((h->geom.n_channels + 255) / 256, VS, batch), 256, 0, st>>>(h->dg, d_sino, h->d_rec, subset, M, VS);
+    k_scale_sino<<<dim3((h->geom.n_channels + 255) / 256, VS, batch), 256, 0, st>>>(h->dg, d_sino, h->d_res, subset, M, VS);
+    const BackPlan p = plan_back(h, VS, batch);
     BackArgs b{};
-    b.g = h->dg; b.rec = h->d_rec; b.subset = subset; b.M = M; b.VS = VS; b.out = d_img;
-    k_back<0><<<back_grid(h, batch), BK_THREADS, 0, st>>>(b);
+    b.g = h->dg; b.res = h->d_res; b.subset = subset; b.M = M; b.VS = VS; b.out = d_img;
+    launch_back<0>(p, b, st);
     return launch_check(h, 2);
 }
 
@@ -345,7 +452,8 @@ int osiv_tv_gradient(osiv_handle* h, const float* d_img, float* d_grad, int32_t 
     if (rc != OSIV_OK) return rc;
     k_pad_transpose<<<dim3((h->geom.nx + 31) / 32, (h->geom.ny + 31) / 32, batch), 256, 0, st>>>(h->dg, d_img, h->d_imgA,
                                                                                              h->d_imgTA);
-    k_tv<<<back_grid(h, batch), BK_THREADS, 0, st>>>(h->dg, h->d_imgA, (float)(tv_eps * tv_eps), d_grad);
+    k_tv<<<dim3((h->geom.nx + 31) / 32, (h->geom.ny + 15) / 16, batch), 128, 0, st>>>(h->dg, h->d_imgA,
+                                                                                     (float)(tv_eps * tv_eps), d_grad);
     return launch_check(h, 2);
 }
 
@@ -364,9 +472,10 @@ int osiv_reconstruct(osiv_handle* h, const float* d_counts, const float* d_blank
     const int VS = h->geom.n_views / M, C = h->geom.n_channels;
     int rc = ensure_images(h, batch, st);
     if (rc != OSIV_OK) return rc;
-    if ((rc = grow(&h->d_rec, &h->rec_elems, (size_t)batch * VS * C)) != OSIV_OK) return rc;
-    const dim3 fg = fwd_grid(h, VS, batch);
-    if ((rc = grow(&h->d_partials, &h->partial_elems, (size_t)batch * fg.x * fg.y)) != OSIV_OK) return rc;
+    if ((rc = grow(&h->d_res, &h->res_elems, (size_t)batch * VS * C)) != OSIV_OK) return rc;
+    const FwdPlan fp = plan_forward(h, 1, VS, batch);
+    const BackPlan bp = plan_back(h, VS, batch);
+    if ((rc = ensure_forward_ws(h, fp, batch, st)) != OSIV_OK) return rc;
     if (h_trace && N > 0 && (rc = grow(&h->d_trace, &h->trace_elems, (size_t)batch * N * 2)) != OSIV_OK) return rc;
     if (prm->forced_lambda && N > 0) {
         if ((rc = grow(&h->d_forced, &h->forced_elems, (size_t)N)) != OSIV_OK) return rc;
@@ -376,24 +485,25 @@ int osiv_reconstruct(osiv_handle* h, const float* d_counts, const float* d_blank
     osiv_get_tau(h, M, prm->kappa, &tau);
 
     float* best = prm->return_best ? h->d_best : nullptr;
-    k_init_state<<<1, 32, 0, st>>>(h->d_state, batch, prm->lambda0, d_blank, blank_scalar, C, h->d_inv_bref);
+    SliceState* state[2] = {h->d_state, h->d_state + h->max_batch};
+    k_init_state<<<1, 32, 0, st>>>(state[0], h->d_not_finite, batch, prm->lambda0, d_blank, blank_scalar, C, h->d_inv_bref);
     k_fill<<<px_grid(h, batch), 256, 0, st>>>(h->dg, (float)prm->mu0, h->d_imgA, h->d_imgTA, best);
     h->launches += 2;
 
     FwdArgs f{};
-    f.g = h->dg; f.M = M; f.VS = VS;
+    f.g = h->dg; f.M = M; f.VS = VS; f.nsplit = fp.nsplit;
     f.counts = d_counts; f.blank = d_blank; f.blank_scalar = blank_scalar; f.inv_bref = h->d_inv_bref;
-    f.rec = h->d_rec; f.partials = h->d_partials; f.state = h->d_state;
-    f.ip.lambda0 = prm->lambda0; f.ip.up = prm->lambda_up; f.ip.down = prm->lambda_down; f.ip.lmin = prm->lambda_min;
-    f.ip.forced = (prm->forced_lambda && N > 0) ? h->d_forced : nullptr;
-    f.ip.trace = (h_trace && N > 0) ? h->d_trace : nullptr;
-    f.ip.n_iters = N; f.ip.return_best = prm->return_best;
+    f.res = h->d_res; f.fpart = h->d_fpart; f.tickets = h->d_tickets; f.dparts = h->d_dparts;
     BackArgs b{};
-    b.g = h->dg; b.rec = h->d_rec; b.M = M; b.VS = VS; b.best = best; b.state = h->d_state;
+    b.g = h->dg; b.res = h->d_res; b.M = M; b.VS = VS; b.best = best;
+    b.dparts = h->d_dparts; b.nparts = fp.groups; b.not_finite = h->d_not_finite;
+    b.ip.lambda0 = prm->lambda0; b.ip.up = prm->lambda_up; b.ip.down = prm->lambda_down; b.ip.lmin = prm->lambda_min;
+    b.ip.forced = (prm->forced_lambda && N > 0) ? h->d_forced : nullptr;
+    b.ip.trace = (h_trace && N > 0) ? h->d_trace : nullptr;
+    b.ip.n_iters = N; b.ip.return_best = prm->return_best;
     b.tau = tau; b.beta_over_M = (float)(prm->beta / M); b.eps2 = (float)(prm->tv_eps * prm->tv_eps);
 
     float *cur = h->d_imgA, *curT = h->d_imgTA, *nxt = h->d_imgB, *nxtT = h->d_imgTB;
-    const dim3 bg = back_grid(h, batch);
     const bool prof = h->profiling && N > 0;
     if (prof) {
         while (h->events.size() < (size_t)2 * N + 1) {
@@ -405,11 +515,12 @@ int osiv_reconstruct(osiv_handle* h, const float* d_counts, const float* d_blank
     }
     for (int n = 0; n < N; ++n) {
         const int m = n % M;                               // PAPER.md:118, C11
-        f.img = cur; f.imgT = curT; f.subset = m; f.monitor_only = 0;
-        k_forward<1><<<fg, FWD_THREADS, 0, st>>>(f);
+        f.img = cur; f.imgT = curT; f.subset = m;
+        launch_forward<1>(fp, f, st);
         if (prof) cudaEventRecord(h->events[2 * n + 1], st);
         b.img = cur; b.img_new = nxt; b.imgT_new = nxtT; b.subset = m;
-        k_back<1><<<bg, BK_THREADS, 0, st>>>(b);
+        b.state_in = state[n & 1]; b.state_out = state[(n + 1) & 1];
+        launch_back<1>(bp, b, st);
         if (prof) cudaEventRecord(h->events[2 * n + 2], st);
         float* t;
         t = cur; cur = nxt; nxt = t;
@@ -426,23 +537,25 @@ int osiv_reconstruct(osiv_handle* h, const float* d_counts, const float* d_blank
         }
         h->prof_n_fwd += N; h->prof_n_back += N;
     }
+    SliceState* fin = state[N & 1];
     if (prm->return_best) {
         // the final iterate competes too, judged on the subset that would come next (C12)
-        f.img = cur; f.imgT = curT; f.subset = N % M; f.monitor_only = 1;
-        k_forward<1><<<fg, FWD_THREADS, 0, st>>>(f);
-        h->launches += 1;
+        f.img = cur; f.imgT = curT; f.subset = N % M;
+        launch_forward<1>(fp, f, st);
+        k_final_monitor<<<batch, 32, 0, st>>>(h->d_dparts, fp.groups, fin, h->d_not_finite);
+        h->launches += 2;
     }
-    k_unpad<<<px_grid(h, batch), 256, 0, st>>>(h->dg, cur, best, h->d_state, d_img_out);
+    k_unpad<<<px_grid(h, batch), 256, 0, st>>>(h->dg, cur, best, fin, d_img_out);
     rc = launch_check(h, 1);
     if (rc != OSIV_OK) return rc;
 
     if (h_trace) {
-        std::vector<SliceState> hs(batch);
+        std::vector<int> nf(batch);
         if (N > 0)
             OSIV_CUDA(cudaMemcpyAsync(h_trace, h->d_trace, (size_t)batch * N * 2 * sizeof(double), cudaMemcpyDeviceToHost, st));
-        OSIV_CUDA(cudaMemcpyAsync(hs.data(), h->d_state, (size_t)batch * sizeof(SliceState), cudaMemcpyDeviceToHost, st));
+        OSIV_CUDA(cudaMemcpyAsync(nf.data(), h->d_not_finite, (size_t)batch * sizeof(int), cudaMemcpyDeviceToHost, st));
         OSIV_CUDA(cudaStreamSynchronize(st));
-        for (int s = 0; s < batch; ++s) if (hs[s].not_finite) return OSIV_ERR_NOT_FINITE;
+        for (int s = 0; s < batch; ++s) if (nf[s]) return OSIV_ERR_NOT_FINITE;
     }
     return OSIV_OK;
 }

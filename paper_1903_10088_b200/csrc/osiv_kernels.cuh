@@ -1,10 +1,11 @@
 // osiv_kernels.cuh -- sm_100a device code of libosiv (see include/osiv.h).
 //
 // Hot path of arxiv 1903.10088: per ordered-subset iteration
-//   K1  k_forward<1>  ray-driven reprojection l = A_S mu, fused Poisson residual, monitor D (fp64,
-//                     fixed-order reduction) and the adaptive-step rule Eq. 4-5 in the last block
-//   K2  k_back<1>     matched atomic-free gather backprojection g = A_S^T r, fused TV gradient,
-//                     Eq. 3 update, mu > 0 clamp, best-image copy; double-buffered image
+//   K1  k_forward<1,NS>  ray-driven reprojection l = A_S mu, fused Poisson residual and the per-ray-group
+//                        fp64 partial sums of the monitor D
+//   K2  k_back<1,NS>     monitor D (fixed-order sum of the partials) and the adaptive-step rule Eq. 4-5,
+//                        matched atomic-free gather backprojection g = A_S^T r, fused TV gradient,
+//                        Eq. 3 update, mu > 0 clamp, best-image copy; double-buffered image
 //
 // System matrix (reading C2): a(i,r) = length of the zero-width ray i inside square pixel r.  With
 // p the signed distance of the pixel centre from the ray, the chord is the trapezoid
@@ -12,9 +13,19 @@
 // p is affine in the centred pixel indices (xc, yc), so after dividing by (hi-lo) every ray carries
 // four floats {alpha, beta, g0, h} with
 //   a(i; xc,yc) = h * sat( (|alpha|+|beta|)/2 - |alpha*xc + beta*yc + g0| ),
-// one of alpha,beta being exactly +1 and the other |k| >= 1.  Forward and back evaluate this same
+// one of alpha,beta being exactly +-1 and the other |k| >= 1.  Forward and back evaluate this same
 // expression, so the pair is matched by construction.  Nothing here is a dense contraction: no
 // tensor cores; the work is FP32 FMA/ALU issue plus L1/L2 gathers.
+//
+// Quarter-turn symmetry (NS = 4).  When the grid is square with nx % 4 == 0, V % 4 == 0 and the subset
+// holds whole orbits {v, v+V/4, v+V/2, v+3V/4}, the scan is invariant under the rotation
+// R: (xc,yc) -> (-yc,xc), i.e. pixel (ix,iy) -> (N-1-iy, ix):  a(v + kV/4, c; R^k P) = a(v, c; P).
+// Every chord weight is then evaluated once and used for the four rotated (ray, pixel) pairs: K1 walks
+// ray (v,c) and gathers mu at P, RP, R^2P, R^3P (row-major and transposed image copies make all four
+// walks contiguous); K2 evaluates a(v,c;T) for its base tile T and feeds the accumulators of T, RT, R^2T,
+// R^3T with the residuals of views v, v+V/4, v+V/2, v+3V/4.  The ray table is built with exactly
+// rotated coefficients (alpha,beta,g0,h) -> (-beta,alpha,g0,h), so both kernels still use one weight per
+// (ray, pixel) pair.  NS = 1 is the general path (any geometry).
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -23,12 +34,13 @@ namespace osiv {
 
 constexpr int PAD = 4;                     // zero columns left and right of every padded image line
 constexpr int PADR = 1;                    // zero rows above and below a padded image
-constexpr int FWD_SEGS = 8;                // a ray is split into this many segments (one warp each)
+constexpr int FWD_SEGS = 8;                // warps per K1 block; each owns one segment of the rays' image lines
 constexpr int FWD_THREADS = 32 * FWD_SEGS;
+constexpr int FWD_MAX_SPLIT = 8;           // K1 blocks that share one ray group (partial sums through global memory)
 constexpr int BK_TX = 2, BK_TY = 2;        // pixels per thread in the backprojector
-constexpr int BK_THREADS = 128;            // 4 warps as 2x2; a warp covers 8x4 tiles = 16x8 pixels
-constexpr int BK_BLOCK_PX_X = 2 * 8 * BK_TX;
-constexpr int BK_BLOCK_PX_Y = 2 * 4 * BK_TY;
+constexpr int BK_WX = 8, BK_WY = 4;        // tiles per warp: a warp covers 16 x 8 pixels
+constexpr int BK_MAX_SPLIT = 8;            // K2 warps per block; each owns a share of the subset's views
+constexpr int BK_MAX_THREADS = 32 * BK_MAX_SPLIT;
 
 struct DevGeom {
     int nx, ny, V, C;
@@ -36,10 +48,9 @@ struct DevGeom {
     long long img_elems, imgT_elems;       // padded floats per slice
     float cx, cy;                          // (nx-1)/2, (ny-1)/2
     float pixel, sad, inv_dgamma, c_center;   // c_center = (C-1)/2 - channel_offset
-    float hw_scale;                        // pixel / dgamma
-    int use_atanf;                         // fan too wide for the short atan series
-    int wide;                              // tiles subtend a large angle: use the enclosing-circle candidate bound
-    float tile_r;                          // half-diagonal of a backprojector tile [mm]
+    float tile_hw;                         // angular half-width of a K2 tile at unit distance, in channels (with asin slack)
+    int use_atanf;                         // fan too wide for the short atan polynomial
+    int sym4;                              // geometry admits the quarter-turn path (square grid, nx%4==0, V%4==0)
     const float4* rays;                    // [V][C] {alpha, beta, g0, h}
     const float2* views;                   // [V] {cos th_v, sin th_v}
 };
@@ -48,8 +59,7 @@ struct SliceState {
     double lambda, D_prev, D_best, D_last;
     int n;                                 // subset updates done = next trace row
     int improved;                          // last monitor value beat D_best (return_best)
-    int not_finite;
-    unsigned int ticket;
+    int pad0, pad1;
 };
 
 struct IterParams {
@@ -65,28 +75,33 @@ struct FwdArgs {
     const float* img;                      // padded mu, slice stride g.img_elems
     const float* imgT;                     // padded transpose, slice stride g.imgT_elems
     int subset, M, VS;
+    int nsplit;                            // blocks per ray group (segments of the rays' lines)
     float* sino;                           // MODE 0: [batch][VS][C]
     const float* counts;                   // MODE 1: [batch][V][C]
     const float* blank;                    // [C] or null
     float blank_scalar;
     const float* inv_bref;                 // device scalar 1/b_ref
-    float4* rec;                           // [batch][VS][C] {alpha, beta, g0, h*r}
-    double* partials;                      // [batch][blocks per slice]
-    SliceState* state;                     // [batch]
-    IterParams ip;
-    int monitor_only;
+    float* res;                            // MODE 1: [batch][VS][C]  h * r
+    float* fpart;                          // [batch][groups][nsplit][NS][32] line-integral partial sums (nsplit > 1)
+    unsigned int* tickets;                 // [batch][groups], zero between launches
+    double* dparts;                        // MODE 1: [batch][groups] partial sums of D
 };
 
 struct BackArgs {
     DevGeom g;
-    const float4* rec;                     // [batch][VS][C]
+    const float* res;                      // [batch][VS][C]  h * (residual or sinogram)
     int subset, M, VS;
     float* out;                            // MODE 0: [batch][ny][nx]
     const float* img;                      // MODE 1: padded mu(n)
     float* img_new;                        // padded mu(n+1)
     float* imgT_new;
     float* best;                           // [batch][ny][nx] or null
-    const SliceState* state;
+    const double* dparts;                  // [batch][nparts]
+    int nparts;
+    const SliceState* state_in;            // [batch] state after iteration n-1
+    SliceState* state_out;                 // [batch] state after iteration n
+    int* not_finite;                       // [batch] sticky flags
+    IterParams ip;
     double tau;
     float beta_over_M, eps2;
 };
@@ -99,28 +114,35 @@ __device__ __forceinline__ size_t padT_off(const DevGeom& g, int ix, int iy) {
 }
 
 // ------------------------------------------------------------------------------------------------
-// K1: forward projection (+ residual, monitor, step rule when MODE == 1).
-// grid (ceil(C/32), V_S, batch), block 32 x FWD_SEGS: lane = channel, warp = segment of the ray.
-// A ray marches over the image lines of its major axis (rows of img when |dy| >= |dx|, else rows of
-// the transposed copy imgT) and touches at most two adjacent pixels per line.
+// K1: forward projection (+ residual and monitor partials when MODE == 1).
+// grid (ceil(C/32), base views * nsplit, batch), block 32 x FWD_SEGS: lane = channel, warp = segment of the
+// ray's image lines, blockIdx.y % nsplit = which share of the segments.  A ray marches over the image lines
+// of its major axis (rows of img when |dy| >= |dx|, else rows of the transposed copy imgT) and touches at
+// most two adjacent pixels per line.  With NS == 4 the same two weights also serve the three rotated rays.
 // ------------------------------------------------------------------------------------------------
-template <int MODE>
+template <int MODE, int NS>
 __global__ void __launch_bounds__(FWD_THREADS) k_forward(const FwdArgs a) {
     const DevGeom& g = a.g;
     const int lane = threadIdx.x & 31, seg = threadIdx.x >> 5;
-    const int c = blockIdx.x * 32 + lane, j = blockIdx.y, s = blockIdx.z;
-    const int v = a.subset < 0 ? j : a.subset + j * a.M;
-    __shared__ float part[FWD_SEGS][32];
+    const int c = blockIdx.x * 32 + lane, s = blockIdx.z;
+    const int jb = blockIdx.y / a.nsplit, split = blockIdx.y - jb * a.nsplit;
+    const int v = a.subset < 0 ? jb : a.subset + jb * a.M;          // base view of the orbit
+    __shared__ float part[FWD_SEGS][NS][32];
+    __shared__ unsigned int s_ticket;
 
-    float acc = 0.f;
-    float4 ray = make_float4(0.f, 0.f, 0.f, 0.f);
+    float acc[NS];
+#pragma unroll
+    for (int k = 0; k < NS; ++k) acc[k] = 0.f;
+    float4 ray = make_float4(1.f, 0.f, 0.f, 0.f);
+    bool rowmaj = true;
     if (c < g.C) {
         ray = __ldg(&g.rays[(size_t)v * g.C + c]);
-        const bool rowmaj = fabsf(ray.x) >= fabsf(ray.y);
+        rowmaj = fabsf(ray.x) >= fabsf(ray.y);
         const float kk = rowmaj ? ray.x : ray.y;          // coefficient of the in-line coordinate, |kk| >= 1
         const float uu = rowmaj ? ray.y : ray.x;          // coefficient of the marching coordinate, +-1
-        const float* base = rowmaj ? a.img + (size_t)s * g.img_elems : a.imgT + (size_t)s * g.imgT_elems;
-        const int pitch = rowmaj ? g.pitch : g.pitchT;
+        const float* bufA = rowmaj ? a.img + (size_t)s * g.img_elems : a.imgT + (size_t)s * g.imgT_elems;
+        const float* bufB = rowmaj ? a.imgT + (size_t)s * g.imgT_elems : a.img + (size_t)s * g.img_elems;
+        const int pitch = rowmaj ? g.pitch : g.pitchT;    // NS == 4: square grid, both pitches are equal
         const int na = rowmaj ? g.nx : g.ny, nb = rowmaj ? g.ny : g.nx;
         const float ca = rowmaj ? g.cx : g.cy, cb = rowmaj ? g.cy : g.cx;
         const float invk = 1.0f / kk;
@@ -133,101 +155,159 @@ __global__ void __launch_bounds__(FWD_THREADS) k_forward(const FwdArgs a) {
         const int jlo = (int)flo, jhi = (int)fhi;
         const int nsteps = jhi - jlo + 1;
         if (nsteps > 0) {
-            const int len = (nsteps + FWD_SEGS - 1) / FWD_SEGS;
-            const int j0 = jlo + seg * len;
+            const int nsegt = FWD_SEGS * a.nsplit;
+            const int len = (nsteps + nsegt - 1) / nsegt;
+            const int j0 = jlo + (split * FWD_SEGS + seg) * len;
             const int j1 = min(j0 + len, jhi + 1);
-            const float* line = base + (size_t)(j0 + PADR) * pitch + PAD;
             const int imax = na + PAD - 2;
-#pragma unroll 4
-            for (int jj = j0; jj < j1; ++jj, line += pitch) {
-                const float b = (float)jj - cb;
-                const float bg = fmaf(uu, b, ray.z);
+            int offP = (j0 + PADR) * pitch + PAD;                 // line j, walking up
+            int offM = (nb - 1 - j0 + PADR) * pitch + PAD;        // line nb-1-j, walking down
+            float bf = (float)j0 - cb;
+#pragma unroll 2
+            for (int jj = j0; jj < j1; ++jj, offP += pitch, offM -= pitch, bf += 1.f) {
+                const float bg = fmaf(uu, bf, ray.z);
                 const float fa = floorf(fmaf(-bg, invk, ca));     // index of the pixel left of the crossing
-                const float a0 = fa - ca;
-                const float q0 = fmaf(kk, a0, bg);
+                const float q0 = fmaf(kk, fa - ca, bg);
                 const float q1 = q0 + kk;
                 const float w0 = __saturatef(hk - fabsf(q0));
                 const float w1 = __saturatef(hk - fabsf(q1));
                 const int i0 = min(max((int)fa, -PAD), imax);
-                acc = fmaf(w0, __ldg(line + i0), acc);
-                acc = fmaf(w1, __ldg(line + i0 + 1), acc);
+                const float* p0 = bufA + (offP + i0);
+                acc[0] = fmaf(w0, __ldg(p0), acc[0]);
+                acc[0] = fmaf(w1, __ldg(p0 + 1), acc[0]);
+                if (NS == 4) {
+                    const int ir = na - 2 - i0;                   // mirrored index of pixel i0+1
+                    const float* p1 = bufB + (offM + i0);         // pattern 1: other copy, line nb-1-j, same order
+                    const float* p2 = bufA + (offM + ir);         // pattern 2: same copy, line nb-1-j, mirrored
+                    const float* p3 = bufB + (offP + ir);         // pattern 3: other copy, line j, mirrored
+                    acc[1] = fmaf(w0, __ldg(p1), acc[1]);
+                    acc[1] = fmaf(w1, __ldg(p1 + 1), acc[1]);
+                    acc[2] = fmaf(w1, __ldg(p2), acc[2]);
+                    acc[2] = fmaf(w0, __ldg(p2 + 1), acc[2]);
+                    acc[3] = fmaf(w1, __ldg(p3), acc[3]);
+                    acc[3] = fmaf(w0, __ldg(p3 + 1), acc[3]);
+                }
             }
         }
     }
-    part[seg][lane] = acc;
+#pragma unroll
+    for (int k = 0; k < NS; ++k) part[seg][k][lane] = acc[k];
     __syncthreads();
     if (seg != 0) return;
 
-    float t = 0.f;
+    // sums over this block's segments, fixed order; pattern -> rotation k (patterns 1 and 3 swap for a
+    // column-major base ray: R maps its walk onto the other copy with the mirrored index first)
+    float t[NS];
 #pragma unroll
-    for (int k = 0; k < FWD_SEGS; ++k) t += part[k][lane];    // fixed order
-    const float l = ray.w * t;
-
-    if (MODE == 0) {
-        if (c < g.C) a.sino[((size_t)s * a.VS + j) * g.C + c] = l;
-        return;
-    }
-
-    // ---- A2: Poisson residual r = (b exp(-l) - y)/b_ref and monitor D = sum (l - ln(b/max(y,1)))^2 ----
-    double d2 = 0.0;
-    if (c < g.C) {
-        const float y = __ldg(&a.counts[((size_t)s * g.V + v) * g.C + c]);
-        const float b = a.blank ? __ldg(&a.blank[c]) : a.blank_scalar;
-        const float ybar = b * expf(-l);
-        const float r = (ybar - y) * __ldg(a.inv_bref);
-        if (!a.monitor_only)
-            a.rec[((size_t)s * a.VS + j) * g.C + c] = make_float4(ray.x, ray.y, ray.z, ray.w * r);
-        const float p = logf(b / fmaxf(y, 1.f));
-        const double d = (double)l - (double)p;
-        d2 = d * d;
-    }
+    for (int k = 0; k < NS; ++k) {
+        float x = 0.f;
 #pragma unroll
-    for (int off = 16; off > 0; off >>= 1) d2 += __shfl_down_sync(0xffffffffu, d2, off);
+        for (int q = 0; q < FWD_SEGS; ++q) x += part[q][k][lane];
+        t[k] = x;
+    }
+    if (NS == 4 && !rowmaj) { const float x = t[1]; t[1] = t[3]; t[3] = x; }
 
-    const unsigned nblk = gridDim.x * gridDim.y;
-    const unsigned blk = blockIdx.y * gridDim.x + blockIdx.x;
-    double* partials = a.partials + (size_t)s * nblk;
-    SliceState* st = a.state + s;
-    unsigned ticket = 0;
-    if (lane == 0) {
-        partials[blk] = d2;
+    const int groups = gridDim.x * (gridDim.y / a.nsplit);
+    const int grp = jb * gridDim.x + blockIdx.x;
+    if (a.nsplit > 1) {
+        float* fp = a.fpart + (((size_t)s * groups + grp) * a.nsplit) * (NS * 32);
+#pragma unroll
+        for (int k = 0; k < NS; ++k) __stcg(&fp[(split * NS + k) * 32 + lane], t[k]);
         __threadfence();
-        ticket = atomicAdd(&st->ticket, 1u);
-    }
-    ticket = __shfl_sync(0xffffffffu, ticket, 0);
-    if (ticket != nblk - 1) return;
-
-    // ---- last block of this slice: D in a fixed order, then A3 (Eq. 4-5) ----
-    __threadfence();
-    double D = 0.0;
-    for (unsigned i = lane; i < nblk; i += 32) D += __ldcg(&partials[i]);
+        __syncwarp();
+        if (lane == 0) s_ticket = atomicAdd(&a.tickets[(size_t)s * groups + grp], 1u);
+        __syncwarp();
+        if (s_ticket != (unsigned)(a.nsplit - 1)) return;
+        __threadfence();
+        if (lane == 0) a.tickets[(size_t)s * groups + grp] = 0u;
 #pragma unroll
-    for (int off = 16; off > 0; off >>= 1) D += __shfl_down_sync(0xffffffffu, D, off);
-    if (lane != 0) return;
-    if (!isfinite(D)) st->not_finite = 1;
-    st->D_last = D;
-    if (a.monitor_only) {
-        st->improved = D < st->D_best;
-    } else {
-        const int n = st->n;
-        double lam;
-        if (a.ip.forced)        lam = a.ip.forced[n];
-        else if (n == 0)        lam = a.ip.lambda0;
-        else if (D < st->D_prev) lam = st->lambda + a.ip.up;
-        else                    lam = fmax(st->lambda - a.ip.down, a.ip.lmin);
-        st->lambda = lam;
-        st->D_prev = D;
+        for (int k = 0; k < NS; ++k) {
+            float x = 0.f;
+            for (int q = 0; q < a.nsplit; ++q) x += __ldcg(&fp[(q * NS + k) * 32 + lane]);   // fixed order
+            t[k] = x;
+        }
+    }
+
+    const int VSb = a.VS / NS, Vq = g.V / NS;
+    double d2 = 0.0;
+#pragma unroll
+    for (int k = 0; k < NS; ++k) {
+        const float l = ray.w * t[k];
+        const int jk = jb + k * VSb;                     // compact view index inside the subset
+        const int vk = v + k * Vq;
+        if (c < g.C) {
+            if (MODE == 0) {
+                a.sino[((size_t)s * a.VS + jk) * g.C + c] = l;
+            } else {
+                // A2: Poisson residual r = (b exp(-l) - y)/b_ref and monitor term (l - ln(b/max(y,1)))^2
+                const float y = __ldg(&a.counts[((size_t)s * g.V + vk) * g.C + c]);
+                const float b = a.blank ? __ldg(&a.blank[c]) : a.blank_scalar;
+                const float ybar = b * expf(-l);
+                const float r = (ybar - y) * __ldg(a.inv_bref);
+                a.res[((size_t)s * a.VS + jk) * g.C + c] = ray.w * r;
+                const float p = logf(b / fmaxf(y, 1.f));
+                const double d = (double)l - (double)p;
+                d2 += d * d;
+            }
+        }
+    }
+    if (MODE == 1) {
+#pragma unroll
+        for (int off = 16; off > 0; off >>= 1) d2 += __shfl_down_sync(0xffffffffu, d2, off);
+        if (lane == 0) a.dparts[(size_t)s * groups + grp] = d2;
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// Monitor D(n) = fixed-order sum of K1's partials (every caller warp computes the same bits), then A3
+// (Eq. 4-5).  Returns lambda(n) and whether D(n) beat D_best; `writer` publishes the state.
+// ------------------------------------------------------------------------------------------------
+struct StepInfo { double lambda; double D; int improved; };
+
+__device__ __forceinline__ double sum_partials(const double* p, int n, int lane) {
+    double D = 0.0;
+    for (int i = lane; i < n; i += 32) D += __ldg(&p[i]);
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) D += __shfl_xor_sync(0xffffffffu, D, off);
+    return D;
+}
+
+__device__ __forceinline__ StepInfo step_rule(const BackArgs& a, int s, int lane, bool writer) {
+    StepInfo si;
+    si.D = sum_partials(a.dparts + (size_t)s * a.nparts, a.nparts, lane);
+    const SliceState st = a.state_in[s];
+    const int n = st.n;
+    double lam;
+    if (a.ip.forced)          lam = a.ip.forced[n];
+    else if (n == 0)          lam = a.ip.lambda0;
+    else if (si.D < st.D_prev) lam = st.lambda + a.ip.up;
+    else                      lam = fmax(st.lambda - a.ip.down, a.ip.lmin);
+    si.lambda = lam;
+    si.improved = a.ip.return_best && si.D < st.D_best;
+    if (writer && lane == 0) {
+        SliceState o;
+        o.lambda = lam; o.D_prev = si.D; o.D_best = si.improved ? si.D : st.D_best; o.D_last = si.D;
+        o.n = n + 1; o.improved = si.improved; o.pad0 = 0; o.pad1 = 0;
+        a.state_out[s] = o;
+        if (!isfinite(si.D)) a.not_finite[s] = 1;
         if (a.ip.trace) {
             double* tr = a.ip.trace + ((size_t)s * a.ip.n_iters + n) * 2;
-            tr[0] = D;
+            tr[0] = si.D;
             tr[1] = lam;
         }
-        const int imp = a.ip.return_best && D < st->D_best;
-        if (imp) st->D_best = D;
-        st->improved = imp;
-        st->n = n + 1;
     }
-    st->ticket = 0;
+    return si;
+}
+
+// final iterate's monitor (return_best): one warp per slice
+__global__ void k_final_monitor(const double* dparts, int nparts, SliceState* state, int* not_finite) {
+    const int s = blockIdx.x, lane = threadIdx.x;
+    const double D = sum_partials(dparts + (size_t)s * nparts, nparts, lane);
+    if (lane == 0) {
+        state[s].D_last = D;
+        state[s].improved = D < state[s].D_best;
+        if (!isfinite(D)) not_finite[s] = 1;
+    }
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -277,103 +357,180 @@ __device__ __forceinline__ void load_nbhd(const DevGeom& g, const float* img, in
     }
 }
 
+// atan(z) for |z| <= 0.75: odd polynomial, max error 3e-7 rad (fit on Chebyshev nodes; checked on the host side of
+// the tests through the candidate-range parity cases)
+__device__ __forceinline__ float atan_small(float z) {
+    const float z2 = z * z;
+    float p = -0.028348274528980255f;
+    p = fmaf(p, z2, 0.08230143785476685f);
+    p = fmaf(p, z2, -0.13596512377262115f);
+    p = fmaf(p, z2, 0.19924239814281464f);
+    p = fmaf(p, z2, -0.33330586552619934f);
+    p = p * z2;
+    return fmaf(z, p, z);
+}
+
 // ------------------------------------------------------------------------------------------------
-// K2: matched gather backprojection of the records written by K1 (+ TV gradient, Eq. 3 update,
+// K2: matched gather backprojection of the residuals written by K1 (+ step rule, TV gradient, Eq. 3 update,
 // positivity clamp, best-image copy when MODE == 1).
-// grid (ceil(nx/32), ceil(ny/16), batch), block 128: each thread owns a 2x2 pixel tile.  For every
-// view the channels whose ray can cross the tile form the interval |c - c*| < hw around the channel
-// coordinate c* of the tile centre; each candidate costs one 16-byte record load.
+// grid (tiles_x/8, tiles_y/4, batch) over the base tiles (NS == 4: the quadrant x,y < N/2), block 32 x nsplit:
+// lane = one 2x2 pixel tile of a 16 x 8 pixel region, warp = a share of the subset's views.  For every view the
+// channels whose ray can cross the tile form the interval |c - c*| <= hw around the channel coordinate c* of the
+// tile centre (every such ray passes within the tile's half-diagonal of the centre, so its fan angle differs
+// from the centre's by at most asin(r/L) <= tile_hw/along channels); each candidate costs one 16-byte ray-table
+// load and NS 4-byte residual loads.  The warps' sums meet in shared memory in a fixed order; warp k then
+// finishes rotation k of the tile (TV gradient, update, stores).
 // ------------------------------------------------------------------------------------------------
-template <int MODE>
-__global__ void __launch_bounds__(BK_THREADS) k_back(const BackArgs a) {
+template <int MODE, int NS>
+__global__ void __launch_bounds__(BK_MAX_THREADS) k_back(const BackArgs a) {
     const DevGeom& g = a.g;
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int tile_x = blockIdx.x * 16 + (warp & 1) * 8 + (lane & 7);
-    const int tile_y = blockIdx.y * 8 + (warp >> 1) * 4 + (lane >> 3);
-    const int x0 = tile_x * BK_TX, y0 = tile_y * BK_TY, s = blockIdx.z;
-    if (x0 >= g.nx || y0 >= g.ny) return;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nsplit = blockDim.x >> 5;
+    const int x0 = (blockIdx.x * BK_WX + (lane & (BK_WX - 1))) * BK_TX;
+    const int y0 = (blockIdx.y * BK_WY + (lane / BK_WX)) * BK_TY;
+    const int s = blockIdx.z;
+    const bool active = NS == 4 ? (x0 < (g.nx >> 1) && y0 < (g.ny >> 1)) : (x0 < g.nx && y0 < g.ny);
+    __shared__ float red[BK_MAX_SPLIT][NS * 4][32];
 
-    const float xc0 = (float)x0 - g.cx, yc0 = (float)y0 - g.cy;
-    const float X = (xc0 + 0.5f * (BK_TX - 1)) * g.pixel, Y = (yc0 + 0.5f * (BK_TY - 1)) * g.pixel;
-    const float4* rec = a.rec + (size_t)s * a.VS * g.C;
+    float acc[NS][4];                                     // acc[k][ty*2+tx]
+#pragma unroll
+    for (int k = 0; k < NS; ++k)
+#pragma unroll
+        for (int p = 0; p < 4; ++p) acc[k][p] = 0.f;
 
-    float acc00 = 0.f, acc01 = 0.f, acc10 = 0.f, acc11 = 0.f;     // acc[ty][tx]
-    for (int jj = 0; jj < a.VS; ++jj, rec += g.C) {
-        const int v = a.subset < 0 ? jj : a.subset + jj * a.M;
-        const float2 cs = __ldg(&g.views[v]);
-        // fan angle of the tile centre: tan(gamma*) = perp/along
-        const float along = g.sad - fmaf(X, cs.x, Y * cs.y);
-        const float perp = fmaf(X, cs.y, -Y * cs.x);
-        const float z = __fdividef(perp, along);
-        float gam;
-        if (g.use_atanf) {
-            gam = atanf(z);
-        } else {
-            const float z2 = z * z;
-            gam = z * fmaf(z2, fmaf(z2, fmaf(z2, -1.f / 7.f, 0.2f), -1.f / 3.f), 1.f);
-        }
-        const float cstar = fmaf(gam, g.inv_dgamma, g.c_center);
-        // half-width of the tile seen from the source, in channels (+2 % and 0.05 channel of slack)
-        const float adX = fabsf(fmaf(-g.sad, cs.x, X)), adY = fabsf(fmaf(-g.sad, cs.y, Y));
-        const float L2 = fmaf(along, along, perp * perp);
-        float hw;
-        if (g.wide) {                      // every ray through the tile lies within asin(R/L) of its centre
-            hw = asinf(fminf(g.tile_r * rsqrtf(L2), 1.f)) * g.inv_dgamma * 1.001f + 0.05f;
-        } else {                           // tight: projected half-width / (L dgamma), direction error < R/L <= 1.5 %
-            hw = __fdividef(g.hw_scale * 0.5f * (BK_TX * adY + BK_TY * adX), L2) * 1.02f + 0.05f;
-        }
-        const int c_lo = max(0, (int)ceilf(cstar - hw));
-        const int c_hi = min(g.C - 1, (int)floorf(cstar + hw));
-        for (int c = c_lo; c <= c_hi; ++c) {
-            const float4 r = __ldg(&rec[c]);
-            const float hk = 0.5f * (fabsf(r.x) + fabsf(r.y));
-            const float q00 = fmaf(r.x, xc0, fmaf(r.y, yc0, r.z));
-            const float q01 = q00 + r.x;          // (ty=0, tx=1)
-            const float q10 = q00 + r.y;          // (ty=1, tx=0)
-            const float q11 = q10 + r.x;
-            acc00 = fmaf(__saturatef(hk - fabsf(q00)), r.w, acc00);
-            acc01 = fmaf(__saturatef(hk - fabsf(q01)), r.w, acc01);
-            acc10 = fmaf(__saturatef(hk - fabsf(q10)), r.w, acc10);
-            acc11 = fmaf(__saturatef(hk - fabsf(q11)), r.w, acc11);
+    if (active) {
+        const float xc0 = (float)x0 - g.cx, yc0 = (float)y0 - g.cy;
+        const float X = (xc0 + 0.5f * (BK_TX - 1)) * g.pixel, Y = (yc0 + 0.5f * (BK_TY - 1)) * g.pixel;
+        const float* res = a.res + (size_t)s * a.VS * g.C;
+        const int VSb = a.VS / NS;
+        for (int jj = warp; jj < a.VS; jj += nsplit) {
+            const int v = a.subset < 0 ? jj : a.subset + jj * a.M;
+            const float2 cs = __ldg(&g.views[v]);
+            // fan angle of the tile centre: tan(gamma*) = perp/along; along >= SAD - r_max > 0
+            const float along = g.sad - fmaf(X, cs.x, Y * cs.y);
+            const float perp = fmaf(X, cs.y, -Y * cs.x);
+            const float rinv = __fdividef(1.f, along);
+            const float z = perp * rinv;
+            const float gam = g.use_atanf ? atanf(z) : atan_small(z);
+            const float cstar = fmaf(gam, g.inv_dgamma, g.c_center);
+            const float hw = fmaf(g.tile_hw, rinv, 0.05f);
+            const int c_lo = max(0, (int)ceilf(cstar - hw));
+            const int c_hi = min(g.C - 1, (int)floorf(cstar + hw));
+            const float4* rays = g.rays + (size_t)v * g.C;
+            const float* r0 = res + (size_t)jj * g.C;
+            const float* r1 = r0;
+            const float* r2 = r0;
+            const float* r3 = r0;
+            if (NS == 4) {
+                int j1 = jj + VSb, j2 = jj + 2 * VSb, j3 = jj + 3 * VSb;
+                if (j1 >= a.VS) j1 -= a.VS;
+                if (j2 >= a.VS) j2 -= a.VS;
+                if (j3 >= a.VS) j3 -= a.VS;
+                r1 = res + (size_t)j1 * g.C;
+                r2 = res + (size_t)j2 * g.C;
+                r3 = res + (size_t)j3 * g.C;
+            }
+            for (int c = c_lo; c <= c_hi; ++c) {
+                const float4 r = __ldg(&rays[c]);
+                const float hk = 0.5f * (fabsf(r.x) + fabsf(r.y));
+                const float q00 = fmaf(r.x, xc0, fmaf(r.y, yc0, r.z));
+                const float q01 = q00 + r.x;          // (ty=0, tx=1)
+                const float q10 = q00 + r.y;          // (ty=1, tx=0)
+                const float q11 = q10 + r.x;
+                const float w00 = __saturatef(hk - fabsf(q00));
+                const float w01 = __saturatef(hk - fabsf(q01));
+                const float w10 = __saturatef(hk - fabsf(q10));
+                const float w11 = __saturatef(hk - fabsf(q11));
+                const float s0 = __ldg(r0 + c);
+                acc[0][0] = fmaf(w00, s0, acc[0][0]);
+                acc[0][1] = fmaf(w01, s0, acc[0][1]);
+                acc[0][2] = fmaf(w10, s0, acc[0][2]);
+                acc[0][3] = fmaf(w11, s0, acc[0][3]);
+                if (NS == 4) {
+                    const float s1 = __ldg(r1 + c), s2 = __ldg(r2 + c), s3 = __ldg(r3 + c);
+                    acc[1][0] = fmaf(w00, s1, acc[1][0]);
+                    acc[1][1] = fmaf(w01, s1, acc[1][1]);
+                    acc[1][2] = fmaf(w10, s1, acc[1][2]);
+                    acc[1][3] = fmaf(w11, s1, acc[1][3]);
+                    acc[2][0] = fmaf(w00, s2, acc[2][0]);
+                    acc[2][1] = fmaf(w01, s2, acc[2][1]);
+                    acc[2][2] = fmaf(w10, s2, acc[2][2]);
+                    acc[2][3] = fmaf(w11, s2, acc[2][3]);
+                    acc[3][0] = fmaf(w00, s3, acc[3][0]);
+                    acc[3][1] = fmaf(w01, s3, acc[3][1]);
+                    acc[3][2] = fmaf(w10, s3, acc[3][2]);
+                    acc[3][3] = fmaf(w11, s3, acc[3][3]);
+                }
+            }
         }
     }
+#pragma unroll
+    for (int k = 0; k < NS; ++k)
+#pragma unroll
+        for (int p = 0; p < 4; ++p) red[warp][k * 4 + p][lane] = acc[k][p];
+    __syncthreads();
+    if (warp >= NS) return;
 
-    const bool vx1 = x0 + 1 < g.nx, vy1 = y0 + 1 < g.ny;
-    if (MODE == 0) {
-        float* out = a.out + (size_t)s * g.nx * g.ny;
-        out[(size_t)y0 * g.nx + x0] = acc00;
-        if (vx1) out[(size_t)y0 * g.nx + x0 + 1] = acc01;
-        if (vy1) out[(size_t)(y0 + 1) * g.nx + x0] = acc10;
-        if (vx1 && vy1) out[(size_t)(y0 + 1) * g.nx + x0 + 1] = acc11;
-        return;
+    StepInfo si;
+    float step = 0.f;
+    if (MODE == 1) {
+        si = step_rule(a, s, lane, blockIdx.x == 0 && blockIdx.y == 0 && warp == 0);
+        step = (float)(si.lambda * a.tau);
     }
+    if (!active) return;
 
-    // ---- A5 TV gradient of mu(n), A6 update (Eq. 3) with mu > 0, A7 best copy ----
-    const float* img = a.img + (size_t)s * g.img_elems;
-    float m[4][4], tv[2][2];
-    load_nbhd(g, img, x0, y0, m);
-    tv_grad_tile(m, x0, y0, g.nx, g.ny, a.eps2, tv);
-    const SliceState* st = a.state + s;
-    const float step = (float)(st->lambda * a.tau);
-    const float u00 = fmaxf(fmaf(step, acc00 - a.beta_over_M * tv[0][0], m[1][1]), 0.f);
-    const float u01 = fmaxf(fmaf(step, acc01 - a.beta_over_M * tv[0][1], m[1][2]), 0.f);
-    const float u10 = fmaxf(fmaf(step, acc10 - a.beta_over_M * tv[1][0], m[2][1]), 0.f);
-    const float u11 = fmaxf(fmaf(step, acc11 - a.beta_over_M * tv[1][1], m[2][2]), 0.f);
+    for (int k = warp; k < NS; k += nsplit) {
+        // sums over the view shares, fixed order
+        float b[4];
+#pragma unroll
+        for (int p = 0; p < 4; ++p) {
+            float x = 0.f;
+            for (int q = 0; q < nsplit; ++q) x += red[q][k * 4 + p][lane];
+            b[p] = x;
+        }
+        // rotation k of the base tile: origin and where base pixel (tx,ty) lands, o[ty'][tx']
+        int xk = x0, yk = y0;
+        float o00 = b[0], o01 = b[1], o10 = b[2], o11 = b[3];
+        if (NS == 4) {
+            const int N = g.nx;
+            if (k == 1)      { xk = N - 2 - y0; yk = x0;         o00 = b[2]; o01 = b[0]; o10 = b[3]; o11 = b[1]; }
+            else if (k == 2) { xk = N - 2 - x0; yk = N - 2 - y0; o00 = b[3]; o01 = b[2]; o10 = b[1]; o11 = b[0]; }
+            else if (k == 3) { xk = y0;         yk = N - 2 - x0; o00 = b[1]; o01 = b[3]; o10 = b[0]; o11 = b[2]; }
+        }
+        const bool vx1 = xk + 1 < g.nx, vy1 = yk + 1 < g.ny;
+        if (MODE == 0) {
+            float* out = a.out + (size_t)s * g.nx * g.ny;
+            out[(size_t)yk * g.nx + xk] = o00;
+            if (vx1) out[(size_t)yk * g.nx + xk + 1] = o01;
+            if (vy1) out[(size_t)(yk + 1) * g.nx + xk] = o10;
+            if (vx1 && vy1) out[(size_t)(yk + 1) * g.nx + xk + 1] = o11;
+            continue;
+        }
 
-    float* nimg = a.img_new + (size_t)s * g.img_elems;
-    float* nimgT = a.imgT_new + (size_t)s * g.imgT_elems;
-    nimg[pad_off(g, y0, x0)] = u00;
-    nimgT[padT_off(g, x0, y0)] = u00;
-    if (vx1) { nimg[pad_off(g, y0, x0 + 1)] = u01; nimgT[padT_off(g, x0 + 1, y0)] = u01; }
-    if (vy1) { nimg[pad_off(g, y0 + 1, x0)] = u10; nimgT[padT_off(g, x0, y0 + 1)] = u10; }
-    if (vx1 && vy1) { nimg[pad_off(g, y0 + 1, x0 + 1)] = u11; nimgT[padT_off(g, x0 + 1, y0 + 1)] = u11; }
+        // ---- A5 TV gradient of mu(n), A6 update (Eq. 3) with mu > 0, A7 best copy ----
+        const float* img = a.img + (size_t)s * g.img_elems;
+        float m[4][4], tv[2][2];
+        load_nbhd(g, img, xk, yk, m);
+        tv_grad_tile(m, xk, yk, g.nx, g.ny, a.eps2, tv);
+        const float u00 = fmaxf(fmaf(step, o00 - a.beta_over_M * tv[0][0], m[1][1]), 0.f);
+        const float u01 = fmaxf(fmaf(step, o01 - a.beta_over_M * tv[0][1], m[1][2]), 0.f);
+        const float u10 = fmaxf(fmaf(step, o10 - a.beta_over_M * tv[1][0], m[2][1]), 0.f);
+        const float u11 = fmaxf(fmaf(step, o11 - a.beta_over_M * tv[1][1], m[2][2]), 0.f);
 
-    if (a.best && st->improved) {
-        float* best = a.best + (size_t)s * g.nx * g.ny;
-        best[(size_t)y0 * g.nx + x0] = m[1][1];
-        if (vx1) best[(size_t)y0 * g.nx + x0 + 1] = m[1][2];
-        if (vy1) best[(size_t)(y0 + 1) * g.nx + x0] = m[2][1];
-        if (vx1 && vy1) best[(size_t)(y0 + 1) * g.nx + x0 + 1] = m[2][2];
+        float* nimg = a.img_new + (size_t)s * g.img_elems;
+        float* nimgT = a.imgT_new + (size_t)s * g.imgT_elems;
+        nimg[pad_off(g, yk, xk)] = u00;
+        nimgT[padT_off(g, xk, yk)] = u00;
+        if (vx1) { nimg[pad_off(g, yk, xk + 1)] = u01; nimgT[padT_off(g, xk + 1, yk)] = u01; }
+        if (vy1) { nimg[pad_off(g, yk + 1, xk)] = u10; nimgT[padT_off(g, xk, yk + 1)] = u10; }
+        if (vx1 && vy1) { nimg[pad_off(g, yk + 1, xk + 1)] = u11; nimgT[padT_off(g, xk + 1, yk + 1)] = u11; }
+
+        if (a.best && si.improved) {
+            float* best = a.best + (size_t)s * g.nx * g.ny;
+            best[(size_t)yk * g.nx + xk] = m[1][1];
+            if (vx1) best[(size_t)yk * g.nx + xk + 1] = m[1][2];
+            if (vy1) best[(size_t)(yk + 1) * g.nx + xk] = m[2][1];
+            if (vx1 && vy1) best[(size_t)(yk + 1) * g.nx + xk + 1] = m[2][2];
+        }
     }
 }
 
@@ -433,14 +590,15 @@ __global__ void __launch_bounds__(256) k_fill(DevGeom g, float mu0, float* __res
 }
 
 // per-slice state reset and 1/b_ref, b_ref = mean_c b_c (one warp, fixed order)
-__global__ void k_init_state(SliceState* state, int batch, double lambda0, const float* blank, float blank_scalar,
-                             int C, float* inv_bref) {
+__global__ void k_init_state(SliceState* state, int* not_finite, int batch, double lambda0, const float* blank,
+                             float blank_scalar, int C, float* inv_bref) {
     const int lane = threadIdx.x;
     for (int s = lane; s < batch; s += 32) {
         SliceState st;
         st.lambda = lambda0; st.D_prev = 0.0; st.D_best = __longlong_as_double(0x7ff0000000000000LL);
-        st.D_last = 0.0; st.n = 0; st.improved = 0; st.not_finite = 0; st.ticket = 0;
+        st.D_last = 0.0; st.n = 0; st.improved = 0; st.pad0 = 0; st.pad1 = 0;
         state[s] = st;
+        not_finite[s] = 0;
     }
     double sum = 0.0;
     if (blank) {
@@ -453,20 +611,20 @@ __global__ void k_init_state(SliceState* state, int batch, double lambda0, const
     if (lane == 0) *inv_bref = (float)(1.0 / sum);
 }
 
-// sinogram [batch][VS][C] -> records {alpha, beta, g0, h*s} for the standalone backprojection
-__global__ void __launch_bounds__(256) k_make_rec(DevGeom g, const float* __restrict__ sino, float4* __restrict__ rec,
-                                                  int subset, int M, int VS) {
+// sinogram [batch][VS][C] -> h * s for the standalone backprojection
+__global__ void __launch_bounds__(256) k_scale_sino(DevGeom g, const float* __restrict__ sino, float* __restrict__ res,
+                                                    int subset, int M, int VS) {
     const int c = blockIdx.x * 256 + threadIdx.x, j = blockIdx.y, s = blockIdx.z;
     if (c >= g.C) return;
     const int v = subset < 0 ? j : subset + j * M;
     const float4 ray = __ldg(&g.rays[(size_t)v * g.C + c]);
     const size_t o = ((size_t)s * VS + j) * g.C + c;
-    rec[o] = make_float4(ray.x, ray.y, ray.z, ray.w * sino[o]);
+    res[o] = ray.w * sino[o];
 }
 
 // standalone TV gradient: [batch][ny][nx] -> [batch][ny][nx] through the padded workspace
-__global__ void __launch_bounds__(BK_THREADS) k_tv(DevGeom g, const float* __restrict__ img, float eps2,
-                                                   float* __restrict__ out) {
+__global__ void __launch_bounds__(128) k_tv(DevGeom g, const float* __restrict__ img, float eps2,
+                                            float* __restrict__ out) {
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int x0 = (blockIdx.x * 16 + (warp & 1) * 8 + (lane & 7)) * 2;
     const int y0 = (blockIdx.y * 8 + (warp >> 1) * 4 + (lane >> 3)) * 2;

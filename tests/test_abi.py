@@ -103,9 +103,9 @@ def test_A0_ray_table_reproduces_the_oracle_chord(kw):
     assert rays.shape == (V, Cn, 4) and views.shape == (V, 2)
     th = gg.theta0_rad + 2 * np.pi * np.arange(V) / V
     assert np.allclose(views[:, 0], np.cos(th), atol=1e-7) and np.allclose(views[:, 1], np.sin(th), atol=1e-7)
-    # one coefficient is exactly +1, the other has magnitude >= 1
+    # one coefficient is exactly +-1 (-1 only in the rotated quarter turns of a V % 4 == 0 scan), the other >= 1 in magnitude
     a, b = rays[..., 0].astype(np.float64), rays[..., 1].astype(np.float64)
-    assert np.all((a == 1.0) | (b == 1.0)) and np.all(np.maximum(np.abs(a), np.abs(b)) >= 1.0)
+    assert np.all((np.abs(a) == 1.0) | (np.abs(b) == 1.0)) and np.all(np.maximum(np.abs(a), np.abs(b)) >= 1.0)
     xc = np.arange(gg.nx) - 0.5 * (gg.nx - 1)
     yc = np.arange(gg.ny) - 0.5 * (gg.ny - 1)
     worst, nz = 0.0, 0

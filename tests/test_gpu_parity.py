@@ -44,6 +44,7 @@ def host(t):
 ODD = si.ScanConfig("odd", 37, 29, 1.3, 24, 45, sad_mm=120.0, theta0_rad=0.3, channel_offset=0.25, seed=7)
 WIDE = si.ScanConfig("wide", 48, 40, 2.0, 30, 70, sad_mm=75.0, seed=8)           # wide fan: atanf branch
 TINY = si.ScanConfig("tiny", 3, 5, 1.0, 4, 3, sad_mm=20.0, seed=9)
+SYM = si.ScanConfig("sym", 36, 36, 1.3, 24, 45, sad_mm=120.0, theta0_rad=0.3, channel_offset=0.25, seed=11)  # quarter-turn path
 NEAR_AXIS = si.ScanConfig("axis", 64, 64, 1.0, 90, 97, theta0_rad=1e-7, seed=10)  # G10: central ray ~ on pixel edges
 
 
@@ -63,7 +64,8 @@ def osiv():
     (WIDE, [(-1, 1), (4, 5)]),
     (TINY, [(-1, 1), (1, 2)]),
     (si.scan_config("2"), [(-1, 1), (7, 10)]),
-], ids=["config1", "odd", "wide", "tiny", "config2"])
+    (SYM, [(-1, 1), (1, 2), (2, 3), (0, 4)]),          # V_S = 24, 12, 8 take the quarter-turn kernels, V_S = 6 the general
+], ids=["config1", "odd", "wide", "tiny", "config2", "sym"])
 def test_forward_and_back_match_oracle(osiv, cfg, subsets):
     og, gg = geoms(cfg)
     rng = np.random.default_rng(cfg.seed)
@@ -82,6 +84,29 @@ def test_forward_and_back_match_oracle(osiv, cfg, subsets):
             lhs = np.dot(got.astype(np.float64).ravel(), sino.astype(np.float64).ravel())
             rhs = np.dot(img.astype(np.float64).ravel(), gotb.astype(np.float64).ravel())
             assert abs(lhs - rhs) / abs(lhs) < 2e-6
+
+
+def test_quarter_turn_path_is_taken_and_agrees_with_the_general_path(osiv):
+    """The NS = 4 kernels (one chord weight per quarter-turn orbit) against the NS = 1 kernels on the same inputs:
+    equal up to float32 rounding, and the plan reports which one runs."""
+    for cfg, sub, M in [(SYM, 1, 2), (si.scan_config("2"), 7, 10), (si.scan_config("2"), -1, 1)]:
+        _, gg = geoms(cfg)
+        rng = np.random.default_rng(cfg.seed + 1)
+        img = rng.uniform(0.0, 0.013, size=(2, cfg.ny, cfg.nx)).astype(np.float32)
+        vs = cfg.n_views if sub < 0 else cfg.n_views // M
+        sino = rng.uniform(0.0, 1.0, size=(2, vs, cfg.n_channels)).astype(np.float32)
+        with osiv.Handle(gg, max_batch=2) as h:
+            plan = h.plan(M if sub >= 0 else 0, 2)
+            assert plan["k1_orbit"] == 4 and plan["k2_orbit"] == 4
+            f4, b4 = host(h.forward(dev(img), sub, M)), host(h.backward(dev(sino), sub, M))
+            h.set_symmetry(False)
+            plan = h.plan(M if sub >= 0 else 0, 2)
+            assert plan["k1_orbit"] == 1 and plan["k2_orbit"] == 1
+            f1, b1 = host(h.forward(dev(img), sub, M)), host(h.backward(dev(sino), sub, M))
+        assert rel(f4, f1) < 2e-6 and rel(b4, b1) < 2e-6
+    _, gg = geoms(si.scan_config("1"))                  # V = 90: no quarter-turn orbits
+    with osiv.Handle(gg, max_batch=1) as h:
+        assert h.plan(1, 1)["k1_orbit"] == 1
 
 
 def test_projector_near_axis_rays(osiv):
@@ -264,7 +289,7 @@ def test_reconstruct_odd_geometry_with_channel_blank_and_zero_counts(osiv):
 
 def test_reconstruct_forced_lambda_and_constant_lambda(osiv):
     cfg = si.scan_config("1")
-    lam = 0.01 + 0.002 * np.arange(30)
+    lam = 0.01 + 0.001 * np.arange(30)          # stays below the stability limit: rounding noise is not amplified
     got, tr, ref, tr_ref, _ = run_pair(osiv, cfg, dict(beta=0.01, n_subsets=2, n_iters=30, forced_lambda=lam))
     check_run(got, tr, ref, tr_ref)
     assert np.array_equal(tr[:, 1], lam)
