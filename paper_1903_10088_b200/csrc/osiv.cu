@@ -27,6 +27,8 @@ struct osiv_handle {
     float *d_imgA = nullptr, *d_imgB = nullptr, *d_imgTA = nullptr, *d_imgTB = nullptr;
     float* d_best = nullptr;
     size_t res_elems = 0;       float* d_res = nullptr;
+    long long res_key = -1;             // layout (V_S, orbit size, batch) whose zero columns d_res currently holds
+    int res_pad = 4;                    // zero columns C..Cp-1 of every residual row (K2 reads past a tile's last candidate)
     size_t fpart_elems = 0;     float* d_fpart = nullptr;
     size_t ticket_elems = 0;    unsigned int* d_tickets = nullptr;
     size_t dpart_elems = 0;     double* d_dparts = nullptr;
@@ -188,9 +190,16 @@ BackPlan plan_back(const osiv_handle* h, int VS, int batch) {
     p.grid = dim3((tx + BK_WX - 1) / BK_WX, (ty + BK_WY - 1) / BK_WY, batch);
     const long long blocks = (long long)p.grid.x * p.grid.y * batch;
     long long want = ((long long)h->num_sms * 40 + blocks - 1) / blocks;      // about 40 resident warps per SM
-    want = std::max<long long>(1, std::min<long long>(want, std::min(BK_MAX_SPLIT, VS)));
-    int best = (int)want;
-    for (int d = (int)want; d >= 1; --d) if (VS % d == 0) { if (2 * d > want) best = d; break; }
+    int best;
+    if (p.ns == 4) {                  // warps come in fours (one per quarter turn), each with a share of the V_S/4 base views
+        const int vb = VS / 4;
+        best = 4;
+        while (best * 2 <= BK_MAX_SPLIT && best * 2 <= want && best / 2 <= vb) best *= 2;
+    } else {
+        want = std::max<long long>(1, std::min<long long>(want, std::min(BK_MAX_SPLIT, VS)));
+        best = (int)want;
+        for (int d = (int)want; d >= 1; --d) if (VS % d == 0) { if (2 * d > want) best = d; break; }
+    }
     p.nsplit = best;
     return p;
 }
@@ -203,8 +212,8 @@ void launch_forward(const FwdPlan& p, const FwdArgs& a, cudaStream_t st) {
 
 template <int MODE>
 void launch_back(const BackPlan& p, const BackArgs& a, cudaStream_t st) {
-    if (p.ns == 4) k_back<MODE, 4><<<p.grid, 32 * p.nsplit, 0, st>>>(a);
-    else           k_back<MODE, 1><<<p.grid, 32 * p.nsplit, 0, st>>>(a);
+    if (p.ns == 4) k_back<MODE, 4><<<p.grid, 32 * p.nsplit, (size_t)p.nsplit * 16 * 32 * sizeof(float), st>>>(a);
+    else           k_back<MODE, 1><<<p.grid, 32 * p.nsplit, (size_t)p.nsplit * 4 * 32 * sizeof(float), st>>>(a);
 }
 
 int ensure_forward_ws(osiv_handle* h, const FwdPlan& p, int batch, cudaStream_t st) {
@@ -217,6 +226,22 @@ int ensure_forward_ws(osiv_handle* h, const FwdPlan& p, int batch, cudaStream_t 
         OSIV_CUDA(cudaMemsetAsync(h->d_tickets, 0, h->ticket_elems * sizeof(unsigned int), st));
     }
     return grow(&h->d_dparts, &h->dpart_elems, nt);
+}
+
+// residual buffer [batch][V_S][Cp] floats (NS == 4: [batch][V_S/4][Cp] float4); columns C..Cp-1 must be zero, and they
+// move when the layout changes, so the buffer is cleared whenever (V_S, orbit size, batch) differs from the last call
+int ensure_res(osiv_handle* h, int VS, int ns, int batch, cudaStream_t st) {
+    const int Cp = h->geom.n_channels + h->res_pad;
+    const size_t want = (size_t)batch * VS * Cp;
+    const long long key = ((long long)VS * 8 + ns) * 100000 + batch;
+    const bool realloc = h->res_elems < want || !h->d_res;
+    int rc = grow(&h->d_res, &h->res_elems, want);
+    if (rc != OSIV_OK) return rc;
+    if (realloc || key != h->res_key) {
+        OSIV_CUDA(cudaMemsetAsync(h->d_res, 0, h->res_elems * sizeof(float), st));
+        h->res_key = key;
+    }
+    return OSIV_OK;
 }
 
 dim3 px_grid(const osiv_handle* h, int batch) { return dim3((h->geom.nx + 31) / 32, (h->geom.ny + 7) / 8, batch); }
@@ -296,6 +321,12 @@ int osiv_create(const osiv_geometry* geom, int32_t max_batch, int32_t device, os
     std::vector<float4> rays;
     std::vector<float2> views;
     build_tables(g, dgamma, rays, views);
+    // K2 reads up to res_pad entries past a view's last channel: zero slack after the last view
+    const double tile_r = 0.5 * g.pixel_mm * std::sqrt((double)(BK_TX * BK_TX + BK_TY * BK_TY));
+    const double xm = std::min(tile_r / (g.sad_mm - rmax), 1.0);
+    const double tile_hw = std::asin(xm) / xm * tile_r / dgamma * 1.0005;
+    h->res_pad = ((2 * (int)std::ceil(tile_hw / (g.sad_mm - rmax) + 0.05) + 3) + 3) / 4 * 4;
+    rays.resize(rays.size() + h->res_pad + 4, make_float4(0.f, 0.f, 0.f, 0.f));
     if (cudaMalloc((void**)&h->d_rays, rays.size() * sizeof(float4)) != cudaSuccess ||
         cudaMalloc((void**)&h->d_views, views.size() * sizeof(float2)) != cudaSuccess ||
         cudaMalloc((void**)&h->d_state, (size_t)2 * max_batch * sizeof(SliceState)) != cudaSuccess ||
@@ -324,9 +355,7 @@ int osiv_create(const osiv_geometry* geom, int32_t max_batch, int32_t device, os
     d.c_center = (float)(0.5 * (g.n_channels - 1) - g.channel_offset);
     // K2 candidate bound: every ray through a tile passes within its half-diagonal r of the tile centre, so its fan
     // angle is within asin(r/L) <= f*r/along of the centre's, f = asin(x)/x at the largest possible x = r/(SAD-r_max)
-    const double tile_r = 0.5 * g.pixel_mm * std::sqrt((double)(BK_TX * BK_TX + BK_TY * BK_TY));
-    const double xm = std::min(tile_r / (g.sad_mm - rmax), 1.0);
-    d.tile_hw = (float)(std::asin(xm) / xm * tile_r / dgamma * 1.0005);
+    d.tile_hw = (float)tile_hw;
     // atan_small: |z| <= 0.75, error 3e-7 rad; demand < 0.01 channel, else atanf
     const double zmax = rmax / (g.sad_mm - rmax);
     d.use_atanf = (zmax > 0.75 || 3e-7 / dgamma > 0.01) ? 1 : 0;
@@ -432,12 +461,14 @@ int osiv_backward(osiv_handle* h, const float* d_sino, float* d_img, int32_t bat
     if (!guard.ok) { cudaGetLastError(); return OSIV_ERR_CUDA; }
     cudaStream_t st = (cudaStream_t)cuda_stream;
     const int VS = subset_views(h, subset, n_subsets), M = subset < 0 ? 1 : n_subsets;
-    int rc = grow(&h->d_res, &h->res_elems, (size_t)batch * VS * h->geom.n_channels);
-    if (rc != OSIV_OK) return rc;
-    k_scale_sino<<<dim3((h->geom.n_channels + 255) / 256, VS, batch), 256, 0, st>>>(h->dg, d_sino, h->d_res, subset, M, VS);
     const BackPlan p = plan_back(h, VS, batch);
+    int rc = ensure_res(h, VS, p.ns, batch, st);
+    if (rc != OSIV_OK) return rc;
+    const int Cp = h->geom.n_channels + h->res_pad;
+    k_scale_sino<<<dim3((h->geom.n_channels + 255) / 256, VS, batch), 256, 0, st>>>(h->dg, d_sino, h->d_res, subset, M, VS,
+                                                                                    p.ns, Cp);
     BackArgs b{};
-    b.g = h->dg; b.res = h->d_res; b.subset = subset; b.M = M; b.VS = VS; b.out = d_img;
+    b.g = h->dg; b.res = h->d_res; b.Cp = Cp; b.subset = subset; b.M = M; b.VS = VS; b.out = d_img;
     launch_back<0>(p, b, st);
     return launch_check(h, 2);
 }
@@ -472,9 +503,10 @@ int osiv_reconstruct(osiv_handle* h, const float* d_counts, const float* d_blank
     const int VS = h->geom.n_views / M, C = h->geom.n_channels;
     int rc = ensure_images(h, batch, st);
     if (rc != OSIV_OK) return rc;
-    if ((rc = grow(&h->d_res, &h->res_elems, (size_t)batch * VS * C)) != OSIV_OK) return rc;
     const FwdPlan fp = plan_forward(h, 1, VS, batch);
     const BackPlan bp = plan_back(h, VS, batch);
+    if ((rc = ensure_res(h, VS, fp.ns, batch, st)) != OSIV_OK) return rc;
+    const int Cp = C + h->res_pad;
     if ((rc = ensure_forward_ws(h, fp, batch, st)) != OSIV_OK) return rc;
     if (h_trace && N > 0 && (rc = grow(&h->d_trace, &h->trace_elems, (size_t)batch * N * 2)) != OSIV_OK) return rc;
     if (prm->forced_lambda && N > 0) {
@@ -493,9 +525,9 @@ int osiv_reconstruct(osiv_handle* h, const float* d_counts, const float* d_blank
     FwdArgs f{};
     f.g = h->dg; f.M = M; f.VS = VS; f.nsplit = fp.nsplit;
     f.counts = d_counts; f.blank = d_blank; f.blank_scalar = blank_scalar; f.inv_bref = h->d_inv_bref;
-    f.res = h->d_res; f.fpart = h->d_fpart; f.tickets = h->d_tickets; f.dparts = h->d_dparts;
+    f.res = h->d_res; f.Cp = Cp; f.fpart = h->d_fpart; f.tickets = h->d_tickets; f.dparts = h->d_dparts;
     BackArgs b{};
-    b.g = h->dg; b.res = h->d_res; b.M = M; b.VS = VS; b.best = best;
+    b.g = h->dg; b.res = h->d_res; b.Cp = Cp; b.M = M; b.VS = VS; b.best = best;
     b.dparts = h->d_dparts; b.nparts = fp.groups; b.not_finite = h->d_not_finite;
     b.ip.lambda0 = prm->lambda0; b.ip.up = prm->lambda_up; b.ip.down = prm->lambda_down; b.ip.lmin = prm->lambda_min;
     b.ip.forced = (prm->forced_lambda && N > 0) ? h->d_forced : nullptr;

@@ -39,7 +39,7 @@ constexpr int FWD_THREADS = 32 * FWD_SEGS;
 constexpr int FWD_MAX_SPLIT = 8;           // K1 blocks that share one ray group (partial sums through global memory)
 constexpr int BK_TX = 2, BK_TY = 2;        // pixels per thread in the backprojector
 constexpr int BK_WX = 8, BK_WY = 4;        // tiles per warp: a warp covers 16 x 8 pixels
-constexpr int BK_MAX_SPLIT = 8;            // K2 warps per block; each owns a share of the subset's views
+constexpr int BK_MAX_SPLIT = 16;           // K2 warps per block; each owns a share of the subset's views
 constexpr int BK_MAX_THREADS = 32 * BK_MAX_SPLIT;
 
 struct DevGeom {
@@ -81,7 +81,9 @@ struct FwdArgs {
     const float* blank;                    // [C] or null
     float blank_scalar;
     const float* inv_bref;                 // device scalar 1/b_ref
-    float* res;                            // MODE 1: [batch][VS][C]  h * r
+    float* res;                            // MODE 1: h * r; NS == 1: [batch][VS][Cp] floats, NS == 4: [batch][VS/4][Cp] float4
+                                           // holding the orbit {j, j+VS/4, j+VS/2, j+3VS/4}; columns C..Cp-1 stay zero
+    int Cp;
     float* fpart;                          // [batch][groups][nsplit][NS][32] line-integral partial sums (nsplit > 1)
     unsigned int* tickets;                 // [batch][groups], zero between launches
     double* dparts;                        // MODE 1: [batch][groups] partial sums of D
@@ -89,7 +91,8 @@ struct FwdArgs {
 
 struct BackArgs {
     DevGeom g;
-    const float* res;                      // [batch][VS][C]  h * (residual or sinogram)
+    const float* res;                      // h * (residual or sinogram), layout as FwdArgs::res
+    int Cp;
     int subset, M, VS;
     float* out;                            // MODE 0: [batch][ny][nx]
     const float* img;                      // MODE 1: padded mu(n)
@@ -133,11 +136,10 @@ __global__ void __launch_bounds__(FWD_THREADS) k_forward(const FwdArgs a) {
     float acc[NS];
 #pragma unroll
     for (int k = 0; k < NS; ++k) acc[k] = 0.f;
-    float4 ray = make_float4(1.f, 0.f, 0.f, 0.f);
-    bool rowmaj = true;
-    if (c < g.C) {
-        ray = __ldg(&g.rays[(size_t)v * g.C + c]);
-        rowmaj = fabsf(ray.x) >= fabsf(ray.y);
+    // lanes past the last channel walk a copy of the last ray (keeps the warp convergent) and store nothing
+    const float4 ray = __ldg(&g.rays[(size_t)v * g.C + min(c, g.C - 1)]);
+    const bool rowmaj = fabsf(ray.x) >= fabsf(ray.y);
+    {
         const float kk = rowmaj ? ray.x : ray.y;          // coefficient of the in-line coordinate, |kk| >= 1
         const float uu = rowmaj ? ray.y : ray.x;          // coefficient of the marching coordinate, +-1
         const float* bufA = rowmaj ? a.img + (size_t)s * g.img_elems : a.imgT + (size_t)s * g.imgT_elems;
@@ -152,13 +154,23 @@ __global__ void __launch_bounds__(FWD_THREADS) k_forward(const FwdArgs a) {
         const float b1 = uu * (-ray.z - A), b2 = uu * (-ray.z + A);
         const float flo = fminf(fmaxf(ceilf(fminf(b1, b2) + cb) - 1.f, 0.f), (float)nb);
         const float fhi = fminf(fmaxf(floorf(fmaxf(b1, b2) + cb) + 1.f, -1.f), (float)(nb - 1));
-        const int jlo = (int)flo, jhi = (int)fhi;
-        const int nsteps = jhi - jlo + 1;
+        // The warp walks the union of its rays' line ranges in lock step, so that at every step its 32 lanes read
+        // neighbouring pixels of ONE image line (1-2 cache lines per load instead of up to 32).  On a line outside a
+        // ray's own range the crossing is more than half a pixel outside the image: the clamped index lands in the
+        // zero padding and the term vanishes.
+        // (Row-major and column-major rays of one warp form two such unions: their lines are different things.)
+        const int big = 1 << 30;
+        const int rlo = __reduce_min_sync(0xffffffffu, rowmaj ? (int)flo : big);
+        const int rhi = __reduce_max_sync(0xffffffffu, rowmaj ? (int)fhi : -big);
+        const int clo = __reduce_min_sync(0xffffffffu, rowmaj ? big : (int)flo);
+        const int chi = __reduce_max_sync(0xffffffffu, rowmaj ? -big : (int)fhi);
+        const int wlo = rowmaj ? rlo : clo, whi = rowmaj ? rhi : chi;
+        const int nsteps = whi - wlo + 1;
         if (nsteps > 0) {
             const int nsegt = FWD_SEGS * a.nsplit;
             const int len = (nsteps + nsegt - 1) / nsegt;
-            const int j0 = jlo + (split * FWD_SEGS + seg) * len;
-            const int j1 = min(j0 + len, jhi + 1);
+            const int j0 = wlo + (split * FWD_SEGS + seg) * len;
+            const int j1 = min(j0 + len, whi + 1);
             const int imax = na + PAD - 2;
             int offP = (j0 + PADR) * pitch + PAD;                 // line j, walking up
             int offM = (nb - 1 - j0 + PADR) * pitch + PAD;        // line nb-1-j, walking down
@@ -230,11 +242,13 @@ __global__ void __launch_bounds__(FWD_THREADS) k_forward(const FwdArgs a) {
 
     const int VSb = a.VS / NS, Vq = g.V / NS;
     double d2 = 0.0;
+    float hr[NS];
 #pragma unroll
     for (int k = 0; k < NS; ++k) {
         const float l = ray.w * t[k];
         const int jk = jb + k * VSb;                     // compact view index inside the subset
         const int vk = v + k * Vq;
+        hr[k] = 0.f;
         if (c < g.C) {
             if (MODE == 0) {
                 a.sino[((size_t)s * a.VS + jk) * g.C + c] = l;
@@ -244,12 +258,17 @@ __global__ void __launch_bounds__(FWD_THREADS) k_forward(const FwdArgs a) {
                 const float b = a.blank ? __ldg(&a.blank[c]) : a.blank_scalar;
                 const float ybar = b * expf(-l);
                 const float r = (ybar - y) * __ldg(a.inv_bref);
-                a.res[((size_t)s * a.VS + jk) * g.C + c] = ray.w * r;
+                hr[k] = ray.w * r;
                 const float p = logf(b / fmaxf(y, 1.f));
                 const double d = (double)l - (double)p;
                 d2 += d * d;
             }
         }
+    }
+    if (MODE == 1 && c < g.C) {
+        // NS == 4: the orbit's four residuals share one float4 (K2 reads them with one load per candidate ray)
+        if (NS == 4) reinterpret_cast<float4*>(a.res)[((size_t)s * VSb + jb) * a.Cp + c] = make_float4(hr[0], hr[1], hr[2], hr[3]);
+        else         a.res[((size_t)s * a.VS + jb) * a.Cp + c] = hr[0];
     }
     if (MODE == 1) {
 #pragma unroll
@@ -378,7 +397,7 @@ __device__ __forceinline__ float atan_small(float z) {
 // channels whose ray can cross the tile form the interval |c - c*| <= hw around the channel coordinate c* of the
 // tile centre (every such ray passes within the tile's half-diagonal of the centre, so its fan angle differs
 // from the centre's by at most asin(r/L) <= tile_hw/along channels); each candidate costs one 16-byte ray-table
-// load and NS 4-byte residual loads.  The warps' sums meet in shared memory in a fixed order; warp k then
+// load and one residual load (NS == 4: the float4 of the view's orbit).  The warps' sums meet in shared memory in a fixed order; warp k then
 // finishes rotation k of the tile (TV gradient, update, stores).
 // ------------------------------------------------------------------------------------------------
 template <int MODE, int NS>
@@ -389,20 +408,27 @@ __global__ void __launch_bounds__(BK_MAX_THREADS) k_back(const BackArgs a) {
     const int y0 = (blockIdx.y * BK_WY + (lane / BK_WX)) * BK_TY;
     const int s = blockIdx.z;
     const bool active = NS == 4 ? (x0 < (g.nx >> 1) && y0 < (g.ny >> 1)) : (x0 < g.nx && y0 < g.ny);
-    __shared__ float red[BK_MAX_SPLIT][NS * 4][32];
+    extern __shared__ float red_dyn[];                    // [nsplit][NS * 4][32]
+    float (*red)[NS * 4][32] = reinterpret_cast<float (*)[NS * 4][32]>(red_dyn);
 
-    float acc[NS][4];                                     // acc[k][ty*2+tx]
+    // acc[m][ty*2+tx]: NS == 4: m = component of the orbit's residual float4 (this warp's views all lie in quarter
+    // turn `quarter`, so rotation k of the tile collects component (quarter + k) % 4)
+    float acc[NS][4];
 #pragma unroll
     for (int k = 0; k < NS; ++k)
 #pragma unroll
         for (int p = 0; p < 4; ++p) acc[k][p] = 0.f;
 
-    if (active) {
+    const int VSb = a.VS / NS;
+    // NS == 4: nsplit is a multiple of 4; warp w takes quarter turn w & 3 and every (nsplit/4)-th base view
+    const int quarter = NS == 4 ? (warp & 3) : 0;
+    const int jfirst = NS == 4 ? (warp >> 2) : warp, jstep = NS == 4 ? (nsplit >> 2) : nsplit;
+    {
         const float xc0 = (float)x0 - g.cx, yc0 = (float)y0 - g.cy;
         const float X = (xc0 + 0.5f * (BK_TX - 1)) * g.pixel, Y = (yc0 + 0.5f * (BK_TY - 1)) * g.pixel;
-        const float* res = a.res + (size_t)s * a.VS * g.C;
-        const int VSb = a.VS / NS;
-        for (int jj = warp; jj < a.VS; jj += nsplit) {
+        const float* res = a.res + (size_t)s * a.VS * a.Cp;      // same float count for both layouts
+        for (int jb = jfirst; jb < VSb; jb += jstep) {
+            const int jj = jb + quarter * VSb;
             const int v = a.subset < 0 ? jj : a.subset + jj * a.M;
             const float2 cs = __ldg(&g.views[v]);
             // fan angle of the tile centre: tan(gamma*) = perp/along; along >= SAD - r_max > 0
@@ -413,60 +439,60 @@ __global__ void __launch_bounds__(BK_MAX_THREADS) k_back(const BackArgs a) {
             const float gam = g.use_atanf ? atanf(z) : atan_small(z);
             const float cstar = fmaf(gam, g.inv_dgamma, g.c_center);
             const float hw = fmaf(g.tile_hw, rinv, 0.05f);
-            const int c_lo = max(0, (int)ceilf(cstar - hw));
+            const int c_lo = min(max(0, (int)ceilf(cstar - hw)), g.C);
             const int c_hi = min(g.C - 1, (int)floorf(cstar + hw));
-            const float4* rays = g.rays + (size_t)v * g.C;
-            const float* r0 = res + (size_t)jj * g.C;
-            const float* r1 = r0;
-            const float* r2 = r0;
-            const float* r3 = r0;
+            // the warp runs max-over-lanes candidates in lock step (no remainder code); a lane's extra candidates
+            // have zero weight (the ray misses its tile) or read the zero columns C..Cp-1 of res
+            const int ncw = __reduce_max_sync(0xffffffffu, active ? c_hi - c_lo + 1 : 0);
+            const float4* rp = g.rays + (size_t)v * g.C + c_lo;
             if (NS == 4) {
-                int j1 = jj + VSb, j2 = jj + 2 * VSb, j3 = jj + 3 * VSb;
-                if (j1 >= a.VS) j1 -= a.VS;
-                if (j2 >= a.VS) j2 -= a.VS;
-                if (j3 >= a.VS) j3 -= a.VS;
-                r1 = res + (size_t)j1 * g.C;
-                r2 = res + (size_t)j2 * g.C;
-                r3 = res + (size_t)j3 * g.C;
-            }
-            for (int c = c_lo; c <= c_hi; ++c) {
-                const float4 r = __ldg(&rays[c]);
-                const float hk = 0.5f * (fabsf(r.x) + fabsf(r.y));
-                const float q00 = fmaf(r.x, xc0, fmaf(r.y, yc0, r.z));
-                const float q01 = q00 + r.x;          // (ty=0, tx=1)
-                const float q10 = q00 + r.y;          // (ty=1, tx=0)
-                const float q11 = q10 + r.x;
-                const float w00 = __saturatef(hk - fabsf(q00));
-                const float w01 = __saturatef(hk - fabsf(q01));
-                const float w10 = __saturatef(hk - fabsf(q10));
-                const float w11 = __saturatef(hk - fabsf(q11));
-                const float s0 = __ldg(r0 + c);
-                acc[0][0] = fmaf(w00, s0, acc[0][0]);
-                acc[0][1] = fmaf(w01, s0, acc[0][1]);
-                acc[0][2] = fmaf(w10, s0, acc[0][2]);
-                acc[0][3] = fmaf(w11, s0, acc[0][3]);
-                if (NS == 4) {
-                    const float s1 = __ldg(r1 + c), s2 = __ldg(r2 + c), s3 = __ldg(r3 + c);
-                    acc[1][0] = fmaf(w00, s1, acc[1][0]);
-                    acc[1][1] = fmaf(w01, s1, acc[1][1]);
-                    acc[1][2] = fmaf(w10, s1, acc[1][2]);
-                    acc[1][3] = fmaf(w11, s1, acc[1][3]);
-                    acc[2][0] = fmaf(w00, s2, acc[2][0]);
-                    acc[2][1] = fmaf(w01, s2, acc[2][1]);
-                    acc[2][2] = fmaf(w10, s2, acc[2][2]);
-                    acc[2][3] = fmaf(w11, s2, acc[2][3]);
-                    acc[3][0] = fmaf(w00, s3, acc[3][0]);
-                    acc[3][1] = fmaf(w01, s3, acc[3][1]);
-                    acc[3][2] = fmaf(w10, s3, acc[3][2]);
-                    acc[3][3] = fmaf(w11, s3, acc[3][3]);
+                const float4* sp = reinterpret_cast<const float4*>(res) + (size_t)jb * a.Cp + c_lo;
+#pragma unroll 2
+                for (int t = 0; t < ncw; ++t) {
+                    const float4 r = __ldg(rp + t);
+                    const float4 sv = __ldg(sp + t);
+                    const float hk = 0.5f * (fabsf(r.x) + fabsf(r.y));
+                    const float q00 = fmaf(r.x, xc0, fmaf(r.y, yc0, r.z));
+                    const float q01 = q00 + r.x;          // (ty=0, tx=1)
+                    const float q10 = q00 + r.y;          // (ty=1, tx=0)
+                    const float q11 = q10 + r.x;
+                    const float w00 = __saturatef(hk - fabsf(q00));
+                    const float w01 = __saturatef(hk - fabsf(q01));
+                    const float w10 = __saturatef(hk - fabsf(q10));
+                    const float w11 = __saturatef(hk - fabsf(q11));
+                    acc[0][0] = fmaf(w00, sv.x, acc[0][0]); acc[0][1] = fmaf(w01, sv.x, acc[0][1]);
+                    acc[0][2] = fmaf(w10, sv.x, acc[0][2]); acc[0][3] = fmaf(w11, sv.x, acc[0][3]);
+                    acc[1 % NS][0] = fmaf(w00, sv.y, acc[1 % NS][0]); acc[1 % NS][1] = fmaf(w01, sv.y, acc[1 % NS][1]);
+                    acc[1 % NS][2] = fmaf(w10, sv.y, acc[1 % NS][2]); acc[1 % NS][3] = fmaf(w11, sv.y, acc[1 % NS][3]);
+                    acc[2 % NS][0] = fmaf(w00, sv.z, acc[2 % NS][0]); acc[2 % NS][1] = fmaf(w01, sv.z, acc[2 % NS][1]);
+                    acc[2 % NS][2] = fmaf(w10, sv.z, acc[2 % NS][2]); acc[2 % NS][3] = fmaf(w11, sv.z, acc[2 % NS][3]);
+                    acc[3 % NS][0] = fmaf(w00, sv.w, acc[3 % NS][0]); acc[3 % NS][1] = fmaf(w01, sv.w, acc[3 % NS][1]);
+                    acc[3 % NS][2] = fmaf(w10, sv.w, acc[3 % NS][2]); acc[3 % NS][3] = fmaf(w11, sv.w, acc[3 % NS][3]);
+                }
+            } else {
+                const float* sp = res + (size_t)jb * a.Cp + c_lo;
+#pragma unroll 2
+                for (int t = 0; t < ncw; ++t) {
+                    const float4 r = __ldg(rp + t);
+                    const float sv = __ldg(sp + t);
+                    const float hk = 0.5f * (fabsf(r.x) + fabsf(r.y));
+                    const float q00 = fmaf(r.x, xc0, fmaf(r.y, yc0, r.z));
+                    const float q01 = q00 + r.x;
+                    const float q10 = q00 + r.y;
+                    const float q11 = q10 + r.x;
+                    acc[0][0] = fmaf(__saturatef(hk - fabsf(q00)), sv, acc[0][0]);
+                    acc[0][1] = fmaf(__saturatef(hk - fabsf(q01)), sv, acc[0][1]);
+                    acc[0][2] = fmaf(__saturatef(hk - fabsf(q10)), sv, acc[0][2]);
+                    acc[0][3] = fmaf(__saturatef(hk - fabsf(q11)), sv, acc[0][3]);
                 }
             }
         }
     }
+    // rotation k of the tile = orbit component (quarter + k) % 4  <=>  component m feeds rotation (m - quarter) % 4
 #pragma unroll
-    for (int k = 0; k < NS; ++k)
+    for (int m = 0; m < NS; ++m)
 #pragma unroll
-        for (int p = 0; p < 4; ++p) red[warp][k * 4 + p][lane] = acc[k][p];
+        for (int p = 0; p < 4; ++p) red[warp][((m - quarter) & (NS - 1)) * 4 + p][lane] = acc[m][p];
     __syncthreads();
     if (warp >= NS) return;
 
@@ -611,15 +637,20 @@ __global__ void k_init_state(SliceState* state, int* not_finite, int batch, doub
     if (lane == 0) *inv_bref = (float)(1.0 / sum);
 }
 
-// sinogram [batch][VS][C] -> h * s for the standalone backprojection
+// sinogram [batch][VS][C] -> h * s in the layout of FwdArgs::res, for the standalone backprojection
 __global__ void __launch_bounds__(256) k_scale_sino(DevGeom g, const float* __restrict__ sino, float* __restrict__ res,
-                                                    int subset, int M, int VS) {
+                                                    int subset, int M, int VS, int ns, int Cp) {
     const int c = blockIdx.x * 256 + threadIdx.x, j = blockIdx.y, s = blockIdx.z;
     if (c >= g.C) return;
     const int v = subset < 0 ? j : subset + j * M;
     const float4 ray = __ldg(&g.rays[(size_t)v * g.C + c]);
-    const size_t o = ((size_t)s * VS + j) * g.C + c;
-    res[o] = ray.w * sino[o];
+    const float val = ray.w * sino[((size_t)s * VS + j) * g.C + c];
+    if (ns == 4) {
+        const int VSb = VS / 4, jb = j % VSb, k = j / VSb;
+        res[(((size_t)s * VSb + jb) * Cp + c) * 4 + k] = val;
+    } else {
+        res[((size_t)s * VS + j) * Cp + c] = val;
+    }
 }
 
 // standalone TV gradient: [batch][ny][nx] -> [batch][ny][nx] through the padded workspace
