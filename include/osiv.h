@@ -116,6 +116,12 @@ int64_t osiv_launch_count(const osiv_handle* h);
  * the general kernels (used by the tests to compare the two paths).  Results differ only by rounding. */
 int osiv_set_symmetry(osiv_handle* h, int32_t enable);
 
+/* Launch overlap inside osiv_reconstruct.  By default (enable = 1) K1 and K2 are chained with programmatic
+ * dependent launches: the next kernel's blocks become resident and run their data-independent prologue while the
+ * current kernel drains, and wait on the device for its completion before they read its output.  enable = 0 uses
+ * plain stream order (same results bit for bit; used by the tests and for A/B timing). */
+int osiv_set_overlap(osiv_handle* h, int32_t enable);
+
 /* Launch plan osiv_reconstruct would use for `n_subsets` subsets (<= 0: all views) and `batch` slices:
  * out8 = {K1 orbit size (1 or 4), K1 blocks per ray group, K1 blocks, K1 threads per block,
  *         K2 orbit size, K2 warps per block, K2 blocks, K2 threads per block}.  Host only. */

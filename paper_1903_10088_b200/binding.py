@@ -17,7 +17,7 @@ OSIV_OK, OSIV_ERR_INVALID_ARG, OSIV_ERR_CUDA, OSIV_ERR_NOT_FINITE = 0, -1, -2, -
 
 EXPORTED_SYMBOLS = (
     "osiv_version", "osiv_strerror", "osiv_default_params", "osiv_create", "osiv_destroy", "osiv_ray_table", "osiv_get_dgamma",
-    "osiv_get_tau", "osiv_launch_count", "osiv_set_symmetry", "osiv_get_plan", "osiv_set_profiling", "osiv_get_profile", "osiv_forward", "osiv_backward", "osiv_tv_gradient", "osiv_reconstruct",
+    "osiv_get_tau", "osiv_launch_count", "osiv_set_symmetry", "osiv_set_overlap", "osiv_get_plan", "osiv_set_profiling", "osiv_get_profile", "osiv_forward", "osiv_backward", "osiv_tv_gradient", "osiv_reconstruct",
     "osiv_reconstruct_host",
 )
 
@@ -101,6 +101,7 @@ def lib():
         L.osiv_launch_count.restype = C.c_int64
         L.osiv_launch_count.argtypes = [vp]
         L.osiv_set_symmetry.argtypes = [vp, ip]
+        L.osiv_set_overlap.argtypes = [vp, ip]
         L.osiv_get_plan.argtypes = [vp, ip, ip, C.POINTER(C.c_int32)]
         L.osiv_set_profiling.argtypes = [vp, ip]
         L.osiv_get_profile.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_int64), C.POINTER(C.c_double),
@@ -216,6 +217,10 @@ class Handle:
     def set_symmetry(self, enable: bool) -> None:
         """enable=False forces the general (NS = 1) kernels even where the quarter-turn path applies"""
         _check(lib().osiv_set_symmetry(self._h, 1 if enable else 0), "osiv_set_symmetry")
+
+    def set_overlap(self, enable: bool) -> None:
+        """enable=False chains K1 and K2 in plain stream order instead of programmatic dependent launches"""
+        _check(lib().osiv_set_overlap(self._h, 1 if enable else 0), "osiv_set_overlap")
 
     def plan(self, n_subsets: int = 0, batch: int = 1) -> dict:
         out = (C.c_int32 * 8)()

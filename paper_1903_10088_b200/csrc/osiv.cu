@@ -29,8 +29,6 @@ struct osiv_handle {
     size_t res_elems = 0;       float* d_res = nullptr;
     long long res_key = -1;             // layout (V_S, orbit size, batch) whose zero columns d_res currently holds
     int res_pad = 4;                    // zero columns C..Cp-1 of every residual row (K2 reads past a tile's last candidate)
-    size_t fpart_elems = 0;     float* d_fpart = nullptr;
-    size_t ticket_elems = 0;    unsigned int* d_tickets = nullptr;
     size_t dpart_elems = 0;     double* d_dparts = nullptr;
     SliceState* d_state = nullptr;      // [2][max_batch], ping-pong between iterations
     int* d_not_finite = nullptr;        // [max_batch]
@@ -45,6 +43,7 @@ struct osiv_handle {
     size_t hi_elems = 0;        float* d_himg = nullptr;
     int64_t launches = 0;
     int force_ns1 = 0;                  // osiv_set_symmetry(h, 0): always take the general path
+    int use_pdl = 1;                    // osiv_set_overlap(h, 0): plain stream order between K1 and K2
     // per-kernel event timing (osiv_set_profiling)
     bool profiling = false;
     std::vector<cudaEvent_t> events;
@@ -165,6 +164,40 @@ int pick_ns(const osiv_handle* h, int VS) { return (h->dg.sym4 && !h->force_ns1 
 struct FwdPlan { dim3 grid; int nsplit, groups, ns; };
 struct BackPlan { dim3 grid; int nsplit, ns; };
 
+// K1 runs as thread-block clusters (1, nsplit, 1): the blocks that share a ray group exchange their partial
+// line integrals through distributed shared memory.
+struct FwdLaunch {
+    cudaLaunchConfig_t cfg;
+    cudaLaunchAttribute attr[2];
+    FwdLaunch(const FwdPlan& p, cudaStream_t st, bool pdl = false) {
+        cfg = cudaLaunchConfig_t{};
+        cfg.gridDim = p.grid; cfg.blockDim = dim3(FWD_THREADS); cfg.dynamicSmemBytes = 0; cfg.stream = st;
+        attr[0].id = cudaLaunchAttributeClusterDimension;
+        attr[0].val.clusterDim.x = 1; attr[0].val.clusterDim.y = (unsigned)p.nsplit; attr[0].val.clusterDim.z = 1;
+        attr[1].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        attr[1].val.programmaticStreamSerializationAllowed = 1;
+        cfg.attrs = attr; cfg.numAttrs = pdl ? 2 : 1;
+    }
+};
+
+template <int MODE>
+cudaError_t launch_forward(const FwdPlan& p, const FwdArgs& a, cudaStream_t st, bool pdl) {
+    FwdLaunch L(p, st, pdl);
+    if (p.ns == 4) return cudaLaunchKernelEx(&L.cfg, k_forward<MODE, 4>, a);
+    return cudaLaunchKernelEx(&L.cfg, k_forward<MODE, 1>, a);
+}
+
+// can all clusters of the plan be resident at once?
+template <int MODE>
+bool forward_fits(const FwdPlan& p) {
+    FwdLaunch L(p, nullptr);
+    int n = 0;
+    const cudaError_t e = p.ns == 4 ? cudaOccupancyMaxActiveClusters(&n, k_forward<MODE, 4>, &L.cfg)
+                                    : cudaOccupancyMaxActiveClusters(&n, k_forward<MODE, 1>, &L.cfg);
+    if (e != cudaSuccess) { cudaGetLastError(); return false; }
+    return (long long)n * p.nsplit >= (long long)p.grid.x * p.grid.y * p.grid.z;
+}
+
 // K1: one block per (32 channels, base view, share of the line segments); the shares are sized so that the
 // whole grid is resident in one wave.
 FwdPlan plan_forward(const osiv_handle* h, int mode, int VS, int batch) {
@@ -178,6 +211,11 @@ FwdPlan plan_forward(const osiv_handle* h, int mode, int VS, int batch) {
     ns = std::min<long long>(ns, std::max(1, nmax / (FWD_SEGS * 4)));      // keep >= 4 image lines per warp
     p.nsplit = (int)std::max<long long>(1, std::min<long long>(ns, FWD_MAX_SPLIT));
     p.grid = dim3(cg, vb * p.nsplit, batch);
+    // clusters are placed whole inside one GPC: step down until every cluster is resident in the first wave
+    while (p.nsplit > 1 && !(mode ? forward_fits<1>(p) : forward_fits<0>(p))) {
+        --p.nsplit;
+        p.grid = dim3(cg, vb * p.nsplit, batch);
+    }
     return p;
 }
 
@@ -205,27 +243,20 @@ BackPlan plan_back(const osiv_handle* h, int VS, int batch) {
 }
 
 template <int MODE>
-void launch_forward(const FwdPlan& p, const FwdArgs& a, cudaStream_t st) {
-    if (p.ns == 4) k_forward<MODE, 4><<<p.grid, FWD_THREADS, 0, st>>>(a);
-    else           k_forward<MODE, 1><<<p.grid, FWD_THREADS, 0, st>>>(a);
+cudaError_t launch_back(const BackPlan& p, const BackArgs& a, cudaStream_t st, bool pdl) {
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = p.grid; cfg.blockDim = dim3(32 * p.nsplit); cfg.stream = st;
+    cfg.dynamicSmemBytes = (size_t)p.nsplit * p.ns * 4 * 32 * sizeof(float);
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr; cfg.numAttrs = pdl ? 1 : 0;
+    if (p.ns == 4) return cudaLaunchKernelEx(&cfg, k_back<MODE, 4>, a);
+    return cudaLaunchKernelEx(&cfg, k_back<MODE, 1>, a);
 }
 
-template <int MODE>
-void launch_back(const BackPlan& p, const BackArgs& a, cudaStream_t st) {
-    if (p.ns == 4) k_back<MODE, 4><<<p.grid, 32 * p.nsplit, (size_t)p.nsplit * 16 * 32 * sizeof(float), st>>>(a);
-    else           k_back<MODE, 1><<<p.grid, 32 * p.nsplit, (size_t)p.nsplit * 4 * 32 * sizeof(float), st>>>(a);
-}
-
-int ensure_forward_ws(osiv_handle* h, const FwdPlan& p, int batch, cudaStream_t st) {
-    int rc;
-    if (p.nsplit > 1 &&
-        (rc = grow(&h->d_fpart, &h->fpart_elems, (size_t)batch * p.groups * p.nsplit * p.ns * 32)) != OSIV_OK) return rc;
-    const size_t nt = (size_t)batch * p.groups;
-    if (h->ticket_elems < nt || !h->d_tickets) {
-        if ((rc = grow(&h->d_tickets, &h->ticket_elems, nt)) != OSIV_OK) return rc;
-        OSIV_CUDA(cudaMemsetAsync(h->d_tickets, 0, h->ticket_elems * sizeof(unsigned int), st));
-    }
-    return grow(&h->d_dparts, &h->dpart_elems, nt);
+int ensure_forward_ws(osiv_handle* h, const FwdPlan& p, int batch) {
+    return grow(&h->d_dparts, &h->dpart_elems, (size_t)batch * p.groups);
 }
 
 // residual buffer [batch][V_S][Cp] floats (NS == 4: [batch][V_S/4][Cp] float4); columns C..Cp-1 must be zero, and they
@@ -371,7 +402,7 @@ int osiv_destroy(osiv_handle* h) {
     if (guard.ok) {
         cudaDeviceSynchronize();
         void* ptrs[] = {h->d_rays, h->d_views, h->d_imgA, h->d_imgB, h->d_imgTA, h->d_imgTB, h->d_best, h->d_res,
-                        h->d_fpart, h->d_tickets, h->d_dparts, h->d_state, h->d_not_finite, h->d_inv_bref, h->d_trace,
+                        h->d_dparts, h->d_state, h->d_not_finite, h->d_inv_bref, h->d_trace,
                         h->d_forced, h->d_hcounts, h->d_hblank, h->d_himg};
         for (void* p : ptrs) if (p) cudaFree(p);
         for (cudaEvent_t e : h->events) cudaEventDestroy(e);
@@ -401,6 +432,12 @@ int64_t osiv_launch_count(const osiv_handle* h) { return h ? h->launches : 0; }
 int osiv_set_symmetry(osiv_handle* h, int32_t enable) {
     if (!h) return OSIV_ERR_INVALID_ARG;
     h->force_ns1 = enable ? 0 : 1;
+    return OSIV_OK;
+}
+
+int osiv_set_overlap(osiv_handle* h, int32_t enable) {
+    if (!h) return OSIV_ERR_INVALID_ARG;
+    h->use_pdl = enable ? 1 : 0;
     return OSIV_OK;
 }
 
@@ -442,14 +479,13 @@ int osiv_forward(osiv_handle* h, const float* d_img, float* d_sino, int32_t batc
     if (rc != OSIV_OK) return rc;
     const int VS = subset_views(h, subset, n_subsets);
     const FwdPlan p = plan_forward(h, 0, VS, batch);
-    if ((rc = ensure_forward_ws(h, p, batch, st)) != OSIV_OK) return rc;
+    if ((rc = ensure_forward_ws(h, p, batch)) != OSIV_OK) return rc;
     k_pad_transpose<<<dim3((h->geom.nx + 31) / 32, (h->geom.ny + 31) / 32, batch), 256, 0, st>>>(h->dg, d_img, h->d_imgA,
                                                                                              h->d_imgTA);
     FwdArgs a{};
     a.g = h->dg; a.img = h->d_imgA; a.imgT = h->d_imgTA;
     a.subset = subset; a.M = subset < 0 ? 1 : n_subsets; a.VS = VS; a.nsplit = p.nsplit; a.sino = d_sino;
-    a.fpart = h->d_fpart; a.tickets = h->d_tickets;
-    launch_forward<0>(p, a, st);
+    launch_forward<0>(p, a, st, false);
     return launch_check(h, 2);
 }
 
@@ -469,7 +505,7 @@ int osiv_backward(osiv_handle* h, const float* d_sino, float* d_img, int32_t bat
                                                                                     p.ns, Cp);
     BackArgs b{};
     b.g = h->dg; b.res = h->d_res; b.Cp = Cp; b.subset = subset; b.M = M; b.VS = VS; b.out = d_img;
-    launch_back<0>(p, b, st);
+    launch_back<0>(p, b, st, false);
     return launch_check(h, 2);
 }
 
@@ -507,7 +543,7 @@ int osiv_reconstruct(osiv_handle* h, const float* d_counts, const float* d_blank
     const BackPlan bp = plan_back(h, VS, batch);
     if ((rc = ensure_res(h, VS, fp.ns, batch, st)) != OSIV_OK) return rc;
     const int Cp = C + h->res_pad;
-    if ((rc = ensure_forward_ws(h, fp, batch, st)) != OSIV_OK) return rc;
+    if ((rc = ensure_forward_ws(h, fp, batch)) != OSIV_OK) return rc;
     if (h_trace && N > 0 && (rc = grow(&h->d_trace, &h->trace_elems, (size_t)batch * N * 2)) != OSIV_OK) return rc;
     if (prm->forced_lambda && N > 0) {
         if ((rc = grow(&h->d_forced, &h->forced_elems, (size_t)N)) != OSIV_OK) return rc;
@@ -525,7 +561,7 @@ int osiv_reconstruct(osiv_handle* h, const float* d_counts, const float* d_blank
     FwdArgs f{};
     f.g = h->dg; f.M = M; f.VS = VS; f.nsplit = fp.nsplit;
     f.counts = d_counts; f.blank = d_blank; f.blank_scalar = blank_scalar; f.inv_bref = h->d_inv_bref;
-    f.res = h->d_res; f.Cp = Cp; f.fpart = h->d_fpart; f.tickets = h->d_tickets; f.dparts = h->d_dparts;
+    f.res = h->d_res; f.Cp = Cp; f.dparts = h->d_dparts;
     BackArgs b{};
     b.g = h->dg; b.res = h->d_res; b.Cp = Cp; b.M = M; b.VS = VS; b.best = best;
     b.dparts = h->d_dparts; b.nparts = fp.groups; b.not_finite = h->d_not_finite;
@@ -537,6 +573,7 @@ int osiv_reconstruct(osiv_handle* h, const float* d_counts, const float* d_blank
 
     float *cur = h->d_imgA, *curT = h->d_imgTA, *nxt = h->d_imgB, *nxtT = h->d_imgTB;
     const bool prof = h->profiling && N > 0;
+    const bool pdl = h->use_pdl != 0;
     if (prof) {
         while (h->events.size() < (size_t)2 * N + 1) {
             cudaEvent_t e;
@@ -548,11 +585,11 @@ int osiv_reconstruct(osiv_handle* h, const float* d_counts, const float* d_blank
     for (int n = 0; n < N; ++n) {
         const int m = n % M;                               // PAPER.md:118, C11
         f.img = cur; f.imgT = curT; f.subset = m;
-        launch_forward<1>(fp, f, st);
+        launch_forward<1>(fp, f, st, pdl);
         if (prof) cudaEventRecord(h->events[2 * n + 1], st);
         b.img = cur; b.img_new = nxt; b.imgT_new = nxtT; b.subset = m;
         b.state_in = state[n & 1]; b.state_out = state[(n + 1) & 1];
-        launch_back<1>(bp, b, st);
+        launch_back<1>(bp, b, st, pdl);
         if (prof) cudaEventRecord(h->events[2 * n + 2], st);
         float* t;
         t = cur; cur = nxt; nxt = t;
@@ -573,7 +610,7 @@ int osiv_reconstruct(osiv_handle* h, const float* d_counts, const float* d_blank
     if (prm->return_best) {
         // the final iterate competes too, judged on the subset that would come next (C12)
         f.img = cur; f.imgT = curT; f.subset = N % M;
-        launch_forward<1>(fp, f, st);
+        launch_forward<1>(fp, f, st, false);
         k_final_monitor<<<batch, 32, 0, st>>>(h->d_dparts, fp.groups, fin, h->d_not_finite);
         h->launches += 2;
     }

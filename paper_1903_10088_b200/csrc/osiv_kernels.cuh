@@ -36,7 +36,13 @@ constexpr int PAD = 4;                     // zero columns left and right of eve
 constexpr int PADR = 1;                    // zero rows above and below a padded image
 constexpr int FWD_SEGS = 8;                // warps per K1 block; each owns one segment of the rays' image lines
 constexpr int FWD_THREADS = 32 * FWD_SEGS;
-constexpr int FWD_MAX_SPLIT = 8;           // K1 blocks that share one ray group (partial sums through global memory)
+#ifndef OSIV_PDL_LATE
+#define OSIV_PDL_LATE 0                    // 1: release the next launch after the main loop instead of right after the wait
+#endif
+#ifndef OSIV_FWD_MIN_BLOCKS
+#define OSIV_FWD_MIN_BLOCKS 5              // K1 blocks per SM the register allocation aims at (5 -> 48 registers)
+#endif
+constexpr int FWD_MAX_SPLIT = 8;           // K1 blocks that share one ray group = one thread-block cluster (portable size limit)
 constexpr int BK_TX = 2, BK_TY = 2;        // pixels per thread in the backprojector
 constexpr int BK_WX = 8, BK_WY = 4;        // tiles per warp: a warp covers 16 x 8 pixels
 constexpr int BK_MAX_SPLIT = 16;           // K2 warps per block; each owns a share of the subset's views
@@ -75,7 +81,7 @@ struct FwdArgs {
     const float* img;                      // padded mu, slice stride g.img_elems
     const float* imgT;                     // padded transpose, slice stride g.imgT_elems
     int subset, M, VS;
-    int nsplit;                            // blocks per ray group (segments of the rays' lines)
+    int nsplit;                            // blocks per ray group = cluster size (1, nsplit, 1); each owns a share of the lines
     float* sino;                           // MODE 0: [batch][VS][C]
     const float* counts;                   // MODE 1: [batch][V][C]
     const float* blank;                    // [C] or null
@@ -84,8 +90,6 @@ struct FwdArgs {
     float* res;                            // MODE 1: h * r; NS == 1: [batch][VS][Cp] floats, NS == 4: [batch][VS/4][Cp] float4
                                            // holding the orbit {j, j+VS/4, j+VS/2, j+3VS/4}; columns C..Cp-1 stay zero
     int Cp;
-    float* fpart;                          // [batch][groups][nsplit][NS][32] line-integral partial sums (nsplit > 1)
-    unsigned int* tickets;                 // [batch][groups], zero between launches
     double* dparts;                        // MODE 1: [batch][groups] partial sums of D
 };
 
@@ -116,28 +120,72 @@ __device__ __forceinline__ size_t padT_off(const DevGeom& g, int ix, int iy) {
     return (size_t)(ix + PADR) * g.pitchT + PAD + iy;
 }
 
+// ---- programmatic dependent launch: both hot kernels are launched while their predecessor in the stream still runs;
+// everything above pdl_wait() touches only constants (geometry tables, indices), pdl_wait() returns once the
+// predecessor has completed and its writes are visible, and pdl_launch_next() -- placed AFTER the wait, so that at
+// most one successor is ever resident early -- lets the successor's blocks move into the SM slots this grid frees.
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void pdl_launch_next() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+
+// ---- thread-block-cluster plumbing for K1 (raw PTX: the cooperative-groups cluster.sync() and every
+// barrier.cluster.wait carry a CCTL.IVALL that empties the SM's L1 under the co-resident blocks) ----
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ uint32_t cluster_map(uint32_t addr, uint32_t rank) {
+    uint32_t r;
+    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(addr), "r"(rank));
+    return r;
+}
+__device__ __forceinline__ void mbar_init_expect(uint64_t* mbar, uint32_t tx_bytes) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(smem_u32(mbar)) : "memory");
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(mbar)), "r"(tx_bytes) : "memory");
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+__device__ __forceinline__ void cluster_arrive() { asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory"); }
+__device__ __forceinline__ void cluster_wait() { asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory"); }
+// remote shared-memory store whose arrival is counted by the destination block's mbarrier (no fence, no L1 flush)
+__device__ __forceinline__ void st_async_f32(uint32_t remote_addr, float v, uint32_t remote_mbar) {
+    asm volatile("st.async.shared::cluster.mbarrier::complete_tx::bytes.b32 [%0], %1, [%2];" ::"r"(remote_addr),
+                 "r"(__float_as_uint(v)), "r"(remote_mbar) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* mbar, uint32_t parity) {
+    uint32_t done = 0;
+    while (!done)
+        asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2; selp.u32 %0, 1, 0, p; }"
+                     : "=r"(done) : "r"(smem_u32(mbar)), "r"(parity) : "memory");
+}
+
 // ------------------------------------------------------------------------------------------------
 // K1: forward projection (+ residual and monitor partials when MODE == 1).
-// grid (ceil(C/32), base views * nsplit, batch), block 32 x FWD_SEGS: lane = channel, warp = segment of the
-// ray's image lines, blockIdx.y % nsplit = which share of the segments.  A ray marches over the image lines
+// grid (ceil(C/32), base views * nsplit, batch), block 32 x FWD_SEGS, cluster (1, nsplit, 1): lane = channel,
+// warp = segment of the ray's image lines, blockIdx.y % nsplit = rank in the cluster = which share of the segments.
+// The cluster's partial line integrals meet in the shared memory of its rank-0 block (st.async + mbarrier over
+// DSMEM, summed in a fixed order), which then runs the per-ray epilogue.  A ray marches over the image lines
 // of its major axis (rows of img when |dy| >= |dx|, else rows of the transposed copy imgT) and touches at
 // most two adjacent pixels per line.  With NS == 4 the same two weights also serve the three rotated rays.
 // ------------------------------------------------------------------------------------------------
 template <int MODE, int NS>
-__global__ void __launch_bounds__(FWD_THREADS) k_forward(const FwdArgs a) {
+__global__ void __launch_bounds__(FWD_THREADS, OSIV_FWD_MIN_BLOCKS) k_forward(const FwdArgs a) {
     const DevGeom& g = a.g;
     const int lane = threadIdx.x & 31, seg = threadIdx.x >> 5;
     const int c = blockIdx.x * 32 + lane, s = blockIdx.z;
     const int jb = blockIdx.y / a.nsplit, split = blockIdx.y - jb * a.nsplit;
     const int v = a.subset < 0 ? jb : a.subset + jb * a.M;          // base view of the orbit
     __shared__ float part[FWD_SEGS][NS][32];
-    __shared__ unsigned int s_ticket;
+    __shared__ float cpart[FWD_MAX_SPLIT][NS][32];        // rank 0: the other ranks' sums (cpart[0] unused)
+    __shared__ __align__(8) uint64_t mbar;
+    if (a.nsplit > 1) {
+        // rank 0 arms its mbarrier for the bytes the other ranks will send; the cluster barrier makes that (and the
+        // fact that rank 0 is running) visible before anybody can send
+        if (split == 0 && threadIdx.x == 0) mbar_init_expect(&mbar, (uint32_t)((a.nsplit - 1) * NS * 32 * sizeof(float)));
+        cluster_arrive();
+    }
 
     float acc[NS];
 #pragma unroll
     for (int k = 0; k < NS; ++k) acc[k] = 0.f;
     // lanes past the last channel walk a copy of the last ray (keeps the warp convergent) and store nothing
     const float4 ray = __ldg(&g.rays[(size_t)v * g.C + min(c, g.C - 1)]);
+    if (a.nsplit > 1) cluster_wait();
     const bool rowmaj = fabsf(ray.x) >= fabsf(ray.y);
     {
         const float kk = rowmaj ? ray.x : ray.y;          // coefficient of the in-line coordinate, |kk| >= 1
@@ -166,6 +214,10 @@ __global__ void __launch_bounds__(FWD_THREADS) k_forward(const FwdArgs a) {
         const int chi = __reduce_max_sync(0xffffffffu, rowmaj ? -big : (int)fhi);
         const int wlo = rowmaj ? rlo : clo, whi = rowmaj ? rhi : chi;
         const int nsteps = whi - wlo + 1;
+        pdl_wait();                                          // mu(n) is the previous launch's output
+#if !OSIV_PDL_LATE
+        pdl_launch_next();
+#endif
         if (nsteps > 0) {
             const int nsegt = FWD_SEGS * a.nsplit;
             const int len = (nsteps + nsegt - 1) / nsegt;
@@ -175,35 +227,70 @@ __global__ void __launch_bounds__(FWD_THREADS) k_forward(const FwdArgs a) {
             int offP = (j0 + PADR) * pitch + PAD;                 // line j, walking up
             int offM = (nb - 1 - j0 + PADR) * pitch + PAD;        // line nb-1-j, walking down
             float bf = (float)j0 - cb;
-#pragma unroll 2
-            for (int jj = j0; jj < j1; ++jj, offP += pitch, offM -= pitch, bf += 1.f) {
-                const float bg = fmaf(uu, bf, ray.z);
-                const float fa = floorf(fmaf(-bg, invk, ca));     // index of the pixel left of the crossing
-                const float q0 = fmaf(kk, fa - ca, bg);
-                const float q1 = q0 + kk;
-                const float w0 = __saturatef(hk - fabsf(q0));
-                const float w1 = __saturatef(hk - fabsf(q1));
-                const int i0 = min(max((int)fa, -PAD), imax);
-                const float* p0 = bufA + (offP + i0);
-                acc[0] = fmaf(w0, __ldg(p0), acc[0]);
-                acc[0] = fmaf(w1, __ldg(p0 + 1), acc[0]);
-                if (NS == 4) {
-                    const int ir = na - 2 - i0;                   // mirrored index of pixel i0+1
-                    const float* p1 = bufB + (offM + i0);         // pattern 1: other copy, line nb-1-j, same order
-                    const float* p2 = bufA + (offM + ir);         // pattern 2: same copy, line nb-1-j, mirrored
-                    const float* p3 = bufB + (offP + ir);         // pattern 3: other copy, line j, mirrored
-                    acc[1] = fmaf(w0, __ldg(p1), acc[1]);
-                    acc[1] = fmaf(w1, __ldg(p1 + 1), acc[1]);
-                    acc[2] = fmaf(w1, __ldg(p2), acc[2]);
-                    acc[2] = fmaf(w0, __ldg(p2 + 1), acc[2]);
-                    acc[3] = fmaf(w1, __ldg(p3), acc[3]);
-                    acc[3] = fmaf(w0, __ldg(p3 + 1), acc[3]);
+            // Two lines per trip, written so that all 2 x 2 x NS gathers of a trip are in flight together: the walk
+            // is bound by load latency, not by issue.  The odd line past j1 (only in the last trip) gets zero weights;
+            // its addresses stay inside the padded buffers because j1 <= nb.
+            for (int jj = j0; jj < j1; jj += 2, offP += 2 * pitch, offM -= 2 * pitch, bf += 2.f) {
+                float w[2][2];
+                int i0[2];
+#pragma unroll
+                for (int u = 0; u < 2; ++u) {
+                    const float bg = fmaf(uu, bf + (float)u, ray.z);
+                    const float fa = floorf(fmaf(-bg, invk, ca)); // index of the pixel left of the crossing
+                    const float q0 = fmaf(kk, fa - ca, bg);
+                    const float q1 = q0 + kk;
+                    w[u][0] = __saturatef(hk - fabsf(q0));
+                    w[u][1] = __saturatef(hk - fabsf(q1));
+                    i0[u] = min(max((int)fa, -PAD), imax);
+                }
+                if (jj + 1 >= j1) { w[1][0] = 0.f; w[1][1] = 0.f; }
+                float x[2][NS][2];
+#pragma unroll
+                for (int u = 0; u < 2; ++u) {
+                    const int oP = offP + u * pitch, oM = offM - u * pitch;
+                    const float* p0 = bufA + (oP + i0[u]);
+                    x[u][0][0] = __ldg(p0); x[u][0][1] = __ldg(p0 + 1);
+                    if (NS == 4) {
+                        const int ir = na - 2 - i0[u];            // mirrored index of pixel i0+1
+                        const float* p1 = bufB + (oM + i0[u]);    // pattern 1: other copy, line nb-1-j, same order
+                        const float* p2 = bufA + (oM + ir);       // pattern 2: same copy, line nb-1-j, mirrored
+                        const float* p3 = bufB + (oP + ir);       // pattern 3: other copy, line j, mirrored
+                        x[u][1 % NS][0] = __ldg(p1); x[u][1 % NS][1] = __ldg(p1 + 1);
+                        x[u][2 % NS][0] = __ldg(p2); x[u][2 % NS][1] = __ldg(p2 + 1);
+                        x[u][3 % NS][0] = __ldg(p3); x[u][3 % NS][1] = __ldg(p3 + 1);
+                    }
+                }
+#pragma unroll
+                for (int u = 0; u < 2; ++u) {
+                    acc[0] = fmaf(w[u][0], x[u][0][0], acc[0]);
+                    acc[0] = fmaf(w[u][1], x[u][0][1], acc[0]);
+                    if (NS == 4) {
+                        acc[1] = fmaf(w[u][0], x[u][1 % NS][0], acc[1]);
+                        acc[1] = fmaf(w[u][1], x[u][1 % NS][1], acc[1]);
+                        acc[2 % NS] = fmaf(w[u][1], x[u][2 % NS][0], acc[2 % NS]);
+                        acc[2 % NS] = fmaf(w[u][0], x[u][2 % NS][1], acc[2 % NS]);
+                        acc[3 % NS] = fmaf(w[u][1], x[u][3 % NS][0], acc[3 % NS]);
+                        acc[3 % NS] = fmaf(w[u][0], x[u][3 % NS][1], acc[3 % NS]);
+                    }
                 }
             }
         }
     }
+#if OSIV_PDL_LATE
+    pdl_launch_next();
+#endif
 #pragma unroll
     for (int k = 0; k < NS; ++k) part[seg][k][lane] = acc[k];
+    // the epilogue's inputs are requested before the barrier so that they arrive while the block drains
+    const int VSb = a.VS / NS, Vq = g.V / NS;
+    const bool epi = MODE == 1 && seg == 0 && split == 0 && c < g.C;
+    float yk[NS] = {}, bl = a.blank_scalar, ib = 0.f;
+    if (epi) {
+#pragma unroll
+        for (int k = 0; k < NS; ++k) yk[k] = __ldg(&a.counts[((size_t)s * g.V + v + k * Vq) * g.C + c]);
+        if (a.blank) bl = __ldg(&a.blank[c]);
+        ib = __ldg(a.inv_bref);
+    }
     __syncthreads();
     if (seg != 0) return;
 
@@ -222,42 +309,33 @@ __global__ void __launch_bounds__(FWD_THREADS) k_forward(const FwdArgs a) {
     const int groups = gridDim.x * (gridDim.y / a.nsplit);
     const int grp = jb * gridDim.x + blockIdx.x;
     if (a.nsplit > 1) {
-        float* fp = a.fpart + (((size_t)s * groups + grp) * a.nsplit) * (NS * 32);
+        if (split != 0) {
+            const uint32_t rmbar = cluster_map(smem_u32(&mbar), 0);
 #pragma unroll
-        for (int k = 0; k < NS; ++k) __stcg(&fp[(split * NS + k) * 32 + lane], t[k]);
-        __threadfence();
-        __syncwarp();
-        if (lane == 0) s_ticket = atomicAdd(&a.tickets[(size_t)s * groups + grp], 1u);
-        __syncwarp();
-        if (s_ticket != (unsigned)(a.nsplit - 1)) return;
-        __threadfence();
-        if (lane == 0) a.tickets[(size_t)s * groups + grp] = 0u;
-#pragma unroll
-        for (int k = 0; k < NS; ++k) {
-            float x = 0.f;
-            for (int q = 0; q < a.nsplit; ++q) x += __ldcg(&fp[(q * NS + k) * 32 + lane]);   // fixed order
-            t[k] = x;
+            for (int k = 0; k < NS; ++k) st_async_f32(cluster_map(smem_u32(&cpart[split][k][lane]), 0), t[k], rmbar);
+            return;
         }
+        mbar_wait(&mbar, 0);
+#pragma unroll
+        for (int k = 0; k < NS; ++k)
+            for (int q = 1; q < a.nsplit; ++q) t[k] += cpart[q][k][lane];          // fixed order
     }
 
-    const int VSb = a.VS / NS, Vq = g.V / NS;
     double d2 = 0.0;
     float hr[NS];
 #pragma unroll
     for (int k = 0; k < NS; ++k) {
         const float l = ray.w * t[k];
         const int jk = jb + k * VSb;                     // compact view index inside the subset
-        const int vk = v + k * Vq;
         hr[k] = 0.f;
         if (c < g.C) {
             if (MODE == 0) {
                 a.sino[((size_t)s * a.VS + jk) * g.C + c] = l;
             } else {
                 // A2: Poisson residual r = (b exp(-l) - y)/b_ref and monitor term (l - ln(b/max(y,1)))^2
-                const float y = __ldg(&a.counts[((size_t)s * g.V + vk) * g.C + c]);
-                const float b = a.blank ? __ldg(&a.blank[c]) : a.blank_scalar;
+                const float y = yk[k], b = bl;
                 const float ybar = b * expf(-l);
-                const float r = (ybar - y) * __ldg(a.inv_bref);
+                const float r = (ybar - y) * ib;
                 hr[k] = ray.w * r;
                 const float p = logf(b / fmaxf(y, 1.f));
                 const double d = (double)l - (double)p;
@@ -427,6 +505,10 @@ __global__ void __launch_bounds__(BK_MAX_THREADS) k_back(const BackArgs a) {
         const float xc0 = (float)x0 - g.cx, yc0 = (float)y0 - g.cy;
         const float X = (xc0 + 0.5f * (BK_TX - 1)) * g.pixel, Y = (yc0 + 0.5f * (BK_TY - 1)) * g.pixel;
         const float* res = a.res + (size_t)s * a.VS * a.Cp;      // same float count for both layouts
+        pdl_wait();                                              // the residuals are the previous launch's output
+#if !OSIV_PDL_LATE
+        pdl_launch_next();
+#endif
         for (int jb = jfirst; jb < VSb; jb += jstep) {
             const int jj = jb + quarter * VSb;
             const int v = a.subset < 0 ? jj : a.subset + jj * a.M;
@@ -488,23 +570,41 @@ __global__ void __launch_bounds__(BK_MAX_THREADS) k_back(const BackArgs a) {
             }
         }
     }
+#if OSIV_PDL_LATE
+    pdl_launch_next();
+#endif
     // rotation k of the tile = orbit component (quarter + k) % 4  <=>  component m feeds rotation (m - quarter) % 4
 #pragma unroll
     for (int m = 0; m < NS; ++m)
 #pragma unroll
         for (int p = 0; p < 4; ++p) red[warp][((m - quarter) & (NS - 1)) * 4 + p][lane] = acc[m][p];
-    __syncthreads();
-    if (warp >= NS) return;
 
+    // warp k < NS finishes rotation k of the base tile: origin (xk, yk) and, below, where base pixel (tx,ty) lands.
+    // Everything that does not depend on the other warps' sums -- monitor, step rule, neighbourhood of mu(n), TV
+    // gradient -- is done before the barrier, so that its loads overlap the wait for the slowest warp.
+    const bool fin = warp < NS;
+    const int k = warp;
+    int xk = x0, yk = y0;
+    if (NS == 4) {
+        const int N = g.nx;
+        if (k == 1)      { xk = N - 2 - y0; yk = x0; }
+        else if (k == 2) { xk = N - 2 - x0; yk = N - 2 - y0; }
+        else if (k == 3) { xk = y0;         yk = N - 2 - x0; }
+    }
     StepInfo si;
     float step = 0.f;
-    if (MODE == 1) {
-        si = step_rule(a, s, lane, blockIdx.x == 0 && blockIdx.y == 0 && warp == 0);
+    float m[4][4], tv[2][2];
+    if (MODE == 1 && fin) {
+        const bool writer = blockIdx.x == 0 && blockIdx.y == 0 && warp == 0;
+        if (active) load_nbhd(g, a.img + (size_t)s * g.img_elems, xk, yk, m);
+        si = step_rule(a, s, lane, writer);
         step = (float)(si.lambda * a.tau);
+        if (active) tv_grad_tile(m, xk, yk, g.nx, g.ny, a.eps2, tv);
     }
-    if (!active) return;
+    __syncthreads();
+    if (!fin || !active) return;
 
-    for (int k = warp; k < NS; k += nsplit) {
+    {
         // sums over the view shares, fixed order
         float b[4];
 #pragma unroll
@@ -513,14 +613,11 @@ __global__ void __launch_bounds__(BK_MAX_THREADS) k_back(const BackArgs a) {
             for (int q = 0; q < nsplit; ++q) x += red[q][k * 4 + p][lane];
             b[p] = x;
         }
-        // rotation k of the base tile: origin and where base pixel (tx,ty) lands, o[ty'][tx']
-        int xk = x0, yk = y0;
         float o00 = b[0], o01 = b[1], o10 = b[2], o11 = b[3];
         if (NS == 4) {
-            const int N = g.nx;
-            if (k == 1)      { xk = N - 2 - y0; yk = x0;         o00 = b[2]; o01 = b[0]; o10 = b[3]; o11 = b[1]; }
-            else if (k == 2) { xk = N - 2 - x0; yk = N - 2 - y0; o00 = b[3]; o01 = b[2]; o10 = b[1]; o11 = b[0]; }
-            else if (k == 3) { xk = y0;         yk = N - 2 - x0; o00 = b[1]; o01 = b[3]; o10 = b[0]; o11 = b[2]; }
+            if (k == 1)      { o00 = b[2]; o01 = b[0]; o10 = b[3]; o11 = b[1]; }
+            else if (k == 2) { o00 = b[3]; o01 = b[2]; o10 = b[1]; o11 = b[0]; }
+            else if (k == 3) { o00 = b[1]; o01 = b[3]; o10 = b[0]; o11 = b[2]; }
         }
         const bool vx1 = xk + 1 < g.nx, vy1 = yk + 1 < g.ny;
         if (MODE == 0) {
@@ -529,14 +626,10 @@ __global__ void __launch_bounds__(BK_MAX_THREADS) k_back(const BackArgs a) {
             if (vx1) out[(size_t)yk * g.nx + xk + 1] = o01;
             if (vy1) out[(size_t)(yk + 1) * g.nx + xk] = o10;
             if (vx1 && vy1) out[(size_t)(yk + 1) * g.nx + xk + 1] = o11;
-            continue;
+            return;
         }
 
         // ---- A5 TV gradient of mu(n), A6 update (Eq. 3) with mu > 0, A7 best copy ----
-        const float* img = a.img + (size_t)s * g.img_elems;
-        float m[4][4], tv[2][2];
-        load_nbhd(g, img, xk, yk, m);
-        tv_grad_tile(m, xk, yk, g.nx, g.ny, a.eps2, tv);
         const float u00 = fmaxf(fmaf(step, o00 - a.beta_over_M * tv[0][0], m[1][1]), 0.f);
         const float u01 = fmaxf(fmaf(step, o01 - a.beta_over_M * tv[0][1], m[1][2]), 0.f);
         const float u10 = fmaxf(fmaf(step, o10 - a.beta_over_M * tv[1][0], m[2][1]), 0.f);
