@@ -34,7 +34,6 @@ struct osiv_handle {
     int* d_not_finite = nullptr;        // [max_batch]
     float* d_inv_bref = nullptr;
     int num_sms = 148;
-    int occ_fwd[2][2] = {{0, 0}, {0, 0}};   // resident K1 blocks per SM, [MODE][NS == 4]
     size_t trace_elems = 0;     double* d_trace = nullptr;
     size_t forced_elems = 0;    double* d_forced = nullptr;
     // staging for osiv_reconstruct_host
@@ -161,62 +160,35 @@ int ensure_images(osiv_handle* h, int batch, cudaStream_t st) {
 // made of whole orbits (V_S % 4 == 0); everything else takes the general NS = 1 kernels.
 int pick_ns(const osiv_handle* h, int VS) { return (h->dg.sym4 && !h->force_ns1 && VS % 4 == 0) ? 4 : 1; }
 
-struct FwdPlan { dim3 grid; int nsplit, groups, ns; };
+struct FwdPlan { int threads, rpb, segs, nparts, ns; size_t smem; };
 struct BackPlan { dim3 grid; int nsplit, ns; };
 
-// K1 runs as thread-block clusters (1, nsplit, 1): the blocks that share a ray group exchange their partial
-// line integrals through distributed shared memory.
-struct FwdLaunch {
-    cudaLaunchConfig_t cfg;
-    cudaLaunchAttribute attr[2];
-    FwdLaunch(const FwdPlan& p, cudaStream_t st, bool pdl = false) {
-        cfg = cudaLaunchConfig_t{};
-        cfg.gridDim = p.grid; cfg.blockDim = dim3(FWD_THREADS); cfg.dynamicSmemBytes = 0; cfg.stream = st;
-        attr[0].id = cudaLaunchAttributeClusterDimension;
-        attr[0].val.clusterDim.x = 1; attr[0].val.clusterDim.y = (unsigned)p.nsplit; attr[0].val.clusterDim.z = 1;
-        attr[1].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-        attr[1].val.programmaticStreamSerializationAllowed = 1;
-        cfg.attrs = attr; cfg.numAttrs = pdl ? 2 : 1;
-    }
-};
-
-template <int MODE>
-cudaError_t launch_forward(const FwdPlan& p, const FwdArgs& a, cudaStream_t st, bool pdl) {
-    FwdLaunch L(p, st, pdl);
-    if (p.ns == 4) return cudaLaunchKernelEx(&L.cfg, k_forward<MODE, 4>, a);
-    return cudaLaunchKernelEx(&L.cfg, k_forward<MODE, 1>, a);
-}
-
-// can all clusters of the plan be resident at once?
-template <int MODE>
-bool forward_fits(const FwdPlan& p) {
-    FwdLaunch L(p, nullptr);
-    int n = 0;
-    const cudaError_t e = p.ns == 4 ? cudaOccupancyMaxActiveClusters(&n, k_forward<MODE, 4>, &L.cfg)
-                                    : cudaOccupancyMaxActiveClusters(&n, k_forward<MODE, 1>, &L.cfg);
-    if (e != cudaSuccess) { cudaGetLastError(); return false; }
-    return (long long)n * p.nsplit >= (long long)p.grid.x * p.grid.y * p.grid.z;
-}
-
-// K1: one block per (32 channels, base view, share of the line segments); the shares are sized so that the
-// whole grid is resident in one wave.
-FwdPlan plan_forward(const osiv_handle* h, int mode, int VS, int batch) {
+// K1: the subset's base rays are dealt out in runs of rpb consecutive rays, one run per block and one block per SM
+// (per slice); a block is rpb rays x segs segments of each ray's line range, as many segments as fit into 1024
+// threads while a segment keeps at least FWD_MIN_LINES image lines.
+FwdPlan plan_forward(const osiv_handle* h, int VS) {
     FwdPlan p;
     p.ns = pick_ns(h, VS);
-    const int cg = (h->geom.n_channels + 31) / 32, vb = VS / p.ns;
-    p.groups = cg * vb;
-    const long long slots = (long long)h->num_sms * std::max(1, h->occ_fwd[mode][p.ns == 4]);
-    long long ns = slots / ((long long)p.groups * batch);
+    const long long R = (long long)(VS / p.ns) * h->geom.n_channels;
+    p.rpb = (int)std::min<long long>(FWD_MAX_THREADS, std::max<long long>(1, (R + h->num_sms - 1) / h->num_sms));
     const int nmax = std::max(h->geom.nx, h->geom.ny);
-    ns = std::min<long long>(ns, std::max(1, nmax / (FWD_SEGS * 4)));      // keep >= 4 image lines per warp
-    p.nsplit = (int)std::max<long long>(1, std::min<long long>(ns, FWD_MAX_SPLIT));
-    p.grid = dim3(cg, vb * p.nsplit, batch);
-    // clusters are placed whole inside one GPC: step down until every cluster is resident in the first wave
-    while (p.nsplit > 1 && !(mode ? forward_fits<1>(p) : forward_fits<0>(p))) {
-        --p.nsplit;
-        p.grid = dim3(cg, vb * p.nsplit, batch);
-    }
+    p.segs = std::max(1, std::min(FWD_MAX_THREADS / p.rpb, nmax / FWD_MIN_LINES));
+    p.threads = (p.rpb * p.segs + 31) / 32 * 32;
+    p.nparts = (int)((R + p.rpb - 1) / p.rpb);
+    p.smem = (size_t)p.segs * p.ns * p.rpb * sizeof(float);
     return p;
+}
+
+template <int MODE>
+cudaError_t launch_forward(FwdPlan p, int batch, const FwdArgs& a, cudaStream_t st, bool pdl) {
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = dim3(p.nparts, 1, batch); cfg.blockDim = dim3(p.threads); cfg.dynamicSmemBytes = p.smem; cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr; cfg.numAttrs = pdl ? 1 : 0;
+    if (p.ns == 4) return cudaLaunchKernelEx(&cfg, k_forward<MODE, 4>, a);
+    return cudaLaunchKernelEx(&cfg, k_forward<MODE, 1>, a);
 }
 
 // K2: one block per 16 x 8 pixel region of base tiles; its warps share the subset's views.
@@ -256,7 +228,7 @@ cudaError_t launch_back(const BackPlan& p, const BackArgs& a, cudaStream_t st, b
 }
 
 int ensure_forward_ws(osiv_handle* h, const FwdPlan& p, int batch) {
-    return grow(&h->d_dparts, &h->dpart_elems, (size_t)batch * p.groups);
+    return grow(&h->d_dparts, &h->dpart_elems, (size_t)batch * p.nparts);
 }
 
 // residual buffer [batch][V_S][Cp] floats (NS == 4: [batch][V_S/4][Cp] float4); columns C..Cp-1 must be zero, and they
@@ -365,11 +337,7 @@ int osiv_create(const osiv_geometry* geom, int32_t max_batch, int32_t device, os
         cudaMalloc((void**)&h->d_inv_bref, sizeof(float)) != cudaSuccess ||
         cudaMemcpy(h->d_rays, rays.data(), rays.size() * sizeof(float4), cudaMemcpyHostToDevice) != cudaSuccess ||
         cudaMemcpy(h->d_views, views.data(), views.size() * sizeof(float2), cudaMemcpyHostToDevice) != cudaSuccess ||
-        cudaDeviceGetAttribute(&h->num_sms, cudaDevAttrMultiProcessorCount, device) != cudaSuccess ||
-        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&h->occ_fwd[0][0], k_forward<0, 1>, FWD_THREADS, 0) != cudaSuccess ||
-        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&h->occ_fwd[0][1], k_forward<0, 4>, FWD_THREADS, 0) != cudaSuccess ||
-        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&h->occ_fwd[1][0], k_forward<1, 1>, FWD_THREADS, 0) != cudaSuccess ||
-        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&h->occ_fwd[1][1], k_forward<1, 4>, FWD_THREADS, 0) != cudaSuccess) {
+        cudaDeviceGetAttribute(&h->num_sms, cudaDevAttrMultiProcessorCount, device) != cudaSuccess) {
         cudaGetLastError();
         osiv_destroy(h);
         return OSIV_ERR_CUDA;
@@ -444,9 +412,9 @@ int osiv_set_overlap(osiv_handle* h, int32_t enable) {
 int osiv_get_plan(const osiv_handle* h, int32_t n_subsets, int32_t batch, int32_t* out8) {
     if (!h || !out8 || batch <= 0 || (n_subsets > 0 && h->geom.n_views % n_subsets != 0)) return OSIV_ERR_INVALID_ARG;
     const int VS = n_subsets > 0 ? h->geom.n_views / n_subsets : h->geom.n_views;
-    const FwdPlan f = plan_forward(h, 1, VS, batch);
+    const FwdPlan f = plan_forward(h, VS);
     const BackPlan b = plan_back(h, VS, batch);
-    out8[0] = f.ns; out8[1] = f.nsplit; out8[2] = (int)(f.grid.x * f.grid.y * f.grid.z); out8[3] = FWD_THREADS;
+    out8[0] = f.ns; out8[1] = f.segs; out8[2] = f.nparts * batch; out8[3] = f.threads;
     out8[4] = b.ns; out8[5] = b.nsplit; out8[6] = (int)(b.grid.x * b.grid.y * b.grid.z); out8[7] = 32 * b.nsplit;
     return OSIV_OK;
 }
@@ -478,14 +446,14 @@ int osiv_forward(osiv_handle* h, const float* d_img, float* d_sino, int32_t batc
     int rc = ensure_images(h, batch, st);
     if (rc != OSIV_OK) return rc;
     const int VS = subset_views(h, subset, n_subsets);
-    const FwdPlan p = plan_forward(h, 0, VS, batch);
+    const FwdPlan p = plan_forward(h, VS);
     if ((rc = ensure_forward_ws(h, p, batch)) != OSIV_OK) return rc;
     k_pad_transpose<<<dim3((h->geom.nx + 31) / 32, (h->geom.ny + 31) / 32, batch), 256, 0, st>>>(h->dg, d_img, h->d_imgA,
                                                                                              h->d_imgTA);
     FwdArgs a{};
     a.g = h->dg; a.img = h->d_imgA; a.imgT = h->d_imgTA;
-    a.subset = subset; a.M = subset < 0 ? 1 : n_subsets; a.VS = VS; a.nsplit = p.nsplit; a.sino = d_sino;
-    launch_forward<0>(p, a, st, false);
+    a.subset = subset; a.M = subset < 0 ? 1 : n_subsets; a.VS = VS; a.rpb = p.rpb; a.segs = p.segs; a.sino = d_sino;
+    launch_forward<0>(p, batch, a, st, false);
     return launch_check(h, 2);
 }
 
@@ -539,7 +507,7 @@ int osiv_reconstruct(osiv_handle* h, const float* d_counts, const float* d_blank
     const int VS = h->geom.n_views / M, C = h->geom.n_channels;
     int rc = ensure_images(h, batch, st);
     if (rc != OSIV_OK) return rc;
-    const FwdPlan fp = plan_forward(h, 1, VS, batch);
+    const FwdPlan fp = plan_forward(h, VS);
     const BackPlan bp = plan_back(h, VS, batch);
     if ((rc = ensure_res(h, VS, fp.ns, batch, st)) != OSIV_OK) return rc;
     const int Cp = C + h->res_pad;
@@ -559,12 +527,12 @@ int osiv_reconstruct(osiv_handle* h, const float* d_counts, const float* d_blank
     h->launches += 2;
 
     FwdArgs f{};
-    f.g = h->dg; f.M = M; f.VS = VS; f.nsplit = fp.nsplit;
+    f.g = h->dg; f.M = M; f.VS = VS; f.rpb = fp.rpb; f.segs = fp.segs;
     f.counts = d_counts; f.blank = d_blank; f.blank_scalar = blank_scalar; f.inv_bref = h->d_inv_bref;
     f.res = h->d_res; f.Cp = Cp; f.dparts = h->d_dparts;
     BackArgs b{};
     b.g = h->dg; b.res = h->d_res; b.Cp = Cp; b.M = M; b.VS = VS; b.best = best;
-    b.dparts = h->d_dparts; b.nparts = fp.groups; b.not_finite = h->d_not_finite;
+    b.dparts = h->d_dparts; b.nparts = fp.nparts; b.not_finite = h->d_not_finite;
     b.ip.lambda0 = prm->lambda0; b.ip.up = prm->lambda_up; b.ip.down = prm->lambda_down; b.ip.lmin = prm->lambda_min;
     b.ip.forced = (prm->forced_lambda && N > 0) ? h->d_forced : nullptr;
     b.ip.trace = (h_trace && N > 0) ? h->d_trace : nullptr;
@@ -585,7 +553,7 @@ int osiv_reconstruct(osiv_handle* h, const float* d_counts, const float* d_blank
     for (int n = 0; n < N; ++n) {
         const int m = n % M;                               // PAPER.md:118, C11
         f.img = cur; f.imgT = curT; f.subset = m;
-        launch_forward<1>(fp, f, st, pdl);
+        launch_forward<1>(fp, batch, f, st, pdl);
         if (prof) cudaEventRecord(h->events[2 * n + 1], st);
         b.img = cur; b.img_new = nxt; b.imgT_new = nxtT; b.subset = m;
         b.state_in = state[n & 1]; b.state_out = state[(n + 1) & 1];
@@ -610,8 +578,8 @@ int osiv_reconstruct(osiv_handle* h, const float* d_counts, const float* d_blank
     if (prm->return_best) {
         // the final iterate competes too, judged on the subset that would come next (C12)
         f.img = cur; f.imgT = curT; f.subset = N % M;
-        launch_forward<1>(fp, f, st, false);
-        k_final_monitor<<<batch, 32, 0, st>>>(h->d_dparts, fp.groups, fin, h->d_not_finite);
+        launch_forward<1>(fp, batch, f, st, false);
+        k_final_monitor<<<batch, 32, 0, st>>>(h->d_dparts, fp.nparts, fin, h->d_not_finite);
         h->launches += 2;
     }
     k_unpad<<<px_grid(h, batch), 256, 0, st>>>(h->dg, cur, best, fin, d_img_out);

@@ -34,15 +34,11 @@ namespace osiv {
 
 constexpr int PAD = 4;                     // zero columns left and right of every padded image line
 constexpr int PADR = 1;                    // zero rows above and below a padded image
-constexpr int FWD_SEGS = 8;                // warps per K1 block; each owns one segment of the rays' image lines
-constexpr int FWD_THREADS = 32 * FWD_SEGS;
+constexpr int FWD_MAX_THREADS = 1024;      // K1: one block per SM, threads = rays per block x line segments per ray
+constexpr int FWD_MIN_LINES = 8;           // K1: a segment is at least this many image lines
 #ifndef OSIV_PDL_LATE
 #define OSIV_PDL_LATE 0                    // 1: release the next launch after the main loop instead of right after the wait
 #endif
-#ifndef OSIV_FWD_MIN_BLOCKS
-#define OSIV_FWD_MIN_BLOCKS 5              // K1 blocks per SM the register allocation aims at (5 -> 48 registers)
-#endif
-constexpr int FWD_MAX_SPLIT = 8;           // K1 blocks that share one ray group = one thread-block cluster (portable size limit)
 constexpr int BK_TX = 2, BK_TY = 2;        // pixels per thread in the backprojector
 constexpr int BK_WX = 8, BK_WY = 4;        // tiles per warp: a warp covers 16 x 8 pixels
 constexpr int BK_MAX_SPLIT = 16;           // K2 warps per block; each owns a share of the subset's views
@@ -81,7 +77,7 @@ struct FwdArgs {
     const float* img;                      // padded mu, slice stride g.img_elems
     const float* imgT;                     // padded transpose, slice stride g.imgT_elems
     int subset, M, VS;
-    int nsplit;                            // blocks per ray group = cluster size (1, nsplit, 1); each owns a share of the lines
+    int rpb, segs;                         // rays per block, line segments per ray (block = rpb * segs threads, rounded up to warps)
     float* sino;                           // MODE 0: [batch][VS][C]
     const float* counts;                   // MODE 1: [batch][V][C]
     const float* blank;                    // [C] or null
@@ -90,7 +86,7 @@ struct FwdArgs {
     float* res;                            // MODE 1: h * r; NS == 1: [batch][VS][Cp] floats, NS == 4: [batch][VS/4][Cp] float4
                                            // holding the orbit {j, j+VS/4, j+VS/2, j+3VS/4}; columns C..Cp-1 stay zero
     int Cp;
-    double* dparts;                        // MODE 1: [batch][groups] partial sums of D
+    double* dparts;                        // MODE 1: [batch][gridDim.x] partial sums of D
 };
 
 struct BackArgs {
@@ -127,65 +123,38 @@ __device__ __forceinline__ size_t padT_off(const DevGeom& g, int ix, int iy) {
 __device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
 __device__ __forceinline__ void pdl_launch_next() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
 
-// ---- thread-block-cluster plumbing for K1 (raw PTX: the cooperative-groups cluster.sync() and every
-// barrier.cluster.wait carry a CCTL.IVALL that empties the SM's L1 under the co-resident blocks) ----
-__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ uint32_t cluster_map(uint32_t addr, uint32_t rank) {
-    uint32_t r;
-    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(addr), "r"(rank));
-    return r;
-}
-__device__ __forceinline__ void mbar_init_expect(uint64_t* mbar, uint32_t tx_bytes) {
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(smem_u32(mbar)) : "memory");
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(mbar)), "r"(tx_bytes) : "memory");
-    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-}
-__device__ __forceinline__ void cluster_arrive() { asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory"); }
-__device__ __forceinline__ void cluster_wait() { asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory"); }
-// remote shared-memory store whose arrival is counted by the destination block's mbarrier (no fence, no L1 flush)
-__device__ __forceinline__ void st_async_f32(uint32_t remote_addr, float v, uint32_t remote_mbar) {
-    asm volatile("st.async.shared::cluster.mbarrier::complete_tx::bytes.b32 [%0], %1, [%2];" ::"r"(remote_addr),
-                 "r"(__float_as_uint(v)), "r"(remote_mbar) : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint64_t* mbar, uint32_t parity) {
-    uint32_t done = 0;
-    while (!done)
-        asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2; selp.u32 %0, 1, 0, p; }"
-                     : "=r"(done) : "r"(smem_u32(mbar)), "r"(parity) : "memory");
-}
-
 // ------------------------------------------------------------------------------------------------
 // K1: forward projection (+ residual and monitor partials when MODE == 1).
-// grid (ceil(C/32), base views * nsplit, batch), block 32 x FWD_SEGS, cluster (1, nsplit, 1): lane = channel,
-// warp = segment of the ray's image lines, blockIdx.y % nsplit = rank in the cluster = which share of the segments.
-// The cluster's partial line integrals meet in the shared memory of its rank-0 block (st.async + mbarrier over
-// DSMEM, summed in a fixed order), which then runs the per-ray epilogue.  A ray marches over the image lines
-// of its major axis (rows of img when |dy| >= |dx|, else rows of the transposed copy imgT) and touches at
-// most two adjacent pixels per line.  With NS == 4 the same two weights also serve the three rotated rays.
+// One block per SM-sized share of the subset's base rays: the R = (V_S/NS) * C base rays are dealt out in runs of
+// `rpb` consecutive rays (view-major), and a block is rpb rays x `segs` segments of each ray's own image-line range
+// [flo, fhi]: thread t walks segment t / rpb of ray t % rpb.  Neighbouring threads are neighbouring channels on
+// the same line (the block walks the union of its rays' ranges in lock step), so a warp's gathers fall into one or two cache lines.  A ray marches over the image lines
+// of its major axis (rows of img when |dy| >= |dx|, else rows of the transposed copy imgT) and touches at most two
+// adjacent pixels per line; with NS == 4 the same two weights also serve the three rotated rays.  Every block has
+// the same amount of work and no block depends on another: the segment sums meet in shared memory in a fixed order
+// and the first rpb threads run the per-ray epilogue.  The host sizes the grid to one block per SM (fwd_plan).
 // ------------------------------------------------------------------------------------------------
 template <int MODE, int NS>
-__global__ void __launch_bounds__(FWD_THREADS, OSIV_FWD_MIN_BLOCKS) k_forward(const FwdArgs a) {
+__global__ void __launch_bounds__(FWD_MAX_THREADS, 1) k_forward(const FwdArgs a) {
     const DevGeom& g = a.g;
-    const int lane = threadIdx.x & 31, seg = threadIdx.x >> 5;
-    const int c = blockIdx.x * 32 + lane, s = blockIdx.z;
-    const int jb = blockIdx.y / a.nsplit, split = blockIdx.y - jb * a.nsplit;
+    const int t = threadIdx.x, s = blockIdx.z;
+    const int rpb = a.rpb, segs = a.segs;
+    const int seg = t / rpb, i = t - seg * rpb;
+    const int VSb = a.VS / NS, Vq = g.V / NS;
+    const int R = VSb * g.C;
+    const int r = blockIdx.x * rpb + i;
+    const bool walker = seg < segs && r < R;
+    const int rr = min(r, R - 1);
+    const int jb = rr / g.C, c = rr - jb * g.C;
     const int v = a.subset < 0 ? jb : a.subset + jb * a.M;          // base view of the orbit
-    __shared__ float part[FWD_SEGS][NS][32];
-    __shared__ float cpart[FWD_MAX_SPLIT][NS][32];        // rank 0: the other ranks' sums (cpart[0] unused)
-    __shared__ __align__(8) uint64_t mbar;
-    if (a.nsplit > 1) {
-        // rank 0 arms its mbarrier for the bytes the other ranks will send; the cluster barrier makes that (and the
-        // fact that rank 0 is running) visible before anybody can send
-        if (split == 0 && threadIdx.x == 0) mbar_init_expect(&mbar, (uint32_t)((a.nsplit - 1) * NS * 32 * sizeof(float)));
-        cluster_arrive();
-    }
+    extern __shared__ float part[];                                 // [segs][NS][rpb]
+    __shared__ double dred[FWD_MAX_THREADS / 32];
+    __shared__ int rng[4];                                          // line ranges of the block's row- / column-major rays
 
     float acc[NS];
 #pragma unroll
     for (int k = 0; k < NS; ++k) acc[k] = 0.f;
-    // lanes past the last channel walk a copy of the last ray (keeps the warp convergent) and store nothing
-    const float4 ray = __ldg(&g.rays[(size_t)v * g.C + min(c, g.C - 1)]);
-    if (a.nsplit > 1) cluster_wait();
+    const float4 ray = __ldg(&g.rays[(size_t)v * g.C + c]);
     const bool rowmaj = fabsf(ray.x) >= fabsf(ray.y);
     {
         const float kk = rowmaj ? ray.x : ray.y;          // coefficient of the in-line coordinate, |kk| >= 1
@@ -200,158 +169,145 @@ __global__ void __launch_bounds__(FWD_THREADS, OSIV_FWD_MIN_BLOCKS) k_forward(co
         // lines where the crossing lies within half a pixel of the image: |uu*b + g0| < |kk|*(na/2 + 1/2)
         const float A = fabsf(kk) * (0.5f * na + 0.5f);
         const float b1 = uu * (-ray.z - A), b2 = uu * (-ray.z + A);
-        const float flo = fminf(fmaxf(ceilf(fminf(b1, b2) + cb) - 1.f, 0.f), (float)nb);
-        const float fhi = fminf(fmaxf(floorf(fmaxf(b1, b2) + cb) + 1.f, -1.f), (float)(nb - 1));
-        // The warp walks the union of its rays' line ranges in lock step, so that at every step its 32 lanes read
-        // neighbouring pixels of ONE image line (1-2 cache lines per load instead of up to 32).  On a line outside a
-        // ray's own range the crossing is more than half a pixel outside the image: the clamped index lands in the
-        // zero padding and the term vanishes.
-        // (Row-major and column-major rays of one warp form two such unions: their lines are different things.)
-        const int big = 1 << 30;
-        const int rlo = __reduce_min_sync(0xffffffffu, rowmaj ? (int)flo : big);
-        const int rhi = __reduce_max_sync(0xffffffffu, rowmaj ? (int)fhi : -big);
-        const int clo = __reduce_min_sync(0xffffffffu, rowmaj ? big : (int)flo);
-        const int chi = __reduce_max_sync(0xffffffffu, rowmaj ? -big : (int)fhi);
-        const int wlo = rowmaj ? rlo : clo, whi = rowmaj ? rhi : chi;
-        const int nsteps = whi - wlo + 1;
-        pdl_wait();                                          // mu(n) is the previous launch's output
-#if !OSIV_PDL_LATE
+        const int flo = (int)fminf(fmaxf(ceilf(fminf(b1, b2) + cb) - 1.f, 0.f), (float)nb);
+        const int fhi = (int)fminf(fmaxf(floorf(fmaxf(b1, b2) + cb) + 1.f, -1.f), (float)(nb - 1));
+        // The block walks the union of its rays' line ranges in lock step, so that at every step the lanes of a warp
+        // read neighbouring pixels of ONE image line (1-2 cache lines per load instead of up to 32; rays clipped by an
+        // image corner start many lines apart).  On a line outside a ray's own range the crossing is more than half a
+        // pixel outside the image: the clamped index lands in the zero padding and the term vanishes.
+        // (Row-major and column-major rays of one block form two such unions: their lines are different things.)
+        if (t < 4) rng[t] = (t & 1) ? -1 : (1 << 30);
+        __syncthreads();
+        {
+            const int big = 1 << 30;
+            const int lo = __reduce_min_sync(0xffffffffu, walker && rowmaj ? flo : big);
+            const int hi = __reduce_max_sync(0xffffffffu, walker && rowmaj ? fhi : -1);
+            const int lo2 = __reduce_min_sync(0xffffffffu, walker && !rowmaj ? flo : big);
+            const int hi2 = __reduce_max_sync(0xffffffffu, walker && !rowmaj ? fhi : -1);
+            if ((t & 31) == 0) {
+                if (hi >= lo) { atomicMin(&rng[0], lo); atomicMax(&rng[1], hi); }
+                if (hi2 >= lo2) { atomicMin(&rng[2], lo2); atomicMax(&rng[3], hi2); }
+            }
+        }
+        __syncthreads();
+        const int wlo = rowmaj ? rng[0] : rng[2], whi = rowmaj ? rng[1] : rng[3];
+        const int nsteps = walker ? whi - wlo + 1 : 0;
+        const int len = (nsteps + segs - 1) / segs;
+        const int j0 = wlo + seg * len;
+        const int j1 = min(j0 + len, wlo + nsteps);
+        const int imax = na + PAD - 2;
+        int offP = (j0 + PADR) * pitch + PAD;                 // line j, walking up
+        int offM = (nb - 1 - j0 + PADR) * pitch + PAD;        // line nb-1-j, walking down
+        float bf = (float)j0 - cb;
+        pdl_wait();                                           // mu(n) is the previous launch's output
         pdl_launch_next();
-#endif
-        if (nsteps > 0) {
-            const int nsegt = FWD_SEGS * a.nsplit;
-            const int len = (nsteps + nsegt - 1) / nsegt;
-            const int j0 = wlo + (split * FWD_SEGS + seg) * len;
-            const int j1 = min(j0 + len, whi + 1);
-            const int imax = na + PAD - 2;
-            int offP = (j0 + PADR) * pitch + PAD;                 // line j, walking up
-            int offM = (nb - 1 - j0 + PADR) * pitch + PAD;        // line nb-1-j, walking down
-            float bf = (float)j0 - cb;
-            // Two lines per trip, written so that all 2 x 2 x NS gathers of a trip are in flight together: the walk
-            // is bound by load latency, not by issue.  The odd line past j1 (only in the last trip) gets zero weights;
-            // its addresses stay inside the padded buffers because j1 <= nb.
-            for (int jj = j0; jj < j1; jj += 2, offP += 2 * pitch, offM -= 2 * pitch, bf += 2.f) {
-                float w[2][2];
-                int i0[2];
+        // Two lines per trip, written so that all 2 x 2 x NS gathers of a trip are in flight together: the walk is
+        // bound by load latency.  The odd line past j1 (only in the last trip) gets zero weights; its addresses stay
+        // inside the padded buffers because j1 <= nb.
+        for (int jj = j0; jj < j1; jj += 2, offP += 2 * pitch, offM -= 2 * pitch, bf += 2.f) {
+            float w[2][2];
+            int i0[2];
 #pragma unroll
-                for (int u = 0; u < 2; ++u) {
-                    const float bg = fmaf(uu, bf + (float)u, ray.z);
-                    const float fa = floorf(fmaf(-bg, invk, ca)); // index of the pixel left of the crossing
-                    const float q0 = fmaf(kk, fa - ca, bg);
-                    const float q1 = q0 + kk;
-                    w[u][0] = __saturatef(hk - fabsf(q0));
-                    w[u][1] = __saturatef(hk - fabsf(q1));
-                    i0[u] = min(max((int)fa, -PAD), imax);
+            for (int u = 0; u < 2; ++u) {
+                const float bg = fmaf(uu, bf + (float)u, ray.z);
+                const float fa = floorf(fmaf(-bg, invk, ca));     // index of the pixel left of the crossing
+                const float q0 = fmaf(kk, fa - ca, bg);
+                const float q1 = q0 + kk;
+                w[u][0] = __saturatef(hk - fabsf(q0));
+                w[u][1] = __saturatef(hk - fabsf(q1));
+                i0[u] = min(max((int)fa, -PAD), imax);
+            }
+            if (jj + 1 >= j1) { w[1][0] = 0.f; w[1][1] = 0.f; }
+            float x[2][NS][2];
+#pragma unroll
+            for (int u = 0; u < 2; ++u) {
+                const int oP = offP + u * pitch, oM = offM - u * pitch;
+                const float* p0 = bufA + (oP + i0[u]);
+                x[u][0][0] = __ldg(p0); x[u][0][1] = __ldg(p0 + 1);
+                if (NS == 4) {
+                    const int ir = na - 2 - i0[u];                // mirrored index of pixel i0+1
+                    const float* p1 = bufB + (oM + i0[u]);        // pattern 1: other copy, line nb-1-j, same order
+                    const float* p2 = bufA + (oM + ir);           // pattern 2: same copy, line nb-1-j, mirrored
+                    const float* p3 = bufB + (oP + ir);           // pattern 3: other copy, line j, mirrored
+                    x[u][1 % NS][0] = __ldg(p1); x[u][1 % NS][1] = __ldg(p1 + 1);
+                    x[u][2 % NS][0] = __ldg(p2); x[u][2 % NS][1] = __ldg(p2 + 1);
+                    x[u][3 % NS][0] = __ldg(p3); x[u][3 % NS][1] = __ldg(p3 + 1);
                 }
-                if (jj + 1 >= j1) { w[1][0] = 0.f; w[1][1] = 0.f; }
-                float x[2][NS][2];
+            }
 #pragma unroll
-                for (int u = 0; u < 2; ++u) {
-                    const int oP = offP + u * pitch, oM = offM - u * pitch;
-                    const float* p0 = bufA + (oP + i0[u]);
-                    x[u][0][0] = __ldg(p0); x[u][0][1] = __ldg(p0 + 1);
-                    if (NS == 4) {
-                        const int ir = na - 2 - i0[u];            // mirrored index of pixel i0+1
-                        const float* p1 = bufB + (oM + i0[u]);    // pattern 1: other copy, line nb-1-j, same order
-                        const float* p2 = bufA + (oM + ir);       // pattern 2: same copy, line nb-1-j, mirrored
-                        const float* p3 = bufB + (oP + ir);       // pattern 3: other copy, line j, mirrored
-                        x[u][1 % NS][0] = __ldg(p1); x[u][1 % NS][1] = __ldg(p1 + 1);
-                        x[u][2 % NS][0] = __ldg(p2); x[u][2 % NS][1] = __ldg(p2 + 1);
-                        x[u][3 % NS][0] = __ldg(p3); x[u][3 % NS][1] = __ldg(p3 + 1);
-                    }
-                }
-#pragma unroll
-                for (int u = 0; u < 2; ++u) {
-                    acc[0] = fmaf(w[u][0], x[u][0][0], acc[0]);
-                    acc[0] = fmaf(w[u][1], x[u][0][1], acc[0]);
-                    if (NS == 4) {
-                        acc[1] = fmaf(w[u][0], x[u][1 % NS][0], acc[1]);
-                        acc[1] = fmaf(w[u][1], x[u][1 % NS][1], acc[1]);
-                        acc[2 % NS] = fmaf(w[u][1], x[u][2 % NS][0], acc[2 % NS]);
-                        acc[2 % NS] = fmaf(w[u][0], x[u][2 % NS][1], acc[2 % NS]);
-                        acc[3 % NS] = fmaf(w[u][1], x[u][3 % NS][0], acc[3 % NS]);
-                        acc[3 % NS] = fmaf(w[u][0], x[u][3 % NS][1], acc[3 % NS]);
-                    }
+            for (int u = 0; u < 2; ++u) {
+                acc[0] = fmaf(w[u][0], x[u][0][0], acc[0]);
+                acc[0] = fmaf(w[u][1], x[u][0][1], acc[0]);
+                if (NS == 4) {
+                    acc[1 % NS] = fmaf(w[u][0], x[u][1 % NS][0], acc[1 % NS]);
+                    acc[1 % NS] = fmaf(w[u][1], x[u][1 % NS][1], acc[1 % NS]);
+                    acc[2 % NS] = fmaf(w[u][1], x[u][2 % NS][0], acc[2 % NS]);
+                    acc[2 % NS] = fmaf(w[u][0], x[u][2 % NS][1], acc[2 % NS]);
+                    acc[3 % NS] = fmaf(w[u][1], x[u][3 % NS][0], acc[3 % NS]);
+                    acc[3 % NS] = fmaf(w[u][0], x[u][3 % NS][1], acc[3 % NS]);
                 }
             }
         }
     }
-#if OSIV_PDL_LATE
-    pdl_launch_next();
-#endif
+    if (seg < segs) {
 #pragma unroll
-    for (int k = 0; k < NS; ++k) part[seg][k][lane] = acc[k];
+        for (int k = 0; k < NS; ++k) part[(seg * NS + k) * rpb + i] = acc[k];
+    }
     // the epilogue's inputs are requested before the barrier so that they arrive while the block drains
-    const int VSb = a.VS / NS, Vq = g.V / NS;
-    const bool epi = MODE == 1 && seg == 0 && split == 0 && c < g.C;
+    const bool epi = t < rpb && r < R;
     float yk[NS] = {}, bl = a.blank_scalar, ib = 0.f;
-    if (epi) {
+    if (MODE == 1 && epi) {
 #pragma unroll
         for (int k = 0; k < NS; ++k) yk[k] = __ldg(&a.counts[((size_t)s * g.V + v + k * Vq) * g.C + c]);
         if (a.blank) bl = __ldg(&a.blank[c]);
         ib = __ldg(a.inv_bref);
     }
     __syncthreads();
-    if (seg != 0) return;
-
-    // sums over this block's segments, fixed order; pattern -> rotation k (patterns 1 and 3 swap for a
-    // column-major base ray: R maps its walk onto the other copy with the mirrored index first)
-    float t[NS];
-#pragma unroll
-    for (int k = 0; k < NS; ++k) {
-        float x = 0.f;
-#pragma unroll
-        for (int q = 0; q < FWD_SEGS; ++q) x += part[q][k][lane];
-        t[k] = x;
-    }
-    if (NS == 4 && !rowmaj) { const float x = t[1]; t[1] = t[3]; t[3] = x; }
-
-    const int groups = gridDim.x * (gridDim.y / a.nsplit);
-    const int grp = jb * gridDim.x + blockIdx.x;
-    if (a.nsplit > 1) {
-        if (split != 0) {
-            const uint32_t rmbar = cluster_map(smem_u32(&mbar), 0);
-#pragma unroll
-            for (int k = 0; k < NS; ++k) st_async_f32(cluster_map(smem_u32(&cpart[split][k][lane]), 0), t[k], rmbar);
-            return;
-        }
-        mbar_wait(&mbar, 0);
-#pragma unroll
-        for (int k = 0; k < NS; ++k)
-            for (int q = 1; q < a.nsplit; ++q) t[k] += cpart[q][k][lane];          // fixed order
-    }
+    if (t >= 32 * ((rpb + 31) / 32)) return;                  // whole warps past the epilogue rays
 
     double d2 = 0.0;
-    float hr[NS];
+    if (epi) {
+        // sums over the ray's segments, fixed order; pattern -> rotation k (patterns 1 and 3 swap for a
+        // column-major base ray: R maps its walk onto the other copy with the mirrored index first)
+        float l[NS], hr[NS];
 #pragma unroll
-    for (int k = 0; k < NS; ++k) {
-        const float l = ray.w * t[k];
-        const int jk = jb + k * VSb;                     // compact view index inside the subset
-        hr[k] = 0.f;
-        if (c < g.C) {
+        for (int k = 0; k < NS; ++k) {
+            float x = 0.f;
+            for (int q = 0; q < segs; ++q) x += part[(q * NS + k) * rpb + i];
+            l[k] = ray.w * x;
+        }
+        if (NS == 4 && !rowmaj) { const float x = l[1]; l[1] = l[3]; l[3] = x; }
+#pragma unroll
+        for (int k = 0; k < NS; ++k) {
             if (MODE == 0) {
-                a.sino[((size_t)s * a.VS + jk) * g.C + c] = l;
+                a.sino[((size_t)s * a.VS + jb + k * VSb) * g.C + c] = l[k];
             } else {
                 // A2: Poisson residual r = (b exp(-l) - y)/b_ref and monitor term (l - ln(b/max(y,1)))^2
-                const float y = yk[k], b = bl;
-                const float ybar = b * expf(-l);
-                const float r = (ybar - y) * ib;
-                hr[k] = ray.w * r;
-                const float p = logf(b / fmaxf(y, 1.f));
-                const double d = (double)l - (double)p;
+                const float ybar = bl * expf(-l[k]);
+                hr[k] = ray.w * ((ybar - yk[k]) * ib);
+                const float p = logf(bl / fmaxf(yk[k], 1.f));
+                const double d = (double)l[k] - (double)p;
                 d2 += d * d;
             }
         }
-    }
-    if (MODE == 1 && c < g.C) {
-        // NS == 4: the orbit's four residuals share one float4 (K2 reads them with one load per candidate ray)
-        if (NS == 4) reinterpret_cast<float4*>(a.res)[((size_t)s * VSb + jb) * a.Cp + c] = make_float4(hr[0], hr[1], hr[2], hr[3]);
-        else         a.res[((size_t)s * a.VS + jb) * a.Cp + c] = hr[0];
+        if (MODE == 1) {
+            // NS == 4: the orbit's four residuals share one float4 (K2 reads them with one load per candidate ray)
+            if (NS == 4) reinterpret_cast<float4*>(a.res)[((size_t)s * VSb + jb) * a.Cp + c] = make_float4(hr[0], hr[1 % NS], hr[2 % NS], hr[3 % NS]);
+            else         a.res[((size_t)s * a.VS + jb) * a.Cp + c] = hr[0];
+        }
     }
     if (MODE == 1) {
+        // block's share of D: warp shuffles, then the (at most 32) warp sums in a fixed order
 #pragma unroll
         for (int off = 16; off > 0; off >>= 1) d2 += __shfl_down_sync(0xffffffffu, d2, off);
-        if (lane == 0) a.dparts[(size_t)s * groups + grp] = d2;
+        const int nw = (rpb + 31) / 32;
+        if ((t & 31) == 0) dred[t >> 5] = d2;
+        asm volatile("bar.sync 1, %0;" ::"r"(32 * nw) : "memory");     // only the epilogue warps meet here
+        if (t == 0) {
+            double D = 0.0;
+            for (int w = 0; w < nw; ++w) D += dred[w];
+            a.dparts[(size_t)s * gridDim.x + blockIdx.x] = D;
+        }
     }
 }
 
