@@ -22,6 +22,7 @@ struct osiv_handle {
     DevGeom dg;
     float4* d_rays = nullptr;
     float2* d_views = nullptr;
+    float* d_hs = nullptr;
     // per-slice workspace, grown lazily
     int ws_batch = 0;
     float *d_imgA = nullptr, *d_imgB = nullptr, *d_imgTA = nullptr, *d_imgTB = nullptr;
@@ -161,7 +162,7 @@ int ensure_images(osiv_handle* h, int batch, cudaStream_t st) {
 int pick_ns(const osiv_handle* h, int VS) { return (h->dg.sym4 && !h->force_ns1 && VS % 4 == 0) ? 4 : 1; }
 
 struct FwdPlan { int threads, rpb, segs, nparts, ns; size_t smem; };
-struct BackPlan { dim3 grid; int nsplit, ns; };
+struct BackPlan { int nblk, threads, tpb, shares, ngx, ns; size_t smem; };
 
 // K1: the subset's base rays are dealt out in runs of rpb consecutive rays, one run per block and one block per SM
 // (per slice); a block is rpb rays x segs segments of each ray's line range, as many segments as fit into 1024
@@ -191,34 +192,35 @@ cudaError_t launch_forward(FwdPlan p, int batch, const FwdArgs& a, cudaStream_t 
     return cudaLaunchKernelEx(&cfg, k_forward<MODE, 1>, a);
 }
 
-// K2: one block per 16 x 8 pixel region of base tiles; its warps share the subset's views.
-BackPlan plan_back(const osiv_handle* h, int VS, int batch) {
+// K2: the base tiles, numbered patch by patch (8 x 4 tiles, patches grouped 2 x 2), are dealt out in runs of tpb
+// consecutive tiles, one run per block and one block per SM (per slice); a block is tpb tiles x `shares` view shares.
+BackPlan plan_back(const osiv_handle* h, int VS) {
     BackPlan p;
     p.ns = pick_ns(h, VS);
     const int tx = p.ns == 4 ? h->geom.nx / 4 : (h->geom.nx + BK_TX - 1) / BK_TX;
     const int ty = p.ns == 4 ? h->geom.ny / 4 : (h->geom.ny + BK_TY - 1) / BK_TY;
-    p.grid = dim3((tx + BK_WX - 1) / BK_WX, (ty + BK_WY - 1) / BK_WY, batch);
-    const long long blocks = (long long)p.grid.x * p.grid.y * batch;
-    long long want = ((long long)h->num_sms * 40 + blocks - 1) / blocks;      // about 40 resident warps per SM
-    int best;
-    if (p.ns == 4) {                  // warps come in fours (one per quarter turn), each with a share of the V_S/4 base views
-        const int vb = VS / 4;
-        best = 4;
-        while (best * 2 <= BK_MAX_SPLIT && best * 2 <= want && best / 2 <= vb) best *= 2;
-    } else {
-        want = std::max<long long>(1, std::min<long long>(want, std::min(BK_MAX_SPLIT, VS)));
-        best = (int)want;
-        for (int d = (int)want; d >= 1; --d) if (VS % d == 0) { if (2 * d > want) best = d; break; }
-    }
-    p.nsplit = best;
+    p.ngx = ((tx + BK_WX - 1) / BK_WX + 1) / 2;
+    const int ngy = ((ty + BK_WY - 1) / BK_WY + 1) / 2;
+    const long long tiles = (long long)p.ngx * ngy * 4 * 32;
+    p.tpb = (int)std::min<long long>(BK_MAX_THREADS / p.ns, std::max<long long>(1, (tiles + h->num_sms - 1) / h->num_sms));
+    p.nblk = (int)((tiles + p.tpb - 1) / p.tpb);
+    const int VSb = VS / p.ns;
+    // shares per quarter turn (NS == 4) or in all: as many as fit, then the fewest that keep the same number of
+    // views per share
+    int sq = std::max(1, std::min(BK_MAX_THREADS / (p.tpb * p.ns), VSb));
+    const int trips = (VSb + sq - 1) / sq;
+    sq = (VSb + trips - 1) / trips;
+    p.shares = sq * p.ns;
+    p.threads = (p.tpb * p.shares + 31) / 32 * 32;
+    p.smem = (size_t)p.shares * p.ns * 4 * p.tpb * sizeof(float);
     return p;
 }
 
 template <int MODE>
-cudaError_t launch_back(const BackPlan& p, const BackArgs& a, cudaStream_t st, bool pdl) {
+cudaError_t launch_back(const BackPlan& p, int batch, const BackArgs& a, cudaStream_t st, bool pdl) {
     cudaLaunchConfig_t cfg{};
-    cfg.gridDim = p.grid; cfg.blockDim = dim3(32 * p.nsplit); cfg.stream = st;
-    cfg.dynamicSmemBytes = (size_t)p.nsplit * p.ns * 4 * 32 * sizeof(float);
+    cfg.gridDim = dim3(p.nblk, 1, batch); cfg.blockDim = dim3(p.threads); cfg.stream = st;
+    cfg.dynamicSmemBytes = p.smem;
     cudaLaunchAttribute attr[1];
     attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     attr[0].val.programmaticStreamSerializationAllowed = 1;
@@ -301,7 +303,7 @@ int osiv_ray_table(const osiv_geometry* geom, float* h_rays, float* h_views) {
     std::vector<float4> rays;
     std::vector<float2> views;
     build_tables(*geom, resolve_dgamma(*geom), rays, views);
-    if (h_rays) std::memcpy(h_rays, rays.data(), rays.size() * sizeof(float4));
+    if (h_rays) std::memcpy(h_rays, rays.data(), rays.size() * sizeof(float4));      // {alpha, beta, g0, h}
     if (h_views) std::memcpy(h_views, views.data(), views.size() * sizeof(float2));
     return OSIV_OK;
 }
@@ -329,15 +331,26 @@ int osiv_create(const osiv_geometry* geom, int32_t max_batch, int32_t device, os
     const double xm = std::min(tile_r / (g.sad_mm - rmax), 1.0);
     const double tile_hw = std::asin(xm) / xm * tile_r / dgamma * 1.0005;
     h->res_pad = ((2 * (int)std::ceil(tile_hw / (g.sad_mm - rmax) + 0.05) + 3) + 3) / 4 * 4;
+    // device layout: float4 {alpha, beta, g0, hk} for the inner loops, h in a table of its own
+    std::vector<float> hs(rays.size());
+    for (size_t i = 0; i < rays.size(); ++i) {
+        hs[i] = rays[i].w;
+        rays[i].w = 0.5f * (std::fabs(rays[i].x) + std::fabs(rays[i].y));
+    }
     rays.resize(rays.size() + h->res_pad + 4, make_float4(0.f, 0.f, 0.f, 0.f));
     if (cudaMalloc((void**)&h->d_rays, rays.size() * sizeof(float4)) != cudaSuccess ||
+        cudaMalloc((void**)&h->d_hs, hs.size() * sizeof(float)) != cudaSuccess ||
+        cudaMemcpy(h->d_hs, hs.data(), hs.size() * sizeof(float), cudaMemcpyHostToDevice) != cudaSuccess ||
         cudaMalloc((void**)&h->d_views, views.size() * sizeof(float2)) != cudaSuccess ||
         cudaMalloc((void**)&h->d_state, (size_t)2 * max_batch * sizeof(SliceState)) != cudaSuccess ||
         cudaMalloc((void**)&h->d_not_finite, (size_t)max_batch * sizeof(int)) != cudaSuccess ||
         cudaMalloc((void**)&h->d_inv_bref, sizeof(float)) != cudaSuccess ||
         cudaMemcpy(h->d_rays, rays.data(), rays.size() * sizeof(float4), cudaMemcpyHostToDevice) != cudaSuccess ||
         cudaMemcpy(h->d_views, views.data(), views.size() * sizeof(float2), cudaMemcpyHostToDevice) != cudaSuccess ||
-        cudaDeviceGetAttribute(&h->num_sms, cudaDevAttrMultiProcessorCount, device) != cudaSuccess) {
+        cudaDeviceGetAttribute(&h->num_sms, cudaDevAttrMultiProcessorCount, device) != cudaSuccess ||
+        // K2's shared-memory reduction buffer: up to 1024 threads x 16 floats
+        cudaFuncSetAttribute(k_back<0, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024) != cudaSuccess ||
+        cudaFuncSetAttribute(k_back<1, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024) != cudaSuccess) {
         cudaGetLastError();
         osiv_destroy(h);
         return OSIV_ERR_CUDA;
@@ -359,7 +372,7 @@ int osiv_create(const osiv_geometry* geom, int32_t max_batch, int32_t device, os
     const double zmax = rmax / (g.sad_mm - rmax);
     d.use_atanf = (zmax > 0.75 || 3e-7 / dgamma > 0.01) ? 1 : 0;
     d.sym4 = (g.nx == g.ny && g.nx % 4 == 0 && g.n_views % 4 == 0) ? 1 : 0;
-    d.rays = h->d_rays; d.views = h->d_views;
+    d.rays = h->d_rays; d.views = h->d_views; d.hs = h->d_hs;
     *out = h;
     return OSIV_OK;
 }
@@ -369,7 +382,7 @@ int osiv_destroy(osiv_handle* h) {
     DeviceGuard guard(h->device);
     if (guard.ok) {
         cudaDeviceSynchronize();
-        void* ptrs[] = {h->d_rays, h->d_views, h->d_imgA, h->d_imgB, h->d_imgTA, h->d_imgTB, h->d_best, h->d_res,
+        void* ptrs[] = {h->d_rays, h->d_views, h->d_hs, h->d_imgA, h->d_imgB, h->d_imgTA, h->d_imgTB, h->d_best, h->d_res,
                         h->d_dparts, h->d_state, h->d_not_finite, h->d_inv_bref, h->d_trace,
                         h->d_forced, h->d_hcounts, h->d_hblank, h->d_himg};
         for (void* p : ptrs) if (p) cudaFree(p);
@@ -413,9 +426,9 @@ int osiv_get_plan(const osiv_handle* h, int32_t n_subsets, int32_t batch, int32_
     if (!h || !out8 || batch <= 0 || (n_subsets > 0 && h->geom.n_views % n_subsets != 0)) return OSIV_ERR_INVALID_ARG;
     const int VS = n_subsets > 0 ? h->geom.n_views / n_subsets : h->geom.n_views;
     const FwdPlan f = plan_forward(h, VS);
-    const BackPlan b = plan_back(h, VS, batch);
+    const BackPlan b = plan_back(h, VS);
     out8[0] = f.ns; out8[1] = f.segs; out8[2] = f.nparts * batch; out8[3] = f.threads;
-    out8[4] = b.ns; out8[5] = b.nsplit; out8[6] = (int)(b.grid.x * b.grid.y * b.grid.z); out8[7] = 32 * b.nsplit;
+    out8[4] = b.ns; out8[5] = b.shares; out8[6] = b.nblk * batch; out8[7] = b.threads;
     return OSIV_OK;
 }
 
@@ -465,15 +478,15 @@ int osiv_backward(osiv_handle* h, const float* d_sino, float* d_img, int32_t bat
     if (!guard.ok) { cudaGetLastError(); return OSIV_ERR_CUDA; }
     cudaStream_t st = (cudaStream_t)cuda_stream;
     const int VS = subset_views(h, subset, n_subsets), M = subset < 0 ? 1 : n_subsets;
-    const BackPlan p = plan_back(h, VS, batch);
+    const BackPlan p = plan_back(h, VS);
     int rc = ensure_res(h, VS, p.ns, batch, st);
     if (rc != OSIV_OK) return rc;
     const int Cp = h->geom.n_channels + h->res_pad;
     k_scale_sino<<<dim3((h->geom.n_channels + 255) / 256, VS, batch), 256, 0, st>>>(h->dg, d_sino, h->d_res, subset, M, VS,
                                                                                     p.ns, Cp);
     BackArgs b{};
-    b.g = h->dg; b.res = h->d_res; b.Cp = Cp; b.subset = subset; b.M = M; b.VS = VS; b.out = d_img;
-    launch_back<0>(p, b, st, false);
+    b.g = h->dg; b.res = h->d_res; b.Cp = Cp; b.subset = subset; b.M = M; b.VS = VS; b.out = d_img; b.tpb = p.tpb; b.shares = p.shares; b.ngx = p.ngx;
+    launch_back<0>(p, batch, b, st, false);
     return launch_check(h, 2);
 }
 
@@ -508,7 +521,7 @@ int osiv_reconstruct(osiv_handle* h, const float* d_counts, const float* d_blank
     int rc = ensure_images(h, batch, st);
     if (rc != OSIV_OK) return rc;
     const FwdPlan fp = plan_forward(h, VS);
-    const BackPlan bp = plan_back(h, VS, batch);
+    const BackPlan bp = plan_back(h, VS);
     if ((rc = ensure_res(h, VS, fp.ns, batch, st)) != OSIV_OK) return rc;
     const int Cp = C + h->res_pad;
     if ((rc = ensure_forward_ws(h, fp, batch)) != OSIV_OK) return rc;
@@ -531,7 +544,7 @@ int osiv_reconstruct(osiv_handle* h, const float* d_counts, const float* d_blank
     f.counts = d_counts; f.blank = d_blank; f.blank_scalar = blank_scalar; f.inv_bref = h->d_inv_bref;
     f.res = h->d_res; f.Cp = Cp; f.dparts = h->d_dparts;
     BackArgs b{};
-    b.g = h->dg; b.res = h->d_res; b.Cp = Cp; b.M = M; b.VS = VS; b.best = best;
+    b.g = h->dg; b.res = h->d_res; b.Cp = Cp; b.M = M; b.VS = VS; b.best = best; b.tpb = bp.tpb; b.shares = bp.shares; b.ngx = bp.ngx;
     b.dparts = h->d_dparts; b.nparts = fp.nparts; b.not_finite = h->d_not_finite;
     b.ip.lambda0 = prm->lambda0; b.ip.up = prm->lambda_up; b.ip.down = prm->lambda_down; b.ip.lmin = prm->lambda_min;
     b.ip.forced = (prm->forced_lambda && N > 0) ? h->d_forced : nullptr;
@@ -557,7 +570,7 @@ int osiv_reconstruct(osiv_handle* h, const float* d_counts, const float* d_blank
         if (prof) cudaEventRecord(h->events[2 * n + 1], st);
         b.img = cur; b.img_new = nxt; b.imgT_new = nxtT; b.subset = m;
         b.state_in = state[n & 1]; b.state_out = state[(n + 1) & 1];
-        launch_back<1>(bp, b, st, pdl);
+        launch_back<1>(bp, batch, b, st, pdl);
         if (prof) cudaEventRecord(h->events[2 * n + 2], st);
         float* t;
         t = cur; cur = nxt; nxt = t;

@@ -11,7 +11,7 @@
 // p the signed distance of the pixel centre from the ray, the chord is the trapezoid
 //   a = h * sat((hi - |p|) / (hi - lo)),  h = D/max(|dx|,|dy|), hi = D(|dx|+|dy|)/2, hi-lo = D*min(|dx|,|dy|).
 // p is affine in the centred pixel indices (xc, yc), so after dividing by (hi-lo) every ray carries
-// four floats {alpha, beta, g0, h} with
+// {alpha, beta, g0, h} (stored as the float4 {alpha, beta, g0, (|alpha|+|beta|)/2} plus a separate h table) with
 //   a(i; xc,yc) = h * sat( (|alpha|+|beta|)/2 - |alpha*xc + beta*yc + g0| ),
 // one of alpha,beta being exactly +-1 and the other |k| >= 1.  Forward and back evaluate this same
 // expression, so the pair is matched by construction.  Nothing here is a dense contraction: no
@@ -41,8 +41,7 @@ constexpr int FWD_MIN_LINES = 8;           // K1: a segment is at least this man
 #endif
 constexpr int BK_TX = 2, BK_TY = 2;        // pixels per thread in the backprojector
 constexpr int BK_WX = 8, BK_WY = 4;        // tiles per warp: a warp covers 16 x 8 pixels
-constexpr int BK_MAX_SPLIT = 16;           // K2 warps per block; each owns a share of the subset's views
-constexpr int BK_MAX_THREADS = 32 * BK_MAX_SPLIT;
+constexpr int BK_MAX_THREADS = 1024;       // K2: one block per SM, threads = tiles per block x view shares
 
 struct DevGeom {
     int nx, ny, V, C;
@@ -53,7 +52,8 @@ struct DevGeom {
     float tile_hw;                         // angular half-width of a K2 tile at unit distance, in channels (with asin slack)
     int use_atanf;                         // fan too wide for the short atan polynomial
     int sym4;                              // geometry admits the quarter-turn path (square grid, nx%4==0, V%4==0)
-    const float4* rays;                    // [V][C] {alpha, beta, g0, h}
+    const float4* rays;                    // [V][C] {alpha, beta, g0, hk}, hk = (|alpha|+|beta|)/2 (both kernels' inner loops)
+    const float* hs;                       // [V][C] chord scale h (per ray, outside the inner loops)
     const float2* views;                   // [V] {cos th_v, sin th_v}
 };
 
@@ -94,6 +94,7 @@ struct BackArgs {
     const float* res;                      // h * (residual or sinogram), layout as FwdArgs::res
     int Cp;
     int subset, M, VS;
+    int tpb, shares, ngx;                  // tiles per block, view shares, 2x2 patch groups per row of groups
     float* out;                            // MODE 0: [batch][ny][nx]
     const float* img;                      // MODE 1: padded mu(n)
     float* img_new;                        // padded mu(n+1)
@@ -122,6 +123,19 @@ __device__ __forceinline__ size_t padT_off(const DevGeom& g, int ix, int iy) {
 // most one successor is ever resident early -- lets the successor's blocks move into the SM slots this grid frees.
 __device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
 __device__ __forceinline__ void pdl_launch_next() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+
+// Packed FP32 pairs (Blackwell FFMA2: two IEEE fp32 FMAs per instruction, the scalar operand broadcast): halves the
+// issue slots of the accumulation, bit-identical to two FFMAs.
+__device__ __forceinline__ uint64_t pack2(float lo, float hi) {
+    uint64_t r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+    return r;
+}
+__device__ __forceinline__ void unpack2(uint64_t v, float& lo, float& hi) { asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v)); }
+__device__ __forceinline__ void ffma2(uint64_t& c, uint64_t a, float b) {       // c += a * (b, b)
+    const uint64_t bb = pack2(b, b);
+    asm("fma.rn.f32x2 %0, %1, %2, %0;" : "+l"(c) : "l"(a), "l"(bb));
+}
 
 // ------------------------------------------------------------------------------------------------
 // K1: forward projection (+ residual and monitor partials when MODE == 1).
@@ -152,6 +166,7 @@ __global__ void __launch_bounds__(FWD_MAX_THREADS, 1) k_forward(const FwdArgs a)
     __shared__ int rng[4];                                          // line ranges of the block's row- / column-major rays
 
     float acc[NS];
+    uint64_t acc01 = 0ull, acc23 = 0ull;
 #pragma unroll
     for (int k = 0; k < NS; ++k) acc[k] = 0.f;
     const float4 ray = __ldg(&g.rays[(size_t)v * g.C + c]);
@@ -165,7 +180,7 @@ __global__ void __launch_bounds__(FWD_MAX_THREADS, 1) k_forward(const FwdArgs a)
         const int na = rowmaj ? g.nx : g.ny, nb = rowmaj ? g.ny : g.nx;
         const float ca = rowmaj ? g.cx : g.cy, cb = rowmaj ? g.cy : g.cx;
         const float invk = 1.0f / kk;
-        const float hk = 0.5f * (fabsf(ray.x) + fabsf(ray.y));
+        const float hk = ray.w;
         // lines where the crossing lies within half a pixel of the image: |uu*b + g0| < |kk|*(na/2 + 1/2)
         const float A = fabsf(kk) * (0.5f * na + 0.5f);
         const float b1 = uu * (-ray.z - A), b2 = uu * (-ray.z + A);
@@ -236,26 +251,27 @@ __global__ void __launch_bounds__(FWD_MAX_THREADS, 1) k_forward(const FwdArgs a)
             }
 #pragma unroll
             for (int u = 0; u < 2; ++u) {
-                acc[0] = fmaf(w[u][0], x[u][0][0], acc[0]);
-                acc[0] = fmaf(w[u][1], x[u][0][1], acc[0]);
-                if (NS == 4) {
-                    acc[1 % NS] = fmaf(w[u][0], x[u][1 % NS][0], acc[1 % NS]);
-                    acc[1 % NS] = fmaf(w[u][1], x[u][1 % NS][1], acc[1 % NS]);
-                    acc[2 % NS] = fmaf(w[u][1], x[u][2 % NS][0], acc[2 % NS]);
-                    acc[2 % NS] = fmaf(w[u][0], x[u][2 % NS][1], acc[2 % NS]);
-                    acc[3 % NS] = fmaf(w[u][1], x[u][3 % NS][0], acc[3 % NS]);
-                    acc[3 % NS] = fmaf(w[u][0], x[u][3 % NS][1], acc[3 % NS]);
+                if (NS == 4) {                                    // (acc0, acc1) and (acc2, acc3) as FFMA2 pairs
+                    ffma2(acc01, pack2(x[u][0][0], x[u][1 % NS][0]), w[u][0]);
+                    ffma2(acc01, pack2(x[u][0][1], x[u][1 % NS][1]), w[u][1]);
+                    ffma2(acc23, pack2(x[u][2 % NS][0], x[u][3 % NS][0]), w[u][1]);
+                    ffma2(acc23, pack2(x[u][2 % NS][1], x[u][3 % NS][1]), w[u][0]);
+                } else {
+                    acc[0] = fmaf(w[u][0], x[u][0][0], acc[0]);
+                    acc[0] = fmaf(w[u][1], x[u][0][1], acc[0]);
                 }
             }
         }
     }
+    if (NS == 4) { unpack2(acc01, acc[0], acc[1 % NS]); unpack2(acc23, acc[2 % NS], acc[3 % NS]); }
     if (seg < segs) {
 #pragma unroll
         for (int k = 0; k < NS; ++k) part[(seg * NS + k) * rpb + i] = acc[k];
     }
     // the epilogue's inputs are requested before the barrier so that they arrive while the block drains
     const bool epi = t < rpb && r < R;
-    float yk[NS] = {}, bl = a.blank_scalar, ib = 0.f;
+    float yk[NS] = {}, bl = a.blank_scalar, ib = 0.f, h = 0.f;
+    if (epi) h = __ldg(&g.hs[(size_t)v * g.C + c]);
     if (MODE == 1 && epi) {
 #pragma unroll
         for (int k = 0; k < NS; ++k) yk[k] = __ldg(&a.counts[((size_t)s * g.V + v + k * Vq) * g.C + c]);
@@ -274,7 +290,7 @@ __global__ void __launch_bounds__(FWD_MAX_THREADS, 1) k_forward(const FwdArgs a)
         for (int k = 0; k < NS; ++k) {
             float x = 0.f;
             for (int q = 0; q < segs; ++q) x += part[(q * NS + k) * rpb + i];
-            l[k] = ray.w * x;
+            l[k] = h * x;
         }
         if (NS == 4 && !rowmaj) { const float x = l[1]; l[1] = l[3]; l[3] = x; }
 #pragma unroll
@@ -284,7 +300,7 @@ __global__ void __launch_bounds__(FWD_MAX_THREADS, 1) k_forward(const FwdArgs a)
             } else {
                 // A2: Poisson residual r = (b exp(-l) - y)/b_ref and monitor term (l - ln(b/max(y,1)))^2
                 const float ybar = bl * expf(-l[k]);
-                hr[k] = ray.w * ((ybar - yk[k]) * ib);
+                hr[k] = h * ((ybar - yk[k]) * ib);
                 const float p = logf(bl / fmaxf(yk[k], 1.f));
                 const double d = (double)l[k] - (double)p;
                 d2 += d * d;
@@ -423,49 +439,119 @@ __device__ __forceinline__ float atan_small(float z) {
     return fmaf(z, p, z);
 }
 
+// K2's accumulators: NS == 4: acc.p[h][px] = the pair (component 2h, component 2h+1) of pixel px = ty*2+tx;
+// NS == 1: acc.s[px].
+template <int NS> struct BackAcc;
+template <> struct BackAcc<4> {
+    uint64_t p[2][4];
+    __device__ __forceinline__ void clear() {
+#pragma unroll
+        for (int h = 0; h < 2; ++h)
+#pragma unroll
+            for (int x = 0; x < 4; ++x) p[h][x] = 0ull;
+    }
+    __device__ __forceinline__ float get(int m, int px) const {
+        float lo, hi;
+        unpack2(p[m >> 1][px], lo, hi);
+        return (m & 1) ? hi : lo;
+    }
+};
+template <> struct BackAcc<1> {
+    float s[4];
+    __device__ __forceinline__ void clear() { s[0] = s[1] = s[2] = s[3] = 0.f; }
+    __device__ __forceinline__ float get(int, int px) const { return s[px]; }
+};
+
+// one candidate ray r = {alpha, beta, g0, hk} against the 2x2 tile whose first pixel has centred indices (xc0, yc0):
+// the four chord weights (over h, which the residuals sv already carry) feed the tile's accumulators; with NS == 4
+// the same weights serve the orbit's four residuals.
+template <int NS>
+__device__ __forceinline__ void back_accumulate(const float4 r, const float4 sv, float xc0, float yc0, BackAcc<NS>& acc);
+template <>
+__device__ __forceinline__ void back_accumulate<4>(const float4 r, const float4 sv, float xc0, float yc0, BackAcc<4>& acc) {
+    const float q00 = fmaf(r.x, xc0, fmaf(r.y, yc0, r.z));
+    const float q01 = q00 + r.x;          // (ty=0, tx=1)
+    const float q10 = q00 + r.y;          // (ty=1, tx=0)
+    const float q11 = q10 + r.x;
+    const float w00 = __saturatef(r.w - fabsf(q00));
+    const float w01 = __saturatef(r.w - fabsf(q01));
+    const float w10 = __saturatef(r.w - fabsf(q10));
+    const float w11 = __saturatef(r.w - fabsf(q11));
+    const uint64_t sxy = pack2(sv.x, sv.y), szw = pack2(sv.z, sv.w);
+    ffma2(acc.p[0][0], sxy, w00); ffma2(acc.p[1][0], szw, w00);
+    ffma2(acc.p[0][1], sxy, w01); ffma2(acc.p[1][1], szw, w01);
+    ffma2(acc.p[0][2], sxy, w10); ffma2(acc.p[1][2], szw, w10);
+    ffma2(acc.p[0][3], sxy, w11); ffma2(acc.p[1][3], szw, w11);
+}
+template <>
+__device__ __forceinline__ void back_accumulate<1>(const float4 r, const float4 sv, float xc0, float yc0, BackAcc<1>& acc) {
+    const float q00 = fmaf(r.x, xc0, fmaf(r.y, yc0, r.z));
+    const float q01 = q00 + r.x;
+    const float q10 = q00 + r.y;
+    const float q11 = q10 + r.x;
+    acc.s[0] = fmaf(__saturatef(r.w - fabsf(q00)), sv.x, acc.s[0]);
+    acc.s[1] = fmaf(__saturatef(r.w - fabsf(q01)), sv.x, acc.s[1]);
+    acc.s[2] = fmaf(__saturatef(r.w - fabsf(q10)), sv.x, acc.s[2]);
+    acc.s[3] = fmaf(__saturatef(r.w - fabsf(q11)), sv.x, acc.s[3]);
+}
+
 // ------------------------------------------------------------------------------------------------
 // K2: matched gather backprojection of the residuals written by K1 (+ step rule, TV gradient, Eq. 3 update,
 // positivity clamp, best-image copy when MODE == 1).
-// grid (tiles_x/8, tiles_y/4, batch) over the base tiles (NS == 4: the quadrant x,y < N/2), block 32 x nsplit:
-// lane = one 2x2 pixel tile of a 16 x 8 pixel region, warp = a share of the subset's views.  For every view the
-// channels whose ray can cross the tile form the interval |c - c*| <= hw around the channel coordinate c* of the
-// tile centre (every such ray passes within the tile's half-diagonal of the centre, so its fan angle differs
-// from the centre's by at most asin(r/L) <= tile_hw/along channels); each candidate costs one 16-byte ray-table
-// load and one residual load (NS == 4: the float4 of the view's orbit).  The warps' sums meet in shared memory in a fixed order; warp k then
-// finishes rotation k of the tile (TV gradient, update, stores).
+// One block per SM-sized share of the base tiles (NS == 4: the 2x2-pixel tiles of the quadrant x,y < N/2): the tiles
+// are numbered patch by patch (a patch = 8 x 4 tiles = 16 x 8 pixels, patches grouped 2 x 2) and dealt out in runs of
+// `tpb` consecutive tiles, so that a block owns a compact piece of the image.  A block is tpb tiles x `shares` view
+// shares: thread t works on tile t % tpb for the views of share t / tpb (NS == 4: share q takes quarter turn q & 3
+// and every (shares/4)-th base view).  For every view the channels whose ray can cross the tile form the interval
+// |c - c*| <= hw around the channel coordinate c* of the tile centre (every such ray passes within the tile's
+// half-diagonal of the centre, so its fan angle differs from the centre's by at most asin(r/L) <= tile_hw/along
+// channels); each candidate costs one 16-byte ray-table load and one residual load (NS == 4: the float4 of the
+// view's orbit).  The shares' sums meet in shared memory in a fixed order; thread (tile, k) then finishes rotation
+// k of the tile (TV gradient, update, stores).  The host sizes the grid to one block per SM (plan_back).
 // ------------------------------------------------------------------------------------------------
 template <int MODE, int NS>
-__global__ void __launch_bounds__(BK_MAX_THREADS) k_back(const BackArgs a) {
+__global__ void __launch_bounds__(BK_MAX_THREADS, 1) k_back(const BackArgs a) {
     const DevGeom& g = a.g;
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nsplit = blockDim.x >> 5;
-    const int x0 = (blockIdx.x * BK_WX + (lane & (BK_WX - 1))) * BK_TX;
-    const int y0 = (blockIdx.y * BK_WY + (lane / BK_WX)) * BK_TY;
-    const int s = blockIdx.z;
-    const bool active = NS == 4 ? (x0 < (g.nx >> 1) && y0 < (g.ny >> 1)) : (x0 < g.nx && y0 < g.ny);
-    extern __shared__ float red_dyn[];                    // [nsplit][NS * 4][32]
-    float (*red)[NS * 4][32] = reinterpret_cast<float (*)[NS * 4][32]>(red_dyn);
+    const int t = threadIdx.x, lane = t & 31, s = blockIdx.z;
+    const int tpb = a.tpb, shares = a.shares;
+    const int q = t / tpb, i = t - q * tpb;
+    extern __shared__ float red[];                        // [shares][NS * 4][tpb]
 
-    // acc[m][ty*2+tx]: NS == 4: m = component of the orbit's residual float4 (this warp's views all lie in quarter
+    // tile number -> patch (2 x 2 patch groups, row-major) -> 2x2-pixel tile origin (x0, y0)
+    auto tile_origin = [&](int T, int& x0, int& y0) {
+        const int patch = T >> 5, w = T & 31;
+        const int grp = patch >> 2, sub = patch & 3;
+        const int gy = grp / a.ngx, gx = grp - gy * a.ngx;
+        x0 = (((gx << 1) + (sub & 1)) * BK_WX + (w & (BK_WX - 1))) * BK_TX;
+        y0 = (((gy << 1) + (sub >> 1)) * BK_WY + (w / BK_WX)) * BK_TY;
+    };
+    const int xlim = NS == 4 ? (g.nx >> 1) : g.nx, ylim = NS == 4 ? (g.ny >> 1) : g.ny;
+    int x0, y0;
+    tile_origin(blockIdx.x * tpb + i, x0, y0);
+    const bool active = q < shares && x0 < xlim && y0 < ylim;
+
+    // acc[m][ty*2+tx]: NS == 4: m = component of the orbit's residual float4 (this thread's views all lie in quarter
     // turn `quarter`, so rotation k of the tile collects component (quarter + k) % 4)
-    float acc[NS][4];
-#pragma unroll
-    for (int k = 0; k < NS; ++k)
-#pragma unroll
-        for (int p = 0; p < 4; ++p) acc[k][p] = 0.f;
+    BackAcc<NS> acc;
+    acc.clear();
 
     const int VSb = a.VS / NS;
-    // NS == 4: nsplit is a multiple of 4; warp w takes quarter turn w & 3 and every (nsplit/4)-th base view
-    const int quarter = NS == 4 ? (warp & 3) : 0;
-    const int jfirst = NS == 4 ? (warp >> 2) : warp, jstep = NS == 4 ? (nsplit >> 2) : nsplit;
+    const int quarter = NS == 4 ? (q & 3) : 0;
+    const int jfirst = NS == 4 ? (q >> 2) : q, jstep = NS == 4 ? (shares >> 2) : shares;
+    const int ntrips = (VSb + jstep - 1) / jstep;         // the same for every thread: the candidate loop is warp-wide
     {
         const float xc0 = (float)x0 - g.cx, yc0 = (float)y0 - g.cy;
         const float X = (xc0 + 0.5f * (BK_TX - 1)) * g.pixel, Y = (yc0 + 0.5f * (BK_TY - 1)) * g.pixel;
         const float* res = a.res + (size_t)s * a.VS * a.Cp;      // same float count for both layouts
-        pdl_wait();                                              // the residuals are the previous launch's output
-#if !OSIV_PDL_LATE
-        pdl_launch_next();
-#endif
-        for (int jb = jfirst; jb < VSb; jb += jstep) {
+
+        // Candidate interval of trip `it` (view jfirst + it * jstep of this thread's share): offsets of its first
+        // candidate in the ray table and in the residual rows, and the warp's candidate count.  The warp runs
+        // max-over-lanes candidates in lock step (no remainder code); a lane's extra candidates have zero weight (the
+        // ray misses its tile) or read the zero columns C..Cp-1 of res, and a lane that is off reads only those.
+        auto interval = [&](int it, int& offR, int& offS) -> int {
+            const int jbr = jfirst + it * jstep;
+            const bool on = active && jbr < VSb;
+            const int jb = min(jbr, VSb - 1);
             const int jj = jb + quarter * VSb;
             const int v = a.subset < 0 ? jj : a.subset + jj * a.M;
             const float2 cs = __ldg(&g.views[v]);
@@ -477,69 +563,75 @@ __global__ void __launch_bounds__(BK_MAX_THREADS) k_back(const BackArgs a) {
             const float gam = g.use_atanf ? atanf(z) : atan_small(z);
             const float cstar = fmaf(gam, g.inv_dgamma, g.c_center);
             const float hw = fmaf(g.tile_hw, rinv, 0.05f);
-            const int c_lo = min(max(0, (int)ceilf(cstar - hw)), g.C);
+            const int c_lo = on ? min(max(0, (int)ceilf(cstar - hw)), g.C) : g.C;
             const int c_hi = min(g.C - 1, (int)floorf(cstar + hw));
-            // the warp runs max-over-lanes candidates in lock step (no remainder code); a lane's extra candidates
-            // have zero weight (the ray misses its tile) or read the zero columns C..Cp-1 of res
-            const int ncw = __reduce_max_sync(0xffffffffu, active ? c_hi - c_lo + 1 : 0);
-            const float4* rp = g.rays + (size_t)v * g.C + c_lo;
-            if (NS == 4) {
-                const float4* sp = reinterpret_cast<const float4*>(res) + (size_t)jb * a.Cp + c_lo;
+            offR = v * g.C + c_lo;
+            offS = jb * a.Cp + c_lo;
+            return __reduce_max_sync(0xffffffffu, on ? c_hi - c_lo + 1 : 0);
+        };
+        // Trips are taken four at a time: the four intervals are independent chains of arithmetic, and the first four
+        // need nothing from K1, so they are worked out before the wait; the candidates of two trips are then walked
+        // together, which keeps 2 x 2 x 2 sixteen-byte loads in flight per thread.
+        constexpr int CH = 4;
+        int offR[CH], offS[CH], ncw[CH];
+#pragma unroll
+        for (int e = 0; e < CH; ++e) {
+            offR[e] = offS[e] = 0; ncw[e] = 0;
+            if (e < ntrips) ncw[e] = interval(e, offR[e], offS[e]);
+        }
+        pdl_wait();                                              // the residuals are the previous launch's output
+        pdl_launch_next();
+        for (int it0 = 0;;) {
+#pragma unroll
+            for (int e = 0; e < CH; e += 2) {
+                const float4* rpA = g.rays + offR[e];
+                const float4* rpB = g.rays + offR[e + 1];
+                const float4* spA = reinterpret_cast<const float4*>(res) + offS[e];      // NS == 4
+                const float4* spB = reinterpret_cast<const float4*>(res) + offS[e + 1];
+                const float* tpA = res + offS[e];                                        // NS == 1
+                const float* tpB = res + offS[e + 1];
+                if (ncw[e + 1] == 0) {                     // odd trip out (warp-uniform): one stream
 #pragma unroll 2
-                for (int t = 0; t < ncw; ++t) {
-                    const float4 r = __ldg(rp + t);
-                    const float4 sv = __ldg(sp + t);
-                    const float hk = 0.5f * (fabsf(r.x) + fabsf(r.y));
-                    const float q00 = fmaf(r.x, xc0, fmaf(r.y, yc0, r.z));
-                    const float q01 = q00 + r.x;          // (ty=0, tx=1)
-                    const float q10 = q00 + r.y;          // (ty=1, tx=0)
-                    const float q11 = q10 + r.x;
-                    const float w00 = __saturatef(hk - fabsf(q00));
-                    const float w01 = __saturatef(hk - fabsf(q01));
-                    const float w10 = __saturatef(hk - fabsf(q10));
-                    const float w11 = __saturatef(hk - fabsf(q11));
-                    acc[0][0] = fmaf(w00, sv.x, acc[0][0]); acc[0][1] = fmaf(w01, sv.x, acc[0][1]);
-                    acc[0][2] = fmaf(w10, sv.x, acc[0][2]); acc[0][3] = fmaf(w11, sv.x, acc[0][3]);
-                    acc[1 % NS][0] = fmaf(w00, sv.y, acc[1 % NS][0]); acc[1 % NS][1] = fmaf(w01, sv.y, acc[1 % NS][1]);
-                    acc[1 % NS][2] = fmaf(w10, sv.y, acc[1 % NS][2]); acc[1 % NS][3] = fmaf(w11, sv.y, acc[1 % NS][3]);
-                    acc[2 % NS][0] = fmaf(w00, sv.z, acc[2 % NS][0]); acc[2 % NS][1] = fmaf(w01, sv.z, acc[2 % NS][1]);
-                    acc[2 % NS][2] = fmaf(w10, sv.z, acc[2 % NS][2]); acc[2 % NS][3] = fmaf(w11, sv.z, acc[2 % NS][3]);
-                    acc[3 % NS][0] = fmaf(w00, sv.w, acc[3 % NS][0]); acc[3 % NS][1] = fmaf(w01, sv.w, acc[3 % NS][1]);
-                    acc[3 % NS][2] = fmaf(w10, sv.w, acc[3 % NS][2]); acc[3 % NS][3] = fmaf(w11, sv.w, acc[3 % NS][3]);
-                }
-            } else {
-                const float* sp = res + (size_t)jb * a.Cp + c_lo;
+                    for (int u = 0; u < ncw[e]; ++u) {
+                        const float4 rA = __ldg(rpA + u);
+                        const float4 sA = NS == 4 ? __ldg(spA + u) : make_float4(__ldg(tpA + u), 0.f, 0.f, 0.f);
+                        back_accumulate<NS>(rA, sA, xc0, yc0, acc);
+                    }
+                } else {
+                    const int n = max(ncw[e], ncw[e + 1]);
 #pragma unroll 2
-                for (int t = 0; t < ncw; ++t) {
-                    const float4 r = __ldg(rp + t);
-                    const float sv = __ldg(sp + t);
-                    const float hk = 0.5f * (fabsf(r.x) + fabsf(r.y));
-                    const float q00 = fmaf(r.x, xc0, fmaf(r.y, yc0, r.z));
-                    const float q01 = q00 + r.x;
-                    const float q10 = q00 + r.y;
-                    const float q11 = q10 + r.x;
-                    acc[0][0] = fmaf(__saturatef(hk - fabsf(q00)), sv, acc[0][0]);
-                    acc[0][1] = fmaf(__saturatef(hk - fabsf(q01)), sv, acc[0][1]);
-                    acc[0][2] = fmaf(__saturatef(hk - fabsf(q10)), sv, acc[0][2]);
-                    acc[0][3] = fmaf(__saturatef(hk - fabsf(q11)), sv, acc[0][3]);
+                    for (int u = 0; u < n; ++u) {
+                        const float4 rA = __ldg(rpA + u), rB = __ldg(rpB + u);
+                        const float4 sA = NS == 4 ? __ldg(spA + u) : make_float4(__ldg(tpA + u), 0.f, 0.f, 0.f);
+                        const float4 sB = NS == 4 ? __ldg(spB + u) : make_float4(__ldg(tpB + u), 0.f, 0.f, 0.f);
+                        back_accumulate<NS>(rA, sA, xc0, yc0, acc);
+                        back_accumulate<NS>(rB, sB, xc0, yc0, acc);
+                    }
                 }
+            }
+            it0 += CH;
+            if (it0 >= ntrips) break;
+#pragma unroll
+            for (int e = 0; e < CH; ++e) {
+                ncw[e] = 0;
+                if (it0 + e < ntrips) ncw[e] = interval(it0 + e, offR[e], offS[e]);
             }
         }
     }
-#if OSIV_PDL_LATE
-    pdl_launch_next();
-#endif
     // rotation k of the tile = orbit component (quarter + k) % 4  <=>  component m feeds rotation (m - quarter) % 4
+    if (q < shares) {
 #pragma unroll
-    for (int m = 0; m < NS; ++m)
+        for (int m = 0; m < NS; ++m)
 #pragma unroll
-        for (int p = 0; p < 4; ++p) red[warp][((m - quarter) & (NS - 1)) * 4 + p][lane] = acc[m][p];
+            for (int p = 0; p < 4; ++p) red[(q * (NS * 4) + ((m - quarter) & (NS - 1)) * 4 + p) * tpb + i] = acc.get(m, p);
+    }
 
-    // warp k < NS finishes rotation k of the base tile: origin (xk, yk) and, below, where base pixel (tx,ty) lands.
-    // Everything that does not depend on the other warps' sums -- monitor, step rule, neighbourhood of mu(n), TV
-    // gradient -- is done before the barrier, so that its loads overlap the wait for the slowest warp.
-    const bool fin = warp < NS;
-    const int k = warp;
+    // thread (tile i, k = q < NS) finishes rotation k of the base tile: origin (xk, yk) and, below, where base pixel
+    // (tx,ty) lands.  Everything that does not depend on the other shares' sums -- monitor, step rule, neighbourhood
+    // of mu(n), TV gradient -- is done before the barrier, so that its loads overlap the wait for the slowest warp.
+    const bool fin = q < NS;
+    const bool fin_active = fin && x0 < xlim && y0 < ylim;
+    const int k = q;
     int xk = x0, yk = y0;
     if (NS == 4) {
         const int N = g.nx;
@@ -550,15 +642,15 @@ __global__ void __launch_bounds__(BK_MAX_THREADS) k_back(const BackArgs a) {
     StepInfo si;
     float step = 0.f;
     float m[4][4], tv[2][2];
-    if (MODE == 1 && fin) {
-        const bool writer = blockIdx.x == 0 && blockIdx.y == 0 && warp == 0;
-        if (active) load_nbhd(g, a.img + (size_t)s * g.img_elems, xk, yk, m);
+    if (MODE == 1 && t < 32 * ((NS * tpb + 31) / 32)) {           // whole warps: step_rule shuffles
+        const bool writer = blockIdx.x == 0 && t < 32;
+        if (fin_active) load_nbhd(g, a.img + (size_t)s * g.img_elems, xk, yk, m);
         si = step_rule(a, s, lane, writer);
         step = (float)(si.lambda * a.tau);
-        if (active) tv_grad_tile(m, xk, yk, g.nx, g.ny, a.eps2, tv);
+        if (fin_active) tv_grad_tile(m, xk, yk, g.nx, g.ny, a.eps2, tv);
     }
     __syncthreads();
-    if (!fin || !active) return;
+    if (!fin_active) return;
 
     {
         // sums over the view shares, fixed order
@@ -566,7 +658,7 @@ __global__ void __launch_bounds__(BK_MAX_THREADS) k_back(const BackArgs a) {
 #pragma unroll
         for (int p = 0; p < 4; ++p) {
             float x = 0.f;
-            for (int q = 0; q < nsplit; ++q) x += red[q][k * 4 + p][lane];
+            for (int qq = 0; qq < shares; ++qq) x += red[(qq * (NS * 4) + k * 4 + p) * tpb + i];
             b[p] = x;
         }
         float o00 = b[0], o01 = b[1], o10 = b[2], o11 = b[3];
@@ -692,8 +784,7 @@ __global__ void __launch_bounds__(256) k_scale_sino(DevGeom g, const float* __re
     const int c = blockIdx.x * 256 + threadIdx.x, j = blockIdx.y, s = blockIdx.z;
     if (c >= g.C) return;
     const int v = subset < 0 ? j : subset + j * M;
-    const float4 ray = __ldg(&g.rays[(size_t)v * g.C + c]);
-    const float val = ray.w * sino[((size_t)s * VS + j) * g.C + c];
+    const float val = __ldg(&g.hs[(size_t)v * g.C + c]) * sino[((size_t)s * VS + j) * g.C + c];
     if (ns == 4) {
         const int VSb = VS / 4, jb = j % VSb, k = j / VSb;
         res[(((size_t)s * VSb + jb) * Cp + c) * 4 + k] = val;
