@@ -36,6 +36,9 @@ UNIT = "iterations/s"
 FP32_FLOP_PER_NNZ = 6          # q (FMA, 2) + half-width minus |q| (1) + clamp (1) + accumulate (FMA, 2)
 NNZ_PER_RAY_PER_N = 1.193      # measured non-zeros per ray / N when the fan spans the inscribed circle
 SM_COUNT, FP32_LANES_PER_SM = 148, 128
+# dram__bytes_read.sum + dram__bytes_write.sum per launch at config 3 from the committed full-set ncu capture
+# (profiles/r1c_ncu_config3.md; ncu flushes the caches before every replay, so this is the cold-cache figure)
+NCU_DRAM_BYTES_PER_LAUNCH = {"3": {"k_forward<1>": 2438912, "k_back<1>": 1511680}}
 
 
 def load_peaks():
@@ -249,10 +252,13 @@ def run_ours(args, cfg, beta):
     hbm_bytes = {"k_forward<1>": (cfg.nx * cfg.ny * 4 + 2 * vs * cfg.n_channels * 4 + vs * cfg.n_channels * 32) * batch,
                  "k_back<1>": (cfg.nx * cfg.ny * 4 * 3 + vs * cfg.n_channels * 16) * batch}
     roof = {"bound": "alu", "kernel": dom, "achieved": kernels[dom]["achieved_tflops"], "peak": alu_peak_tflops,
-            "unit": "TFLOP/s", "frac": kernels[dom]["frac"], "traffic": None,
+            "unit": "TFLOP/s", "frac": kernels[dom]["frac"],
+            "traffic": NCU_DRAM_BYTES_PER_LAUNCH.get(cfg.name, {}).get(dom),
             "peak_source": f"148 SMs x 128 FP32 lanes x 2 flop x {sm_mhz_peak:.0f} MHz ({peak_kind} sm_max_mhz)",
             "algorithmic_flop_per_launch": nnz * FP32_FLOP_PER_NNZ, "nnz_per_launch": nnz,
-            "timing": "CUDA events around every launch on the launching stream, 2 extra steps after the timed region",
+            "timing": "CUDA events around every launch on the launching stream, 2 extra steps after the timed region; "
+                      "an event between two launches serialises them, so these are stand-alone kernel durations "
+                      "(in the timed region K1 and K2 overlap their prologues through programmatic dependent launch)",
             "kernels": kernels,
             "hbm": {"compulsory_bytes_per_launch": hbm_bytes[dom],
                     "achieved_gbs": hbm_bytes[dom] / (kernels[dom]["avg_us"] * 1e-6) / 1e9,
