@@ -56,7 +56,7 @@ def workload_desc(cfg, beta, batch):
             "slices_per_gpu": batch, "image": [cfg.ny, cfg.nx], "views": cfg.n_views, "channels": cfg.n_channels,
             "subsets": cfg.n_subsets, "iterations_per_step": cfg.n_iters, "beta": beta,
             "l2": "flushed between steps (256 MiB memset, outside the per-step events)",
-            "parallelism": "one slice per GPU, no collective"}
+            "parallelism": f"{batch} slice(s) per GPU, no collective"}
 
 
 class ClockSampler:
@@ -170,7 +170,7 @@ def run_ours(args, cfg, beta):
 
     geom = osiv.Geometry(cfg.nx, cfg.ny, cfg.pixel_mm, cfg.n_views, cfg.n_channels, cfg.sad_mm, cfg.sdd_mm,
                          cfg.dgamma_rad, cfg.channel_offset, cfg.theta0_rad)
-    batch = 1
+    batch = args.slices if args.slices > 0 else (64 if args.workload == "4" else 1)
     lo, hi = sharding.slice_range(rank, world, world * batch)     # weak scaling: `batch` slices per rank
     counts_np = np.stack([si.make_case(cfg, slice_index=s)[2] for s in range(lo, hi)])
     prm = osiv.Params(beta=beta, n_subsets=cfg.n_subsets, n_iters=cfg.n_iters)
@@ -270,6 +270,7 @@ def run_ours(args, cfg, beta):
             "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
             "config": workload_desc(cfg, beta, batch),
             "seconds_per_500_iter_recon": (t_dev / args.steps) * 500.0 / cfg.n_iters,
+            "slices_per_s": world * batch * args.steps / t_dev,
             "wall_ms_per_step_incl_flush": 1e3 * wall / args.steps,
             "paper_context": {"gtx1080ti_s_per_slice_thinning_1_20": 3.71, "iterations_per_s": 134.8,
                               "source": "PAPER.md:156,164 Table I (other hardware, real data; context only)"},
@@ -298,7 +299,8 @@ def main():
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="3", choices=["1", "2", "3"])
+    ap.add_argument("--workload", default="3", choices=["1", "2", "3", "4"])
+    ap.add_argument("--slices", type=int, default=0, help="slices per GPU (default 1; 64 for workload 4)")
     ap.add_argument("--beta", type=float, default=None)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()

@@ -161,19 +161,23 @@ int ensure_images(osiv_handle* h, int batch, cudaStream_t st) {
 // made of whole orbits (V_S % 4 == 0); everything else takes the general NS = 1 kernels.
 int pick_ns(const osiv_handle* h, int VS) { return (h->dg.sym4 && !h->force_ns1 && VS % 4 == 0) ? 4 : 1; }
 
+constexpr int BATCH_THREADS = 512;      // block size cap when a launch carries several slices: two blocks per SM
+
 struct FwdPlan { int threads, rpb, segs, nparts, ns; size_t smem; };
 struct BackPlan { int nblk, threads, tpb, shares, ngx, ns; size_t smem; };
 
 // K1: the subset's base rays are dealt out in runs of rpb consecutive rays, one run per block and one block per SM
 // (per slice); a block is rpb rays x segs segments of each ray's line range, as many segments as fit into 1024
 // threads while a segment keeps at least FWD_MIN_LINES image lines.
-FwdPlan plan_forward(const osiv_handle* h, int VS) {
+FwdPlan plan_forward(const osiv_handle* h, int VS, int batch) {
     FwdPlan p;
     p.ns = pick_ns(h, VS);
     const long long R = (long long)(VS / p.ns) * h->geom.n_channels;
     p.rpb = (int)std::min<long long>(FWD_MAX_THREADS, std::max<long long>(1, (R + h->num_sms - 1) / h->num_sms));
     const int nmax = std::max(h->geom.nx, h->geom.ny);
-    p.segs = std::max(1, std::min(FWD_MAX_THREADS / p.rpb, nmax / FWD_MIN_LINES));
+    // several slices: two half-size blocks (of different slices) per SM fill each other's stalls (A8)
+    const int tmax = std::max(p.rpb, batch > 1 ? BATCH_THREADS : FWD_MAX_THREADS);
+    p.segs = std::max(1, std::min(tmax / p.rpb, nmax / FWD_MIN_LINES));
     p.threads = (p.rpb * p.segs + 31) / 32 * 32;
     p.nparts = (int)((R + p.rpb - 1) / p.rpb);
     p.smem = (size_t)p.segs * p.ns * p.rpb * sizeof(float);
@@ -194,7 +198,7 @@ cudaError_t launch_forward(FwdPlan p, int batch, const FwdArgs& a, cudaStream_t 
 
 // K2: the base tiles, numbered patch by patch (8 x 4 tiles, patches grouped 2 x 2), are dealt out in runs of tpb
 // consecutive tiles, one run per block and one block per SM (per slice); a block is tpb tiles x `shares` view shares.
-BackPlan plan_back(const osiv_handle* h, int VS) {
+BackPlan plan_back(const osiv_handle* h, int VS, int batch) {
     BackPlan p;
     p.ns = pick_ns(h, VS);
     const int tx = p.ns == 4 ? h->geom.nx / 4 : (h->geom.nx + BK_TX - 1) / BK_TX;
@@ -207,7 +211,8 @@ BackPlan plan_back(const osiv_handle* h, int VS) {
     const int VSb = VS / p.ns;
     // shares per quarter turn (NS == 4) or in all: as many as fit, then the fewest that keep the same number of
     // views per share
-    int sq = std::max(1, std::min(BK_MAX_THREADS / (p.tpb * p.ns), VSb));
+    const int tmax = std::max(p.tpb * p.ns, batch > 1 ? BATCH_THREADS : BK_MAX_THREADS);
+    int sq = std::max(1, std::min(tmax / (p.tpb * p.ns), VSb));
     const int trips = (VSb + sq - 1) / sq;
     sq = (VSb + trips - 1) / trips;
     p.shares = sq * p.ns;
@@ -425,8 +430,8 @@ int osiv_set_overlap(osiv_handle* h, int32_t enable) {
 int osiv_get_plan(const osiv_handle* h, int32_t n_subsets, int32_t batch, int32_t* out8) {
     if (!h || !out8 || batch <= 0 || (n_subsets > 0 && h->geom.n_views % n_subsets != 0)) return OSIV_ERR_INVALID_ARG;
     const int VS = n_subsets > 0 ? h->geom.n_views / n_subsets : h->geom.n_views;
-    const FwdPlan f = plan_forward(h, VS);
-    const BackPlan b = plan_back(h, VS);
+    const FwdPlan f = plan_forward(h, VS, batch);
+    const BackPlan b = plan_back(h, VS, batch);
     out8[0] = f.ns; out8[1] = f.segs; out8[2] = f.nparts * batch; out8[3] = f.threads;
     out8[4] = b.ns; out8[5] = b.shares; out8[6] = b.nblk * batch; out8[7] = b.threads;
     return OSIV_OK;
@@ -459,7 +464,7 @@ int osiv_forward(osiv_handle* h, const float* d_img, float* d_sino, int32_t batc
     int rc = ensure_images(h, batch, st);
     if (rc != OSIV_OK) return rc;
     const int VS = subset_views(h, subset, n_subsets);
-    const FwdPlan p = plan_forward(h, VS);
+    const FwdPlan p = plan_forward(h, VS, batch);
     if ((rc = ensure_forward_ws(h, p, batch)) != OSIV_OK) return rc;
     k_pad_transpose<<<dim3((h->geom.nx + 31) / 32, (h->geom.ny + 31) / 32, batch), 256, 0, st>>>(h->dg, d_img, h->d_imgA,
                                                                                              h->d_imgTA);
@@ -478,7 +483,7 @@ int osiv_backward(osiv_handle* h, const float* d_sino, float* d_img, int32_t bat
     if (!guard.ok) { cudaGetLastError(); return OSIV_ERR_CUDA; }
     cudaStream_t st = (cudaStream_t)cuda_stream;
     const int VS = subset_views(h, subset, n_subsets), M = subset < 0 ? 1 : n_subsets;
-    const BackPlan p = plan_back(h, VS);
+    const BackPlan p = plan_back(h, VS, batch);
     int rc = ensure_res(h, VS, p.ns, batch, st);
     if (rc != OSIV_OK) return rc;
     const int Cp = h->geom.n_channels + h->res_pad;
@@ -520,8 +525,8 @@ int osiv_reconstruct(osiv_handle* h, const float* d_counts, const float* d_blank
     const int VS = h->geom.n_views / M, C = h->geom.n_channels;
     int rc = ensure_images(h, batch, st);
     if (rc != OSIV_OK) return rc;
-    const FwdPlan fp = plan_forward(h, VS);
-    const BackPlan bp = plan_back(h, VS);
+    const FwdPlan fp = plan_forward(h, VS, batch);
+    const BackPlan bp = plan_back(h, VS, batch);
     if ((rc = ensure_res(h, VS, fp.ns, batch, st)) != OSIV_OK) return rc;
     const int Cp = C + h->res_pad;
     if ((rc = ensure_forward_ws(h, fp, batch)) != OSIV_OK) return rc;

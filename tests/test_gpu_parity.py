@@ -360,8 +360,11 @@ def test_reconstruct_batch_is_independent_and_deterministic(osiv):
         b, trb = h.reconstruct(dev(counts), cfg.i0, prm, trace=True)
         assert torch.equal(a, b) and np.array_equal(tra, trb)          # atomic-free, fixed-order reductions
         for s in range(3):
+            # a launch that carries several slices splits rays and views differently (two half-size blocks per SM), so a
+            # slice reconstructed alone agrees up to the rounding order of the sums, with the same lambda decisions
             one, tr1 = h.reconstruct(dev(counts[s:s + 1]), cfg.i0, prm, trace=True)
-            assert torch.equal(one[0], a[s]) and np.array_equal(tr1[0], tra[s])
+            assert rel(host(one)[0], host(a)[s].astype(np.float64)) < 2e-6
+            assert np.array_equal(tr1[0, :, 1], tra[s, :, 1]) and np.allclose(tr1[0, :, 0], tra[s, :, 0], rtol=1e-6, atol=0)
         assert not torch.equal(a[0], a[1])
         # the host-buffer entry point gives the same bits
         hst = h.reconstruct_host(counts, cfg.i0, prm)
