@@ -293,19 +293,63 @@ def run_ours(args, cfg, beta):
     return 0
 
 
+def run_projector_pair(args, cfg):
+    """Config 5 (BASELINE.json): forward A and adjoint A^T alone, all views, on a uniform-random image / sinogram.
+    Not the headline metric: one extra JSON line with ms per pass, nnz/s ("rays.pixels/s" = ray-pixel intersections),
+    algorithmic GB/s against the measured HBM peak and the adjoint-identity error of the fp32 outputs."""
+    import torch
+    import paper_1903_10088_b200 as osiv
+    torch.cuda.set_device(0)
+    geom = osiv.Geometry(cfg.nx, cfg.ny, cfg.pixel_mm, cfg.n_views, cfg.n_channels, cfg.sad_mm, cfg.sdd_mm)
+    img_np, sino_np = si.uniform_image(cfg), si.uniform_sinogram(cfg)
+    img, sino = torch.from_numpy(img_np)[None].cuda(), torch.from_numpy(sino_np)[None].cuda()
+    flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device="cuda")
+    h = osiv.Handle(geom, max_batch=1, device=0)
+    out = {}
+    for name, fn in (("forward", lambda: h.forward(img)), ("back", lambda: h.backward(sino))):
+        for _ in range(max(args.warmup, 3)):
+            res = fn()
+        ts = []
+        for _ in range(args.steps):
+            flush.zero_()
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(); res = fn(); b.record()
+            torch.cuda.synchronize()
+            ts.append(a.elapsed_time(b))
+        out[name] = (float(np.median(ts)), res.cpu().numpy()[0].astype(np.float64))
+    nnz = NNZ_PER_RAY_PER_N * max(cfg.nx, cfg.ny) * cfg.n_views * cfg.n_channels
+    bytes_alg = 4.0 * (cfg.nx * cfg.ny + cfg.n_views * cfg.n_channels)          # image + sinogram, once each
+    peaks, kind = load_peaks()
+    lhs = float(np.dot(out["forward"][1].ravel(), sino_np.astype(np.float64).ravel()))
+    rhs = float(np.dot(img_np.astype(np.float64).ravel(), out["back"][1].ravel()))
+    line = {"metric": "projector_pair", "workload": f"config{cfg.name}: {cfg.nx}x{cfg.ny}, {cfg.n_views}x{cfg.n_channels}, all views",
+            "n_gpus": 1, "steps": args.steps, "dtype": "f32", "data": "synthetic", "nnz_per_pass": nnz,
+            "adjoint_rel_error": abs(lhs - rhs) / abs(lhs), "l2": "flushed between passes"}
+    for name in ("forward", "back"):
+        ms = out[name][0]
+        line[name] = {"ms_per_pass": ms, "nnz_per_s": nnz / (ms * 1e-3), "algorithmic_gbs": bytes_alg / (ms * 1e-3) / 1e9,
+                      "hbm_frac": bytes_alg / (ms * 1e-3) / 1e9 / float(peaks["hbm_gbs"]), "hbm_peak_kind": kind,
+                      "alu_frac": nnz * FP32_FLOP_PER_NNZ / (ms * 1e-3) / 1e12 /
+                                  (SM_COUNT * FP32_LANES_PER_SM * 2 * float(peaks.get("sm_max_mhz", 1965.0)) * 1e6 / 1e12)}
+    print(json.dumps(line))
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="3", choices=["1", "2", "3", "4"])
+    ap.add_argument("--workload", default="3", choices=["1", "2", "3", "4", "5a", "5b"])
     ap.add_argument("--slices", type=int, default=0, help="slices per GPU (default 1; 64 for workload 4)")
     ap.add_argument("--beta", type=float, default=None)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     cfg = si.scan_config(args.workload)
-    beta = args.beta if args.beta is not None else (0.005 if args.workload == "3" else cfg.betas[0])
+    beta = args.beta if args.beta is not None else (0.005 if args.workload == "3" else (cfg.betas[0] if cfg.betas else 0.0))
+    if args.workload in ("5a", "5b"):
+        return run_projector_pair(args, cfg)
     if args.impl == "reference":
         return run_reference(args, cfg, beta)
     return run_ours(args, cfg, beta)

@@ -30,7 +30,7 @@ class _CParams(C.Structure):
     _fields_ = [("beta", C.c_double), ("n_subsets", C.c_int32), ("n_iters", C.c_int32),
                 ("mu0", C.c_double), ("lambda0", C.c_double), ("lambda_up", C.c_double),
                 ("lambda_down", C.c_double), ("lambda_min", C.c_double), ("kappa", C.c_double),
-                ("tv_eps", C.c_double), ("return_best", C.c_int32), ("_pad", C.c_int32),
+                ("tv_eps", C.c_double), ("return_best", C.c_int32), ("monitor_mode", C.c_int32),
                 ("forced_lambda", C.POINTER(C.c_double))]
 
 
@@ -64,6 +64,7 @@ class Params:
     kappa: float = 100.0
     tv_eps: float = 1e-5
     return_best: int = 0
+    monitor_mode: int = 0         # 0: Eq. 4-5 compare with D(n-1) (C10); 1: with D(n-M), the same subset (G3)
     forced_lambda: Optional[np.ndarray] = None
 
 
@@ -224,7 +225,7 @@ def reconstruct(g: Geometry, counts, blank, prm: Params):
     if forced is not None:
         assert forced.shape == (prm.n_iters,)
     cp = _CParams(prm.beta, prm.n_subsets, prm.n_iters, prm.mu0, prm.lambda0, prm.lambda_up, prm.lambda_down,
-                  prm.lambda_min, prm.kappa, prm.tv_eps, prm.return_best, 0, _dp(forced))
+                  prm.lambda_min, prm.kappa, prm.tv_eps, prm.return_best, prm.monitor_mode, _dp(forced))
     img = np.zeros((g.ny, g.nx), dtype=np.float64)
     trace = np.zeros((prm.n_iters, 2), dtype=np.float64)
     status = lib().oracle_reconstruct(C.byref(g.c()), _dp(counts), _dp(b), bs, C.byref(cp), _dp(img), _dp(trace))

@@ -54,7 +54,8 @@ typedef struct {
     double  kappa;           /* step scale (C6) */
     double  tv_eps;          /* TV smoothing (C9) */
     int32_t return_best;
-    int32_t _pad;
+    int32_t monitor_mode;    /* which earlier D Eq. 4-5 compare D(n) with: 0 = D(n-1), the previous iteration (C10);
+                                1 = D(n-M), the same subset one pass earlier (reading G3; lambda(n) = lambda0 for n < M) */
     const double* forced_lambda;   /* NULL or n_iters values replayed instead of Eq. 4-5 */
 } oracle_params;
 
@@ -359,6 +360,7 @@ int oracle_reconstruct(const oracle_geometry* g, const double* counts, const dou
     double* resid = (double*)malloc(sizeof(double) * nray);
     const double tau = oracle_tau(g, M, prm->kappa);
     double lambda = prm->lambda0, Dprev = 0.0, Dbest = INFINITY;
+    double* Dsub  = (double*)malloc(sizeof(double) * M);      /* monitor_mode 1: D of each subset's last visit */
     int status = 0;
 
     for (size_t r = 0; r < npix; ++r) mu[r] = prm->mu0;                      /* PAPER.md:114 */
@@ -370,11 +372,12 @@ int oracle_reconstruct(const oracle_geometry* g, const double* counts, const dou
         double D = oracle_residual(g, l, counts, blank, blank_scalar, m, M, resid);
         if (!isfinite(D)) status = -3;
         if (prm->forced_lambda) lambda = prm->forced_lambda[n];
-        else if (n == 0)        lambda = prm->lambda0;                        /* PAPER.md:108 */
-        else if (D < Dprev)     lambda = lambda + prm->lambda_up;             /* Eq. 4 */
+        else if (n < (prm->monitor_mode ? M : 1)) lambda = prm->lambda0;      /* PAPER.md:108 */
+        else if (D < (prm->monitor_mode ? Dsub[m] : Dprev)) lambda = lambda + prm->lambda_up;   /* Eq. 4 */
         else { lambda = lambda - prm->lambda_down;                            /* Eq. 5 */
                if (lambda < prm->lambda_min) lambda = prm->lambda_min; }      /* floor, C10 */
         Dprev = D;
+        Dsub[m] = D;
         if (trace) { trace[2 * n] = D; trace[2 * n + 1] = lambda; }
         if (prm->return_best && D < Dbest) { Dbest = D; memcpy(best, mu, sizeof(double) * npix); }
         oracle_backward(g, resid, grad, m, M);                                /* "estimation" */
@@ -394,6 +397,6 @@ int oracle_reconstruct(const oracle_geometry* g, const double* counts, const dou
     } else {
         memcpy(img_out, mu, sizeof(double) * npix);
     }
-    free(mu); free(best); free(grad); free(tvg); free(l); free(resid);
+    free(mu); free(best); free(grad); free(tvg); free(l); free(resid); free(Dsub);
     return status;
 }

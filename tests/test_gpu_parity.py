@@ -374,6 +374,23 @@ def test_reconstruct_batch_is_independent_and_deterministic(osiv):
         assert h.launch_count() - n0 >= 2 * prm.n_iters
 
 
+def test_dependent_launch_chain_gives_the_same_bits_as_stream_order(osiv):
+    """K1/K2 chained by programmatic dependent launch (default) vs plain stream order: the overlap moves only
+    constant-dependent prologues ahead of the wait, so images and traces must be identical bit for bit."""
+    cfg = si.scan_config("2")
+    _, gg = geoms(cfg)
+    counts = si.make_case(cfg)[2]
+    prm = osiv.Params(beta=cfg.betas[0], n_subsets=cfg.n_subsets, n_iters=60, return_best=1)
+    with osiv.Handle(gg, max_batch=1) as h:
+        a, tra = h.reconstruct(dev(counts)[None], cfg.i0, prm, trace=True)
+        h.set_overlap(False)
+        b, trb = h.reconstruct(dev(counts)[None], cfg.i0, prm, trace=True)
+        h.set_overlap(True)
+        c2, trc = h.reconstruct(dev(counts)[None], cfg.i0, prm, trace=True)
+    assert torch.equal(a, b) and np.array_equal(tra, trb)
+    assert torch.equal(a, c2) and np.array_equal(tra, trc)
+
+
 def test_reconstruct_zero_iterations_and_errors(osiv):
     cfg = si.scan_config("1")
     _, gg = geoms(cfg)

@@ -146,6 +146,41 @@ def test_P10_step_rule_replay_and_oscillation():
     assert D3 <= trace3[:, 0].min() * (1 + 1e-12)
 
 
+def replay_step_rule_same_subset(D, prm):
+    M, lam = prm.n_subsets, np.zeros(len(D))
+    for n in range(len(D)):
+        if n < M:
+            lam[n] = prm.lambda0
+        elif D[n] < D[n - M]:
+            lam[n] = lam[n - 1] + prm.lambda_up
+        else:
+            lam[n] = max(lam[n - 1] - prm.lambda_down, prm.lambda_min)
+    return lam
+
+
+def test_P10b_same_subset_monitor_variant():
+    # reading G3's alternative: D(n) is compared with D(n-M), the last visit of the same subset.  With one subset the
+    # two rules are the same rule; with M > 1 lambda stays at lambda0 for the first pass, the trace replays from its own
+    # D values, and the step no longer collapses under strong thinning (the literal rule compares different subsets'
+    # D, which differ by more than one update changes them; "the oscillation behavior is emphasized").
+    cfg, g = small_case(n=16, V=24, C=24, i0=2e4, seed=5)
+    _, _, counts = si.make_case(cfg)
+    a = oracle.reconstruct(g, counts, cfg.i0, oracle.Params(beta=0.002, n_subsets=1, n_iters=300))
+    b = oracle.reconstruct(g, counts, cfg.i0, oracle.Params(beta=0.002, n_subsets=1, n_iters=300, monitor_mode=1))
+    assert np.array_equal(a[0], b[0]) and np.array_equal(a[1], b[1])
+    for M in (3, 6):
+        prm = oracle.Params(beta=0.002, n_subsets=M, n_iters=240, monitor_mode=1)
+        img, trace, status = oracle.reconstruct(g, counts, cfg.i0, prm)
+        assert status == 0
+        assert np.all(trace[:M, 1] == prm.lambda0)
+        assert np.array_equal(trace[:, 1], replay_step_rule_same_subset(trace[:, 0], prm))
+        lit = oracle.reconstruct(g, counts, cfg.i0, oracle.Params(beta=0.002, n_subsets=M, n_iters=240))[1]
+        assert not np.array_equal(lit[:, 1], trace[:, 1])
+        # per-subset D falls pass after pass at first, so lambda climbs by lambda_up every iteration after the first pass
+        per = trace[:, 0].reshape(-1, M)
+        assert np.all(np.diff(per[:5], axis=0) < 0) and abs(trace[5 * M - 1, 1] - (prm.lambda0 + 4 * M * prm.lambda_up)) < 1e-12
+
+
 def test_P11_adaptive_lambda_is_about_three_times_faster():
     # "a similar degree of convergence is achieved with 500 iterations compared to 1500
     # iterations using a constant convergence parameter" -- same counts, on a 32x32 body-sized phantom
