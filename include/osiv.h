@@ -73,7 +73,8 @@ typedef struct {
     double  kappa;           /* step scale, 100 (C6): tau_S = kappa*SAD*dgamma/(V_S*max(nx,ny)*pixel^3) */
     double  tv_eps;          /* TV smoothing, 1e-5 /mm (C9) */
     int32_t return_best;     /* 0: final iterate; 1: iterate with the smallest monitor D */
-    int32_t reserved;        /* must be 0 */
+    int32_t monitor_mode;    /* which earlier D Eq. 4-5 compare D(n) with: 0 = D(n-1), the previous iteration (C10, default);
+                                1 = D(n-M), the same subset one pass earlier (G3; lambda(n) = lambda0 for n < M) */
     const double* forced_lambda;  /* HOST pointer: NULL, or n_iters values used instead of Eq. 4-5 */
 } osiv_params;
 

@@ -38,7 +38,7 @@ class _CParams(C.Structure):
     _fields_ = [("beta", C.c_double), ("n_subsets", C.c_int32), ("n_iters", C.c_int32), ("mu0", C.c_double),
                 ("lambda0", C.c_double), ("lambda_up", C.c_double), ("lambda_down", C.c_double),
                 ("lambda_min", C.c_double), ("kappa", C.c_double), ("tv_eps", C.c_double),
-                ("return_best", C.c_int32), ("reserved", C.c_int32), ("forced_lambda", C.POINTER(C.c_double))]
+                ("return_best", C.c_int32), ("monitor_mode", C.c_int32), ("forced_lambda", C.POINTER(C.c_double))]
 
 
 @dataclass
@@ -72,6 +72,7 @@ class Params:
     kappa: float = 100.0
     tv_eps: float = 1e-5
     return_best: int = 0
+    monitor_mode: int = 0
     forced_lambda: Optional[np.ndarray] = None
 
 
@@ -128,7 +129,7 @@ def default_params() -> Params:
     _check(lib().osiv_default_params(C.byref(cp)), "osiv_default_params")
     return Params(beta=cp.beta, n_subsets=cp.n_subsets, n_iters=cp.n_iters, mu0=cp.mu0, lambda0=cp.lambda0,
                   lambda_up=cp.lambda_up, lambda_down=cp.lambda_down, lambda_min=cp.lambda_min, kappa=cp.kappa,
-                  tv_eps=cp.tv_eps, return_best=cp.return_best)
+                  tv_eps=cp.tv_eps, return_best=cp.return_best, monitor_mode=cp.monitor_mode)
 
 
 def ray_table(geom: "Geometry"):
@@ -168,7 +169,7 @@ def _cparams(p: Params):
             raise ValueError("forced_lambda must have n_iters entries")
         fptr = forced.ctypes.data_as(C.POINTER(C.c_double))
     cp = _CParams(p.beta, p.n_subsets, p.n_iters, p.mu0, p.lambda0, p.lambda_up, p.lambda_down, p.lambda_min,
-                  p.kappa, p.tv_eps, p.return_best, 0, fptr)
+                  p.kappa, p.tv_eps, p.return_best, p.monitor_mode, fptr)
     return cp, forced
 
 

@@ -37,6 +37,7 @@ struct osiv_handle {
     int num_sms = 148;
     size_t trace_elems = 0;     double* d_trace = nullptr;
     size_t forced_elems = 0;    double* d_forced = nullptr;
+    size_t dhist_elems = 0;     double* d_dhist = nullptr;
     // staging for osiv_reconstruct_host
     size_t hc_elems = 0;        float* d_hcounts = nullptr;
     float* d_hblank = nullptr;
@@ -285,7 +286,7 @@ int osiv_default_params(osiv_params* p) {
     p->mu0 = 0.005;                                     // PAPER.md:140 (0.05 /cm)
     p->lambda0 = 0.01; p->lambda_up = 1e-4; p->lambda_down = 2e-4;
     p->lambda_min = 1e-4; p->kappa = 100.0; p->tv_eps = 1e-5;
-    p->return_best = 0; p->reserved = 0; p->forced_lambda = nullptr;
+    p->return_best = 0; p->monitor_mode = 0; p->forced_lambda = nullptr;
     return OSIV_OK;
 }
 
@@ -389,7 +390,7 @@ int osiv_destroy(osiv_handle* h) {
         cudaDeviceSynchronize();
         void* ptrs[] = {h->d_rays, h->d_views, h->d_hs, h->d_imgA, h->d_imgB, h->d_imgTA, h->d_imgTB, h->d_best, h->d_res,
                         h->d_dparts, h->d_state, h->d_not_finite, h->d_inv_bref, h->d_trace,
-                        h->d_forced, h->d_hcounts, h->d_hblank, h->d_himg};
+                        h->d_forced, h->d_dhist, h->d_hcounts, h->d_hblank, h->d_himg};
         for (void* p : ptrs) if (p) cudaFree(p);
         for (cudaEvent_t e : h->events) cudaEventDestroy(e);
         cudaGetLastError();
@@ -514,7 +515,7 @@ int osiv_reconstruct(osiv_handle* h, const float* d_counts, const float* d_blank
                      const osiv_params* prm, int32_t batch, float* d_img_out, double* h_trace, void* cuda_stream) {
     if (!h || !d_counts || !prm || !d_img_out || batch <= 0 || batch > h->max_batch) return OSIV_ERR_INVALID_ARG;
     const int M = prm->n_subsets, N = prm->n_iters;
-    if (M <= 0 || N < 0 || h->geom.n_views % M != 0 || prm->reserved != 0) return OSIV_ERR_INVALID_ARG;
+    if (M <= 0 || N < 0 || h->geom.n_views % M != 0 || (prm->monitor_mode != 0 && prm->monitor_mode != 1)) return OSIV_ERR_INVALID_ARG;
     if (!d_blank && !(blank_scalar > 0.f)) return OSIV_ERR_INVALID_ARG;
     if (!(prm->tv_eps >= 0.0) || !std::isfinite(prm->beta) || !std::isfinite(prm->mu0) || !(prm->kappa > 0.0))
         return OSIV_ERR_INVALID_ARG;
@@ -535,6 +536,7 @@ int osiv_reconstruct(osiv_handle* h, const float* d_counts, const float* d_blank
         if ((rc = grow(&h->d_forced, &h->forced_elems, (size_t)N)) != OSIV_OK) return rc;
         OSIV_CUDA(cudaMemcpyAsync(h->d_forced, prm->forced_lambda, (size_t)N * sizeof(double), cudaMemcpyHostToDevice, st));
     }
+    if (prm->monitor_mode && (rc = grow(&h->d_dhist, &h->dhist_elems, (size_t)batch * 2 * M)) != OSIV_OK) return rc;
     double tau;
     osiv_get_tau(h, M, prm->kappa, &tau);
 
@@ -555,6 +557,7 @@ int osiv_reconstruct(osiv_handle* h, const float* d_counts, const float* d_blank
     b.ip.forced = (prm->forced_lambda && N > 0) ? h->d_forced : nullptr;
     b.ip.trace = (h_trace && N > 0) ? h->d_trace : nullptr;
     b.ip.n_iters = N; b.ip.return_best = prm->return_best;
+    b.ip.monitor_mode = prm->monitor_mode; b.ip.M = M; b.ip.dhist = h->d_dhist;
     b.tau = tau; b.beta_over_M = (float)(prm->beta / M); b.eps2 = (float)(prm->tv_eps * prm->tv_eps);
 
     float *cur = h->d_imgA, *curT = h->d_imgTA, *nxt = h->d_imgB, *nxtT = h->d_imgTB;

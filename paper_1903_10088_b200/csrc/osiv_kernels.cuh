@@ -70,6 +70,9 @@ struct IterParams {
     double* trace;                         // device, [batch][n_iters][2] or null
     int n_iters;
     int return_best;
+    int monitor_mode;                      // 0: compare with D(n-1); 1: with D(n-M) (same subset)
+    int M;
+    double* dhist;                         // monitor_mode 1: [batch][2M] ring of the last 2M monitor values
 };
 
 struct FwdArgs {
@@ -348,8 +351,8 @@ __device__ __forceinline__ StepInfo step_rule(const BackArgs& a, int s, int lane
     const int n = st.n;
     double lam;
     if (a.ip.forced)          lam = a.ip.forced[n];
-    else if (n == 0)          lam = a.ip.lambda0;
-    else if (si.D < st.D_prev) lam = st.lambda + a.ip.up;
+    else if (n < (a.ip.monitor_mode ? a.ip.M : 1)) lam = a.ip.lambda0;
+    else if (si.D < (a.ip.monitor_mode ? a.ip.dhist[(size_t)s * 2 * a.ip.M + (n - a.ip.M) % (2 * a.ip.M)] : st.D_prev)) lam = st.lambda + a.ip.up;
     else                      lam = fmax(st.lambda - a.ip.down, a.ip.lmin);
     si.lambda = lam;
     si.improved = a.ip.return_best && si.D < st.D_best;
@@ -359,6 +362,8 @@ __device__ __forceinline__ StepInfo step_rule(const BackArgs& a, int s, int lane
         o.n = n + 1; o.improved = si.improved; o.pad0 = 0; o.pad1 = 0;
         a.state_out[s] = o;
         if (!isfinite(si.D)) a.not_finite[s] = 1;
+        // slot n % 2M is written while every block may still read slot (n - M) % 2M: never the same slot
+        if (a.ip.monitor_mode) a.ip.dhist[(size_t)s * 2 * a.ip.M + n % (2 * a.ip.M)] = si.D;
         if (a.ip.trace) {
             double* tr = a.ip.trace + ((size_t)s * a.ip.n_iters + n) * 2;
             tr[0] = si.D;

@@ -374,6 +374,31 @@ def test_reconstruct_batch_is_independent_and_deterministic(osiv):
         assert h.launch_count() - n0 >= 2 * prm.n_iters
 
 
+def test_reconstruct_same_subset_monitor_variant(osiv):
+    """monitor_mode = 1 (reading G3): Eq. 4-5 compare D(n) with D(n-M).  Config 2 (10 subsets) and an
+    odd geometry in a batch of two; lambda traces equal to the oracle's, images within the bar."""
+    cfg = si.scan_config("2")
+    og, gg = geoms(cfg)
+    counts = si.make_case(cfg)[2]
+    kw = dict(beta=cfg.betas[0], n_subsets=cfg.n_subsets, n_iters=cfg.n_iters, monitor_mode=1, return_best=1)
+    ref, tr_ref, status = oracle.reconstruct(og, counts, cfg.i0, oracle.Params(**kw))
+    assert status == 0 and not np.array_equal(
+        tr_ref[:, 1], oracle.reconstruct(og, counts, cfg.i0, oracle.Params(**dict(kw, monitor_mode=0)))[1][:, 1])
+    with osiv.Handle(gg, max_batch=1) as h:
+        got, tr = h.reconstruct(dev(counts)[None], cfg.i0, osiv.Params(**kw), trace=True)
+    assert np.array_equal(tr[0, :, 1], tr_ref[:, 1])
+    assert np.all(np.abs(tr[0, :, 0] - tr_ref[:, 0]) <= 1e-5 * tr_ref[:, 0])
+    assert rel(host(got)[0], ref) < IMG_TOL
+    og, gg = geoms(ODD)
+    cs = np.stack([si.make_case(ODD, slice_index=s)[2] for s in range(2)])
+    kw = dict(beta=0.003, n_subsets=4, n_iters=30, monitor_mode=1)
+    with osiv.Handle(gg, max_batch=2) as h:
+        got, tr = h.reconstruct(dev(cs), ODD.i0, osiv.Params(**kw), trace=True)
+    for s in range(2):
+        ref, tr_ref, _ = oracle.reconstruct(og, cs[s], ODD.i0, oracle.Params(**kw))
+        assert np.array_equal(tr[s, :, 1], tr_ref[:, 1]) and rel(host(got)[s], ref) < IMG_TOL
+
+
 def test_dependent_launch_chain_gives_the_same_bits_as_stream_order(osiv):
     """K1/K2 chained by programmatic dependent launch (default) vs plain stream order: the overlap moves only
     constant-dependent prologues ahead of the wait, so images and traces must be identical bit for bit."""
