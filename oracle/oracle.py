@@ -23,7 +23,8 @@ _lib = None
 class _CGeometry(C.Structure):
     _fields_ = [("nx", C.c_int32), ("ny", C.c_int32), ("pixel_mm", C.c_double),
                 ("n_views", C.c_int32), ("n_channels", C.c_int32), ("sad_mm", C.c_double),
-                ("dgamma_rad", C.c_double), ("channel_offset", C.c_double), ("theta0_rad", C.c_double)]
+                ("dgamma_rad", C.c_double), ("channel_offset", C.c_double), ("theta0_rad", C.c_double),
+                ("model", C.c_int32), ("_pad", C.c_int32)]
 
 
 class _CParams(C.Structure):
@@ -45,10 +46,11 @@ class Geometry:
     dgamma_rad: float = 0.0
     channel_offset: float = 0.0
     theta0_rad: float = 0.0
+    model: int = 0                # 0: exact chord length (C2); 1: Joseph's interpolating model (8(f)-2)
 
     def c(self) -> _CGeometry:
         return _CGeometry(self.nx, self.ny, self.pixel_mm, self.n_views, self.n_channels, self.sad_mm,
-                          self.dgamma_rad, self.channel_offset, self.theta0_rad)
+                          self.dgamma_rad, self.channel_offset, self.theta0_rad, self.model, 0)
 
 
 @dataclass

@@ -44,6 +44,8 @@ typedef struct {
     double  dgamma_rad;      /* channel pitch; <=0 -> 2*asin(R_FOV/SAD)/C, R_FOV = min(nx,ny)*pixel/2  (C1) */
     double  channel_offset;  /* gamma_c = (c-(C-1)/2+off)*dgamma */
     double  theta0_rad;      /* theta_v = theta0 + 2*pi*v/V */
+    int32_t model;           /* system matrix: 0 = exact chord length (C2); 1 = Joseph's interpolating model */
+    int32_t _pad;
 } oracle_geometry;
 
 typedef struct {
@@ -118,13 +120,28 @@ static double chord_closed_form(double dx, double dy, double delta, double p) {
     return 0.0;
 }
 
+/* ---- second system matrix: Joseph's model.  The ray is sampled once on every image line of its
+ * major axis (rows if |dy| >= |dx|, else columns), at the line's centre; the sample is the linear interpolation of
+ * the line's two pixels next to the crossing, times the path length per line h = D/max(|dx|,|dy|).  As a function of
+ * the perpendicular distance p of a pixel centre from the ray: the in-line distance between the centre and the
+ * crossing is |p|/max(|dx|,|dy|), so a = h * max(0, 1 - |p| / (D*max(|dx|,|dy|))). ---- */
+static double joseph_closed_form(double dx, double dy, double delta, double p) {
+    double m = fabs(dx) > fabs(dy) ? fabs(dx) : fabs(dy);
+    double t = 1.0 - fabs(p) / (delta * m);
+    return t > 0.0 ? (delta / m) * t : 0.0;
+}
+
+static double weight_closed_form(int model, double dx, double dy, double delta, double p) {
+    return model == 1 ? joseph_closed_form(dx, dy, delta, p) : chord_closed_form(dx, dy, delta, p);
+}
+
 /* a(i,r) for ray i=(v,c), pixel r=(ix,iy) */
 double oracle_weight(const oracle_geometry* g, int v, int c, int ix, int iy) {
     double sx, sy, dx, dy;
     oracle_ray(g, v, c, &sx, &sy, &dx, &dy);
     double px = pix_x(g, ix), py = pix_y(g, iy);
     double p = (px - sx) * dy - (py - sy) * dx;      /* signed distance of the pixel centre from the ray */
-    return chord_closed_form(dx, dy, g->pixel_mm, p);
+    return weight_closed_form(g->model, dx, dy, g->pixel_mm, p);
 }
 
 static int subset_views(const oracle_geometry* g, int subset, int n_subsets) {
@@ -166,7 +183,8 @@ void oracle_forward(const oracle_geometry* g, const double* img, double* sino, i
         double sum = 0.0;
         if (fabs(dy) >= fabs(dx)) {
             /* the ray crosses every pixel row once; inside a row strip it deviates at most D/2 in x
-             * from its position at the row centre, so it can only touch pixels ixc-1..ixc+1 */
+             * from its position at the row centre, so it can only touch pixels ixc-1..ixc+1 (Joseph: the two pixel
+             * centres next to the crossing at the row centre are among these three) */
             for (int iy = 0; iy < g->ny; ++iy) {
                 double y = pix_y(g, iy);
                 double x = sx + (y - sy) / dy * dx;
@@ -174,7 +192,7 @@ void oracle_forward(const oracle_geometry* g, const double* img, double* sino, i
                 for (int ix = ixc - 1; ix <= ixc + 1; ++ix) {
                     if (ix < 0 || ix >= g->nx) continue;
                     double p = (pix_x(g, ix) - sx) * dy - (y - sy) * dx;
-                    sum += chord_closed_form(dx, dy, delta, p) * img[(size_t)iy * g->nx + ix];
+                    sum += weight_closed_form(g->model, dx, dy, delta, p) * img[(size_t)iy * g->nx + ix];
                 }
             }
         } else {
@@ -185,7 +203,7 @@ void oracle_forward(const oracle_geometry* g, const double* img, double* sino, i
                 for (int iy = iyc - 1; iy <= iyc + 1; ++iy) {
                     if (iy < 0 || iy >= g->ny) continue;
                     double p = (x - sx) * dy - (pix_y(g, iy) - sy) * dx;
-                    sum += chord_closed_form(dx, dy, delta, p) * img[(size_t)iy * g->nx + ix];
+                    sum += weight_closed_form(g->model, dx, dy, delta, p) * img[(size_t)iy * g->nx + ix];
                 }
             }
         }
@@ -212,7 +230,9 @@ void oracle_forward_brute(const oracle_geometry* g, const double* img, double* s
 int oracle_candidate_K(const oracle_geometry* g) {
     double rmax = 0.5 * g->pixel_mm * sqrt((double)g->nx * g->nx + (double)g->ny * g->ny);
     double spacing = (g->sad_mm - rmax) * oracle_dgamma(g);
-    return (int)ceil((g->pixel_mm / sqrt(2.0)) / spacing) + 1;
+    /* Joseph: a pixel is touched by rays within D*max(|dx|,|dy|) <= D of its centre */
+    double reach = g->model == 1 ? g->pixel_mm : g->pixel_mm / sqrt(2.0);
+    return (int)ceil(reach / spacing) + 1;
 }
 
 /* ---- C3 back: g_r = sum_{i in S} a(i,r) r_i, gather per pixel ---- */
@@ -238,7 +258,7 @@ void oracle_backward(const oracle_geometry* g, const double* sino, double* img, 
                 if (c < 0 || c >= C) continue;
                 double dx = t.dx[(size_t)j * C + c], dy = t.dy[(size_t)j * C + c];
                 double p = (px - sx) * dy - (py - sy) * dx;
-                sum += chord_closed_form(dx, dy, g->pixel_mm, p) * sino[(size_t)j * C + c];
+                sum += weight_closed_form(g->model, dx, dy, g->pixel_mm, p) * sino[(size_t)j * C + c];
             }
         }
         img[r] = sum;
