@@ -57,6 +57,11 @@ typedef struct {
     double  dgamma_rad;      /* channel pitch; <= 0 selects 2*asin(R_FOV/SAD)/C, R_FOV = min(nx,ny)*pixel/2 */
     double  channel_offset;  /* in channels */
     double  theta0_rad;
+    int32_t model;           /* system matrix a(i,r): 0 = exact length of the ray inside the pixel (reading C2, default);
+                                1 = Joseph's interpolating model: one sample per image line of the ray's major axis,
+                                linear interpolation between the line's two nearest pixels, times the path length per
+                                line.  Forward and back use the same a(i,r) in either case. */
+    int32_t reserved;        /* must be 0 */
 } osiv_geometry;
 
 /* Iteration parameters.  osiv_default_params() fills the paper's values. */

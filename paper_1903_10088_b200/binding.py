@@ -31,7 +31,7 @@ class OsivError(RuntimeError):
 class _CGeometry(C.Structure):
     _fields_ = [("nx", C.c_int32), ("ny", C.c_int32), ("pixel_mm", C.c_double), ("n_views", C.c_int32),
                 ("n_channels", C.c_int32), ("sad_mm", C.c_double), ("sdd_mm", C.c_double), ("dgamma_rad", C.c_double),
-                ("channel_offset", C.c_double), ("theta0_rad", C.c_double)]
+                ("channel_offset", C.c_double), ("theta0_rad", C.c_double), ("model", C.c_int32), ("reserved", C.c_int32)]
 
 
 class _CParams(C.Structure):
@@ -53,10 +53,11 @@ class Geometry:
     dgamma_rad: float = 0.0
     channel_offset: float = 0.0
     theta0_rad: float = 0.0
+    model: int = 0
 
     def c(self) -> _CGeometry:
         return _CGeometry(self.nx, self.ny, self.pixel_mm, self.n_views, self.n_channels, self.sad_mm, self.sdd_mm,
-                          self.dgamma_rad, self.channel_offset, self.theta0_rad)
+                          self.dgamma_rad, self.channel_offset, self.theta0_rad, self.model, 0)
 
 
 @dataclass

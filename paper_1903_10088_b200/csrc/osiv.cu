@@ -121,6 +121,14 @@ void build_tables(const osiv_geometry& g, double dgamma, std::vector<float4>& ra
                 r.z = (float)(S / (D * dy));
                 r.w = (float)(D / std::fabs(dx));
             }
+            if (g.model == 1) {
+                // Joseph: a = h * sat(1 - |xc - x*|) on the ray's major-axis line, and |xc - x*| = |q| / |k| with k the
+                // in-line coefficient: the same expression with the ray's three coefficients divided by |k|
+                // (in-line coefficient +-1, marching coefficient +-1/|k|) and a half-width of 1
+                const double ak = std::fabs(dy) >= std::fabs(dx) ? std::fabs(dy / dx) : std::fabs(dx / dy);
+                if (std::fabs(dy) >= std::fabs(dx)) { r.x = (-dy / dx) > 0 ? 1.f : -1.f; r.y = (float)(1.0 / ak); r.z = (float)(-S / (D * dx) / ak); }
+                else                                { r.x = (float)(1.0 / ak); r.y = (-dx / dy) > 0 ? 1.f : -1.f; r.z = (float)(S / (D * dy) / ak); }
+            }
             rays[(size_t)v * C + c] = r;
         }
     }
@@ -291,7 +299,8 @@ int osiv_default_params(osiv_params* p) {
 }
 
 static int check_geometry(const osiv_geometry& g) {
-    if (g.nx <= 0 || g.ny <= 0 || g.n_views <= 0 || g.n_channels <= 0 || g.nx > 16384 || g.ny > 16384)
+    if (g.nx <= 0 || g.ny <= 0 || g.n_views <= 0 || g.n_channels <= 0 || g.nx > 16384 || g.ny > 16384 ||
+        (g.model != 0 && g.model != 1) || g.reserved != 0)
         return OSIV_ERR_INVALID_ARG;
     if (!(g.pixel_mm > 0.0) || !(g.sad_mm > 0.0) || !std::isfinite(g.pixel_mm) || !std::isfinite(g.sad_mm) ||
         !std::isfinite(g.dgamma_rad) || !std::isfinite(g.channel_offset) || !std::isfinite(g.theta0_rad))
@@ -333,7 +342,11 @@ int osiv_create(const osiv_geometry* geom, int32_t max_batch, int32_t device, os
     std::vector<float2> views;
     build_tables(g, dgamma, rays, views);
     // K2 reads up to res_pad entries past a view's last channel: zero slack after the last view
-    const double tile_r = 0.5 * g.pixel_mm * std::sqrt((double)(BK_TX * BK_TX + BK_TY * BK_TY));
+    // rays that can have a non-zero weight for one of a tile's pixels pass within tile_r of the tile's centre: exact
+    // chord -- they cross the tile's square; Joseph -- within pixel*max(|dx|,|dy|) <= pixel of a pixel centre
+    const double tile_r = g.model == 1
+        ? 0.5 * g.pixel_mm * std::sqrt((double)((BK_TX - 1) * (BK_TX - 1) + (BK_TY - 1) * (BK_TY - 1))) + g.pixel_mm
+        : 0.5 * g.pixel_mm * std::sqrt((double)(BK_TX * BK_TX + BK_TY * BK_TY));
     const double xm = std::min(tile_r / (g.sad_mm - rmax), 1.0);
     const double tile_hw = std::asin(xm) / xm * tile_r / dgamma * 1.0005;
     h->res_pad = ((2 * (int)std::ceil(tile_hw / (g.sad_mm - rmax) + 0.05) + 3) + 3) / 4 * 4;
@@ -341,7 +354,7 @@ int osiv_create(const osiv_geometry* geom, int32_t max_batch, int32_t device, os
     std::vector<float> hs(rays.size());
     for (size_t i = 0; i < rays.size(); ++i) {
         hs[i] = rays[i].w;
-        rays[i].w = 0.5f * (std::fabs(rays[i].x) + std::fabs(rays[i].y));
+        rays[i].w = g.model == 1 ? 1.f : 0.5f * (std::fabs(rays[i].x) + std::fabs(rays[i].y));
     }
     rays.resize(rays.size() + h->res_pad + 4, make_float4(0.f, 0.f, 0.f, 0.f));
     if (cudaMalloc((void**)&h->d_rays, rays.size() * sizeof(float4)) != cudaSuccess ||

@@ -13,7 +13,9 @@
 // p is affine in the centred pixel indices (xc, yc), so after dividing by (hi-lo) every ray carries
 // {alpha, beta, g0, h} (stored as the float4 {alpha, beta, g0, (|alpha|+|beta|)/2} plus a separate h table) with
 //   a(i; xc,yc) = h * sat( (|alpha|+|beta|)/2 - |alpha*xc + beta*yc + g0| ),
-// one of alpha,beta being exactly +-1 and the other |k| >= 1.  Forward and back evaluate this same
+// one of alpha,beta being exactly +-1 and the other |k| >= 1 (second model, Joseph's interpolation: the table holds
+// the coefficients divided by |k| and a half-width of 1, a = h * sat(1 - |q|/|k|); the kernels do not change).
+// Forward and back evaluate this same
 // expression, so the pair is matched by construction.  Nothing here is a dense contraction: no
 // tensor cores; the work is FP32 FMA/ALU issue plus L1/L2 gathers.
 //
@@ -175,8 +177,8 @@ __global__ void __launch_bounds__(FWD_MAX_THREADS, 1) k_forward(const FwdArgs a)
     const float4 ray = __ldg(&g.rays[(size_t)v * g.C + c]);
     const bool rowmaj = fabsf(ray.x) >= fabsf(ray.y);
     {
-        const float kk = rowmaj ? ray.x : ray.y;          // coefficient of the in-line coordinate, |kk| >= 1
-        const float uu = rowmaj ? ray.y : ray.x;          // coefficient of the marching coordinate, +-1
+        const float kk = rowmaj ? ray.x : ray.y;          // coefficient of the in-line coordinate, |kk| >= 1 (Joseph: +-1)
+        const float uu = rowmaj ? ray.y : ray.x;          // coefficient of the marching coordinate (+-1; Joseph: +-1/|k|)
         const float* bufA = rowmaj ? a.img + (size_t)s * g.img_elems : a.imgT + (size_t)s * g.imgT_elems;
         const float* bufB = rowmaj ? a.imgT + (size_t)s * g.imgT_elems : a.img + (size_t)s * g.img_elems;
         const int pitch = rowmaj ? g.pitch : g.pitchT;    // NS == 4: square grid, both pitches are equal
@@ -186,7 +188,8 @@ __global__ void __launch_bounds__(FWD_MAX_THREADS, 1) k_forward(const FwdArgs a)
         const float hk = ray.w;
         // lines where the crossing lies within half a pixel of the image: |uu*b + g0| < |kk|*(na/2 + 1/2)
         const float A = fabsf(kk) * (0.5f * na + 0.5f);
-        const float b1 = uu * (-ray.z - A), b2 = uu * (-ray.z + A);
+        const float iu = 1.0f / uu;                       // exact chord: uu = +-1; Joseph: |uu| <= 1
+        const float b1 = iu * (-ray.z - A), b2 = iu * (-ray.z + A);
         const int flo = (int)fminf(fmaxf(ceilf(fminf(b1, b2) + cb) - 1.f, 0.f), (float)nb);
         const int fhi = (int)fminf(fmaxf(floorf(fmaxf(b1, b2) + cb) + 1.f, -1.f), (float)(nb - 1));
         // The block walks the union of its rays' line ranges in lock step, so that at every step the lanes of a warp

@@ -211,6 +211,48 @@ def test_projector_pair_max_size_config5b_subset(osiv):
             assert abs(full[v, c] - one[0, c]) < 2e-5 * abs(one[0, c]) + 1e-7
 
 
+# ------------------------------------------------------------------ second system matrix (Joseph, 8(f)-2)
+@pytest.mark.parametrize("cfg,subsets", [
+    (si.scan_config("1"), [(-1, 1), (2, 5)]),           # general path (V = 90)
+    (si.scan_config("2"), [(-1, 1), (3, 10)]),          # quarter-turn path
+    (ODD, [(-1, 1), (1, 3)]),
+    (WIDE, [(-1, 1)]),
+    (NEAR_AXIS, [(-1, 1)]),
+])
+def test_joseph_model_forward_and_back_match_oracle(osiv, cfg, subsets):
+    from dataclasses import replace
+    og, gg = geoms(cfg)
+    og, gg = replace(og, model=1), replace(gg, model=1)
+    rng = np.random.default_rng(cfg.seed + 5)
+    with osiv.Handle(gg, max_batch=1) as h:
+        for sub, M in subsets:
+            img = rng.uniform(0.0, 0.013, size=(cfg.ny, cfg.nx)).astype(np.float32)
+            vs = cfg.n_views if sub < 0 else cfg.n_views // M
+            sino = rng.uniform(0.0, 1.0, size=(vs, cfg.n_channels)).astype(np.float32)
+            f = host(h.forward(dev(img)[None], sub, M))[0]
+            b = host(h.backward(dev(sino)[None], sub, M))[0]
+            assert rel(f, oracle.forward(og, img, sub, M)) < PROJ_TOL
+            assert rel(b, oracle.backward(og, sino, sub, M)) < PROJ_TOL
+            lhs = np.dot(f.astype(np.float64).ravel(), sino.astype(np.float64).ravel())
+            rhs = np.dot(img.astype(np.float64).ravel(), b.astype(np.float64).ravel())
+            assert abs(lhs - rhs) / abs(lhs) < 5e-6
+
+
+def test_joseph_model_reconstruct_config2(osiv):
+    from dataclasses import replace
+    cfg = si.scan_config("2")
+    og, gg = geoms(cfg)
+    og, gg = replace(og, model=1), replace(gg, model=1)
+    counts = si.make_case(cfg)[2]
+    kw = dict(beta=cfg.betas[0], n_subsets=cfg.n_subsets, n_iters=cfg.n_iters)
+    ref, tr_ref, status = oracle.reconstruct(og, counts, cfg.i0, oracle.Params(**kw))
+    with osiv.Handle(gg, max_batch=1) as h:
+        got, tr = h.reconstruct(dev(counts)[None], cfg.i0, osiv.Params(**kw), trace=True)
+    assert status == 0 and np.array_equal(tr[0, :, 1], tr_ref[:, 1])
+    assert np.all(np.abs(tr[0, :, 0] - tr_ref[:, 0]) <= 1e-5 * tr_ref[:, 0])
+    assert rel(host(got)[0], ref) < IMG_TOL
+
+
 # ------------------------------------------------------------------ TV gradient
 
 @pytest.mark.parametrize("shape", [(29, 37), (64, 64), (5, 3), (1, 7)])
