@@ -274,55 +274,49 @@ __global__ void __launch_bounds__(FWD_MAX_THREADS, 1) k_forward(const FwdArgs a)
 #pragma unroll
         for (int k = 0; k < NS; ++k) part[(seg * NS + k) * rpb + i] = acc[k];
     }
-    // the epilogue's inputs are requested before the barrier so that they arrive while the block drains
-    const bool epi = t < rpb && r < R;
-    float yk[NS] = {}, bl = a.blank_scalar, ib = 0.f, h = 0.f;
+    // Epilogue: thread (seg = ko < NS, ray i) finishes ray i of rotation ko -- its own ray, so everything about the ray
+    // is in registers already.  Its inputs are requested before the barrier so that they arrive while the block drains.
+    const int ne = min(segs, NS);                             // epilogue threads per ray
+    const bool epi = seg < ne && r < R;
+    float y0 = 0.f, bl = a.blank_scalar, ib = 0.f, h = 0.f;
     if (epi) h = __ldg(&g.hs[(size_t)v * g.C + c]);
     if (MODE == 1 && epi) {
-#pragma unroll
-        for (int k = 0; k < NS; ++k) yk[k] = __ldg(&a.counts[((size_t)s * g.V + v + k * Vq) * g.C + c]);
+        y0 = __ldg(&a.counts[((size_t)s * g.V + v + seg * Vq) * g.C + c]);
         if (a.blank) bl = __ldg(&a.blank[c]);
         ib = __ldg(a.inv_bref);
     }
     __syncthreads();
-    if (t >= 32 * ((rpb + 31) / 32)) return;                  // whole warps past the epilogue rays
+    const int nw = (ne * rpb + 31) / 32;                      // epilogue warps
+    if (t >= 32 * nw) return;
 
     double d2 = 0.0;
     if (epi) {
-        // sums over the ray's segments, fixed order; pattern -> rotation k (patterns 1 and 3 swap for a
-        // column-major base ray: R maps its walk onto the other copy with the mirrored index first)
-        float l[NS], hr[NS];
-#pragma unroll
-        for (int k = 0; k < NS; ++k) {
+        for (int ko = seg; ko < NS; ko += ne) {
+            // pattern -> rotation (patterns 1 and 3 swap for a column-major base ray: R maps its walk onto the other
+            // copy with the mirrored index first); sum over the ray's segments in a fixed order
+            const int pk = (NS == 4 && !rowmaj && (ko & 1)) ? 4 - ko : ko;
             float x = 0.f;
-            for (int q = 0; q < segs; ++q) x += part[(q * NS + k) * rpb + i];
-            l[k] = h * x;
-        }
-        if (NS == 4 && !rowmaj) { const float x = l[1]; l[1] = l[3]; l[3] = x; }
-#pragma unroll
-        for (int k = 0; k < NS; ++k) {
+            for (int q = 0; q < segs; ++q) x += part[(q * NS + pk) * rpb + i];
+            const float l = h * x;
             if (MODE == 0) {
-                a.sino[((size_t)s * a.VS + jb + k * VSb) * g.C + c] = l[k];
+                a.sino[((size_t)s * a.VS + jb + ko * VSb) * g.C + c] = l;
             } else {
                 // A2: Poisson residual r = (b exp(-l) - y)/b_ref and monitor term (l - ln(b/max(y,1)))^2
-                const float ybar = bl * expf(-l[k]);
-                hr[k] = h * ((ybar - yk[k]) * ib);
-                const float p = logf(bl / fmaxf(yk[k], 1.f));
-                const double d = (double)l[k] - (double)p;
+                const float y = ko == seg ? y0 : __ldg(&a.counts[((size_t)s * g.V + v + ko * Vq) * g.C + c]);
+                const float ybar = bl * expf(-l);
+                const float hr = h * ((ybar - y) * ib);
+                const float p = logf(bl / fmaxf(y, 1.f));
+                const double d = (double)l - (double)p;
                 d2 += d * d;
+                // NS == 4: the orbit's four residuals share one float4 (K2 reads them with one load per candidate ray)
+                a.res[(((size_t)s * VSb + jb) * a.Cp + c) * NS + ko] = hr;
             }
-        }
-        if (MODE == 1) {
-            // NS == 4: the orbit's four residuals share one float4 (K2 reads them with one load per candidate ray)
-            if (NS == 4) reinterpret_cast<float4*>(a.res)[((size_t)s * VSb + jb) * a.Cp + c] = make_float4(hr[0], hr[1 % NS], hr[2 % NS], hr[3 % NS]);
-            else         a.res[((size_t)s * a.VS + jb) * a.Cp + c] = hr[0];
         }
     }
     if (MODE == 1) {
         // block's share of D: warp shuffles, then the (at most 32) warp sums in a fixed order
 #pragma unroll
         for (int off = 16; off > 0; off >>= 1) d2 += __shfl_down_sync(0xffffffffu, d2, off);
-        const int nw = (rpb + 31) / 32;
         if ((t & 31) == 0) dred[t >> 5] = d2;
         asm volatile("bar.sync 1, %0;" ::"r"(32 * nw) : "memory");     // only the epilogue warps meet here
         if (t == 0) {
