@@ -24,7 +24,7 @@ struct osiv_handle {
     float2* d_views = nullptr;
     float* d_hs = nullptr;
     // per-slice workspace, grown lazily
-    int ws_batch = 0;
+    int ws_batch = 0, ws_sb = 1;        // slices the image buffers hold, and their interleave (DevGeom::sb)
     float *d_imgA = nullptr, *d_imgB = nullptr, *d_imgTA = nullptr, *d_imgTB = nullptr;
     float* d_best = nullptr;
     size_t res_elems = 0;       float* d_res = nullptr;
@@ -144,24 +144,31 @@ int check_subset(const osiv_handle* h, int subset, int n_subsets) {
     return OSIV_OK;
 }
 
-// padded image buffers for `batch` slices (pads are zeroed once and never written again)
-int ensure_images(osiv_handle* h, int batch, cudaStream_t st) {
-    if (h->ws_batch >= batch) return OSIV_OK;
-    float** bufs[4] = {&h->d_imgA, &h->d_imgB, &h->d_imgTA, &h->d_imgTB};
-    for (auto b : bufs) if (*b) { OSIV_CUDA(cudaFree(*b)); *b = nullptr; }
-    if (h->d_best) { OSIV_CUDA(cudaFree(h->d_best)); h->d_best = nullptr; }
-    h->ws_batch = 0;
-    const size_t ne = (size_t)h->dg.img_elems * batch, nt = (size_t)h->dg.imgT_elems * batch;
-    OSIV_CUDA(cudaMalloc((void**)&h->d_imgA, ne * sizeof(float)));
-    OSIV_CUDA(cudaMalloc((void**)&h->d_imgB, ne * sizeof(float)));
-    OSIV_CUDA(cudaMalloc((void**)&h->d_imgTA, nt * sizeof(float)));
-    OSIV_CUDA(cudaMalloc((void**)&h->d_imgTB, nt * sizeof(float)));
-    OSIV_CUDA(cudaMalloc((void**)&h->d_best, (size_t)h->geom.nx * h->geom.ny * batch * sizeof(float)));
+// padded image buffers for `batch` slices in the layout DevGeom::sb = sb (slices interleaved per pixel in groups of
+// sb); the pads are zeroed when the buffers are made or the layout changes and never written again
+int ensure_images(osiv_handle* h, int batch, int sb, cudaStream_t st) {
+    const int slices = (batch + sb - 1) / sb * sb;
+    h->dg.sb = sb;
+    if (h->ws_batch >= slices && h->ws_sb == sb) return OSIV_OK;
+    const int n = std::max(slices, h->ws_batch);
+    const size_t ne = (size_t)h->dg.img_elems * n, nt = (size_t)h->dg.imgT_elems * n;
+    if (h->ws_batch < slices) {
+        float** bufs[4] = {&h->d_imgA, &h->d_imgB, &h->d_imgTA, &h->d_imgTB};
+        for (auto b : bufs) if (*b) { OSIV_CUDA(cudaFree(*b)); *b = nullptr; }
+        if (h->d_best) { OSIV_CUDA(cudaFree(h->d_best)); h->d_best = nullptr; }
+        h->ws_batch = 0;
+        OSIV_CUDA(cudaMalloc((void**)&h->d_imgA, ne * sizeof(float)));
+        OSIV_CUDA(cudaMalloc((void**)&h->d_imgB, ne * sizeof(float)));
+        OSIV_CUDA(cudaMalloc((void**)&h->d_imgTA, nt * sizeof(float)));
+        OSIV_CUDA(cudaMalloc((void**)&h->d_imgTB, nt * sizeof(float)));
+        OSIV_CUDA(cudaMalloc((void**)&h->d_best, (size_t)h->geom.nx * h->geom.ny * n * sizeof(float)));
+    }
     OSIV_CUDA(cudaMemsetAsync(h->d_imgA, 0, ne * sizeof(float), st));
     OSIV_CUDA(cudaMemsetAsync(h->d_imgB, 0, ne * sizeof(float), st));
     OSIV_CUDA(cudaMemsetAsync(h->d_imgTA, 0, nt * sizeof(float), st));
     OSIV_CUDA(cudaMemsetAsync(h->d_imgTB, 0, nt * sizeof(float), st));
-    h->ws_batch = batch;
+    h->ws_batch = n;
+    h->ws_sb = sb;
     return OSIV_OK;
 }
 
@@ -170,10 +177,23 @@ int ensure_images(osiv_handle* h, int batch, cudaStream_t st) {
 // made of whole orbits (V_S % 4 == 0); everything else takes the general NS = 1 kernels.
 int pick_ns(const osiv_handle* h, int VS) { return (h->dg.sym4 && !h->force_ns1 && VS % 4 == 0) ? 4 : 1; }
 
-constexpr int BATCH_THREADS = 512;      // block size cap when a launch carries several slices: two blocks per SM
+constexpr int BATCH_THREADS = 512;      // K1 block size cap when a launch carries several slices: two blocks per SM
+constexpr int BATCH_MIN_SLICES = 4;     // fewer slices than this run one after the other in full-size blocks
 
-struct FwdPlan { int threads, rpb, segs, nparts, ns; size_t smem; };
-struct BackPlan { int nblk, threads, tpb, shares, ngx, ns; size_t smem; };
+// Launches with several slices serve pairs of slices per block (SB = 2: interleaved images, shared chord weights) when
+// K2's tiles per block leave room for at least one view share in its 448-thread blocks.
+int pick_sb(const osiv_handle* h, int VS, int batch) {
+    if (batch < BATCH_MIN_SLICES) return 1;
+    const int ns = pick_ns(h, VS);
+    const int tx = ns == 4 ? h->geom.nx / 4 : (h->geom.nx + BK_TX - 1) / BK_TX;
+    const int ty = ns == 4 ? h->geom.ny / 4 : (h->geom.ny + BK_TY - 1) / BK_TY;
+    const long long tiles = (long long)(((tx + BK_WX - 1) / BK_WX + 1) / 2) * (((ty + BK_WY - 1) / BK_WY + 1) / 2) * 4 * 32;
+    const long long tpb = std::max<long long>(1, (tiles + h->num_sms - 1) / h->num_sms);
+    return tpb * ns <= BKB_MAX_THREADS ? 2 : 1;
+}
+
+struct FwdPlan { int threads, rpb, segs, nparts, ns, sb; size_t smem; };
+struct BackPlan { int nblk, threads, tpb, shares, ngx, ns, sb; size_t smem; };
 
 // K1: the subset's base rays are dealt out in runs of rpb consecutive rays, one run per block and one block per SM
 // (per slice); a block is rpb rays x segs segments of each ray's line range, as many segments as fit into 1024
@@ -184,25 +204,28 @@ FwdPlan plan_forward(const osiv_handle* h, int VS, int batch) {
     const long long R = (long long)(VS / p.ns) * h->geom.n_channels;
     p.rpb = (int)std::min<long long>(FWD_MAX_THREADS, std::max<long long>(1, (R + h->num_sms - 1) / h->num_sms));
     const int nmax = std::max(h->geom.nx, h->geom.ny);
-    // several slices: two half-size blocks (of different slices) per SM fill each other's stalls (A8)
-    const int tmax = std::max(p.rpb, batch > 1 ? BATCH_THREADS : FWD_MAX_THREADS);
+    // several slices (A8): pairs of slices share the chord weights (SB = 2), in half-size blocks, two per SM, which
+    // fill each other's stalls
+    p.sb = pick_sb(h, VS, batch);
+    const int tmax = std::max(p.rpb, p.sb == 2 ? BATCH_THREADS : FWD_MAX_THREADS);
     p.segs = std::max(1, std::min(tmax / p.rpb, nmax / FWD_MIN_LINES));
     p.threads = (p.rpb * p.segs + 31) / 32 * 32;
     p.nparts = (int)((R + p.rpb - 1) / p.rpb);
-    p.smem = (size_t)p.segs * p.ns * p.rpb * sizeof(float);
+    p.smem = (size_t)p.sb * p.segs * p.ns * p.rpb * sizeof(float);
     return p;
 }
 
 template <int MODE>
 cudaError_t launch_forward(FwdPlan p, int batch, const FwdArgs& a, cudaStream_t st, bool pdl) {
     cudaLaunchConfig_t cfg{};
-    cfg.gridDim = dim3(p.nparts, 1, batch); cfg.blockDim = dim3(p.threads); cfg.dynamicSmemBytes = p.smem; cfg.stream = st;
+    cfg.gridDim = dim3(p.nparts, 1, (batch + p.sb - 1) / p.sb); cfg.blockDim = dim3(p.threads);
+    cfg.dynamicSmemBytes = p.smem; cfg.stream = st;
     cudaLaunchAttribute attr[1];
     attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     attr[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = attr; cfg.numAttrs = pdl ? 1 : 0;
-    if (p.ns == 4) return cudaLaunchKernelEx(&cfg, k_forward<MODE, 4>, a);
-    return cudaLaunchKernelEx(&cfg, k_forward<MODE, 1>, a);
+    if (p.sb == 2) return p.ns == 4 ? cudaLaunchKernelEx(&cfg, k_forward<MODE, 4, 2>, a) : cudaLaunchKernelEx(&cfg, k_forward<MODE, 1, 2>, a);
+    return p.ns == 4 ? cudaLaunchKernelEx(&cfg, k_forward<MODE, 4, 1>, a) : cudaLaunchKernelEx(&cfg, k_forward<MODE, 1, 1>, a);
 }
 
 // K2: the base tiles, numbered patch by patch (8 x 4 tiles, patches grouped 2 x 2), are dealt out in runs of tpb
@@ -220,27 +243,29 @@ BackPlan plan_back(const osiv_handle* h, int VS, int batch) {
     const int VSb = VS / p.ns;
     // shares per quarter turn (NS == 4) or in all: as many as fit, then the fewest that keep the same number of
     // views per share
-    const int tmax = std::max(p.tpb * p.ns, batch > 1 ? BATCH_THREADS : BK_MAX_THREADS);
+    // several slices: pairs of slices share the chord weights in blocks of at most 448 threads, two blocks per SM (A8)
+    p.sb = pick_sb(h, VS, batch);
+    const int tmax = std::max(p.tpb * p.ns, p.sb == 2 ? BKB_MAX_THREADS : BK_MAX_THREADS);
     int sq = std::max(1, std::min(tmax / (p.tpb * p.ns), VSb));
     const int trips = (VSb + sq - 1) / sq;
     sq = (VSb + trips - 1) / trips;
     p.shares = sq * p.ns;
     p.threads = (p.tpb * p.shares + 31) / 32 * 32;
-    p.smem = (size_t)p.shares * p.ns * 4 * p.tpb * sizeof(float);
+    p.smem = (size_t)p.sb * p.shares * p.ns * 4 * p.tpb * sizeof(float);
     return p;
 }
 
 template <int MODE>
 cudaError_t launch_back(const BackPlan& p, int batch, const BackArgs& a, cudaStream_t st, bool pdl) {
     cudaLaunchConfig_t cfg{};
-    cfg.gridDim = dim3(p.nblk, 1, batch); cfg.blockDim = dim3(p.threads); cfg.stream = st;
+    cfg.gridDim = dim3(p.nblk, 1, (batch + p.sb - 1) / p.sb); cfg.blockDim = dim3(p.threads); cfg.stream = st;
     cfg.dynamicSmemBytes = p.smem;
     cudaLaunchAttribute attr[1];
     attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     attr[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = attr; cfg.numAttrs = pdl ? 1 : 0;
-    if (p.ns == 4) return cudaLaunchKernelEx(&cfg, k_back<MODE, 4>, a);
-    return cudaLaunchKernelEx(&cfg, k_back<MODE, 1>, a);
+    if (p.sb == 2) return p.ns == 4 ? cudaLaunchKernelEx(&cfg, k_back<MODE, 4, 2>, a) : cudaLaunchKernelEx(&cfg, k_back<MODE, 1, 2>, a);
+    return p.ns == 4 ? cudaLaunchKernelEx(&cfg, k_back<MODE, 4, 1>, a) : cudaLaunchKernelEx(&cfg, k_back<MODE, 1, 1>, a);
 }
 
 int ensure_forward_ws(osiv_handle* h, const FwdPlan& p, int batch) {
@@ -368,8 +393,10 @@ int osiv_create(const osiv_geometry* geom, int32_t max_batch, int32_t device, os
         cudaMemcpy(h->d_views, views.data(), views.size() * sizeof(float2), cudaMemcpyHostToDevice) != cudaSuccess ||
         cudaDeviceGetAttribute(&h->num_sms, cudaDevAttrMultiProcessorCount, device) != cudaSuccess ||
         // K2's shared-memory reduction buffer: up to 1024 threads x 16 floats
-        cudaFuncSetAttribute(k_back<0, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024) != cudaSuccess ||
-        cudaFuncSetAttribute(k_back<1, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024) != cudaSuccess) {
+        cudaFuncSetAttribute(k_back<0, 4, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024) != cudaSuccess ||
+        cudaFuncSetAttribute(k_back<1, 4, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024) != cudaSuccess ||
+        cudaFuncSetAttribute(k_back<0, 4, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024) != cudaSuccess ||
+        cudaFuncSetAttribute(k_back<1, 4, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024) != cudaSuccess) {
         cudaGetLastError();
         osiv_destroy(h);
         return OSIV_ERR_CUDA;
@@ -391,6 +418,7 @@ int osiv_create(const osiv_geometry* geom, int32_t max_batch, int32_t device, os
     const double zmax = rmax / (g.sad_mm - rmax);
     d.use_atanf = (zmax > 0.75 || 3e-7 / dgamma > 0.01) ? 1 : 0;
     d.sym4 = (g.nx == g.ny && g.nx % 4 == 0 && g.n_views % 4 == 0) ? 1 : 0;
+    d.sb = 1;
     d.rays = h->d_rays; d.views = h->d_views; d.hs = h->d_hs;
     *out = h;
     return OSIV_OK;
@@ -447,7 +475,7 @@ int osiv_get_plan(const osiv_handle* h, int32_t n_subsets, int32_t batch, int32_
     const FwdPlan f = plan_forward(h, VS, batch);
     const BackPlan b = plan_back(h, VS, batch);
     out8[0] = f.ns; out8[1] = f.segs; out8[2] = f.nparts * batch; out8[3] = f.threads;
-    out8[4] = b.ns; out8[5] = b.shares; out8[6] = b.nblk * batch; out8[7] = b.threads;
+    out8[4] = b.ns; out8[5] = b.shares; out8[6] = b.nblk * ((batch + b.sb - 1) / b.sb); out8[7] = b.threads;
     return OSIV_OK;
 }
 
@@ -475,16 +503,16 @@ int osiv_forward(osiv_handle* h, const float* d_img, float* d_sino, int32_t batc
     DeviceGuard guard(h->device);
     if (!guard.ok) { cudaGetLastError(); return OSIV_ERR_CUDA; }
     cudaStream_t st = (cudaStream_t)cuda_stream;
-    int rc = ensure_images(h, batch, st);
-    if (rc != OSIV_OK) return rc;
     const int VS = subset_views(h, subset, n_subsets);
     const FwdPlan p = plan_forward(h, VS, batch);
+    int rc = ensure_images(h, batch, p.sb, st);
+    if (rc != OSIV_OK) return rc;
     if ((rc = ensure_forward_ws(h, p, batch)) != OSIV_OK) return rc;
     k_pad_transpose<<<dim3((h->geom.nx + 31) / 32, (h->geom.ny + 31) / 32, batch), 256, 0, st>>>(h->dg, d_img, h->d_imgA,
                                                                                              h->d_imgTA);
     FwdArgs a{};
     a.g = h->dg; a.img = h->d_imgA; a.imgT = h->d_imgTA;
-    a.subset = subset; a.M = subset < 0 ? 1 : n_subsets; a.VS = VS; a.rpb = p.rpb; a.segs = p.segs; a.sino = d_sino;
+    a.subset = subset; a.M = subset < 0 ? 1 : n_subsets; a.VS = VS; a.batch = batch; a.rpb = p.rpb; a.segs = p.segs; a.sino = d_sino;
     launch_forward<0>(p, batch, a, st, false);
     return launch_check(h, 2);
 }
@@ -504,7 +532,7 @@ int osiv_backward(osiv_handle* h, const float* d_sino, float* d_img, int32_t bat
     k_scale_sino<<<dim3((h->geom.n_channels + 255) / 256, VS, batch), 256, 0, st>>>(h->dg, d_sino, h->d_res, subset, M, VS,
                                                                                     p.ns, Cp);
     BackArgs b{};
-    b.g = h->dg; b.res = h->d_res; b.Cp = Cp; b.subset = subset; b.M = M; b.VS = VS; b.out = d_img; b.tpb = p.tpb; b.shares = p.shares; b.ngx = p.ngx;
+    b.g = h->dg; b.res = h->d_res; b.Cp = Cp; b.subset = subset; b.M = M; b.VS = VS; b.batch = batch; b.out = d_img; b.tpb = p.tpb; b.shares = p.shares; b.ngx = p.ngx;
     launch_back<0>(p, batch, b, st, false);
     return launch_check(h, 2);
 }
@@ -515,7 +543,7 @@ int osiv_tv_gradient(osiv_handle* h, const float* d_img, float* d_grad, int32_t 
     DeviceGuard guard(h->device);
     if (!guard.ok) { cudaGetLastError(); return OSIV_ERR_CUDA; }
     cudaStream_t st = (cudaStream_t)cuda_stream;
-    int rc = ensure_images(h, batch, st);
+    int rc = ensure_images(h, batch, 1, st);
     if (rc != OSIV_OK) return rc;
     k_pad_transpose<<<dim3((h->geom.nx + 31) / 32, (h->geom.ny + 31) / 32, batch), 256, 0, st>>>(h->dg, d_img, h->d_imgA,
                                                                                              h->d_imgTA);
@@ -537,9 +565,9 @@ int osiv_reconstruct(osiv_handle* h, const float* d_counts, const float* d_blank
     cudaStream_t st = (cudaStream_t)cuda_stream;
 
     const int VS = h->geom.n_views / M, C = h->geom.n_channels;
-    int rc = ensure_images(h, batch, st);
-    if (rc != OSIV_OK) return rc;
     const FwdPlan fp = plan_forward(h, VS, batch);
+    int rc = ensure_images(h, batch, fp.sb, st);
+    if (rc != OSIV_OK) return rc;
     const BackPlan bp = plan_back(h, VS, batch);
     if ((rc = ensure_res(h, VS, fp.ns, batch, st)) != OSIV_OK) return rc;
     const int Cp = C + h->res_pad;
@@ -560,11 +588,11 @@ int osiv_reconstruct(osiv_handle* h, const float* d_counts, const float* d_blank
     h->launches += 2;
 
     FwdArgs f{};
-    f.g = h->dg; f.M = M; f.VS = VS; f.rpb = fp.rpb; f.segs = fp.segs;
+    f.g = h->dg; f.M = M; f.VS = VS; f.batch = batch; f.rpb = fp.rpb; f.segs = fp.segs;
     f.counts = d_counts; f.blank = d_blank; f.blank_scalar = blank_scalar; f.inv_bref = h->d_inv_bref;
     f.res = h->d_res; f.Cp = Cp; f.dparts = h->d_dparts;
     BackArgs b{};
-    b.g = h->dg; b.res = h->d_res; b.Cp = Cp; b.M = M; b.VS = VS; b.best = best; b.tpb = bp.tpb; b.shares = bp.shares; b.ngx = bp.ngx;
+    b.g = h->dg; b.res = h->d_res; b.Cp = Cp; b.M = M; b.VS = VS; b.batch = batch; b.best = best; b.tpb = bp.tpb; b.shares = bp.shares; b.ngx = bp.ngx;
     b.dparts = h->d_dparts; b.nparts = fp.nparts; b.not_finite = h->d_not_finite;
     b.ip.lambda0 = prm->lambda0; b.ip.up = prm->lambda_up; b.ip.down = prm->lambda_down; b.ip.lmin = prm->lambda_min;
     b.ip.forced = (prm->forced_lambda && N > 0) ? h->d_forced : nullptr;

@@ -43,12 +43,14 @@ constexpr int FWD_MIN_LINES = 8;           // K1: a segment is at least this man
 #endif
 constexpr int BK_TX = 2, BK_TY = 2;        // pixels per thread in the backprojector
 constexpr int BK_WX = 8, BK_WY = 4;        // tiles per warp: a warp covers 16 x 8 pixels
+constexpr int BKB_MAX_THREADS = 448;       // K2 serving two slices per block (SB == 2): two such blocks per SM
 constexpr int BK_MAX_THREADS = 1024;       // K2: one block per SM, threads = tiles per block x view shares
 
 struct DevGeom {
     int nx, ny, V, C;
     int pitch, pitchT;                     // floats per padded line of img ([ny+2][nx+8]) and imgT ([nx+2][ny+8])
-    long long img_elems, imgT_elems;       // padded floats per slice
+    long long img_elems, imgT_elems;       // padded pixels per slice
+    int sb;                                // slices interleaved per pixel in the padded images: 1, or 2 (launches with several slices)
     float cx, cy;                          // (nx-1)/2, (ny-1)/2
     float pixel, sad, inv_dgamma, c_center;   // c_center = (C-1)/2 - channel_offset
     float tile_hw;                         // angular half-width of a K2 tile at unit distance, in channels (with asin slack)
@@ -82,6 +84,7 @@ struct FwdArgs {
     const float* img;                      // padded mu, slice stride g.img_elems
     const float* imgT;                     // padded transpose, slice stride g.imgT_elems
     int subset, M, VS;
+    int batch;                             // slices in this launch (SB == 2: the last pair may be half empty)
     int rpb, segs;                         // rays per block, line segments per ray (block = rpb * segs threads, rounded up to warps)
     float* sino;                           // MODE 0: [batch][VS][C]
     const float* counts;                   // MODE 1: [batch][V][C]
@@ -99,6 +102,7 @@ struct BackArgs {
     const float* res;                      // h * (residual or sinogram), layout as FwdArgs::res
     int Cp;
     int subset, M, VS;
+    int batch;                             // slices in this launch (SB == 2: the last pair may be half empty)
     int tpb, shares, ngx;                  // tiles per block, view shares, 2x2 patch groups per row of groups
     float* out;                            // MODE 0: [batch][ny][nx]
     const float* img;                      // MODE 1: padded mu(n)
@@ -120,6 +124,11 @@ __device__ __forceinline__ size_t pad_off(const DevGeom& g, int iy, int ix) {
 }
 __device__ __forceinline__ size_t padT_off(const DevGeom& g, int ix, int iy) {
     return (size_t)(ix + PADR) * g.pitchT + PAD + iy;
+}
+// float index of padded pixel 0 of slice s: slices are stored in groups of g.sb, interleaved per pixel, so pixel p of
+// slice s lives at slice_base + p * g.sb
+__device__ __forceinline__ size_t slice_base(const DevGeom& g, long long elems, int s) {
+    return (size_t)(s / g.sb) * (size_t)elems * g.sb + (size_t)(s % g.sb);
 }
 
 // ---- programmatic dependent launch: both hot kernels are launched while their predecessor in the stream still runs;
@@ -153,10 +162,18 @@ __device__ __forceinline__ void ffma2(uint64_t& c, uint64_t a, float b) {       
 // the same amount of work and no block depends on another: the segment sums meet in shared memory in a fixed order
 // and the first rpb threads run the per-ray epilogue.  The host sizes the grid to one block per SM (fwd_plan).
 // ------------------------------------------------------------------------------------------------
-template <int MODE, int NS>
+// SB == 2 (launches with several slices, A8): a block serves a pair of slices whose padded images are interleaved per
+// pixel (DevGeom::sb == 2), so every gather is one float2 = the pixel in both slices, the chord weights -- the bulk of
+// K1's instructions -- are worked out once per pair, and the FFMA2 pairs run over the two slices.
+template <int SB> struct Px;
+template <> struct Px<1> { typedef float T; };
+template <> struct Px<2> { typedef float2 T; };
+
+template <int MODE, int NS, int SB>
 __global__ void __launch_bounds__(FWD_MAX_THREADS, 1) k_forward(const FwdArgs a) {
+    typedef typename Px<SB>::T PX;
     const DevGeom& g = a.g;
-    const int t = threadIdx.x, s = blockIdx.z;
+    const int t = threadIdx.x, s0 = blockIdx.z * SB;             // slices s0 .. s0 + SB - 1
     const int rpb = a.rpb, segs = a.segs;
     const int seg = t / rpb, i = t - seg * rpb;
     const int VSb = a.VS / NS, Vq = g.V / NS;
@@ -166,21 +183,24 @@ __global__ void __launch_bounds__(FWD_MAX_THREADS, 1) k_forward(const FwdArgs a)
     const int rr = min(r, R - 1);
     const int jb = rr / g.C, c = rr - jb * g.C;
     const int v = a.subset < 0 ? jb : a.subset + jb * a.M;          // base view of the orbit
-    extern __shared__ float part[];                                 // [segs][NS][rpb]
-    __shared__ double dred[FWD_MAX_THREADS / 32];
+    extern __shared__ float part[];                                 // [segs][NS][SB][rpb]
+    __shared__ double dred[2][FWD_MAX_THREADS / 32];
     __shared__ int rng[4];                                          // line ranges of the block's row- / column-major rays
 
-    float acc[NS];
-    uint64_t acc01 = 0ull, acc23 = 0ull;
+    float acc[NS];                                                  // SB == 1, NS == 1
+    uint64_t acc01 = 0ull, acc23 = 0ull;                            // SB == 1, NS == 4: pairs of patterns
+    uint64_t acc2[NS];                                              // SB == 2: per pattern, the pair of slices
 #pragma unroll
-    for (int k = 0; k < NS; ++k) acc[k] = 0.f;
+    for (int k = 0; k < NS; ++k) { acc[k] = 0.f; acc2[k] = 0ull; }
     const float4 ray = __ldg(&g.rays[(size_t)v * g.C + c]);
     const bool rowmaj = fabsf(ray.x) >= fabsf(ray.y);
     {
         const float kk = rowmaj ? ray.x : ray.y;          // coefficient of the in-line coordinate, |kk| >= 1 (Joseph: +-1)
         const float uu = rowmaj ? ray.y : ray.x;          // coefficient of the marching coordinate (+-1; Joseph: +-1/|k|)
-        const float* bufA = rowmaj ? a.img + (size_t)s * g.img_elems : a.imgT + (size_t)s * g.imgT_elems;
-        const float* bufB = rowmaj ? a.imgT + (size_t)s * g.imgT_elems : a.img + (size_t)s * g.img_elems;
+        const PX* im = reinterpret_cast<const PX*>(a.img) + (size_t)blockIdx.z * g.img_elems;
+        const PX* imT = reinterpret_cast<const PX*>(a.imgT) + (size_t)blockIdx.z * g.imgT_elems;
+        const PX* bufA = rowmaj ? im : imT;
+        const PX* bufB = rowmaj ? imT : im;
         const int pitch = rowmaj ? g.pitch : g.pitchT;    // NS == 4: square grid, both pitches are equal
         const int na = rowmaj ? g.nx : g.ny, nb = rowmaj ? g.ny : g.nx;
         const float ca = rowmaj ? g.cx : g.cy, cb = rowmaj ? g.cy : g.cx;
@@ -239,17 +259,17 @@ __global__ void __launch_bounds__(FWD_MAX_THREADS, 1) k_forward(const FwdArgs a)
                 i0[u] = min(max((int)fa, -PAD), imax);
             }
             if (jj + 1 >= j1) { w[1][0] = 0.f; w[1][1] = 0.f; }
-            float x[2][NS][2];
+            PX x[2][NS][2];
 #pragma unroll
             for (int u = 0; u < 2; ++u) {
                 const int oP = offP + u * pitch, oM = offM - u * pitch;
-                const float* p0 = bufA + (oP + i0[u]);
+                const PX* p0 = bufA + (oP + i0[u]);
                 x[u][0][0] = __ldg(p0); x[u][0][1] = __ldg(p0 + 1);
                 if (NS == 4) {
                     const int ir = na - 2 - i0[u];                // mirrored index of pixel i0+1
-                    const float* p1 = bufB + (oM + i0[u]);        // pattern 1: other copy, line nb-1-j, same order
-                    const float* p2 = bufA + (oM + ir);           // pattern 2: same copy, line nb-1-j, mirrored
-                    const float* p3 = bufB + (oP + ir);           // pattern 3: other copy, line j, mirrored
+                    const PX* p1 = bufB + (oM + i0[u]);        // pattern 1: other copy, line nb-1-j, same order
+                    const PX* p2 = bufA + (oM + ir);           // pattern 2: same copy, line nb-1-j, mirrored
+                    const PX* p3 = bufB + (oP + ir);           // pattern 3: other copy, line j, mirrored
                     x[u][1 % NS][0] = __ldg(p1); x[u][1 % NS][1] = __ldg(p1 + 1);
                     x[u][2 % NS][0] = __ldg(p2); x[u][2 % NS][1] = __ldg(p2 + 1);
                     x[u][3 % NS][0] = __ldg(p3); x[u][3 % NS][1] = __ldg(p3 + 1);
@@ -257,7 +277,14 @@ __global__ void __launch_bounds__(FWD_MAX_THREADS, 1) k_forward(const FwdArgs a)
             }
 #pragma unroll
             for (int u = 0; u < 2; ++u) {
-                if (NS == 4) {                                    // (acc0, acc1) and (acc2, acc3) as FFMA2 pairs
+                if constexpr (SB == 2) {                          // per pattern, the two slices as an FFMA2 pair
+#pragma unroll
+                    for (int k = 0; k < NS; ++k) {
+                        const float wa = k < 2 ? w[u][0] : w[u][1], wb = k < 2 ? w[u][1] : w[u][0];   // patterns 2, 3 walk mirrored
+                        ffma2(acc2[k], pack2(x[u][k][0].x, x[u][k][0].y), wa);
+                        ffma2(acc2[k], pack2(x[u][k][1].x, x[u][k][1].y), wb);
+                    }
+                } else if constexpr (NS == 4) {                   // (acc0, acc1) and (acc2, acc3) as FFMA2 pairs
                     ffma2(acc01, pack2(x[u][0][0], x[u][1 % NS][0]), w[u][0]);
                     ffma2(acc01, pack2(x[u][0][1], x[u][1 % NS][1]), w[u][1]);
                     ffma2(acc23, pack2(x[u][2 % NS][0], x[u][3 % NS][0]), w[u][1]);
@@ -269,10 +296,21 @@ __global__ void __launch_bounds__(FWD_MAX_THREADS, 1) k_forward(const FwdArgs a)
             }
         }
     }
-    if (NS == 4) { unpack2(acc01, acc[0], acc[1 % NS]); unpack2(acc23, acc[2 % NS], acc[3 % NS]); }
+    // this thread's sums: fin[pattern][slice of the block]
+    float fin[NS][SB];
+    if constexpr (SB == 2) {
+#pragma unroll
+        for (int k = 0; k < NS; ++k) unpack2(acc2[k], fin[k][0], fin[k][SB - 1]);
+    } else {
+        if (NS == 4) { unpack2(acc01, acc[0], acc[1 % NS]); unpack2(acc23, acc[2 % NS], acc[3 % NS]); }
+#pragma unroll
+        for (int k = 0; k < NS; ++k) fin[k][0] = acc[k];
+    }
     if (seg < segs) {
 #pragma unroll
-        for (int k = 0; k < NS; ++k) part[(seg * NS + k) * rpb + i] = acc[k];
+        for (int k = 0; k < NS; ++k)
+#pragma unroll
+            for (int sl = 0; sl < SB; ++sl) part[((seg * NS + k) * SB + sl) * rpb + i] = fin[k][sl];
     }
     // Epilogue: thread (seg = ko < NS, ray i) finishes ray i of rotation ko -- its own ray, so everything about the ray
     // is in registers already.  Its inputs are requested before the barrier so that they arrive while the block drains.
@@ -281,7 +319,7 @@ __global__ void __launch_bounds__(FWD_MAX_THREADS, 1) k_forward(const FwdArgs a)
     float y0 = 0.f, bl = a.blank_scalar, ib = 0.f, h = 0.f;
     if (epi) h = __ldg(&g.hs[(size_t)v * g.C + c]);
     if (MODE == 1 && epi) {
-        y0 = __ldg(&a.counts[((size_t)s * g.V + v + seg * Vq) * g.C + c]);
+        y0 = __ldg(&a.counts[((size_t)s0 * g.V + v + seg * Vq) * g.C + c]);
         if (a.blank) bl = __ldg(&a.blank[c]);
         ib = __ldg(a.inv_bref);
     }
@@ -289,40 +327,50 @@ __global__ void __launch_bounds__(FWD_MAX_THREADS, 1) k_forward(const FwdArgs a)
     const int nw = (ne * rpb + 31) / 32;                      // epilogue warps
     if (t >= 32 * nw) return;
 
-    double d2 = 0.0;
+    double d2[SB];
+#pragma unroll
+    for (int sl = 0; sl < SB; ++sl) d2[sl] = 0.0;
     if (epi) {
         for (int ko = seg; ko < NS; ko += ne) {
             // pattern -> rotation (patterns 1 and 3 swap for a column-major base ray: R maps its walk onto the other
-            // copy with the mirrored index first); sum over the ray's segments in a fixed order
+            // copy with the mirrored index first)
             const int pk = (NS == 4 && !rowmaj && (ko & 1)) ? 4 - ko : ko;
-            float x = 0.f;
-            for (int q = 0; q < segs; ++q) x += part[(q * NS + pk) * rpb + i];
-            const float l = h * x;
-            if (MODE == 0) {
-                a.sino[((size_t)s * a.VS + jb + ko * VSb) * g.C + c] = l;
-            } else {
-                // A2: Poisson residual r = (b exp(-l) - y)/b_ref and monitor term (l - ln(b/max(y,1)))^2
-                const float y = ko == seg ? y0 : __ldg(&a.counts[((size_t)s * g.V + v + ko * Vq) * g.C + c]);
-                const float ybar = bl * expf(-l);
-                const float hr = h * ((ybar - y) * ib);
-                const float p = logf(bl / fmaxf(y, 1.f));
-                const double d = (double)l - (double)p;
-                d2 += d * d;
-                // NS == 4: the orbit's four residuals share one float4 (K2 reads them with one load per candidate ray)
-                a.res[(((size_t)s * VSb + jb) * a.Cp + c) * NS + ko] = hr;
+#pragma unroll
+            for (int sl = 0; sl < SB; ++sl) {
+                const int s = s0 + sl;
+                if (s >= a.batch) break;
+                float x = 0.f;                                    // sum over the ray's segments in a fixed order
+                for (int q = 0; q < segs; ++q) x += part[((q * NS + pk) * SB + sl) * rpb + i];
+                const float l = h * x;
+                if (MODE == 0) {
+                    a.sino[((size_t)s * a.VS + jb + ko * VSb) * g.C + c] = l;
+                } else {
+                    // A2: Poisson residual r = (b exp(-l) - y)/b_ref and monitor term (l - ln(b/max(y,1)))^2
+                    const float y = (ko == seg && sl == 0) ? y0 : __ldg(&a.counts[((size_t)s * g.V + v + ko * Vq) * g.C + c]);
+                    const float ybar = bl * expf(-l);
+                    const float hr = h * ((ybar - y) * ib);
+                    const float p = logf(bl / fmaxf(y, 1.f));
+                    const double d = (double)l - (double)p;
+                    d2[sl] += d * d;
+                    // NS == 4: the orbit's four residuals share one float4 (K2 reads them with one load per candidate ray)
+                    a.res[(((size_t)s * VSb + jb) * a.Cp + c) * NS + ko] = hr;
+                }
             }
         }
     }
     if (MODE == 1) {
-        // block's share of D: warp shuffles, then the (at most 32) warp sums in a fixed order
+        // block's share of each slice's D: warp shuffles, then the (at most 32) warp sums in a fixed order
 #pragma unroll
-        for (int off = 16; off > 0; off >>= 1) d2 += __shfl_down_sync(0xffffffffu, d2, off);
-        if ((t & 31) == 0) dred[t >> 5] = d2;
+        for (int sl = 0; sl < SB; ++sl) {
+#pragma unroll
+            for (int off = 16; off > 0; off >>= 1) d2[sl] += __shfl_down_sync(0xffffffffu, d2[sl], off);
+            if ((t & 31) == 0) dred[sl][t >> 5] = d2[sl];
+        }
         asm volatile("bar.sync 1, %0;" ::"r"(32 * nw) : "memory");     // only the epilogue warps meet here
-        if (t == 0) {
+        if (t < SB && s0 + t < a.batch) {
             double D = 0.0;
-            for (int w = 0; w < nw; ++w) D += dred[w];
-            a.dparts[(size_t)s * gridDim.x + blockIdx.x] = D;
+            for (int w = 0; w < nw; ++w) D += dred[t][w];
+            a.dparts[(size_t)(s0 + t) * gridDim.x + blockIdx.x] = D;
         }
     }
 }
@@ -419,11 +467,11 @@ __device__ __forceinline__ void load_nbhd(const DevGeom& g, const float* img, in
 #pragma unroll
     for (int r = 0; r < 4; ++r) {
         const int y = min(max(y0 - 1 + r, -PADR), g.ny + PADR - 1);
-        const float* row = img + (size_t)(y + PADR) * g.pitch + PAD;
+        const size_t row = (size_t)(y + PADR) * g.pitch + PAD;
 #pragma unroll
         for (int c = 0; c < 4; ++c) {
             const int x = min(x0 - 1 + c, g.nx + PAD - 1);
-            m[r][c] = __ldg(row + x);
+            m[r][c] = __ldg(img + (row + x) * g.sb);
         }
     }
 }
@@ -466,35 +514,32 @@ template <> struct BackAcc<1> {
 
 // one candidate ray r = {alpha, beta, g0, hk} against the 2x2 tile whose first pixel has centred indices (xc0, yc0):
 // the four chord weights (over h, which the residuals sv already carry) feed the tile's accumulators; with NS == 4
-// the same weights serve the orbit's four residuals.
-template <int NS>
-__device__ __forceinline__ void back_accumulate(const float4 r, const float4 sv, float xc0, float yc0, BackAcc<NS>& acc);
-template <>
-__device__ __forceinline__ void back_accumulate<4>(const float4 r, const float4 sv, float xc0, float yc0, BackAcc<4>& acc) {
+// the same weights serve the orbit's four residuals, and with SB == 2 the two slices of the block.
+__device__ __forceinline__ void back_weights(const float4 r, float xc0, float yc0, float (&w)[4]) {
     const float q00 = fmaf(r.x, xc0, fmaf(r.y, yc0, r.z));
     const float q01 = q00 + r.x;          // (ty=0, tx=1)
     const float q10 = q00 + r.y;          // (ty=1, tx=0)
     const float q11 = q10 + r.x;
-    const float w00 = __saturatef(r.w - fabsf(q00));
-    const float w01 = __saturatef(r.w - fabsf(q01));
-    const float w10 = __saturatef(r.w - fabsf(q10));
-    const float w11 = __saturatef(r.w - fabsf(q11));
-    const uint64_t sxy = pack2(sv.x, sv.y), szw = pack2(sv.z, sv.w);
-    ffma2(acc.p[0][0], sxy, w00); ffma2(acc.p[1][0], szw, w00);
-    ffma2(acc.p[0][1], sxy, w01); ffma2(acc.p[1][1], szw, w01);
-    ffma2(acc.p[0][2], sxy, w10); ffma2(acc.p[1][2], szw, w10);
-    ffma2(acc.p[0][3], sxy, w11); ffma2(acc.p[1][3], szw, w11);
+    w[0] = __saturatef(r.w - fabsf(q00));
+    w[1] = __saturatef(r.w - fabsf(q01));
+    w[2] = __saturatef(r.w - fabsf(q10));
+    w[3] = __saturatef(r.w - fabsf(q11));
 }
-template <>
-__device__ __forceinline__ void back_accumulate<1>(const float4 r, const float4 sv, float xc0, float yc0, BackAcc<1>& acc) {
-    const float q00 = fmaf(r.x, xc0, fmaf(r.y, yc0, r.z));
-    const float q01 = q00 + r.x;
-    const float q10 = q00 + r.y;
-    const float q11 = q10 + r.x;
-    acc.s[0] = fmaf(__saturatef(r.w - fabsf(q00)), sv.x, acc.s[0]);
-    acc.s[1] = fmaf(__saturatef(r.w - fabsf(q01)), sv.x, acc.s[1]);
-    acc.s[2] = fmaf(__saturatef(r.w - fabsf(q10)), sv.x, acc.s[2]);
-    acc.s[3] = fmaf(__saturatef(r.w - fabsf(q11)), sv.x, acc.s[3]);
+__device__ __forceinline__ void back_fma(const float (&w)[4], const float4 sv, BackAcc<4>& acc) {
+    const uint64_t sxy = pack2(sv.x, sv.y), szw = pack2(sv.z, sv.w);
+#pragma unroll
+    for (int p = 0; p < 4; ++p) { ffma2(acc.p[0][p], sxy, w[p]); ffma2(acc.p[1][p], szw, w[p]); }
+}
+__device__ __forceinline__ void back_fma(const float (&w)[4], const float4 sv, BackAcc<1>& acc) {
+#pragma unroll
+    for (int p = 0; p < 4; ++p) acc.s[p] = fmaf(w[p], sv.x, acc.s[p]);
+}
+// the residuals of candidate u of one view for the SB slices of the block (NS == 1: the scalar in .x)
+template <int NS, int SB>
+__device__ __forceinline__ void back_load(const float* const (&res)[SB], int off, float4 (&sv)[SB]) {
+#pragma unroll
+    for (int j = 0; j < SB; ++j)
+        sv[j] = NS == 4 ? __ldg(reinterpret_cast<const float4*>(res[j]) + off) : make_float4(__ldg(res[j] + off), 0.f, 0.f, 0.f);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -511,13 +556,13 @@ __device__ __forceinline__ void back_accumulate<1>(const float4 r, const float4 
 // view's orbit).  The shares' sums meet in shared memory in a fixed order; thread (tile, k) then finishes rotation
 // k of the tile (TV gradient, update, stores).  The host sizes the grid to one block per SM (plan_back).
 // ------------------------------------------------------------------------------------------------
-template <int MODE, int NS>
-__global__ void __launch_bounds__(BK_MAX_THREADS, 1) k_back(const BackArgs a) {
+template <int MODE, int NS, int SB>
+__global__ void __launch_bounds__(SB == 1 ? BK_MAX_THREADS : BKB_MAX_THREADS, SB == 1 ? 1 : 2) k_back(const BackArgs a) {
     const DevGeom& g = a.g;
-    const int t = threadIdx.x, lane = t & 31, s = blockIdx.z;
+    const int t = threadIdx.x, lane = t & 31, s0 = blockIdx.z * SB;       // slices s0 .. s0 + SB - 1
     const int tpb = a.tpb, shares = a.shares;
     const int q = t / tpb, i = t - q * tpb;
-    extern __shared__ float red[];                        // [shares][NS * 4][tpb]
+    extern __shared__ float red[];                        // [SB][shares][NS * 4][tpb]
 
     // tile number -> patch (2 x 2 patch groups, row-major) -> 2x2-pixel tile origin (x0, y0)
     auto tile_origin = [&](int T, int& x0, int& y0) {
@@ -534,8 +579,9 @@ __global__ void __launch_bounds__(BK_MAX_THREADS, 1) k_back(const BackArgs a) {
 
     // acc[m][ty*2+tx]: NS == 4: m = component of the orbit's residual float4 (this thread's views all lie in quarter
     // turn `quarter`, so rotation k of the tile collects component (quarter + k) % 4)
-    BackAcc<NS> acc;
-    acc.clear();
+    BackAcc<NS> acc[SB];
+#pragma unroll
+    for (int j = 0; j < SB; ++j) acc[j].clear();
 
     const int VSb = a.VS / NS;
     const int quarter = NS == 4 ? (q & 3) : 0;
@@ -544,7 +590,9 @@ __global__ void __launch_bounds__(BK_MAX_THREADS, 1) k_back(const BackArgs a) {
     {
         const float xc0 = (float)x0 - g.cx, yc0 = (float)y0 - g.cy;
         const float X = (xc0 + 0.5f * (BK_TX - 1)) * g.pixel, Y = (yc0 + 0.5f * (BK_TY - 1)) * g.pixel;
-        const float* res = a.res + (size_t)s * a.VS * a.Cp;      // same float count for both layouts
+        const float* res[SB];                                    // same float count for both layouts; a slice past the
+#pragma unroll
+        for (int j = 0; j < SB; ++j) res[j] = a.res + (size_t)min(s0 + j, a.batch - 1) * a.VS * a.Cp;   // batch repeats the last
 
         // Candidate interval of trip `it` (view jfirst + it * jstep of this thread's share): offsets of its first
         // candidate in the ray table and in the residual rows, and the warp's candidate count.  The warp runs
@@ -588,26 +636,30 @@ __global__ void __launch_bounds__(BK_MAX_THREADS, 1) k_back(const BackArgs a) {
             for (int e = 0; e < CH; e += 2) {
                 const float4* rpA = g.rays + offR[e];
                 const float4* rpB = g.rays + offR[e + 1];
-                const float4* spA = reinterpret_cast<const float4*>(res) + offS[e];      // NS == 4
-                const float4* spB = reinterpret_cast<const float4*>(res) + offS[e + 1];
-                const float* tpA = res + offS[e];                                        // NS == 1
-                const float* tpB = res + offS[e + 1];
                 if (ncw[e + 1] == 0) {                     // odd trip out (warp-uniform): one stream
 #pragma unroll 2
                     for (int u = 0; u < ncw[e]; ++u) {
                         const float4 rA = __ldg(rpA + u);
-                        const float4 sA = NS == 4 ? __ldg(spA + u) : make_float4(__ldg(tpA + u), 0.f, 0.f, 0.f);
-                        back_accumulate<NS>(rA, sA, xc0, yc0, acc);
+                        float4 sA[SB];
+                        back_load<NS, SB>(res, offS[e] + u, sA);
+                        float wA[4];
+                        back_weights(rA, xc0, yc0, wA);
+#pragma unroll
+                        for (int j = 0; j < SB; ++j) back_fma(wA, sA[j], acc[j]);
                     }
                 } else {
                     const int n = max(ncw[e], ncw[e + 1]);
 #pragma unroll 2
                     for (int u = 0; u < n; ++u) {
                         const float4 rA = __ldg(rpA + u), rB = __ldg(rpB + u);
-                        const float4 sA = NS == 4 ? __ldg(spA + u) : make_float4(__ldg(tpA + u), 0.f, 0.f, 0.f);
-                        const float4 sB = NS == 4 ? __ldg(spB + u) : make_float4(__ldg(tpB + u), 0.f, 0.f, 0.f);
-                        back_accumulate<NS>(rA, sA, xc0, yc0, acc);
-                        back_accumulate<NS>(rB, sB, xc0, yc0, acc);
+                        float4 sA[SB], sB[SB];
+                        back_load<NS, SB>(res, offS[e] + u, sA);
+                        back_load<NS, SB>(res, offS[e + 1] + u, sB);
+                        float wA[4], wB[4];
+                        back_weights(rA, xc0, yc0, wA);
+                        back_weights(rB, xc0, yc0, wB);
+#pragma unroll
+                        for (int j = 0; j < SB; ++j) { back_fma(wA, sA[j], acc[j]); back_fma(wB, sB[j], acc[j]); }
                     }
                 }
             }
@@ -623,9 +675,12 @@ __global__ void __launch_bounds__(BK_MAX_THREADS, 1) k_back(const BackArgs a) {
     // rotation k of the tile = orbit component (quarter + k) % 4  <=>  component m feeds rotation (m - quarter) % 4
     if (q < shares) {
 #pragma unroll
-        for (int m = 0; m < NS; ++m)
+        for (int j = 0; j < SB; ++j)
 #pragma unroll
-            for (int p = 0; p < 4; ++p) red[(q * (NS * 4) + ((m - quarter) & (NS - 1)) * 4 + p) * tpb + i] = acc.get(m, p);
+            for (int m = 0; m < NS; ++m)
+#pragma unroll
+                for (int p = 0; p < 4; ++p)
+                    red[((j * shares + q) * (NS * 4) + ((m - quarter) & (NS - 1)) * 4 + p) * tpb + i] = acc[j].get(m, p);
     }
 
     // thread (tile i, k = q < NS) finishes rotation k of the base tile: origin (xk, yk) and, below, where base pixel
@@ -641,26 +696,33 @@ __global__ void __launch_bounds__(BK_MAX_THREADS, 1) k_back(const BackArgs a) {
         else if (k == 2) { xk = N - 2 - x0; yk = N - 2 - y0; }
         else if (k == 3) { xk = y0;         yk = N - 2 - x0; }
     }
-    StepInfo si;
-    float step = 0.f;
-    float m[4][4], tv[2][2];
+    StepInfo si[SB];
+    float step[SB], m[SB][4][4], tv[SB][2][2];
     if (MODE == 1 && t < 32 * ((NS * tpb + 31) / 32)) {           // whole warps: step_rule shuffles
         const bool writer = blockIdx.x == 0 && t < 32;
-        if (fin_active) load_nbhd(g, a.img + (size_t)s * g.img_elems, xk, yk, m);
-        si = step_rule(a, s, lane, writer);
-        step = (float)(si.lambda * a.tau);
-        if (fin_active) tv_grad_tile(m, xk, yk, g.nx, g.ny, a.eps2, tv);
+#pragma unroll
+        for (int j = 0; j < SB; ++j) {
+            const int s = s0 + j;
+            if (s >= a.batch) break;
+            if (fin_active) load_nbhd(g, a.img + slice_base(g, g.img_elems, s), xk, yk, m[j]);
+            si[j] = step_rule(a, s, lane, writer);
+            step[j] = (float)(si[j].lambda * a.tau);
+            if (fin_active) tv_grad_tile(m[j], xk, yk, g.nx, g.ny, a.eps2, tv[j]);
+        }
     }
     __syncthreads();
     if (!fin_active) return;
 
-    {
+#pragma unroll
+    for (int j = 0; j < SB; ++j) {
+        const int s = s0 + j;
+        if (s >= a.batch) break;
         // sums over the view shares, fixed order
         float b[4];
 #pragma unroll
         for (int p = 0; p < 4; ++p) {
             float x = 0.f;
-            for (int qq = 0; qq < shares; ++qq) x += red[(qq * (NS * 4) + k * 4 + p) * tpb + i];
+            for (int qq = 0; qq < shares; ++qq) x += red[((j * shares + qq) * (NS * 4) + k * 4 + p) * tpb + i];
             b[p] = x;
         }
         float o00 = b[0], o01 = b[1], o10 = b[2], o11 = b[3];
@@ -676,29 +738,30 @@ __global__ void __launch_bounds__(BK_MAX_THREADS, 1) k_back(const BackArgs a) {
             if (vx1) out[(size_t)yk * g.nx + xk + 1] = o01;
             if (vy1) out[(size_t)(yk + 1) * g.nx + xk] = o10;
             if (vx1 && vy1) out[(size_t)(yk + 1) * g.nx + xk + 1] = o11;
-            return;
+            continue;
         }
 
         // ---- A5 TV gradient of mu(n), A6 update (Eq. 3) with mu > 0, A7 best copy ----
-        const float u00 = fmaxf(fmaf(step, o00 - a.beta_over_M * tv[0][0], m[1][1]), 0.f);
-        const float u01 = fmaxf(fmaf(step, o01 - a.beta_over_M * tv[0][1], m[1][2]), 0.f);
-        const float u10 = fmaxf(fmaf(step, o10 - a.beta_over_M * tv[1][0], m[2][1]), 0.f);
-        const float u11 = fmaxf(fmaf(step, o11 - a.beta_over_M * tv[1][1], m[2][2]), 0.f);
+        const float u00 = fmaxf(fmaf(step[j], o00 - a.beta_over_M * tv[j][0][0], m[j][1][1]), 0.f);
+        const float u01 = fmaxf(fmaf(step[j], o01 - a.beta_over_M * tv[j][0][1], m[j][1][2]), 0.f);
+        const float u10 = fmaxf(fmaf(step[j], o10 - a.beta_over_M * tv[j][1][0], m[j][2][1]), 0.f);
+        const float u11 = fmaxf(fmaf(step[j], o11 - a.beta_over_M * tv[j][1][1], m[j][2][2]), 0.f);
 
-        float* nimg = a.img_new + (size_t)s * g.img_elems;
-        float* nimgT = a.imgT_new + (size_t)s * g.imgT_elems;
-        nimg[pad_off(g, yk, xk)] = u00;
-        nimgT[padT_off(g, xk, yk)] = u00;
-        if (vx1) { nimg[pad_off(g, yk, xk + 1)] = u01; nimgT[padT_off(g, xk + 1, yk)] = u01; }
-        if (vy1) { nimg[pad_off(g, yk + 1, xk)] = u10; nimgT[padT_off(g, xk, yk + 1)] = u10; }
-        if (vx1 && vy1) { nimg[pad_off(g, yk + 1, xk + 1)] = u11; nimgT[padT_off(g, xk + 1, yk + 1)] = u11; }
+        float* nimg = a.img_new + slice_base(g, g.img_elems, s);
+        float* nimgT = a.imgT_new + slice_base(g, g.imgT_elems, s);
+        const int sb = g.sb;
+        nimg[pad_off(g, yk, xk) * sb] = u00;
+        nimgT[padT_off(g, xk, yk) * sb] = u00;
+        if (vx1) { nimg[pad_off(g, yk, xk + 1) * sb] = u01; nimgT[padT_off(g, xk + 1, yk) * sb] = u01; }
+        if (vy1) { nimg[pad_off(g, yk + 1, xk) * sb] = u10; nimgT[padT_off(g, xk, yk + 1) * sb] = u10; }
+        if (vx1 && vy1) { nimg[pad_off(g, yk + 1, xk + 1) * sb] = u11; nimgT[padT_off(g, xk + 1, yk + 1) * sb] = u11; }
 
-        if (a.best && si.improved) {
+        if (a.best && si[j].improved) {
             float* best = a.best + (size_t)s * g.nx * g.ny;
-            best[(size_t)yk * g.nx + xk] = m[1][1];
-            if (vx1) best[(size_t)yk * g.nx + xk + 1] = m[1][2];
-            if (vy1) best[(size_t)(yk + 1) * g.nx + xk] = m[2][1];
-            if (vx1 && vy1) best[(size_t)(yk + 1) * g.nx + xk + 1] = m[2][2];
+            best[(size_t)yk * g.nx + xk] = m[j][1][1];
+            if (vx1) best[(size_t)yk * g.nx + xk + 1] = m[j][1][2];
+            if (vy1) best[(size_t)(yk + 1) * g.nx + xk] = m[j][2][1];
+            if (vx1 && vy1) best[(size_t)(yk + 1) * g.nx + xk + 1] = m[j][2][2];
         }
     }
 }
@@ -715,21 +778,21 @@ __global__ void __launch_bounds__(256) k_pad_transpose(DevGeom g, const float* _
     const int bx = blockIdx.x * 32, by = blockIdx.y * 32;
     const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;       // 32 x 8
     src += (size_t)s * g.nx * g.ny;
-    img += (size_t)s * g.img_elems;
-    imgT += (size_t)s * g.imgT_elems;
+    img += slice_base(g, g.img_elems, s);
+    imgT += slice_base(g, g.imgT_elems, s);
     for (int r = ty; r < 32; r += 8) {
         const int x = bx + tx, y = by + r;
         float v = 0.f;
         if (x < g.nx && y < g.ny) {
             v = src[(size_t)y * g.nx + x];
-            img[pad_off(g, y, x)] = v;
+            img[pad_off(g, y, x) * g.sb] = v;
         }
         tile[r][tx] = v;
     }
     __syncthreads();
     for (int r = ty; r < 32; r += 8) {
         const int x = bx + r, y = by + tx;
-        if (x < g.nx && y < g.ny) imgT[padT_off(g, x, y)] = tile[tx][r];
+        if (x < g.nx && y < g.ny) imgT[padT_off(g, x, y) * g.sb] = tile[tx][r];
     }
 }
 
@@ -743,7 +806,7 @@ __global__ void __launch_bounds__(256) k_unpad(DevGeom g, const float* __restric
     if (x >= g.nx || y >= g.ny) return;
     const size_t o = (size_t)s * g.nx * g.ny + (size_t)y * g.nx + x;
     if (best && !state[s].improved) out[o] = best[o];
-    else out[o] = img[(size_t)s * g.img_elems + pad_off(g, y, x)];
+    else out[o] = img[slice_base(g, g.img_elems, s) + pad_off(g, y, x) * g.sb];
 }
 
 // homogeneous initial image into both padded layouts, and into best
@@ -753,8 +816,8 @@ __global__ void __launch_bounds__(256) k_fill(DevGeom g, float mu0, float* __res
     const int x = blockIdx.x * 32 + (threadIdx.x & 31);
     const int y = blockIdx.y * 8 + (threadIdx.x >> 5);
     if (x >= g.nx || y >= g.ny) return;
-    img[(size_t)s * g.img_elems + pad_off(g, y, x)] = mu0;
-    imgT[(size_t)s * g.imgT_elems + padT_off(g, x, y)] = mu0;
+    img[slice_base(g, g.img_elems, s) + pad_off(g, y, x) * g.sb] = mu0;
+    imgT[slice_base(g, g.imgT_elems, s) + padT_off(g, x, y) * g.sb] = mu0;
     if (best) best[(size_t)s * g.nx * g.ny + (size_t)y * g.nx + x] = mu0;
 }
 
@@ -804,7 +867,7 @@ __global__ void __launch_bounds__(128) k_tv(DevGeom g, const float* __restrict__
     const int s = blockIdx.z;
     if (x0 >= g.nx || y0 >= g.ny) return;
     float m[4][4], tv[2][2];
-    load_nbhd(g, img + (size_t)s * g.img_elems, x0, y0, m);
+    load_nbhd(g, img + slice_base(g, g.img_elems, s), x0, y0, m);
     tv_grad_tile(m, x0, y0, g.nx, g.ny, eps2, tv);
     out += (size_t)s * g.nx * g.ny;
     const bool vx1 = x0 + 1 < g.nx, vy1 = y0 + 1 < g.ny;
