@@ -476,6 +476,21 @@ __device__ __forceinline__ void load_nbhd(const DevGeom& g, const float* img, in
     }
 }
 
+// the same neighbourhood in the two slices of a pair (images interleaved per pixel: one float2 per pixel)
+__device__ __forceinline__ void load_nbhd2(const DevGeom& g, const float2* img2, int x0, int y0, float (&m0)[4][4], float (&m1)[4][4]) {
+#pragma unroll
+    for (int r = 0; r < 4; ++r) {
+        const int y = min(max(y0 - 1 + r, -PADR), g.ny + PADR - 1);
+        const float2* row = img2 + (size_t)(y + PADR) * g.pitch + PAD;
+#pragma unroll
+        for (int c = 0; c < 4; ++c) {
+            const int x = min(x0 - 1 + c, g.nx + PAD - 1);
+            const float2 v = __ldg(row + x);
+            m0[r][c] = v.x; m1[r][c] = v.y;
+        }
+    }
+}
+
 // atan(z) for |z| <= 0.75: odd polynomial, max error 3e-7 rad (fit on Chebyshev nodes; checked on the host side of
 // the tests through the candidate-range parity cases)
 __device__ __forceinline__ float atan_small(float z) {
@@ -700,11 +715,14 @@ __global__ void __launch_bounds__(SB == 1 ? BK_MAX_THREADS : BKB_MAX_THREADS, SB
     float step[SB], m[SB][4][4], tv[SB][2][2];
     if (MODE == 1 && t < 32 * ((NS * tpb + 31) / 32)) {           // whole warps: step_rule shuffles
         const bool writer = blockIdx.x == 0 && t < 32;
+        if constexpr (SB == 2) {
+            if (fin_active) load_nbhd2(g, reinterpret_cast<const float2*>(a.img) + (size_t)blockIdx.z * g.img_elems, xk, yk, m[0], m[SB - 1]);
+        }
 #pragma unroll
         for (int j = 0; j < SB; ++j) {
             const int s = s0 + j;
             if (s >= a.batch) break;
-            if (fin_active) load_nbhd(g, a.img + slice_base(g, g.img_elems, s), xk, yk, m[j]);
+            if (SB == 1 && fin_active) load_nbhd(g, a.img + slice_base(g, g.img_elems, s), xk, yk, m[j]);
             si[j] = step_rule(a, s, lane, writer);
             step[j] = (float)(si[j].lambda * a.tau);
             if (fin_active) tv_grad_tile(m[j], xk, yk, g.nx, g.ny, a.eps2, tv[j]);
@@ -713,6 +731,7 @@ __global__ void __launch_bounds__(SB == 1 ? BK_MAX_THREADS : BKB_MAX_THREADS, SB
     __syncthreads();
     if (!fin_active) return;
 
+    float un[SB][4] = {};                                     // SB == 2: mu(n+1) of the tile in both slices (0 in an empty one)
 #pragma unroll
     for (int j = 0; j < SB; ++j) {
         const int s = s0 + j;
@@ -746,15 +765,17 @@ __global__ void __launch_bounds__(SB == 1 ? BK_MAX_THREADS : BKB_MAX_THREADS, SB
         const float u01 = fmaxf(fmaf(step[j], o01 - a.beta_over_M * tv[j][0][1], m[j][1][2]), 0.f);
         const float u10 = fmaxf(fmaf(step[j], o10 - a.beta_over_M * tv[j][1][0], m[j][2][1]), 0.f);
         const float u11 = fmaxf(fmaf(step[j], o11 - a.beta_over_M * tv[j][1][1], m[j][2][2]), 0.f);
-
-        float* nimg = a.img_new + slice_base(g, g.img_elems, s);
-        float* nimgT = a.imgT_new + slice_base(g, g.imgT_elems, s);
-        const int sb = g.sb;
-        nimg[pad_off(g, yk, xk) * sb] = u00;
-        nimgT[padT_off(g, xk, yk) * sb] = u00;
-        if (vx1) { nimg[pad_off(g, yk, xk + 1) * sb] = u01; nimgT[padT_off(g, xk + 1, yk) * sb] = u01; }
-        if (vy1) { nimg[pad_off(g, yk + 1, xk) * sb] = u10; nimgT[padT_off(g, xk, yk + 1) * sb] = u10; }
-        if (vx1 && vy1) { nimg[pad_off(g, yk + 1, xk + 1) * sb] = u11; nimgT[padT_off(g, xk + 1, yk + 1) * sb] = u11; }
+        if constexpr (SB == 2) {
+            un[j][0] = u00; un[j][1] = u01; un[j][2] = u10; un[j][3] = u11;      // stored below, both slices at once
+        } else {
+            float* nimg = a.img_new + slice_base(g, g.img_elems, s);
+            float* nimgT = a.imgT_new + slice_base(g, g.imgT_elems, s);
+            nimg[pad_off(g, yk, xk)] = u00;
+            nimgT[padT_off(g, xk, yk)] = u00;
+            if (vx1) { nimg[pad_off(g, yk, xk + 1)] = u01; nimgT[padT_off(g, xk + 1, yk)] = u01; }
+            if (vy1) { nimg[pad_off(g, yk + 1, xk)] = u10; nimgT[padT_off(g, xk, yk + 1)] = u10; }
+            if (vx1 && vy1) { nimg[pad_off(g, yk + 1, xk + 1)] = u11; nimgT[padT_off(g, xk + 1, yk + 1)] = u11; }
+        }
 
         if (a.best && si[j].improved) {
             float* best = a.best + (size_t)s * g.nx * g.ny;
@@ -763,6 +784,18 @@ __global__ void __launch_bounds__(SB == 1 ? BK_MAX_THREADS : BKB_MAX_THREADS, SB
             if (vy1) best[(size_t)(yk + 1) * g.nx + xk] = m[j][2][1];
             if (vx1 && vy1) best[(size_t)(yk + 1) * g.nx + xk + 1] = m[j][2][2];
         }
+    }
+    if constexpr (SB == 2 && MODE == 1) {
+        float2* nimg = reinterpret_cast<float2*>(a.img_new) + (size_t)blockIdx.z * g.img_elems;
+        float2* nimgT = reinterpret_cast<float2*>(a.imgT_new) + (size_t)blockIdx.z * g.imgT_elems;
+        const bool vx1 = xk + 1 < g.nx, vy1 = yk + 1 < g.ny;
+        const float2 u00 = make_float2(un[0][0], un[SB - 1][0]), u01 = make_float2(un[0][1], un[SB - 1][1]);
+        const float2 u10 = make_float2(un[0][2], un[SB - 1][2]), u11 = make_float2(un[0][3], un[SB - 1][3]);
+        nimg[pad_off(g, yk, xk)] = u00;
+        nimgT[padT_off(g, xk, yk)] = u00;
+        if (vx1) { nimg[pad_off(g, yk, xk + 1)] = u01; nimgT[padT_off(g, xk + 1, yk)] = u01; }
+        if (vy1) { nimg[pad_off(g, yk + 1, xk)] = u10; nimgT[padT_off(g, xk, yk + 1)] = u10; }
+        if (vx1 && vy1) { nimg[pad_off(g, yk + 1, xk + 1)] = u11; nimgT[padT_off(g, xk + 1, yk + 1)] = u11; }
     }
 }
 
