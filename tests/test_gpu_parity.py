@@ -441,6 +441,38 @@ def test_reconstruct_same_subset_monitor_variant(osiv):
         assert np.array_equal(tr[s, :, 1], tr_ref[:, 1]) and rel(host(got)[s], ref) < IMG_TOL
 
 
+@pytest.mark.parametrize("cfg,M", [(si.scan_config("1"), 3), (SYM, 2), (ODD, 4)])
+def test_pairs_of_slices_path_matches_oracle(osiv, cfg, M):
+    """Launches with >= 4 slices serve a pair of slices per block (interleaved images, shared chord weights): an odd
+    batch (the last pair half empty) of different slices against the oracle, slice by slice -- projector pair,
+    reconstruction with return_best, traces -- on the general path (config 1, ODD) and the quarter-turn path (SYM)."""
+    og, gg = geoms(cfg)
+    B = 5
+    rng = np.random.default_rng(cfg.seed + 9)
+    with osiv.Handle(gg, max_batch=B) as h:
+        assert h.plan(M, B)["k2_threads"] <= 448            # the pair path is the one being planned
+        img = rng.uniform(0.0, 0.013, size=(B, cfg.ny, cfg.nx)).astype(np.float32)
+        vs = cfg.n_views // M
+        sino = rng.uniform(0.0, 1.0, size=(B, vs, cfg.n_channels)).astype(np.float32)
+        f, b = host(h.forward(dev(img), 1, M)), host(h.backward(dev(sino), 1, M))
+        for s in range(B):
+            assert rel(f[s], oracle.forward(og, img[s], 1, M)) < PROJ_TOL
+            assert rel(b[s], oracle.backward(og, sino[s], 1, M)) < PROJ_TOL
+        counts = np.stack([si.make_case(cfg, slice_index=s)[2] for s in range(B)])
+        kw = dict(beta=0.004, n_subsets=M, n_iters=24, return_best=1)
+        got, tr = h.reconstruct(dev(counts), cfg.i0, osiv.Params(**kw), trace=True)
+        again, tr2 = h.reconstruct(dev(counts), cfg.i0, osiv.Params(**kw), trace=True)
+        assert torch.equal(got, again) and np.array_equal(tr, tr2)
+        for s in range(B):
+            ref, tr_ref, _ = oracle.reconstruct(og, counts[s], cfg.i0, oracle.Params(**kw))
+            assert np.array_equal(tr[s, :, 1], tr_ref[:, 1])
+            assert np.all(np.abs(tr[s, :, 0] - tr_ref[:, 0]) <= 1e-5 * tr_ref[:, 0])
+            assert rel(host(got)[s], ref) < IMG_TOL
+        # a single slice on the same handle afterwards (the image buffers change their layout back)
+        one = h.reconstruct(dev(counts[:1]), cfg.i0, osiv.Params(**kw))
+        assert rel(host(one)[0], host(got)[0].astype(np.float64)) < 2e-6
+
+
 def test_dependent_launch_chain_gives_the_same_bits_as_stream_order(osiv):
     """K1/K2 chained by programmatic dependent launch (default) vs plain stream order: the overlap moves only
     constant-dependent prologues ahead of the wait, so images and traces must be identical bit for bit."""
