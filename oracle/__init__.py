@@ -10,5 +10,5 @@ it with gcc and marshals numpy arrays through ctypes.
 from .oracle import (  # noqa: F401
     Geometry, Params, build, lib, num_threads, set_num_threads, dgamma, ray, weight, candidate_K,
     forward, forward_brute, backward, backward_brute, tv_value, tv_grad, loglik, residual, tau,
-    reconstruct,
+    reconstruct, tv3_value, tv3_grad, reconstruct_stack,
 )

@@ -105,6 +105,11 @@ def lib():
         L.oracle_residual.argtypes = [gp, dp, dp, dp, C.c_double, C.c_int, C.c_int, dp]
         L.oracle_tau.restype = C.c_double
         L.oracle_tau.argtypes = [gp, C.c_int, C.c_double]
+        L.oracle_tv3_value.restype = C.c_double
+        L.oracle_tv3_value.argtypes = [dp, C.c_int, C.c_int, C.c_int, C.c_double, C.c_double]
+        L.oracle_tv3_grad.argtypes = [dp, dp, C.c_int, C.c_int, C.c_int, C.c_double, C.c_double]
+        L.oracle_reconstruct_stack.restype = C.c_int
+        L.oracle_reconstruct_stack.argtypes = [gp, C.c_int, dp, dp, C.c_double, C.POINTER(_CParams), C.c_int, C.c_double, dp, dp]
         L.oracle_reconstruct.restype = C.c_int
         L.oracle_reconstruct.argtypes = [gp, dp, dp, C.c_double, C.POINTER(_CParams), dp, dp]
         _lib = L
@@ -231,4 +236,33 @@ def reconstruct(g: Geometry, counts, blank, prm: Params):
     img = np.zeros((g.ny, g.nx), dtype=np.float64)
     trace = np.zeros((prm.n_iters, 2), dtype=np.float64)
     status = lib().oracle_reconstruct(C.byref(g.c()), _dp(counts), _dp(b), bs, C.byref(cp), _dp(img), _dp(trace))
+    return img, trace, status
+
+
+def tv3_value(mu, eps: float, wz: float) -> float:
+    """3-D smoothed isotropic TV of a stack [S][ny][nx] (reading H2)"""
+    mu = _f64(mu)
+    return lib().oracle_tv3_value(_dp(mu), mu.shape[2], mu.shape[1], mu.shape[0], eps, wz)
+
+
+def tv3_grad(mu, eps: float, wz: float):
+    mu = _f64(mu)
+    out = np.zeros_like(mu)
+    lib().oracle_tv3_grad(_dp(mu), _dp(out), mu.shape[2], mu.shape[1], mu.shape[0], eps, wz)
+    return out
+
+
+def reconstruct_stack(g: Geometry, counts, blank, prm: Params, view_shift: int = 0, tv_z: float = 0.0):
+    """Stack of S slices (readings H1-H3): counts [S][V][C] -> (images [S][ny][nx], trace [S][n_iters][2], status)"""
+    counts = _f64(counts)
+    S = counts.shape[0]
+    assert counts.shape[1:] == (g.n_views, g.n_channels) and g.n_views % prm.n_subsets == 0
+    assert prm.forced_lambda is None and not prm.return_best
+    b, bs = _blank(blank)
+    cp = _CParams(prm.beta, prm.n_subsets, prm.n_iters, prm.mu0, prm.lambda0, prm.lambda_up, prm.lambda_down,
+                  prm.lambda_min, prm.kappa, prm.tv_eps, 0, prm.monitor_mode, None)
+    img = np.zeros((S, g.ny, g.nx), dtype=np.float64)
+    trace = np.zeros((S, prm.n_iters, 2), dtype=np.float64)
+    status = lib().oracle_reconstruct_stack(C.byref(g.c()), S, _dp(counts), _dp(b), bs, C.byref(cp), view_shift, tv_z,
+                                            _dp(img), _dp(trace))
     return img, trace, status

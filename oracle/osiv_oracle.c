@@ -420,3 +420,102 @@ int oracle_reconstruct(const oracle_geometry* g, const double* counts, const dou
     free(mu); free(best); free(grad); free(tvg); free(l); free(resid); free(Dsub);
     return status;
 }
+
+/* ======================================================================================================
+ * Stack of slices (readings H1-H3): TomoTherapy acquires helically
+ * (PAPER.md:51), so neighbouring slices see the gantry at shifted angles and belong to one volume.
+ *   H1  slice s of S is a 2-D fan slice whose view j was taken at gantry angle theta0 + 2*pi*(j + k*s)/V:
+ *       the couch advances one slice every k views (view_shift = k, an integer number of views).
+ *   H2  the prior is the 3-D smoothed isotropic TV  sum_{x,y,s} sqrt(eps^2 + dx^2 + dy^2 + Dz^2),
+ *       Dz = w_z * (mu_{s+1} - mu_s), forward differences, 0 across the volume's border (w_z = tv_z).
+ *   H3  every slice keeps its own monitor D_s (its own data) and its own step lambda_s by Eq. 4-5; all slices
+ *       are updated together from mu(n) (the coupling enters only through the TV gradient).
+ * ====================================================================================================== */
+static double tv3_cell(const double* mu, int nx, int ny, int S, int x, int y, int s, double eps, double wz) {
+    const size_t np = (size_t)nx * ny;
+    double c = mu[s * np + (size_t)y * nx + x];
+    double dxv = (x + 1 < nx) ? mu[s * np + (size_t)y * nx + x + 1] - c : 0.0;
+    double dyv = (y + 1 < ny) ? mu[s * np + (size_t)(y + 1) * nx + x] - c : 0.0;
+    double dzv = (s + 1 < S) ? wz * (mu[(s + 1) * np + (size_t)y * nx + x] - c) : 0.0;
+    return sqrt(eps * eps + dxv * dxv + dyv * dyv + dzv * dzv);
+}
+
+double oracle_tv3_value(const double* mu, int nx, int ny, int S, double eps, double wz) {
+    double t = 0.0;
+    for (int s = 0; s < S; ++s)
+        for (int y = 0; y < ny; ++y)
+            for (int x = 0; x < nx; ++x) t += tv3_cell(mu, nx, ny, S, x, y, s, eps, wz);
+    return t;
+}
+
+/* d/dmu_{x,y,s}: own cell -(dx + dy + w_z*Dz)/t, cell (x-1,y,s) +dx/t, cell (x,y-1,s) +dy/t,
+ * cell (x,y,s-1) +w_z*Dz/t; out-of-range terms dropped */
+void oracle_tv3_grad(const double* mu, double* grad, int nx, int ny, int S, double eps, double wz) {
+    const size_t np = (size_t)nx * ny;
+    #pragma omp parallel for collapse(2)
+    for (int s = 0; s < S; ++s)
+        for (int y = 0; y < ny; ++y)
+            for (int x = 0; x < nx; ++x) {
+                const size_t o = s * np + (size_t)y * nx + x;
+                double c = mu[o], g = 0.0;
+                if (x > 0) g += (c - mu[o - 1]) / tv3_cell(mu, nx, ny, S, x - 1, y, s, eps, wz);
+                if (y > 0) g += (c - mu[o - nx]) / tv3_cell(mu, nx, ny, S, x, y - 1, s, eps, wz);
+                if (s > 0) g += wz * wz * (c - mu[o - np]) / tv3_cell(mu, nx, ny, S, x, y, s - 1, eps, wz);
+                double dxv = (x + 1 < nx) ? mu[o + 1] - c : 0.0;
+                double dyv = (y + 1 < ny) ? mu[o + nx] - c : 0.0;
+                double dzv = (s + 1 < S) ? wz * (mu[o + np] - c) : 0.0;
+                g -= (dxv + dyv + wz * dzv) / tv3_cell(mu, nx, ny, S, x, y, s, eps, wz);
+                grad[o] = g;
+            }
+}
+
+/* counts [S][V][C]; img_out [S][ny][nx]; trace NULL or [S][n_iters][2].  view_shift = k (H1), tv_z = w_z (H2;
+ * 0 = the 2-D prior slice by slice).  return_best and forced_lambda are not offered for stacks. */
+int oracle_reconstruct_stack(const oracle_geometry* g, int S, const double* counts, const double* blank,
+                             double blank_scalar, const oracle_params* prm, int view_shift, double tv_z,
+                             double* img_out, double* trace) {
+    const int M = prm->n_subsets, C = g->n_channels, nv = g->n_views / M, N = prm->n_iters;
+    const size_t npix = (size_t)g->nx * g->ny, nray = (size_t)nv * C, nsino = (size_t)g->n_views * C;
+    double* mu    = (double*)malloc(sizeof(double) * npix * S);
+    double* nxt   = (double*)malloc(sizeof(double) * npix * S);
+    double* tvg   = (double*)malloc(sizeof(double) * npix * S);
+    double* grad  = (double*)malloc(sizeof(double) * npix);
+    double* l     = (double*)malloc(sizeof(double) * nray);
+    double* resid = (double*)malloc(sizeof(double) * nray);
+    double* lambda = (double*)malloc(sizeof(double) * S);
+    double* Dprev  = (double*)malloc(sizeof(double) * S);
+    double* Dsub   = (double*)malloc(sizeof(double) * S * M);
+    const double tau = oracle_tau(g, M, prm->kappa);
+    int status = 0;
+    for (size_t r = 0; r < npix * S; ++r) mu[r] = prm->mu0;
+    for (int s = 0; s < S; ++s) { lambda[s] = prm->lambda0; Dprev[s] = 0.0; }
+
+    for (int n = 0; n < N; ++n) {
+        const int m = n % M;
+        if (tv_z > 0.0) oracle_tv3_grad(mu, tvg, g->nx, g->ny, S, prm->tv_eps, tv_z);
+        else for (int s = 0; s < S; ++s) oracle_tv_grad(mu + s * npix, tvg + s * npix, g->nx, g->ny, prm->tv_eps);
+        for (int s = 0; s < S; ++s) {
+            oracle_geometry gs = *g;                                           /* H1: the gantry angle of slice s */
+            gs.theta0_rad = g->theta0_rad + 2.0 * M_PI * (double)view_shift * (double)s / (double)g->n_views;
+            const double* mus = mu + s * npix;
+            oracle_forward(&gs, mus, l, m, M);
+            double D = oracle_residual(&gs, l, counts + s * nsino, blank, blank_scalar, m, M, resid);
+            if (!isfinite(D)) status = -3;
+            double lam = lambda[s];
+            if (n < (prm->monitor_mode ? M : 1)) lam = prm->lambda0;
+            else if (D < (prm->monitor_mode ? Dsub[s * M + m] : Dprev[s])) lam = lam + prm->lambda_up;
+            else { lam = lam - prm->lambda_down; if (lam < prm->lambda_min) lam = prm->lambda_min; }
+            lambda[s] = lam; Dprev[s] = D; Dsub[s * M + m] = D;
+            if (trace) { trace[((size_t)s * N + n) * 2] = D; trace[((size_t)s * N + n) * 2 + 1] = lam; }
+            oracle_backward(&gs, resid, grad, m, M);
+            for (size_t r = 0; r < npix; ++r) {
+                double u = mus[r] + lam * tau * (grad[r] - (prm->beta / M) * tvg[s * npix + r]);
+                nxt[s * npix + r] = u > 0.0 ? u : 0.0;
+            }
+        }
+        double* t = mu; mu = nxt; nxt = t;
+    }
+    memcpy(img_out, mu, sizeof(double) * npix * S);
+    free(mu); free(nxt); free(tvg); free(grad); free(l); free(resid); free(lambda); free(Dprev); free(Dsub);
+    return status;
+}
