@@ -80,6 +80,14 @@ typedef struct {
     int32_t return_best;     /* 0: final iterate; 1: iterate with the smallest monitor D */
     int32_t monitor_mode;    /* which earlier D Eq. 4-5 compare D(n) with: 0 = D(n-1), the previous iteration (C10, default);
                                 1 = D(n-M), the same subset one pass earlier (G3; lambda(n) = lambda0 for n < M) */
+    /* Stack of slices (readings H1-H3): the `batch` slices of a call form one volume, slice 0 first. */
+    int32_t view_shift;      /* H1: views the gantry advances per slice; view j of slice s was taken at angle
+                                theta0 + 2*pi*(j + view_shift*s)/V.  0 = every slice at the same angles (default) */
+    int32_t reserved;        /* must be 0 */
+    double  tv_z;            /* H2: > 0 couples neighbouring slices through the 3-D smoothed TV
+                                sum sqrt(eps^2 + dx^2 + dy^2 + (tv_z*(mu_{s+1} - mu_s))^2); 0 = 2-D TV per slice (default).
+                                Every slice keeps its own monitor and step (H3).  With view_shift != 0 or tv_z > 0,
+                                return_best and forced_lambda must be off. */
     const double* forced_lambda;  /* HOST pointer: NULL, or n_iters values used instead of Eq. 4-5 */
 } osiv_params;
 

@@ -38,7 +38,8 @@ class _CParams(C.Structure):
     _fields_ = [("beta", C.c_double), ("n_subsets", C.c_int32), ("n_iters", C.c_int32), ("mu0", C.c_double),
                 ("lambda0", C.c_double), ("lambda_up", C.c_double), ("lambda_down", C.c_double),
                 ("lambda_min", C.c_double), ("kappa", C.c_double), ("tv_eps", C.c_double),
-                ("return_best", C.c_int32), ("monitor_mode", C.c_int32), ("forced_lambda", C.POINTER(C.c_double))]
+                ("return_best", C.c_int32), ("monitor_mode", C.c_int32), ("view_shift", C.c_int32), ("reserved", C.c_int32),
+                ("tv_z", C.c_double), ("forced_lambda", C.POINTER(C.c_double))]
 
 
 @dataclass
@@ -74,6 +75,8 @@ class Params:
     tv_eps: float = 1e-5
     return_best: int = 0
     monitor_mode: int = 0
+    view_shift: int = 0
+    tv_z: float = 0.0
     forced_lambda: Optional[np.ndarray] = None
 
 
@@ -130,7 +133,8 @@ def default_params() -> Params:
     _check(lib().osiv_default_params(C.byref(cp)), "osiv_default_params")
     return Params(beta=cp.beta, n_subsets=cp.n_subsets, n_iters=cp.n_iters, mu0=cp.mu0, lambda0=cp.lambda0,
                   lambda_up=cp.lambda_up, lambda_down=cp.lambda_down, lambda_min=cp.lambda_min, kappa=cp.kappa,
-                  tv_eps=cp.tv_eps, return_best=cp.return_best, monitor_mode=cp.monitor_mode)
+                  tv_eps=cp.tv_eps, return_best=cp.return_best, monitor_mode=cp.monitor_mode,
+                  view_shift=cp.view_shift, tv_z=cp.tv_z)
 
 
 def ray_table(geom: "Geometry"):
@@ -170,7 +174,7 @@ def _cparams(p: Params):
             raise ValueError("forced_lambda must have n_iters entries")
         fptr = forced.ctypes.data_as(C.POINTER(C.c_double))
     cp = _CParams(p.beta, p.n_subsets, p.n_iters, p.mu0, p.lambda0, p.lambda_up, p.lambda_down, p.lambda_min,
-                  p.kappa, p.tv_eps, p.return_best, p.monitor_mode, fptr)
+                  p.kappa, p.tv_eps, p.return_best, p.monitor_mode, p.view_shift, 0, p.tv_z, fptr)
     return cp, forced
 
 

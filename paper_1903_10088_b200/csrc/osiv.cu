@@ -43,6 +43,7 @@ struct osiv_handle {
     float* d_hblank = nullptr;
     size_t hi_elems = 0;        float* d_himg = nullptr;
     int64_t launches = 0;
+    int stack_mode = 0;                 // set while osiv_reconstruct runs a stack of slices (view_shift / tv_z)
     int force_ns1 = 0;                  // osiv_set_symmetry(h, 0): always take the general path
     int use_pdl = 1;                    // osiv_set_overlap(h, 0): plain stream order between K1 and K2
     // per-kernel event timing (osiv_set_profiling)
@@ -183,7 +184,7 @@ constexpr int BATCH_MIN_SLICES = 4;     // fewer slices than this run one after 
 // Launches with several slices serve pairs of slices per block (SB = 2: interleaved images, shared chord weights) when
 // K2's tiles per block leave room for at least one view share in its 448-thread blocks.
 int pick_sb(const osiv_handle* h, int VS, int batch) {
-    if (batch < BATCH_MIN_SLICES) return 1;
+    if (batch < BATCH_MIN_SLICES || h->stack_mode) return 1;      // a stack's slices differ in their views: no pairs
     const int ns = pick_ns(h, VS);
     const int tx = ns == 4 ? h->geom.nx / 4 : (h->geom.nx + BK_TX - 1) / BK_TX;
     const int ty = ns == 4 ? h->geom.ny / 4 : (h->geom.ny + BK_TY - 1) / BK_TY;
@@ -319,7 +320,7 @@ int osiv_default_params(osiv_params* p) {
     p->mu0 = 0.005;                                     // PAPER.md:140 (0.05 /cm)
     p->lambda0 = 0.01; p->lambda_up = 1e-4; p->lambda_down = 2e-4;
     p->lambda_min = 1e-4; p->kappa = 100.0; p->tv_eps = 1e-5;
-    p->return_best = 0; p->monitor_mode = 0; p->forced_lambda = nullptr;
+    p->return_best = 0; p->monitor_mode = 0; p->view_shift = 0; p->reserved = 0; p->tv_z = 0.0; p->forced_lambda = nullptr;
     return OSIV_OK;
 }
 
@@ -503,6 +504,7 @@ int osiv_forward(osiv_handle* h, const float* d_img, float* d_sino, int32_t batc
     DeviceGuard guard(h->device);
     if (!guard.ok) { cudaGetLastError(); return OSIV_ERR_CUDA; }
     cudaStream_t st = (cudaStream_t)cuda_stream;
+    h->stack_mode = 0;
     const int VS = subset_views(h, subset, n_subsets);
     const FwdPlan p = plan_forward(h, VS, batch);
     int rc = ensure_images(h, batch, p.sb, st);
@@ -524,6 +526,7 @@ int osiv_backward(osiv_handle* h, const float* d_sino, float* d_img, int32_t bat
     DeviceGuard guard(h->device);
     if (!guard.ok) { cudaGetLastError(); return OSIV_ERR_CUDA; }
     cudaStream_t st = (cudaStream_t)cuda_stream;
+    h->stack_mode = 0;
     const int VS = subset_views(h, subset, n_subsets), M = subset < 0 ? 1 : n_subsets;
     const BackPlan p = plan_back(h, VS, batch);
     int rc = ensure_res(h, VS, p.ns, batch, st);
@@ -560,6 +563,12 @@ int osiv_reconstruct(osiv_handle* h, const float* d_counts, const float* d_blank
     if (!d_blank && !(blank_scalar > 0.f)) return OSIV_ERR_INVALID_ARG;
     if (!(prm->tv_eps >= 0.0) || !std::isfinite(prm->beta) || !std::isfinite(prm->mu0) || !(prm->kappa > 0.0))
         return OSIV_ERR_INVALID_ARG;
+    const bool stack = prm->view_shift != 0 || prm->tv_z > 0.0;
+    if (prm->reserved != 0 || !(prm->tv_z >= 0.0) || !std::isfinite(prm->tv_z) ||
+        (stack && (prm->return_best || prm->forced_lambda)))
+        return OSIV_ERR_INVALID_ARG;
+    h->stack_mode = stack ? 1 : 0;
+    const int vshift = (int)(((long long)prm->view_shift % h->geom.n_views + h->geom.n_views) % h->geom.n_views);
     DeviceGuard guard(h->device);
     if (!guard.ok) { cudaGetLastError(); return OSIV_ERR_CUDA; }
     cudaStream_t st = (cudaStream_t)cuda_stream;
@@ -588,11 +597,11 @@ int osiv_reconstruct(osiv_handle* h, const float* d_counts, const float* d_blank
     h->launches += 2;
 
     FwdArgs f{};
-    f.g = h->dg; f.M = M; f.VS = VS; f.batch = batch; f.rpb = fp.rpb; f.segs = fp.segs;
+    f.g = h->dg; f.M = M; f.VS = VS; f.batch = batch; f.view_shift = vshift; f.rpb = fp.rpb; f.segs = fp.segs;
     f.counts = d_counts; f.blank = d_blank; f.blank_scalar = blank_scalar; f.inv_bref = h->d_inv_bref;
     f.res = h->d_res; f.Cp = Cp; f.dparts = h->d_dparts;
     BackArgs b{};
-    b.g = h->dg; b.res = h->d_res; b.Cp = Cp; b.M = M; b.VS = VS; b.batch = batch; b.best = best; b.tpb = bp.tpb; b.shares = bp.shares; b.ngx = bp.ngx;
+    b.g = h->dg; b.res = h->d_res; b.Cp = Cp; b.M = M; b.VS = VS; b.batch = batch; b.view_shift = vshift; b.tv_z = (float)prm->tv_z; b.best = best; b.tpb = bp.tpb; b.shares = bp.shares; b.ngx = bp.ngx;
     b.dparts = h->d_dparts; b.nparts = fp.nparts; b.not_finite = h->d_not_finite;
     b.ip.lambda0 = prm->lambda0; b.ip.up = prm->lambda_up; b.ip.down = prm->lambda_down; b.ip.lmin = prm->lambda_min;
     b.ip.forced = (prm->forced_lambda && N > 0) ? h->d_forced : nullptr;

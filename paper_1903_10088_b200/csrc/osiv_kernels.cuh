@@ -85,6 +85,7 @@ struct FwdArgs {
     const float* imgT;                     // padded transpose, slice stride g.imgT_elems
     int subset, M, VS;
     int batch;                             // slices in this launch (SB == 2: the last pair may be half empty)
+    int view_shift;                        // stack of slices (H1): slice s uses the table's view (v + view_shift*s) mod V
     int rpb, segs;                         // rays per block, line segments per ray (block = rpb * segs threads, rounded up to warps)
     float* sino;                           // MODE 0: [batch][VS][C]
     const float* counts;                   // MODE 1: [batch][V][C]
@@ -103,6 +104,8 @@ struct BackArgs {
     int Cp;
     int subset, M, VS;
     int batch;                             // slices in this launch (SB == 2: the last pair may be half empty)
+    int view_shift;                        // stack of slices (H1), as in FwdArgs
+    float tv_z;                            // stack of slices (H2): > 0 adds the z term of the 3-D TV (SB == 1 only)
     int tpb, shares, ngx;                  // tiles per block, view shares, 2x2 patch groups per row of groups
     float* out;                            // MODE 0: [batch][ny][nx]
     const float* img;                      // MODE 1: padded mu(n)
@@ -192,7 +195,9 @@ __global__ void __launch_bounds__(FWD_MAX_THREADS, 1) k_forward(const FwdArgs a)
     uint64_t acc2[NS];                                              // SB == 2: per pattern, the pair of slices
 #pragma unroll
     for (int k = 0; k < NS; ++k) { acc[k] = 0.f; acc2[k] = 0ull; }
-    const float4 ray = __ldg(&g.rays[(size_t)v * g.C + c]);
+    // H1: a slice of a stack sees the gantry view_shift views further on per slice; the counts keep the acquisition index
+    const int vt = a.view_shift ? (int)((v + (long long)a.view_shift * s0) % g.V) : v;
+    const float4 ray = __ldg(&g.rays[(size_t)vt * g.C + c]);
     const bool rowmaj = fabsf(ray.x) >= fabsf(ray.y);
     {
         const float kk = rowmaj ? ray.x : ray.y;          // coefficient of the in-line coordinate, |kk| >= 1 (Joseph: +-1)
@@ -317,7 +322,7 @@ __global__ void __launch_bounds__(FWD_MAX_THREADS, 1) k_forward(const FwdArgs a)
     const int ne = min(segs, NS);                             // epilogue threads per ray
     const bool epi = seg < ne && r < R;
     float y0 = 0.f, bl = a.blank_scalar, ib = 0.f, h = 0.f;
-    if (epi) h = __ldg(&g.hs[(size_t)v * g.C + c]);
+    if (epi) h = __ldg(&g.hs[(size_t)vt * g.C + c]);
     if (MODE == 1 && epi) {
         y0 = __ldg(&a.counts[((size_t)s0 * g.V + v + seg * Vq) * g.C + c]);
         if (a.blank) bl = __ldg(&a.blank[c]);
@@ -459,6 +464,45 @@ __device__ __forceinline__ void tv_grad_tile(const float (&m)[4][4], int x0, int
             const float dxv = (x + 1 < nx) ? m[r][c + 1] - cv : 0.f;
             const float dyv = (y + 1 < ny) ? m[r + 1][c] - cv : 0.f;
             sgrad -= (dxv + dyv) * it[r][c];
+            out[ty][tx] = sgrad;
+        }
+}
+
+// The same with the z term of the 3-D TV (reading H2): up / dn = the neighbourhood in slices s+1 / s-1, wz = tv_z.
+// Own cell: -(dx + dy + wz*Dz)/t with Dz = wz*(up - mu); cell below: +wz*Dz'/t' with Dz' = wz*(mu - dn).
+__device__ __forceinline__ void tv_grad_tile3(const float (&m)[4][4], const float (&up)[4][4], const float (&dn)[4][4],
+                                              bool has_up, bool has_dn, float wz, int x0, int y0, int nx, int ny,
+                                              float eps2, float (&out)[2][2]) {
+    float it[3][3];
+#pragma unroll
+    for (int r = 0; r < 3; ++r)
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            const int x = x0 - 1 + c, y = y0 - 1 + r;
+            const float dxv = (x + 1 < nx) ? m[r][c + 1] - m[r][c] : 0.f;
+            const float dyv = (y + 1 < ny) ? m[r + 1][c] - m[r][c] : 0.f;
+            const float dzv = has_up ? wz * (up[r][c] - m[r][c]) : 0.f;
+            it[r][c] = rsqrtf(eps2 + dxv * dxv + dyv * dyv + dzv * dzv);
+        }
+#pragma unroll
+    for (int ty = 0; ty < 2; ++ty)
+#pragma unroll
+        for (int tx = 0; tx < 2; ++tx) {
+            const int x = x0 + tx, y = y0 + ty, r = ty + 1, c = tx + 1;
+            const float cv = m[r][c];
+            float sgrad = 0.f;
+            if (x > 0) sgrad += (cv - m[r][c - 1]) * it[r][c - 1];
+            if (y > 0) sgrad += (cv - m[r - 1][c]) * it[r - 1][c];
+            if (has_dn) {
+                const float dxd = (x + 1 < nx) ? dn[r][c + 1] - dn[r][c] : 0.f;
+                const float dyd = (y + 1 < ny) ? dn[r + 1][c] - dn[r][c] : 0.f;
+                const float dzd = wz * (cv - dn[r][c]);
+                sgrad += wz * dzd * rsqrtf(eps2 + dxd * dxd + dyd * dyd + dzd * dzd);
+            }
+            const float dxv = (x + 1 < nx) ? m[r][c + 1] - cv : 0.f;
+            const float dyv = (y + 1 < ny) ? m[r + 1][c] - cv : 0.f;
+            const float dzv = has_up ? wz * (up[r][c] - cv) : 0.f;
+            sgrad -= (dxv + dyv + wz * dzv) * it[r][c];
             out[ty][tx] = sgrad;
         }
 }
@@ -618,7 +662,8 @@ __global__ void __launch_bounds__(SB == 1 ? BK_MAX_THREADS : BKB_MAX_THREADS, SB
             const bool on = active && jbr < VSb;
             const int jb = min(jbr, VSb - 1);
             const int jj = jb + quarter * VSb;
-            const int v = a.subset < 0 ? jj : a.subset + jj * a.M;
+            const int va = a.subset < 0 ? jj : a.subset + jj * a.M;
+            const int v = a.view_shift ? (int)((va + (long long)a.view_shift * s0) % g.V) : va;   // H1: the table's view
             const float2 cs = __ldg(&g.views[v]);
             // fan angle of the tile centre: tan(gamma*) = perp/along; along >= SAD - r_max > 0
             const float along = g.sad - fmaf(X, cs.x, Y * cs.y);
@@ -725,7 +770,17 @@ __global__ void __launch_bounds__(SB == 1 ? BK_MAX_THREADS : BKB_MAX_THREADS, SB
             if (SB == 1 && fin_active) load_nbhd(g, a.img + slice_base(g, g.img_elems, s), xk, yk, m[j]);
             si[j] = step_rule(a, s, lane, writer);
             step[j] = (float)(si[j].lambda * a.tau);
-            if (fin_active) tv_grad_tile(m[j], xk, yk, g.nx, g.ny, a.eps2, tv[j]);
+            if (fin_active) {
+                if (SB == 1 && a.tv_z > 0.f) {                  // stack of slices: the z term needs slices s-1 and s+1
+                    const bool has_up = s + 1 < a.batch, has_dn = s > 0;
+                    float up[4][4], dn[4][4];
+                    load_nbhd(g, a.img + slice_base(g, g.img_elems, has_up ? s + 1 : s), xk, yk, up);
+                    load_nbhd(g, a.img + slice_base(g, g.img_elems, has_dn ? s - 1 : s), xk, yk, dn);
+                    tv_grad_tile3(m[j], up, dn, has_up, has_dn, a.tv_z, xk, yk, g.nx, g.ny, a.eps2, tv[j]);
+                } else {
+                    tv_grad_tile(m[j], xk, yk, g.nx, g.ny, a.eps2, tv[j]);
+                }
+            }
         }
     }
     __syncthreads();

@@ -473,6 +473,30 @@ def test_pairs_of_slices_path_matches_oracle(osiv, cfg, M):
         assert rel(host(one)[0], host(got)[0].astype(np.float64)) < 2e-6
 
 
+@pytest.mark.parametrize("cfg,M,k,tvz", [(SYM, 2, 5, 0.8), (si.scan_config("1"), 3, 7, 1.0), (ODD, 4, -3, 0.5),
+                                         (SYM, 2, 0, 1.0), (SYM, 2, 5, 0.0)])
+def test_stack_of_slices_matches_oracle(osiv, cfg, M, k, tvz):
+    """SURVEY.md 8(f)-3 (readings H1-H3): the slices of a call as one volume -- the gantry advanced by k views per slice,
+    3-D TV coupling neighbouring slices, per-slice monitor and step -- against oracle.reconstruct_stack."""
+    og, gg = geoms(cfg)
+    S = 4
+    counts = np.stack([si.make_case(cfg, slice_index=s)[2] for s in range(S)])
+    kw = dict(beta=0.01, n_subsets=M, n_iters=30)
+    ref, tr_ref, status = oracle.reconstruct_stack(og, counts, cfg.i0, oracle.Params(**kw), view_shift=k, tv_z=tvz)
+    assert status == 0
+    with osiv.Handle(gg, max_batch=S) as h:
+        got, tr = h.reconstruct(dev(counts), cfg.i0, osiv.Params(view_shift=k, tv_z=tvz, **kw), trace=True)
+        for s in range(S):
+            assert np.array_equal(tr[s, :, 1], tr_ref[s, :, 1])
+            assert np.all(np.abs(tr[s, :, 0] - tr_ref[s, :, 0]) <= 1e-5 * tr_ref[s, :, 0])
+            assert rel(host(got)[s], ref[s]) < IMG_TOL
+        if tvz > 0:                                             # the coupling is really on: not the independent slices
+            free = h.reconstruct(dev(counts), cfg.i0, osiv.Params(view_shift=k, **kw))
+            assert rel(host(free)[1], ref[1]) > 1e-3
+        with pytest.raises(osiv.OsivError):                     # stacks offer neither return_best nor forced lambda
+            h.reconstruct(dev(counts), cfg.i0, osiv.Params(view_shift=k, tv_z=tvz, return_best=1, **kw))
+
+
 def test_dependent_launch_chain_gives_the_same_bits_as_stream_order(osiv):
     """K1/K2 chained by programmatic dependent launch (default) vs plain stream order: the overlap moves only
     constant-dependent prologues ahead of the wait, so images and traces must be identical bit for bit."""
