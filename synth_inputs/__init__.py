@@ -18,5 +18,5 @@ are not available; shapes follow BASELINE.json ``configs``, the attenuation scal
 """
 from .phantom import (  # noqa: F401
     CONFIGS, MU_WATER, ScanConfig, scan_config, dgamma, ray_geometry, draw_ellipses, ellipse_sinogram,
-    rasterize, make_counts, make_case, uniform_image, uniform_sinogram,
+    rasterize, make_counts, make_case, uniform_image, uniform_sinogram, insert_phantom,
 )

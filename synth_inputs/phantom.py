@@ -157,3 +157,25 @@ def uniform_sinogram(cfg: ScanConfig, n_views: int = None, seed: int = None) -> 
     rng = np.random.default_rng((cfg.seed + 1) if seed is None else seed)
     nv = cfg.n_views if n_views is None else n_views
     return rng.uniform(0.0, 1.0, size=(nv, cfg.n_channels)).astype(np.float32)
+
+
+def insert_phantom(cfg: ScanConfig, n_inserts: int = 11):
+    """Insert phantom for the parameter study (stands in for the Gammex phantom of PAPER.md:96, whose
+    scans and ROI definitions are not available): a water disk of radius 0.8 R_FOV with `n_inserts` circular rods of
+    radius 0.075 R_FOV on a ring of radius 0.5 R_FOV, contrasts from -30 % to +60 % of water in equal steps (the rod
+    nearest 0 % is given +2 %).  Returns (ellipses, rois): ellipses as in draw_ellipses (densities add), rois = list of
+    (x0, y0, radius, mu) in mm and /mm, plus the background ROI at the centre as the last entry."""
+    rfov = 0.5 * min(cfg.nx, cfg.ny) * cfg.pixel_mm
+    ell = [(0.0, 0.0, 0.8 * rfov, 0.8 * rfov, 0.0, MU_WATER)]
+    rois = []
+    rad = 0.075 * rfov
+    for i in range(n_inserts):
+        ang = 2.0 * np.pi * i / n_inserts
+        contrast = -0.30 + 0.90 * i / max(n_inserts - 1, 1)
+        if abs(contrast) < 0.02:
+            contrast = 0.02
+        x0, y0 = 0.5 * rfov * np.cos(ang), 0.5 * rfov * np.sin(ang)
+        ell.append((x0, y0, rad, rad, 0.0, MU_WATER * contrast))
+        rois.append((x0, y0, rad, MU_WATER * (1.0 + contrast)))
+    rois.append((0.0, 0.0, 2.0 * rad, MU_WATER))
+    return ell, rois
