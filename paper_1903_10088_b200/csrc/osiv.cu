@@ -265,8 +265,10 @@ cudaError_t launch_back(const BackPlan& p, int batch, const BackArgs& a, cudaStr
     attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     attr[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = attr; cfg.numAttrs = pdl ? 1 : 0;
-    if (p.sb == 2) return p.ns == 4 ? cudaLaunchKernelEx(&cfg, k_back<MODE, 4, 2>, a) : cudaLaunchKernelEx(&cfg, k_back<MODE, 1, 2>, a);
-    return p.ns == 4 ? cudaLaunchKernelEx(&cfg, k_back<MODE, 4, 1>, a) : cudaLaunchKernelEx(&cfg, k_back<MODE, 1, 1>, a);
+    if (p.sb == 2) return p.ns == 4 ? cudaLaunchKernelEx(&cfg, k_back<MODE, 4, 2, 0>, a) : cudaLaunchKernelEx(&cfg, k_back<MODE, 1, 2, 0>, a);
+    if (MODE == 1 && (a.view_shift != 0 || a.tv_z > 0.f))
+        return p.ns == 4 ? cudaLaunchKernelEx(&cfg, k_back<1, 4, 1, 1>, a) : cudaLaunchKernelEx(&cfg, k_back<1, 1, 1, 1>, a);
+    return p.ns == 4 ? cudaLaunchKernelEx(&cfg, k_back<MODE, 4, 1, 0>, a) : cudaLaunchKernelEx(&cfg, k_back<MODE, 1, 1, 0>, a);
 }
 
 int ensure_forward_ws(osiv_handle* h, const FwdPlan& p, int batch) {
@@ -394,10 +396,11 @@ int osiv_create(const osiv_geometry* geom, int32_t max_batch, int32_t device, os
         cudaMemcpy(h->d_views, views.data(), views.size() * sizeof(float2), cudaMemcpyHostToDevice) != cudaSuccess ||
         cudaDeviceGetAttribute(&h->num_sms, cudaDevAttrMultiProcessorCount, device) != cudaSuccess ||
         // K2's shared-memory reduction buffer: up to 1024 threads x 16 floats
-        cudaFuncSetAttribute(k_back<0, 4, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024) != cudaSuccess ||
-        cudaFuncSetAttribute(k_back<1, 4, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024) != cudaSuccess ||
-        cudaFuncSetAttribute(k_back<0, 4, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024) != cudaSuccess ||
-        cudaFuncSetAttribute(k_back<1, 4, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024) != cudaSuccess) {
+        cudaFuncSetAttribute(k_back<0, 4, 1, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024) != cudaSuccess ||
+        cudaFuncSetAttribute(k_back<1, 4, 1, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024) != cudaSuccess ||
+        cudaFuncSetAttribute(k_back<1, 4, 1, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024) != cudaSuccess ||
+        cudaFuncSetAttribute(k_back<0, 4, 2, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024) != cudaSuccess ||
+        cudaFuncSetAttribute(k_back<1, 4, 2, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024) != cudaSuccess) {
         cudaGetLastError();
         osiv_destroy(h);
         return OSIV_ERR_CUDA;

@@ -511,11 +511,11 @@ __device__ __forceinline__ void load_nbhd(const DevGeom& g, const float* img, in
 #pragma unroll
     for (int r = 0; r < 4; ++r) {
         const int y = min(max(y0 - 1 + r, -PADR), g.ny + PADR - 1);
-        const size_t row = (size_t)(y + PADR) * g.pitch + PAD;
+        const float* row = img + (size_t)(y + PADR) * g.pitch + PAD;       // one slice per image (DevGeom::sb == 1)
 #pragma unroll
         for (int c = 0; c < 4; ++c) {
             const int x = min(x0 - 1 + c, g.nx + PAD - 1);
-            m[r][c] = __ldg(img + (row + x) * g.sb);
+            m[r][c] = __ldg(row + x);
         }
     }
 }
@@ -594,11 +594,12 @@ __device__ __forceinline__ void back_fma(const float (&w)[4], const float4 sv, B
     for (int p = 0; p < 4; ++p) acc.s[p] = fmaf(w[p], sv.x, acc.s[p]);
 }
 // the residuals of candidate u of one view for the SB slices of the block (NS == 1: the scalar in .x)
+// (sp = the view's first candidate in each slice's residual rows, u = candidate)
 template <int NS, int SB>
-__device__ __forceinline__ void back_load(const float* const (&res)[SB], int off, float4 (&sv)[SB]) {
+__device__ __forceinline__ void back_load(const float* const (&sp)[SB], int u, float4 (&sv)[SB]) {
 #pragma unroll
     for (int j = 0; j < SB; ++j)
-        sv[j] = NS == 4 ? __ldg(reinterpret_cast<const float4*>(res[j]) + off) : make_float4(__ldg(res[j] + off), 0.f, 0.f, 0.f);
+        sv[j] = NS == 4 ? __ldg(reinterpret_cast<const float4*>(sp[j]) + u) : make_float4(__ldg(sp[j] + u), 0.f, 0.f, 0.f);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -615,7 +616,9 @@ __device__ __forceinline__ void back_load(const float* const (&res)[SB], int off
 // view's orbit).  The shares' sums meet in shared memory in a fixed order; thread (tile, k) then finishes rotation
 // k of the tile (TV gradient, update, stores).  The host sizes the grid to one block per SM (plan_back).
 // ------------------------------------------------------------------------------------------------
-template <int MODE, int NS, int SB>
+// STACK == 1 (SB == 1 only): the slices of the launch form a volume (readings H1-H3) -- per-slice view shift and the z
+// term of the 3-D TV; kept out of the default instantiation, whose registers are tight.
+template <int MODE, int NS, int SB, int STACK>
 __global__ void __launch_bounds__(SB == 1 ? BK_MAX_THREADS : BKB_MAX_THREADS, SB == 1 ? 1 : 2) k_back(const BackArgs a) {
     const DevGeom& g = a.g;
     const int t = threadIdx.x, lane = t & 31, s0 = blockIdx.z * SB;       // slices s0 .. s0 + SB - 1
@@ -643,6 +646,7 @@ __global__ void __launch_bounds__(SB == 1 ? BK_MAX_THREADS : BKB_MAX_THREADS, SB
     for (int j = 0; j < SB; ++j) acc[j].clear();
 
     const int VSb = a.VS / NS;
+    const int vshift = STACK ? (int)(((long long)a.view_shift * s0) % g.V) : 0;
     const int quarter = NS == 4 ? (q & 3) : 0;
     const int jfirst = NS == 4 ? (q >> 2) : q, jstep = NS == 4 ? (shares >> 2) : shares;
     const int ntrips = (VSb + jstep - 1) / jstep;         // the same for every thread: the candidate loop is warp-wide
@@ -651,7 +655,7 @@ __global__ void __launch_bounds__(SB == 1 ? BK_MAX_THREADS : BKB_MAX_THREADS, SB
         const float X = (xc0 + 0.5f * (BK_TX - 1)) * g.pixel, Y = (yc0 + 0.5f * (BK_TY - 1)) * g.pixel;
         const float* res[SB];                                    // same float count for both layouts; a slice past the
 #pragma unroll
-        for (int j = 0; j < SB; ++j) res[j] = a.res + (size_t)min(s0 + j, a.batch - 1) * a.VS * a.Cp;   // batch repeats the last
+        for (int j = 0; j < SB; ++j) res[j] = a.res + (size_t)(SB == 1 ? s0 : min(s0 + j, a.batch - 1)) * a.VS * a.Cp;   // batch repeats the last
 
         // Candidate interval of trip `it` (view jfirst + it * jstep of this thread's share): offsets of its first
         // candidate in the ray table and in the residual rows, and the warp's candidate count.  The warp runs
@@ -662,8 +666,8 @@ __global__ void __launch_bounds__(SB == 1 ? BK_MAX_THREADS : BKB_MAX_THREADS, SB
             const bool on = active && jbr < VSb;
             const int jb = min(jbr, VSb - 1);
             const int jj = jb + quarter * VSb;
-            const int va = a.subset < 0 ? jj : a.subset + jj * a.M;
-            const int v = a.view_shift ? (int)((va + (long long)a.view_shift * s0) % g.V) : va;   // H1: the table's view
+            int v = a.subset < 0 ? jj : a.subset + jj * a.M;
+            if (STACK) { v += vshift; if (v >= g.V) v -= g.V; }      // H1: the table's view
             const float2 cs = __ldg(&g.views[v]);
             // fan angle of the tile centre: tan(gamma*) = perp/along; along >= SAD - r_max > 0
             const float along = g.sad - fmaf(X, cs.x, Y * cs.y);
@@ -696,30 +700,67 @@ __global__ void __launch_bounds__(SB == 1 ? BK_MAX_THREADS : BKB_MAX_THREADS, SB
             for (int e = 0; e < CH; e += 2) {
                 const float4* rpA = g.rays + offR[e];
                 const float4* rpB = g.rays + offR[e + 1];
-                if (ncw[e + 1] == 0) {                     // odd trip out (warp-uniform): one stream
+                if constexpr (SB == 1) {                   // one slice: plain pointers (the register budget is tight)
+                    const float4* spA = reinterpret_cast<const float4*>(res[0]) + offS[e];      // NS == 4
+                    const float4* spB = reinterpret_cast<const float4*>(res[0]) + offS[e + 1];
+                    const float* tpA = res[0] + offS[e];                                        // NS == 1
+                    const float* tpB = res[0] + offS[e + 1];
+                    if (ncw[e + 1] == 0) {                 // odd trip out (warp-uniform): one stream
 #pragma unroll 2
-                    for (int u = 0; u < ncw[e]; ++u) {
-                        const float4 rA = __ldg(rpA + u);
-                        float4 sA[SB];
-                        back_load<NS, SB>(res, offS[e] + u, sA);
-                        float wA[4];
-                        back_weights(rA, xc0, yc0, wA);
-#pragma unroll
-                        for (int j = 0; j < SB; ++j) back_fma(wA, sA[j], acc[j]);
+                        for (int u = 0; u < ncw[e]; ++u) {
+                            const float4 rA = __ldg(rpA + u);
+                            const float4 sA = NS == 4 ? __ldg(spA + u) : make_float4(__ldg(tpA + u), 0.f, 0.f, 0.f);
+                            float wA[4];
+                            back_weights(rA, xc0, yc0, wA);
+                            back_fma(wA, sA, acc[0]);
+                        }
+                    } else {
+                        const int n = max(ncw[e], ncw[e + 1]);
+#pragma unroll 2
+                        for (int u = 0; u < n; ++u) {
+                            const float4 rA = __ldg(rpA + u), rB = __ldg(rpB + u);
+                            const float4 sA = NS == 4 ? __ldg(spA + u) : make_float4(__ldg(tpA + u), 0.f, 0.f, 0.f);
+                            const float4 sB = NS == 4 ? __ldg(spB + u) : make_float4(__ldg(tpB + u), 0.f, 0.f, 0.f);
+                            float wA[4], wB[4];
+                            back_weights(rA, xc0, yc0, wA);
+                            back_fma(wA, sA, acc[0]);
+                            back_weights(rB, xc0, yc0, wB);
+                            back_fma(wB, sB, acc[0]);
+                        }
                     }
                 } else {
-                    const int n = max(ncw[e], ncw[e + 1]);
-#pragma unroll 2
-                    for (int u = 0; u < n; ++u) {
-                        const float4 rA = __ldg(rpA + u), rB = __ldg(rpB + u);
-                        float4 sA[SB], sB[SB];
-                        back_load<NS, SB>(res, offS[e] + u, sA);
-                        back_load<NS, SB>(res, offS[e + 1] + u, sB);
-                        float wA[4], wB[4];
-                        back_weights(rA, xc0, yc0, wA);
-                        back_weights(rB, xc0, yc0, wB);
+                    const float* spA[SB];
+                    const float* spB[SB];
 #pragma unroll
-                        for (int j = 0; j < SB; ++j) { back_fma(wA, sA[j], acc[j]); back_fma(wB, sB[j], acc[j]); }
+                    for (int j = 0; j < SB; ++j) {
+                        spA[j] = res[j] + (size_t)offS[e] * NS;          // NS == 4: float4 entries
+                        spB[j] = res[j] + (size_t)offS[e + 1] * NS;
+                    }
+                    if (ncw[e + 1] == 0) {                 // odd trip out (warp-uniform): one stream
+#pragma unroll 2
+                        for (int u = 0; u < ncw[e]; ++u) {
+                            const float4 rA = __ldg(rpA + u);
+                            float4 sA[SB];
+                            back_load<NS, SB>(spA, u, sA);
+                            float wA[4];
+                            back_weights(rA, xc0, yc0, wA);
+#pragma unroll
+                            for (int j = 0; j < SB; ++j) back_fma(wA, sA[j], acc[j]);
+                        }
+                    } else {
+                        const int n = max(ncw[e], ncw[e + 1]);
+#pragma unroll 2
+                        for (int u = 0; u < n; ++u) {
+                            const float4 rA = __ldg(rpA + u), rB = __ldg(rpB + u);
+                            float4 sA[SB], sB[SB];
+                            back_load<NS, SB>(spA, u, sA);
+                            back_load<NS, SB>(spB, u, sB);
+                            float wA[4], wB[4];
+                            back_weights(rA, xc0, yc0, wA);
+                            back_weights(rB, xc0, yc0, wB);
+#pragma unroll
+                            for (int j = 0; j < SB; ++j) { back_fma(wA, sA[j], acc[j]); back_fma(wB, sB[j], acc[j]); }
+                        }
                     }
                 }
             }
@@ -732,125 +773,220 @@ __global__ void __launch_bounds__(SB == 1 ? BK_MAX_THREADS : BKB_MAX_THREADS, SB
             }
         }
     }
-    // rotation k of the tile = orbit component (quarter + k) % 4  <=>  component m feeds rotation (m - quarter) % 4
-    if (q < shares) {
-#pragma unroll
-        for (int j = 0; j < SB; ++j)
+    if constexpr (SB == 1) {                               // one slice per block: scalars (the register budget is tight)
+        const int s = s0;
+        // rotation k of the tile = orbit component (quarter + k) % 4  <=>  component m feeds rotation (m - quarter) % 4
+        if (q < shares) {
 #pragma unroll
             for (int m = 0; m < NS; ++m)
 #pragma unroll
-                for (int p = 0; p < 4; ++p)
-                    red[((j * shares + q) * (NS * 4) + ((m - quarter) & (NS - 1)) * 4 + p) * tpb + i] = acc[j].get(m, p);
-    }
-
-    // thread (tile i, k = q < NS) finishes rotation k of the base tile: origin (xk, yk) and, below, where base pixel
-    // (tx,ty) lands.  Everything that does not depend on the other shares' sums -- monitor, step rule, neighbourhood
-    // of mu(n), TV gradient -- is done before the barrier, so that its loads overlap the wait for the slowest warp.
-    const bool fin = q < NS;
-    const bool fin_active = fin && x0 < xlim && y0 < ylim;
-    const int k = q;
-    int xk = x0, yk = y0;
-    if (NS == 4) {
-        const int N = g.nx;
-        if (k == 1)      { xk = N - 2 - y0; yk = x0; }
-        else if (k == 2) { xk = N - 2 - x0; yk = N - 2 - y0; }
-        else if (k == 3) { xk = y0;         yk = N - 2 - x0; }
-    }
-    StepInfo si[SB];
-    float step[SB], m[SB][4][4], tv[SB][2][2];
-    if (MODE == 1 && t < 32 * ((NS * tpb + 31) / 32)) {           // whole warps: step_rule shuffles
-        const bool writer = blockIdx.x == 0 && t < 32;
-        if constexpr (SB == 2) {
-            if (fin_active) load_nbhd2(g, reinterpret_cast<const float2*>(a.img) + (size_t)blockIdx.z * g.img_elems, xk, yk, m[0], m[SB - 1]);
+                for (int p = 0; p < 4; ++p) red[(q * (NS * 4) + ((m - quarter) & (NS - 1)) * 4 + p) * tpb + i] = acc[0].get(m, p);
         }
+
+        // thread (tile i, k = q < NS) finishes rotation k of the base tile: origin (xk, yk) and, below, where base pixel
+        // (tx,ty) lands.  Everything that does not depend on the other shares' sums -- monitor, step rule, neighbourhood
+        // of mu(n), TV gradient -- is done before the barrier, so that its loads overlap the wait for the slowest warp.
+        const bool fin = q < NS;
+        const bool fin_active = fin && x0 < xlim && y0 < ylim;
+        const int k = q;
+        int xk = x0, yk = y0;
+        if (NS == 4) {
+            const int N = g.nx;
+            if (k == 1)      { xk = N - 2 - y0; yk = x0; }
+            else if (k == 2) { xk = N - 2 - x0; yk = N - 2 - y0; }
+            else if (k == 3) { xk = y0;         yk = N - 2 - x0; }
+        }
+        StepInfo si;
+        float step = 0.f;
+        float m[4][4], tv[2][2];
+        if (MODE == 1 && t < 32 * ((NS * tpb + 31) / 32)) {           // whole warps: step_rule shuffles
+            const bool writer = blockIdx.x == 0 && t < 32;
+            if (fin_active) load_nbhd(g, a.img + (size_t)s * g.img_elems, xk, yk, m);
+            si = step_rule(a, s, lane, writer);
+            step = (float)(si.lambda * a.tau);
+            if (fin_active) {
+                if (STACK && a.tv_z > 0.f) {                        // stack of slices: the z term needs slices s-1 and s+1
+                    const bool has_up = s + 1 < a.batch, has_dn = s > 0;
+                    float up[4][4], dn[4][4];
+                    load_nbhd(g, a.img + (size_t)(has_up ? s + 1 : s) * g.img_elems, xk, yk, up);
+                    load_nbhd(g, a.img + (size_t)(has_dn ? s - 1 : s) * g.img_elems, xk, yk, dn);
+                    tv_grad_tile3(m, up, dn, has_up, has_dn, a.tv_z, xk, yk, g.nx, g.ny, a.eps2, tv);
+                } else {
+                    tv_grad_tile(m, xk, yk, g.nx, g.ny, a.eps2, tv);
+                }
+            }
+        }
+        __syncthreads();
+        if (!fin_active) return;
+
+        {
+            // sums over the view shares, fixed order
+            float b[4];
+#pragma unroll
+            for (int p = 0; p < 4; ++p) {
+                float x = 0.f;
+                for (int qq = 0; qq < shares; ++qq) x += red[(qq * (NS * 4) + k * 4 + p) * tpb + i];
+                b[p] = x;
+            }
+            float o00 = b[0], o01 = b[1], o10 = b[2], o11 = b[3];
+            if (NS == 4) {
+                if (k == 1)      { o00 = b[2]; o01 = b[0]; o10 = b[3]; o11 = b[1]; }
+                else if (k == 2) { o00 = b[3]; o01 = b[2]; o10 = b[1]; o11 = b[0]; }
+                else if (k == 3) { o00 = b[1]; o01 = b[3]; o10 = b[0]; o11 = b[2]; }
+            }
+            const bool vx1 = xk + 1 < g.nx, vy1 = yk + 1 < g.ny;
+            if (MODE == 0) {
+                float* out = a.out + (size_t)s * g.nx * g.ny;
+                out[(size_t)yk * g.nx + xk] = o00;
+                if (vx1) out[(size_t)yk * g.nx + xk + 1] = o01;
+                if (vy1) out[(size_t)(yk + 1) * g.nx + xk] = o10;
+                if (vx1 && vy1) out[(size_t)(yk + 1) * g.nx + xk + 1] = o11;
+                return;
+            }
+
+            // ---- A5 TV gradient of mu(n), A6 update (Eq. 3) with mu > 0, A7 best copy ----
+            const float u00 = fmaxf(fmaf(step, o00 - a.beta_over_M * tv[0][0], m[1][1]), 0.f);
+            const float u01 = fmaxf(fmaf(step, o01 - a.beta_over_M * tv[0][1], m[1][2]), 0.f);
+            const float u10 = fmaxf(fmaf(step, o10 - a.beta_over_M * tv[1][0], m[2][1]), 0.f);
+            const float u11 = fmaxf(fmaf(step, o11 - a.beta_over_M * tv[1][1], m[2][2]), 0.f);
+
+            float* nimg = a.img_new + (size_t)s * g.img_elems;
+            float* nimgT = a.imgT_new + (size_t)s * g.imgT_elems;
+            nimg[pad_off(g, yk, xk)] = u00;
+            nimgT[padT_off(g, xk, yk)] = u00;
+            if (vx1) { nimg[pad_off(g, yk, xk + 1)] = u01; nimgT[padT_off(g, xk + 1, yk)] = u01; }
+            if (vy1) { nimg[pad_off(g, yk + 1, xk)] = u10; nimgT[padT_off(g, xk, yk + 1)] = u10; }
+            if (vx1 && vy1) { nimg[pad_off(g, yk + 1, xk + 1)] = u11; nimgT[padT_off(g, xk + 1, yk + 1)] = u11; }
+
+            if (a.best && si.improved) {
+                float* best = a.best + (size_t)s * g.nx * g.ny;
+                best[(size_t)yk * g.nx + xk] = m[1][1];
+                if (vx1) best[(size_t)yk * g.nx + xk + 1] = m[1][2];
+                if (vy1) best[(size_t)(yk + 1) * g.nx + xk] = m[2][1];
+                if (vx1 && vy1) best[(size_t)(yk + 1) * g.nx + xk + 1] = m[2][2];
+            }
+        }
+    } else {                                               // a pair of slices per block
+        // rotation k of the tile = orbit component (quarter + k) % 4  <=>  component m feeds rotation (m - quarter) % 4
+        if (q < shares) {
+#pragma unroll
+            for (int j = 0; j < SB; ++j)
+#pragma unroll
+                for (int m = 0; m < NS; ++m)
+#pragma unroll
+                    for (int p = 0; p < 4; ++p)
+                        red[((j * shares + q) * (NS * 4) + ((m - quarter) & (NS - 1)) * 4 + p) * tpb + i] = acc[j].get(m, p);
+        }
+
+        // thread (tile i, k = q < NS) finishes rotation k of the base tile: origin (xk, yk) and, below, where base pixel
+        // (tx,ty) lands.  Everything that does not depend on the other shares' sums -- monitor, step rule, neighbourhood
+        // of mu(n), TV gradient -- is done before the barrier, so that its loads overlap the wait for the slowest warp.
+        const bool fin = q < NS;
+        const bool fin_active = fin && x0 < xlim && y0 < ylim;
+        const int k = q;
+        int xk = x0, yk = y0;
+        if (NS == 4) {
+            const int N = g.nx;
+            if (k == 1)      { xk = N - 2 - y0; yk = x0; }
+            else if (k == 2) { xk = N - 2 - x0; yk = N - 2 - y0; }
+            else if (k == 3) { xk = y0;         yk = N - 2 - x0; }
+        }
+        StepInfo si[SB];
+        float step[SB], m[SB][4][4], tv[SB][2][2];
+        if (MODE == 1 && t < 32 * ((NS * tpb + 31) / 32)) {           // whole warps: step_rule shuffles
+            const bool writer = blockIdx.x == 0 && t < 32;
+            if constexpr (SB == 2) {
+                if (fin_active) load_nbhd2(g, reinterpret_cast<const float2*>(a.img) + (size_t)blockIdx.z * g.img_elems, xk, yk, m[0], m[SB - 1]);
+            }
+#pragma unroll
+            for (int j = 0; j < SB; ++j) {
+                const int s = s0 + j;
+                if (s >= a.batch) break;
+                if (SB == 1 && fin_active) load_nbhd(g, a.img + (size_t)s * g.img_elems, xk, yk, m[j]);
+                si[j] = step_rule(a, s, lane, writer);
+                step[j] = (float)(si[j].lambda * a.tau);
+                if (fin_active) {
+                    if (STACK && a.tv_z > 0.f) {                    // stack of slices: the z term needs slices s-1 and s+1
+                        const bool has_up = s + 1 < a.batch, has_dn = s > 0;
+                        float up[4][4], dn[4][4];
+                        load_nbhd(g, a.img + (size_t)(has_up ? s + 1 : s) * g.img_elems, xk, yk, up);
+                        load_nbhd(g, a.img + (size_t)(has_dn ? s - 1 : s) * g.img_elems, xk, yk, dn);
+                        tv_grad_tile3(m[j], up, dn, has_up, has_dn, a.tv_z, xk, yk, g.nx, g.ny, a.eps2, tv[j]);
+                    } else {
+                        tv_grad_tile(m[j], xk, yk, g.nx, g.ny, a.eps2, tv[j]);
+                    }
+                }
+            }
+        }
+        __syncthreads();
+        if (!fin_active) return;
+
+        float un[SB][4] = {};                                     // SB == 2: mu(n+1) of the tile in both slices (0 in an empty one)
 #pragma unroll
         for (int j = 0; j < SB; ++j) {
             const int s = s0 + j;
             if (s >= a.batch) break;
-            if (SB == 1 && fin_active) load_nbhd(g, a.img + slice_base(g, g.img_elems, s), xk, yk, m[j]);
-            si[j] = step_rule(a, s, lane, writer);
-            step[j] = (float)(si[j].lambda * a.tau);
-            if (fin_active) {
-                if (SB == 1 && a.tv_z > 0.f) {                  // stack of slices: the z term needs slices s-1 and s+1
-                    const bool has_up = s + 1 < a.batch, has_dn = s > 0;
-                    float up[4][4], dn[4][4];
-                    load_nbhd(g, a.img + slice_base(g, g.img_elems, has_up ? s + 1 : s), xk, yk, up);
-                    load_nbhd(g, a.img + slice_base(g, g.img_elems, has_dn ? s - 1 : s), xk, yk, dn);
-                    tv_grad_tile3(m[j], up, dn, has_up, has_dn, a.tv_z, xk, yk, g.nx, g.ny, a.eps2, tv[j]);
-                } else {
-                    tv_grad_tile(m[j], xk, yk, g.nx, g.ny, a.eps2, tv[j]);
-                }
+            // sums over the view shares, fixed order
+            float b[4];
+#pragma unroll
+            for (int p = 0; p < 4; ++p) {
+                float x = 0.f;
+                for (int qq = 0; qq < shares; ++qq) x += red[((j * shares + qq) * (NS * 4) + k * 4 + p) * tpb + i];
+                b[p] = x;
+            }
+            float o00 = b[0], o01 = b[1], o10 = b[2], o11 = b[3];
+            if (NS == 4) {
+                if (k == 1)      { o00 = b[2]; o01 = b[0]; o10 = b[3]; o11 = b[1]; }
+                else if (k == 2) { o00 = b[3]; o01 = b[2]; o10 = b[1]; o11 = b[0]; }
+                else if (k == 3) { o00 = b[1]; o01 = b[3]; o10 = b[0]; o11 = b[2]; }
+            }
+            const bool vx1 = xk + 1 < g.nx, vy1 = yk + 1 < g.ny;
+            if (MODE == 0) {
+                float* out = a.out + (size_t)s * g.nx * g.ny;
+                out[(size_t)yk * g.nx + xk] = o00;
+                if (vx1) out[(size_t)yk * g.nx + xk + 1] = o01;
+                if (vy1) out[(size_t)(yk + 1) * g.nx + xk] = o10;
+                if (vx1 && vy1) out[(size_t)(yk + 1) * g.nx + xk + 1] = o11;
+                continue;
+            }
+
+            // ---- A5 TV gradient of mu(n), A6 update (Eq. 3) with mu > 0, A7 best copy ----
+            const float u00 = fmaxf(fmaf(step[j], o00 - a.beta_over_M * tv[j][0][0], m[j][1][1]), 0.f);
+            const float u01 = fmaxf(fmaf(step[j], o01 - a.beta_over_M * tv[j][0][1], m[j][1][2]), 0.f);
+            const float u10 = fmaxf(fmaf(step[j], o10 - a.beta_over_M * tv[j][1][0], m[j][2][1]), 0.f);
+            const float u11 = fmaxf(fmaf(step[j], o11 - a.beta_over_M * tv[j][1][1], m[j][2][2]), 0.f);
+            if constexpr (SB == 2) {
+                un[j][0] = u00; un[j][1] = u01; un[j][2] = u10; un[j][3] = u11;      // stored below, both slices at once
+            } else {
+                float* nimg = a.img_new + (size_t)s * g.img_elems;
+                float* nimgT = a.imgT_new + (size_t)s * g.imgT_elems;
+                nimg[pad_off(g, yk, xk)] = u00;
+                nimgT[padT_off(g, xk, yk)] = u00;
+                if (vx1) { nimg[pad_off(g, yk, xk + 1)] = u01; nimgT[padT_off(g, xk + 1, yk)] = u01; }
+                if (vy1) { nimg[pad_off(g, yk + 1, xk)] = u10; nimgT[padT_off(g, xk, yk + 1)] = u10; }
+                if (vx1 && vy1) { nimg[pad_off(g, yk + 1, xk + 1)] = u11; nimgT[padT_off(g, xk + 1, yk + 1)] = u11; }
+            }
+
+            if (a.best && si[j].improved) {
+                float* best = a.best + (size_t)s * g.nx * g.ny;
+                best[(size_t)yk * g.nx + xk] = m[j][1][1];
+                if (vx1) best[(size_t)yk * g.nx + xk + 1] = m[j][1][2];
+                if (vy1) best[(size_t)(yk + 1) * g.nx + xk] = m[j][2][1];
+                if (vx1 && vy1) best[(size_t)(yk + 1) * g.nx + xk + 1] = m[j][2][2];
             }
         }
-    }
-    __syncthreads();
-    if (!fin_active) return;
-
-    float un[SB][4] = {};                                     // SB == 2: mu(n+1) of the tile in both slices (0 in an empty one)
-#pragma unroll
-    for (int j = 0; j < SB; ++j) {
-        const int s = s0 + j;
-        if (s >= a.batch) break;
-        // sums over the view shares, fixed order
-        float b[4];
-#pragma unroll
-        for (int p = 0; p < 4; ++p) {
-            float x = 0.f;
-            for (int qq = 0; qq < shares; ++qq) x += red[((j * shares + qq) * (NS * 4) + k * 4 + p) * tpb + i];
-            b[p] = x;
-        }
-        float o00 = b[0], o01 = b[1], o10 = b[2], o11 = b[3];
-        if (NS == 4) {
-            if (k == 1)      { o00 = b[2]; o01 = b[0]; o10 = b[3]; o11 = b[1]; }
-            else if (k == 2) { o00 = b[3]; o01 = b[2]; o10 = b[1]; o11 = b[0]; }
-            else if (k == 3) { o00 = b[1]; o01 = b[3]; o10 = b[0]; o11 = b[2]; }
-        }
-        const bool vx1 = xk + 1 < g.nx, vy1 = yk + 1 < g.ny;
-        if (MODE == 0) {
-            float* out = a.out + (size_t)s * g.nx * g.ny;
-            out[(size_t)yk * g.nx + xk] = o00;
-            if (vx1) out[(size_t)yk * g.nx + xk + 1] = o01;
-            if (vy1) out[(size_t)(yk + 1) * g.nx + xk] = o10;
-            if (vx1 && vy1) out[(size_t)(yk + 1) * g.nx + xk + 1] = o11;
-            continue;
-        }
-
-        // ---- A5 TV gradient of mu(n), A6 update (Eq. 3) with mu > 0, A7 best copy ----
-        const float u00 = fmaxf(fmaf(step[j], o00 - a.beta_over_M * tv[j][0][0], m[j][1][1]), 0.f);
-        const float u01 = fmaxf(fmaf(step[j], o01 - a.beta_over_M * tv[j][0][1], m[j][1][2]), 0.f);
-        const float u10 = fmaxf(fmaf(step[j], o10 - a.beta_over_M * tv[j][1][0], m[j][2][1]), 0.f);
-        const float u11 = fmaxf(fmaf(step[j], o11 - a.beta_over_M * tv[j][1][1], m[j][2][2]), 0.f);
-        if constexpr (SB == 2) {
-            un[j][0] = u00; un[j][1] = u01; un[j][2] = u10; un[j][3] = u11;      // stored below, both slices at once
-        } else {
-            float* nimg = a.img_new + slice_base(g, g.img_elems, s);
-            float* nimgT = a.imgT_new + slice_base(g, g.imgT_elems, s);
+        if constexpr (SB == 2 && MODE == 1) {
+            float2* nimg = reinterpret_cast<float2*>(a.img_new) + (size_t)blockIdx.z * g.img_elems;
+            float2* nimgT = reinterpret_cast<float2*>(a.imgT_new) + (size_t)blockIdx.z * g.imgT_elems;
+            const bool vx1 = xk + 1 < g.nx, vy1 = yk + 1 < g.ny;
+            const float2 u00 = make_float2(un[0][0], un[SB - 1][0]), u01 = make_float2(un[0][1], un[SB - 1][1]);
+            const float2 u10 = make_float2(un[0][2], un[SB - 1][2]), u11 = make_float2(un[0][3], un[SB - 1][3]);
             nimg[pad_off(g, yk, xk)] = u00;
             nimgT[padT_off(g, xk, yk)] = u00;
             if (vx1) { nimg[pad_off(g, yk, xk + 1)] = u01; nimgT[padT_off(g, xk + 1, yk)] = u01; }
             if (vy1) { nimg[pad_off(g, yk + 1, xk)] = u10; nimgT[padT_off(g, xk, yk + 1)] = u10; }
             if (vx1 && vy1) { nimg[pad_off(g, yk + 1, xk + 1)] = u11; nimgT[padT_off(g, xk + 1, yk + 1)] = u11; }
         }
-
-        if (a.best && si[j].improved) {
-            float* best = a.best + (size_t)s * g.nx * g.ny;
-            best[(size_t)yk * g.nx + xk] = m[j][1][1];
-            if (vx1) best[(size_t)yk * g.nx + xk + 1] = m[j][1][2];
-            if (vy1) best[(size_t)(yk + 1) * g.nx + xk] = m[j][2][1];
-            if (vx1 && vy1) best[(size_t)(yk + 1) * g.nx + xk + 1] = m[j][2][2];
-        }
-    }
-    if constexpr (SB == 2 && MODE == 1) {
-        float2* nimg = reinterpret_cast<float2*>(a.img_new) + (size_t)blockIdx.z * g.img_elems;
-        float2* nimgT = reinterpret_cast<float2*>(a.imgT_new) + (size_t)blockIdx.z * g.imgT_elems;
-        const bool vx1 = xk + 1 < g.nx, vy1 = yk + 1 < g.ny;
-        const float2 u00 = make_float2(un[0][0], un[SB - 1][0]), u01 = make_float2(un[0][1], un[SB - 1][1]);
-        const float2 u10 = make_float2(un[0][2], un[SB - 1][2]), u11 = make_float2(un[0][3], un[SB - 1][3]);
-        nimg[pad_off(g, yk, xk)] = u00;
-        nimgT[padT_off(g, xk, yk)] = u00;
-        if (vx1) { nimg[pad_off(g, yk, xk + 1)] = u01; nimgT[padT_off(g, xk + 1, yk)] = u01; }
-        if (vy1) { nimg[pad_off(g, yk + 1, xk)] = u10; nimgT[padT_off(g, xk, yk + 1)] = u10; }
-        if (vx1 && vy1) { nimg[pad_off(g, yk + 1, xk + 1)] = u11; nimgT[padT_off(g, xk + 1, yk + 1)] = u11; }
     }
 }
 
@@ -955,7 +1091,7 @@ __global__ void __launch_bounds__(128) k_tv(DevGeom g, const float* __restrict__
     const int s = blockIdx.z;
     if (x0 >= g.nx || y0 >= g.ny) return;
     float m[4][4], tv[2][2];
-    load_nbhd(g, img + slice_base(g, g.img_elems, s), x0, y0, m);
+    load_nbhd(g, img + (size_t)s * g.img_elems, x0, y0, m);
     tv_grad_tile(m, x0, y0, g.nx, g.ny, eps2, tv);
     out += (size_t)s * g.nx * g.ny;
     const bool vx1 = x0 + 1 < g.nx, vy1 = y0 + 1 < g.ny;
