@@ -570,6 +570,7 @@ int osiv_reconstruct(osiv_handle* h, const float* d_counts, const float* d_blank
     if (prm->reserved != 0 || !(prm->tv_z >= 0.0) || !std::isfinite(prm->tv_z) ||
         (stack && (prm->return_best || prm->forced_lambda)))
         return OSIV_ERR_INVALID_ARG;
+    if ((long long)h->geom.n_views * batch >= (1ll << 31)) return OSIV_ERR_INVALID_ARG;     // view_shift * slice stays in 32 bits
     h->stack_mode = stack ? 1 : 0;
     const int vshift = (int)(((long long)prm->view_shift % h->geom.n_views + h->geom.n_views) % h->geom.n_views);
     DeviceGuard guard(h->device);

@@ -196,16 +196,15 @@ __global__ void __launch_bounds__(FWD_MAX_THREADS, 1) k_forward(const FwdArgs a)
 #pragma unroll
     for (int k = 0; k < NS; ++k) { acc[k] = 0.f; acc2[k] = 0ull; }
     // H1: a slice of a stack sees the gantry view_shift views further on per slice; the counts keep the acquisition index
-    const int vt = a.view_shift ? (int)((v + (long long)a.view_shift * s0) % g.V) : v;
+    int vt = v;                                                     // (a real branch: the default path must not pay for the modulo)
+    if (a.view_shift) { vt = v + (int)(((unsigned)a.view_shift * (unsigned)s0) % (unsigned)g.V); if (vt >= g.V) vt -= g.V; }
     const float4 ray = __ldg(&g.rays[(size_t)vt * g.C + c]);
     const bool rowmaj = fabsf(ray.x) >= fabsf(ray.y);
     {
         const float kk = rowmaj ? ray.x : ray.y;          // coefficient of the in-line coordinate, |kk| >= 1 (Joseph: +-1)
         const float uu = rowmaj ? ray.y : ray.x;          // coefficient of the marching coordinate (+-1; Joseph: +-1/|k|)
-        const PX* im = reinterpret_cast<const PX*>(a.img) + (size_t)blockIdx.z * g.img_elems;
-        const PX* imT = reinterpret_cast<const PX*>(a.imgT) + (size_t)blockIdx.z * g.imgT_elems;
-        const PX* bufA = rowmaj ? im : imT;
-        const PX* bufB = rowmaj ? imT : im;
+        const PX* bufA = rowmaj ? reinterpret_cast<const PX*>(a.img) + (size_t)blockIdx.z * g.img_elems : reinterpret_cast<const PX*>(a.imgT) + (size_t)blockIdx.z * g.imgT_elems;
+        const PX* bufB = rowmaj ? reinterpret_cast<const PX*>(a.imgT) + (size_t)blockIdx.z * g.imgT_elems : reinterpret_cast<const PX*>(a.img) + (size_t)blockIdx.z * g.img_elems;
         const int pitch = rowmaj ? g.pitch : g.pitchT;    // NS == 4: square grid, both pitches are equal
         const int na = rowmaj ? g.nx : g.ny, nb = rowmaj ? g.ny : g.nx;
         const float ca = rowmaj ? g.cx : g.cy, cb = rowmaj ? g.cy : g.cx;
@@ -646,7 +645,7 @@ __global__ void __launch_bounds__(SB == 1 ? BK_MAX_THREADS : BKB_MAX_THREADS, SB
     for (int j = 0; j < SB; ++j) acc[j].clear();
 
     const int VSb = a.VS / NS;
-    const int vshift = STACK ? (int)(((long long)a.view_shift * s0) % g.V) : 0;
+    const int vshift = STACK ? (int)(((unsigned)a.view_shift * (unsigned)s0) % (unsigned)g.V) : 0;
     const int quarter = NS == 4 ? (q & 3) : 0;
     const int jfirst = NS == 4 ? (q >> 2) : q, jstep = NS == 4 ? (shares >> 2) : shares;
     const int ntrips = (VSb + jstep - 1) / jstep;         // the same for every thread: the candidate loop is warp-wide
