@@ -37,7 +37,7 @@ FP32_FLOP_PER_NNZ = 6          # q (FMA, 2) + half-width mi
 NNZ_PER_RAY_PER_N = 1.193      # measured non-zeros per ray / N when the fan spans the inscribed circle
 SM_COUNT, FP32_LANES_PER_SM = 148, 128
 # dram__bytes_read.sum + dram__bytes_write.sum per launch at config 3 from the committed full-set ncu capture
-# (profiles/r1e_ncu_config3.md; ncu flushes the caches before every replay, so this is the cold-cache figure)
+# (profiles/r1f_ncu_config3.md; ncu flushes the caches before every replay, so this is the cold-cache figure)
 NCU_DRAM_BYTES_PER_LAUNCH = {"3": {"k_forward<1>": 2434048, "k_back<1>": 1514752}}
 
 
