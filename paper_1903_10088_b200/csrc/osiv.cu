@@ -31,6 +31,8 @@ struct osiv_handle {
     long long res_key = -1;             // layout (V_S, orbit size, batch) whose zero columns d_res currently holds
     int res_pad = 4;                    // zero columns C..Cp-1 of every residual row (K2 reads past a tile's last candidate)
     size_t dpart_elems = 0;     double* d_dparts = nullptr;
+    int* d_itab[2] = {nullptr, nullptr};    // K2's candidate intervals [V][ntiles], built on first use; [0]: NS = 1, [1]: NS = 4
+    int itab_tiles[2] = {0, 0};
     SliceState* d_state = nullptr;      // [2][max_batch], ping-pong between iterations
     int* d_not_finite = nullptr;        // [max_batch]
     float* d_inv_bref = nullptr;
@@ -194,7 +196,7 @@ int pick_sb(const osiv_handle* h, int VS, int batch) {
 }
 
 struct FwdPlan { int threads, rpb, segs, nparts, ns, sb; size_t smem; };
-struct BackPlan { int nblk, threads, tpb, shares, ngx, ns, sb; size_t smem; };
+struct BackPlan { int nblk, threads, tpb, shares, ngx, ns, sb, ntiles; size_t smem; };
 
 // K1: the subset's base rays are dealt out in runs of rpb consecutive rays, one run per block and one block per SM
 // (per slice); a block is rpb rays x segs segments of each ray's line range, as many segments as fit into 1024
@@ -239,6 +241,7 @@ BackPlan plan_back(const osiv_handle* h, int VS, int batch) {
     p.ngx = ((tx + BK_WX - 1) / BK_WX + 1) / 2;
     const int ngy = ((ty + BK_WY - 1) / BK_WY + 1) / 2;
     const long long tiles = (long long)p.ngx * ngy * 4 * 32;
+    p.ntiles = (int)tiles;
     p.tpb = (int)std::min<long long>(BK_MAX_THREADS / p.ns, std::max<long long>(1, (tiles + h->num_sms - 1) / h->num_sms));
     p.nblk = (int)((tiles + p.tpb - 1) / p.tpb);
     const int VSb = VS / p.ns;
@@ -269,6 +272,19 @@ cudaError_t launch_back(const BackPlan& p, int batch, const BackArgs& a, cudaStr
     if (MODE == 1 && (a.view_shift != 0 || a.tv_z > 0.f))
         return p.ns == 4 ? cudaLaunchKernelEx(&cfg, k_back<1, 4, 1, 1>, a) : cudaLaunchKernelEx(&cfg, k_back<1, 1, 1, 1>, a);
     return p.ns == 4 ? cudaLaunchKernelEx(&cfg, k_back<MODE, 4, 1, 0>, a) : cudaLaunchKernelEx(&cfg, k_back<MODE, 1, 1, 0>, a);
+}
+
+// K2's candidate intervals for this orbit size: one pass of k_build_intervals over all views, on first use
+int ensure_intervals(osiv_handle* h, const BackPlan& p, cudaStream_t st) {
+    const int w = p.ns == 4 ? 1 : 0;
+    if (h->d_itab[w] && h->itab_tiles[w] == p.ntiles) return OSIV_OK;
+    if (h->d_itab[w]) { OSIV_CUDA(cudaFree(h->d_itab[w])); h->d_itab[w] = nullptr; }
+    OSIV_CUDA(cudaMalloc((void**)&h->d_itab[w], (size_t)h->geom.n_views * p.ntiles * sizeof(int)));
+    k_build_intervals<<<dim3((p.ntiles + 255) / 256, h->geom.n_views), 256, 0, st>>>(h->dg, p.ns, p.ngx, p.ntiles, h->d_itab[w]);
+    h->itab_tiles[w] = p.ntiles;
+    h->launches += 1;
+    OSIV_CUDA(cudaGetLastError());
+    return OSIV_OK;
 }
 
 int ensure_forward_ws(osiv_handle* h, const FwdPlan& p, int batch) {
@@ -435,7 +451,7 @@ int osiv_destroy(osiv_handle* h) {
         cudaDeviceSynchronize();
         void* ptrs[] = {h->d_rays, h->d_views, h->d_hs, h->d_imgA, h->d_imgB, h->d_imgTA, h->d_imgTB, h->d_best, h->d_res,
                         h->d_dparts, h->d_state, h->d_not_finite, h->d_inv_bref, h->d_trace,
-                        h->d_forced, h->d_dhist, h->d_hcounts, h->d_hblank, h->d_himg};
+                        h->d_forced, h->d_dhist, h->d_itab[0], h->d_itab[1], h->d_hcounts, h->d_hblank, h->d_himg};
         for (void* p : ptrs) if (p) cudaFree(p);
         for (cudaEvent_t e : h->events) cudaEventDestroy(e);
         cudaGetLastError();
@@ -539,6 +555,8 @@ int osiv_backward(osiv_handle* h, const float* d_sino, float* d_img, int32_t bat
                                                                                     p.ns, Cp);
     BackArgs b{};
     b.g = h->dg; b.res = h->d_res; b.Cp = Cp; b.subset = subset; b.M = M; b.VS = VS; b.batch = batch; b.out = d_img; b.tpb = p.tpb; b.shares = p.shares; b.ngx = p.ngx;
+    if ((rc = ensure_intervals(h, p, st)) != OSIV_OK) return rc;
+    b.itab = h->d_itab[p.ns == 4]; b.ntiles = p.ntiles;
     launch_back<0>(p, batch, b, st, false);
     return launch_check(h, 2);
 }
@@ -606,6 +624,8 @@ int osiv_reconstruct(osiv_handle* h, const float* d_counts, const float* d_blank
     f.res = h->d_res; f.Cp = Cp; f.dparts = h->d_dparts;
     BackArgs b{};
     b.g = h->dg; b.res = h->d_res; b.Cp = Cp; b.M = M; b.VS = VS; b.batch = batch; b.view_shift = vshift; b.tv_z = (float)prm->tv_z; b.best = best; b.tpb = bp.tpb; b.shares = bp.shares; b.ngx = bp.ngx;
+    if ((rc = ensure_intervals(h, bp, st)) != OSIV_OK) return rc;
+    b.itab = h->d_itab[bp.ns == 4]; b.ntiles = bp.ntiles;
     b.dparts = h->d_dparts; b.nparts = fp.nparts; b.not_finite = h->d_not_finite;
     b.ip.lambda0 = prm->lambda0; b.ip.up = prm->lambda_up; b.ip.down = prm->lambda_down; b.ip.lmin = prm->lambda_min;
     b.ip.forced = (prm->forced_lambda && N > 0) ? h->d_forced : nullptr;

@@ -107,6 +107,8 @@ struct BackArgs {
     int view_shift;                        // stack of slices (H1), as in FwdArgs
     float tv_z;                            // stack of slices (H2): > 0 adds the z term of the 3-D TV (SB == 1 only)
     int tpb, shares, ngx;                  // tiles per block, view shares, 2x2 patch groups per row of groups
+    const int* itab;                       // [V][ntiles] candidate intervals (k_build_intervals)
+    int ntiles;
     float* out;                            // MODE 0: [batch][ny][nx]
     const float* img;                      // MODE 1: padded mu(n)
     float* img_new;                        // padded mu(n+1)
@@ -615,6 +617,46 @@ __device__ __forceinline__ void back_load(const float* const (&sp)[SB], int u, f
 // view's orbit).  The shares' sums meet in shared memory in a fixed order; thread (tile, k) then finishes rotation
 // k of the tile (TV gradient, update, stores).  The host sizes the grid to one block per SM (plan_back).
 // ------------------------------------------------------------------------------------------------
+// tile number -> patch (8 x 4 tiles; patches grouped 2 x 2, groups row-major) -> origin (x0, y0) of the 2x2-pixel tile
+__device__ __forceinline__ void tile_origin(int T, int ngx, int& x0, int& y0) {
+    const int patch = T >> 5, w = T & 31;
+    const int grp = patch >> 2, sub = patch & 3;
+    const int gy = grp / ngx, gx = grp - gy * ngx;
+    x0 = (((gx << 1) + (sub & 1)) * BK_WX + (w & (BK_WX - 1))) * BK_TX;
+    y0 = (((gy << 1) + (sub >> 1)) * BK_WY + (w / BK_WX)) * BK_TY;
+}
+
+// Candidate interval of the tile at (x0, y0) in table view v: the channels whose ray can cross the tile form the interval
+// |c - c*| <= hw around the channel coordinate c* of the tile centre (every such ray passes within tile_r of the centre,
+// so its fan angle differs from the centre's by at most asin(r/L) <= tile_hw/along channels).  Packed as
+// first channel | count << 20; an empty interval starts at C (the zero columns of the residuals).
+__device__ __forceinline__ int tile_interval(const DevGeom& g, int x0, int y0, int v) {
+    const float X = ((float)x0 - g.cx + 0.5f * (BK_TX - 1)) * g.pixel, Y = ((float)y0 - g.cy + 0.5f * (BK_TY - 1)) * g.pixel;
+    const float2 cs = __ldg(&g.views[v]);
+    // fan angle of the tile centre: tan(gamma*) = perp/along; along >= SAD - r_max > 0
+    const float along = g.sad - fmaf(X, cs.x, Y * cs.y);
+    const float perp = fmaf(X, cs.y, -Y * cs.x);
+    const float rinv = __fdividef(1.f, along);
+    const float z = perp * rinv;
+    const float gam = g.use_atanf ? atanf(z) : atan_small(z);
+    const float cstar = fmaf(gam, g.inv_dgamma, g.c_center);
+    const float hw = fmaf(g.tile_hw, rinv, 0.05f);
+    const int c_lo = min(max(0, (int)ceilf(cstar - hw)), g.C);
+    const int c_hi = min(g.C - 1, (int)floorf(cstar + hw));
+    return c_lo | (max(c_hi - c_lo + 1, 0) << 20);
+}
+
+// A0 for K2: the intervals of every (view, tile) once per handle and orbit size -- they depend on the geometry only, and
+// worked out inside K2 they were a sixth of its instructions and most of its start-up path.  tab [V][ntiles].
+__global__ void __launch_bounds__(256) k_build_intervals(DevGeom g, int ns, int ngx, int ntiles, int* __restrict__ tab) {
+    const int T = blockIdx.x * 256 + threadIdx.x, v = blockIdx.y;
+    if (T >= ntiles) return;
+    int x0, y0;
+    tile_origin(T, ngx, x0, y0);
+    const int xlim = ns == 4 ? (g.nx >> 1) : g.nx, ylim = ns == 4 ? (g.ny >> 1) : g.ny;
+    tab[(size_t)v * ntiles + T] = (x0 < xlim && y0 < ylim) ? tile_interval(g, x0, y0, v) : g.C;
+}
+
 // STACK == 1 (SB == 1 only): the slices of the launch form a volume (readings H1-H3) -- per-slice view shift and the z
 // term of the 3-D TV; kept out of the default instantiation, whose registers are tight.
 template <int MODE, int NS, int SB, int STACK>
@@ -625,17 +667,10 @@ __global__ void __launch_bounds__(SB == 1 ? BK_MAX_THREADS : BKB_MAX_THREADS, SB
     const int q = t / tpb, i = t - q * tpb;
     extern __shared__ float red[];                        // [SB][shares][NS * 4][tpb]
 
-    // tile number -> patch (2 x 2 patch groups, row-major) -> 2x2-pixel tile origin (x0, y0)
-    auto tile_origin = [&](int T, int& x0, int& y0) {
-        const int patch = T >> 5, w = T & 31;
-        const int grp = patch >> 2, sub = patch & 3;
-        const int gy = grp / a.ngx, gx = grp - gy * a.ngx;
-        x0 = (((gx << 1) + (sub & 1)) * BK_WX + (w & (BK_WX - 1))) * BK_TX;
-        y0 = (((gy << 1) + (sub >> 1)) * BK_WY + (w / BK_WX)) * BK_TY;
-    };
     const int xlim = NS == 4 ? (g.nx >> 1) : g.nx, ylim = NS == 4 ? (g.ny >> 1) : g.ny;
     int x0, y0;
-    tile_origin(blockIdx.x * tpb + i, x0, y0);
+    const int T = blockIdx.x * tpb + i;
+    tile_origin(T, a.ngx, x0, y0);
     const bool active = q < shares && x0 < xlim && y0 < ylim;
 
     // acc[m][ty*2+tx]: NS == 4: m = component of the orbit's residual float4 (this thread's views all lie in quarter
@@ -651,7 +686,6 @@ __global__ void __launch_bounds__(SB == 1 ? BK_MAX_THREADS : BKB_MAX_THREADS, SB
     const int ntrips = (VSb + jstep - 1) / jstep;         // the same for every thread: the candidate loop is warp-wide
     {
         const float xc0 = (float)x0 - g.cx, yc0 = (float)y0 - g.cy;
-        const float X = (xc0 + 0.5f * (BK_TX - 1)) * g.pixel, Y = (yc0 + 0.5f * (BK_TY - 1)) * g.pixel;
         const float* res[SB];                                    // same float count for both layouts; a slice past the
 #pragma unroll
         for (int j = 0; j < SB; ++j) res[j] = a.res + (size_t)(SB == 1 ? s0 : min(s0 + j, a.batch - 1)) * a.VS * a.Cp;   // batch repeats the last
@@ -667,20 +701,11 @@ __global__ void __launch_bounds__(SB == 1 ? BK_MAX_THREADS : BKB_MAX_THREADS, SB
             const int jj = jb + quarter * VSb;
             int v = a.subset < 0 ? jj : a.subset + jj * a.M;
             if (STACK) { v += vshift; if (v >= g.V) v -= g.V; }      // H1: the table's view
-            const float2 cs = __ldg(&g.views[v]);
-            // fan angle of the tile centre: tan(gamma*) = perp/along; along >= SAD - r_max > 0
-            const float along = g.sad - fmaf(X, cs.x, Y * cs.y);
-            const float perp = fmaf(X, cs.y, -Y * cs.x);
-            const float rinv = __fdividef(1.f, along);
-            const float z = perp * rinv;
-            const float gam = g.use_atanf ? atanf(z) : atan_small(z);
-            const float cstar = fmaf(gam, g.inv_dgamma, g.c_center);
-            const float hw = fmaf(g.tile_hw, rinv, 0.05f);
-            const int c_lo = on ? min(max(0, (int)ceilf(cstar - hw)), g.C) : g.C;
-            const int c_hi = min(g.C - 1, (int)floorf(cstar + hw));
+            const int packed = on ? __ldg(&a.itab[(size_t)v * a.ntiles + T]) : g.C;      // k_build_intervals
+            const int c_lo = packed & 0xfffff;
             offR = v * g.C + c_lo;
             offS = jb * a.Cp + c_lo;
-            return __reduce_max_sync(0xffffffffu, on ? c_hi - c_lo + 1 : 0);
+            return __reduce_max_sync(0xffffffffu, packed >> 20);
         };
         // Trips are taken four at a time: the four intervals are independent chains of arithmetic, and the first four
         // need nothing from K1, so they are worked out before the wait; the candidates of two trips are then walked
