@@ -37,8 +37,8 @@ FP32_FLOP_PER_NNZ = 6          # q (FMA, 2) + half-width mi
 NNZ_PER_RAY_PER_N = 1.193      # measured non-zeros per ray / N when the fan spans the inscribed circle
 SM_COUNT, FP32_LANES_PER_SM = 148, 128
 # dram__bytes_read.sum + dram__bytes_write.sum per launch at config 3 from the committed full-set ncu capture
-# (profiles/r1f_ncu_config3.md; ncu flushes the caches before every replay, so this is the cold-cache figure)
-NCU_DRAM_BYTES_PER_LAUNCH = {"3": {"k_forward<1>": 2434048, "k_back<1>": 1514752}}
+# (profiles/r1g_ncu_config3.md; ncu flushes the caches before every replay, so this is the cold-cache figure)
+NCU_DRAM_BYTES_PER_LAUNCH = {"3": {"k_forward<1>": 2431744, "k_back<1>": 4125184}}
 
 
 def load_peaks():
@@ -250,7 +250,8 @@ def run_ours(args, cfg, beta):
     dom = max(kernels, key=lambda k: kernels[k]["avg_us"])
     # compulsory HBM bytes per launch: everything is L2-resident, so this is a floor
     hbm_bytes = {"k_forward<1>": (cfg.nx * cfg.ny * 4 + 2 * vs * cfg.n_channels * 4 + vs * cfg.n_channels * 32) * batch,
-                 "k_back<1>": (cfg.nx * cfg.ny * 4 * 3 + vs * cfg.n_channels * 16) * batch}
+                 # + K2's candidate-interval table: one int per (view of the subset, 2x2 tile of the base quadrant)
+                 "k_back<1>": (cfg.nx * cfg.ny * 4 * 3 + vs * cfg.n_channels * 16) * batch + vs * (cfg.nx // 4) * (cfg.ny // 4) * 4}
     roof = {"bound": "alu", "kernel": dom, "achieved": kernels[dom]["achieved_tflops"], "peak": alu_peak_tflops,
             "unit": "TFLOP/s", "frac": kernels[dom]["frac"],
             "traffic": NCU_DRAM_BYTES_PER_LAUNCH.get(cfg.name, {}).get(dom),
