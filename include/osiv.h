@@ -137,8 +137,9 @@ int osiv_set_symmetry(osiv_handle* h, int32_t enable);
 int osiv_set_overlap(osiv_handle* h, int32_t enable);
 
 /* Launch plan osiv_reconstruct would use for `n_subsets` subsets (<= 0: all views) and `batch` slices:
- * out8 = {K1 orbit size (1 or 4), K1 blocks per ray group, K1 blocks, K1 threads per block,
- *         K2 orbit size, K2 warps per block, K2 blocks, K2 threads per block}.  Host only. */
+ * out8 = {K1 orbit size (1 or 4), K1 line segments per ray, K1 blocks, K1 threads per block,
+ *         K2 orbit size, K2 view shares per tile, K2 blocks, K2 threads per block}; both kernels run one block per SM
+ *         and slice (launches with >= 4 slices: per pair of slices, in half-size blocks).  Host only. */
 int osiv_get_plan(const osiv_handle* h, int32_t n_subsets, int32_t batch, int32_t* out8);
 
 /* Per-kernel device timing for the roofline report.  While enabled (enable != 0), osiv_reconstruct records a
