@@ -494,7 +494,7 @@ int osiv_get_plan(const osiv_handle* h, int32_t n_subsets, int32_t batch, int32_
     const int VS = n_subsets > 0 ? h->geom.n_views / n_subsets : h->geom.n_views;
     const FwdPlan f = plan_forward(h, VS, batch);
     const BackPlan b = plan_back(h, VS, batch);
-    out8[0] = f.ns; out8[1] = f.segs; out8[2] = f.nparts * batch; out8[3] = f.threads;
+    out8[0] = f.ns; out8[1] = f.segs; out8[2] = f.nparts * ((batch + f.sb - 1) / f.sb); out8[3] = f.threads;
     out8[4] = b.ns; out8[5] = b.shares; out8[6] = b.nblk * ((batch + b.sb - 1) / b.sb); out8[7] = b.threads;
     return OSIV_OK;
 }
