@@ -261,6 +261,10 @@ def run_ours(args, cfg, beta):
                       "an event between two launches serialises them, so these are stand-alone kernel durations "
                       "(in the timed region K1 and K2 overlap their prologues through programmatic dependent launch)",
             "kernels": kernels,
+            # in the timed region K1 and K2 are chained by dependent launches: the step's time over its hot launches
+            "chain": {"us_per_launch": 1e6 * t_dev / args.steps / (2 * cfg.n_iters),
+                      "achieved_tflops": nnz * FP32_FLOP_PER_NNZ / (t_dev / args.steps / (2 * cfg.n_iters)) / 1e12,
+                      "frac": nnz * FP32_FLOP_PER_NNZ / (t_dev / args.steps / (2 * cfg.n_iters)) / 1e12 / alu_peak_tflops},
             "hbm": {"compulsory_bytes_per_launch": hbm_bytes[dom],
                     "achieved_gbs": hbm_bytes[dom] / (kernels[dom]["avg_us"] * 1e-6) / 1e9,
                     "peak_gbs": float(peaks["hbm_gbs"]), "peak_kind": peak_kind,
