@@ -216,3 +216,103 @@ def test_P12_initial_image_matters_little_and_subsets_run():
     assert status == 0 and trace.shape == (200, 2)
     truth = si.rasterize(cfg, ell)
     assert np.linalg.norm(img - truth) / np.linalg.norm(truth) < 0.15
+
+
+# ---- pins of the update itself: thinning scale beta/M, subset order (C11), sign of the prior
+# (Eq. 2-3), positivity, zero counts in the monitor (G11).  None of these replays
+# the oracle's own trace: every expected value is composed here, in numpy, from the individually pinned pieces
+# (forward P2-P5, backward P4, residual P7, tv_grad P6, tau P8). ----
+
+def asymmetric_case():
+    # no symmetry of the phantom or the scan maps one subset onto another: every subset sees different data
+    cfg = si.ScanConfig("t", 20, 20, 1.0, 36, 30, i0=5e3, seed=31, n_ellipses=4, theta0_rad=0.13, channel_offset=0.25)
+    g = oracle.Geometry(nx=20, ny=20, pixel_mm=1.0, n_views=36, n_channels=30, theta0_rad=0.13, channel_offset=0.25)
+    _, _, counts = si.make_case(cfg)
+    return cfg, g, counts.astype(np.float64)
+
+
+def one_update(g, mu, counts, blank, m, M, lam, beta, eps, kappa=100.0):
+    """Eq. 3 on subset m with the regulariser weight multiplied by the thinning 1/M,
+    then mu >= 0; returns (mu_next, D, unclamped)."""
+    l = oracle.forward(g, mu, m, M)
+    r, D = oracle.residual(g, l, counts, blank, m, M)
+    grad = oracle.backward(g, r, m, M)
+    u = mu + lam * oracle.tau(g, M, kappa) * (grad - (beta / M) * oracle.tv_grad(mu, eps))
+    return np.maximum(u, 0.0), D, u
+
+
+@pytest.mark.parametrize("M", [3, 4])
+def test_update_replay_pins_thinning_scale_and_subset_order(M):
+    cfg, g, counts = asymmetric_case()
+    beta, eps = 0.5, 1e-4                 # strong prior: the beta/M term is far above rounding in every step
+    N = M + 2
+    # mu0 = 0 with a doubled first step: some pixels overshoot below zero in most steps, so the clamp is exercised
+    base = dict(beta=beta, n_subsets=M, mu0=0.0, lambda0=0.02, tv_eps=eps)
+    prm = oracle.Params(n_iters=N, **base)
+    runs = [oracle.reconstruct(g, counts, cfg.i0, oracle.Params(n_iters=n, **base)) for n in range(1, N + 1)]
+    trace = runs[-1][1]
+    mu = np.zeros((g.ny, g.nx))
+    lam, D_prev = prm.lambda0, None
+    clamp_bites = 0
+    for n in range(N):
+        m = n % M                                                      # C11: natural order
+        D = oracle.residual(g, oracle.forward(g, mu, m, M), counts, cfg.i0, m, M)[1]
+        if n > 0:                                                      # Eq. 4-5 from the D values composed here
+            lam = lam + prm.lambda_up if D < D_prev else max(lam - prm.lambda_down, prm.lambda_min)
+        D_prev = D
+        assert trace[n, 0] == pytest.approx(D, rel=1e-13)              # D(n) is the monitor of subset n mod M ...
+        assert trace[n, 1] == lam
+        for other in range(M):                                         # ... and of no other subset
+            if other != m:
+                Do = oracle.residual(g, oracle.forward(g, mu, other, M), counts, cfg.i0, other, M)[1]
+                assert abs(Do - D) > 1e-6 * D
+        nxt, _, u = one_update(g, mu, counts, cfg.i0, m, M, lam, beta, eps)
+        assert np.allclose(runs[n][0], nxt, rtol=0, atol=1e-15)
+        clamp_bites += int((u < 0).sum())
+        assert (u < 0).sum() < u.size // 2                             # the clamp acts on a part of the image only
+        if n > 0:
+            # the readings the paper excludes must be visibly different updates of this very step:
+            # un-thinned weight beta instead of beta/M, another subset's data, the prior with the other sign
+            for alt in (one_update(g, mu, counts, cfg.i0, m, M, lam, beta * M, eps)[0],
+                        one_update(g, mu, counts, cfg.i0, (m + 1) % M, M, lam, beta, eps)[0],
+                        one_update(g, mu, counts, cfg.i0, m, M, lam, -beta, eps)[0]):
+                assert np.abs(alt - nxt).max() > 1e-4 * np.abs(nxt).max()
+        mu = nxt
+    assert clamp_bites > 0, "the positivity clamp never acted: the case does not pin it"
+
+
+def test_zero_counts_only_touch_the_monitor():
+    # G11: p_i = ln(b_i / max(y_i, 1)).  A ray that counted nothing has the monitor term of a ray that counted one
+    # photon, stays finite, and enters the gradient with its true count 0.
+    cfg, g, counts = asymmetric_case()
+    mu = np.full((g.ny, g.nx), 0.004)
+    l = oracle.forward(g, mu, 1, 3)
+    ys = counts[1::3].copy()
+    zero = np.zeros_like(ys, dtype=bool)
+    zero[2, 5] = zero[7, 11] = zero[0, 0] = True
+    c0, c1 = counts.copy(), counts.copy()
+    c0[1::3][zero] = 0.0
+    c1[1::3][zero] = 1.0
+    r0, D0 = oracle.residual(g, l, c0, cfg.i0, 1, 3)
+    r1, D1 = oracle.residual(g, l, c1, cfg.i0, 1, 3)
+    assert np.isfinite(D0) and D0 == D1
+    assert np.allclose((r0 - r1)[zero], 1.0 / cfg.i0, rtol=1e-12) and np.array_equal(r0[~zero], r1[~zero])
+    # the term itself: (l - ln b)^2 for those rays
+    base = counts.copy()
+    base[1::3][zero] = 1.0
+    expect = ((l - np.log(cfg.i0 / np.maximum(base[1::3], 1.0))) ** 2).sum()
+    assert D0 == pytest.approx(float(expect), rel=1e-13)
+    # a whole reconstruction on data with dead rays stays finite
+    img, trace, status = oracle.reconstruct(g, c0, cfg.i0, oracle.Params(beta=0.01, n_subsets=3, n_iters=12))
+    assert status == 0 and np.all(np.isfinite(trace)) and np.all(np.isfinite(img))
+
+
+def test_prior_sign_more_beta_means_less_total_variation():
+    # Eq. 2-3 (PAPER.md:68,74): the prior enters the ascent as +alpha*R with R = -TV, so a larger weight must give an
+    # image of smaller total variation from the same data, at equal data iterations, and at beta = 0 the TV term is absent
+    cfg, g, counts = asymmetric_case()
+    tvs = []
+    for beta in (0.0, 0.05, 0.5):
+        img, _, _ = oracle.reconstruct(g, counts, cfg.i0, oracle.Params(beta=beta, n_subsets=3, n_iters=60, tv_eps=1e-4))
+        tvs.append(tv_plain(img, 1e-4))
+    assert tvs[0] > tvs[1] > tvs[2] and tvs[2] < 0.8 * tvs[0]
