@@ -37,8 +37,8 @@ extern "C" {
 
 typedef enum {
     OSIV_OK              =  0,
-    OSIV_ERR_INVALID_ARG = -1,  /* null pointer, non-positive size, n_views % n_subsets != 0,
-                                   batch > max_batch, source inside the grid's circumscribed circle */
+    OSIV_ERR_INVALID_ARG = -1,  /* null pointer, non-positive size, n_views % n_subsets != 0, n_views > 65535,
+                                   batch > max_batch, tv_eps <= 0, source inside the grid's circumscribed circle */
     OSIV_ERR_CUDA        = -2,  /* a CUDA runtime call failed (no device, out of memory, launch error) */
     OSIV_ERR_NOT_FINITE  = -3   /* the monitor D became NaN/Inf for at least one slice */
 } osiv_status;
@@ -112,43 +112,16 @@ int osiv_destroy(osiv_handle* h);
 
 /* A0 setup, host only (no GPU needed): the per-ray coefficients the kernels use.  Writes, for every ray
  * (v,c), four floats {alpha, beta, g0, h} to h_rays [V][C][4] and {cos th_v, sin th_v} to h_views [V][2]
- * (either may be NULL), such that the chord of reading C2 is
- *   a(v,c; ix,iy) = h * clamp( (|alpha|+|beta|)/2 - |alpha*(ix-(nx-1)/2) + beta*(iy-(ny-1)/2) + g0|, 0, 1 ).
- * Computed in float64, rounded once to float32. */
+ * (either may be NULL), such that the weight is
+ *   a(v,c; ix,iy) = h * clamp( w - |alpha*(ix-(nx-1)/2) + beta*(iy-(ny-1)/2) + g0|, 0, 1 ),
+ * with half-width w = (|alpha|+|beta|)/2 for the exact chord of reading C2 (model 0; one of alpha, beta is +-1, the
+ * other has magnitude >= 1) and w = 1 for Joseph's model (model 1; one of alpha, beta is +-1, the other has
+ * magnitude <= 1).  Computed in float64, rounded once to float32. */
 int osiv_ray_table(const osiv_geometry* geom, float* h_rays, float* h_views);
 
 /* Resolved channel pitch (after the dgamma_rad <= 0 rule) and step constant tau_S for M subsets. */
 int osiv_get_dgamma(const osiv_handle* h, double* dgamma_rad);
 int osiv_get_tau(const osiv_handle* h, int32_t n_subsets, double kappa, double* tau);
-
-/* Number of CUDA kernels this handle has launched since osiv_create (for launch accounting). */
-int64_t osiv_launch_count(const osiv_handle* h);
-
-/* Quarter-turn symmetry.  When the grid is square with nx % 4 == 0, n_views % 4 == 0 and a subset holds whole
- * orbits {v, v+V/4, v+V/2, v+3V/4} (V_S % 4 == 0), the kernels evaluate each chord weight once for the four
- * rotated (ray, pixel) pairs (DESIGN.md section 6).  It is on by default wherever it applies; enable = 0 forces
- * the general kernels (used by the tests to compare the two paths).  Results differ only by rounding. */
-int osiv_set_symmetry(osiv_handle* h, int32_t enable);
-
-/* Launch overlap inside osiv_reconstruct.  By default (enable = 1) K1 and K2 are chained with programmatic
- * dependent launches: the next kernel's blocks become resident and run their data-independent prologue while the
- * current kernel drains, and wait on the device for its completion before they read its output.  enable = 0 uses
- * plain stream order (same results bit for bit; used by the tests and for A/B timing). */
-int osiv_set_overlap(osiv_handle* h, int32_t enable);
-
-/* Launch plan osiv_reconstruct would use for `n_subsets` subsets (<= 0: all views) and `batch` slices:
- * out8 = {K1 orbit size (1 or 4), K1 line segments per ray, K1 blocks, K1 threads per block,
- *         K2 orbit size, K2 view shares per tile, K2 blocks, K2 threads per block}; both kernels run one block per SM
- *         and slice (launches with >= 4 slices: per pair of slices, in half-size blocks).  Host only. */
-int osiv_get_plan(const osiv_handle* h, int32_t n_subsets, int32_t batch, int32_t* out8);
-
-/* Per-kernel device timing for the roofline report.  While enabled (enable != 0), osiv_reconstruct records a
- * CUDA event on cuda_stream before and after every K1 (forward + residual + monitor partials) and K2
- * (step rule + backprojection + TV + update) launch and synchronises the stream at the end of the call to accumulate the
- * elapsed times; use it on extra steps, not on the steps whose throughput is reported.
- * osiv_get_profile returns the sums since the last osiv_set_profiling call: milliseconds and launch counts. */
-int osiv_set_profiling(osiv_handle* h, int32_t enable);
-int osiv_get_profile(const osiv_handle* h, double* ms_forward, int64_t* n_forward, double* ms_back, int64_t* n_back);
 
 /* Forward projection ("reprojection"):  l_i = sum_r a(i,r) mu_r  for the rays of
  * subset `subset` of `n_subsets` (subset < 0: all views; then n_subsets is ignored), where a(i,r) is
@@ -180,18 +153,56 @@ int osiv_tv_gradient(osiv_handle* h, const float* d_img, float* d_grad, int32_t 
  *   d_img_out   [batch][ny][nx] result
  *   h_trace     HOST pointer: NULL, or [batch][n_iters][2] doubles receiving (D(n), lambda(n)).
  * All work is enqueued on cuda_stream with no host round-trip inside the loop.  If h_trace is NULL the
- * call returns without synchronising; otherwise it synchronises the stream, fills h_trace and returns
- * OSIV_ERR_NOT_FINITE if any slice's monitor was not finite. */
+ * call returns without synchronising (a non-finite monitor then shows only in the image; use
+ * osiv_reconstruct_host or a trace to have it reported); otherwise it synchronises the stream, fills h_trace
+ * and returns OSIV_ERR_NOT_FINITE if any slice's monitor was not finite.  tv_eps must be > 0.  A failed kernel
+ * launch ends the call at that launch with OSIV_ERR_CUDA. */
 int osiv_reconstruct(osiv_handle* h, const float* d_counts, const float* d_blank, float blank_scalar,
                      const osiv_params* params, int32_t batch, float* d_img_out, double* h_trace,
                      void* cuda_stream);
 
 /* Same reconstruction with HOST buffers (the end-to-end call): copies h_counts (and h_blank) to the
  * device, runs osiv_reconstruct, copies the images back to h_img_out and synchronises the stream.
- * Pinned host memory makes the copies asynchronous but is not required. */
+ * Pinned host memory makes the copies asynchronous but is not required.  Returns OSIV_ERR_NOT_FINITE (image
+ * still delivered) if any slice's monitor was not finite, with or without h_trace. */
 int osiv_reconstruct_host(osiv_handle* h, const float* h_counts, const float* h_blank, float blank_scalar,
                           const osiv_params* params, int32_t batch, float* h_img_out, double* h_trace,
                           void* cuda_stream);
+
+/* =====================================================================================================
+ * DIAGNOSTICS -- not part of the method.  Launch accounting, A/B switches and per-kernel timing used by the
+ * tests and by bench.py's roofline report; a caller who only reconstructs needs none of them.
+ * ===================================================================================================== */
+
+/* Number of CUDA kernels this handle has launched since osiv_create (for launch accounting). */
+int64_t osiv_launch_count(const osiv_handle* h);
+
+/* Quarter-turn symmetry.  When the grid is square with nx % 4 == 0, n_views % 4 == 0 and a subset holds whole
+ * orbits {v, v+V/4, v+V/2, v+3V/4} (V_S % 4 == 0), the kernels evaluate each chord weight once for the four
+ * rotated (ray, pixel) pairs (DESIGN.md section 6).  It is on by default wherever it applies; enable = 0 forces
+ * the general kernels (used by the tests to compare the two paths).  Results differ only by rounding. */
+int osiv_set_symmetry(osiv_handle* h, int32_t enable);
+
+/* Launch overlap inside osiv_reconstruct.  By default (enable = 1) K1 and K2 are chained with programmatic
+ * dependent launches: the next kernel's blocks become resident and run their data-independent prologue while the
+ * current kernel drains, and wait on the device for its completion before they read its output.  enable = 0 uses
+ * plain stream order (same results bit for bit; used by the tests and for A/B timing). */
+int osiv_set_overlap(osiv_handle* h, int32_t enable);
+
+/* Launch plan osiv_reconstruct would use for `n_subsets` subsets (<= 0: all views) and `batch` slices:
+ * (independent slices: a stack with view_shift or tv_z never pairs slices)
+ * out8 = {K1 orbit size (1 or 4), K1 line segments per ray, K1 blocks, K1 threads per block,
+ *         K2 orbit size, K2 view shares per tile, K2 blocks, K2 threads per block}; both kernels run one block per SM
+ *         and slice (launches with >= 4 slices: per pair of slices, in half-size blocks).  Host only. */
+int osiv_get_plan(const osiv_handle* h, int32_t n_subsets, int32_t batch, int32_t* out8);
+
+/* Per-kernel device timing for the roofline report.  While enabled (enable != 0), osiv_reconstruct records a
+ * CUDA event on cuda_stream before and after every K1 (forward + residual + monitor partials) and K2
+ * (step rule + backprojection + TV + update) launch and synchronises the stream at the end of the call to accumulate the
+ * elapsed times; use it on extra steps, not on the steps whose throughput is reported.
+ * osiv_get_profile returns the sums since the last osiv_set_profiling call: milliseconds and launch counts. */
+int osiv_set_profiling(osiv_handle* h, int32_t enable);
+int osiv_get_profile(const osiv_handle* h, double* ms_forward, int64_t* n_forward, double* ms_back, int64_t* n_back);
 
 #ifdef __cplusplus
 }

@@ -45,7 +45,6 @@ struct osiv_handle {
     float* d_hblank = nullptr;
     size_t hi_elems = 0;        float* d_himg = nullptr;
     int64_t launches = 0;
-    int stack_mode = 0;                 // set while osiv_reconstruct runs a stack of slices (view_shift / tv_z)
     int force_ns1 = 0;                  // osiv_set_symmetry(h, 0): always take the general path
     int use_pdl = 1;                    // osiv_set_overlap(h, 0): plain stream order between K1 and K2
     // per-kernel event timing (osiv_set_profiling)
@@ -185,8 +184,8 @@ constexpr int BATCH_MIN_SLICES = 4;     // fewer slices than this run one after 
 
 // Launches with several slices serve pairs of slices per block (SB = 2: interleaved images, shared chord weights) when
 // K2's tiles per block leave room for at least one view share in its 448-thread blocks.
-int pick_sb(const osiv_handle* h, int VS, int batch) {
-    if (batch < BATCH_MIN_SLICES || h->stack_mode) return 1;      // a stack's slices differ in their views: no pairs
+int pick_sb(const osiv_handle* h, int VS, int batch, bool stack) {
+    if (batch < BATCH_MIN_SLICES || stack) return 1;      // a stack's slices differ in their views: no pairs
     const int ns = pick_ns(h, VS);
     const int tx = ns == 4 ? h->geom.nx / 4 : (h->geom.nx + BK_TX - 1) / BK_TX;
     const int ty = ns == 4 ? h->geom.ny / 4 : (h->geom.ny + BK_TY - 1) / BK_TY;
@@ -201,7 +200,7 @@ struct BackPlan { int nblk, threads, tpb, shares, ngx, ns, sb, ntiles; size_t sm
 // K1: the subset's base rays are dealt out in runs of rpb consecutive rays, one run per block and one block per SM
 // (per slice); a block is rpb rays x segs segments of each ray's line range, as many segments as fit into 1024
 // threads while a segment keeps at least FWD_MIN_LINES image lines.
-FwdPlan plan_forward(const osiv_handle* h, int VS, int batch) {
+FwdPlan plan_forward(const osiv_handle* h, int VS, int batch, bool stack = false) {
     FwdPlan p;
     p.ns = pick_ns(h, VS);
     const long long R = (long long)(VS / p.ns) * h->geom.n_channels;
@@ -209,7 +208,7 @@ FwdPlan plan_forward(const osiv_handle* h, int VS, int batch) {
     const int nmax = std::max(h->geom.nx, h->geom.ny);
     // several slices (A8): pairs of slices share the chord weights (SB = 2), in half-size blocks, two per SM, which
     // fill each other's stalls
-    p.sb = pick_sb(h, VS, batch);
+    p.sb = pick_sb(h, VS, batch, stack);
     const int tmax = std::max(p.rpb, p.sb == 2 ? BATCH_THREADS : FWD_MAX_THREADS);
     p.segs = std::max(1, std::min(tmax / p.rpb, nmax / FWD_MIN_LINES));
     p.threads = (p.rpb * p.segs + 31) / 32 * 32;
@@ -233,7 +232,7 @@ cudaError_t launch_forward(FwdPlan p, int batch, const FwdArgs& a, cudaStream_t 
 
 // K2: the base tiles, numbered patch by patch (8 x 4 tiles, patches grouped 2 x 2), are dealt out in runs of tpb
 // consecutive tiles, one run per block and one block per SM (per slice); a block is tpb tiles x `shares` view shares.
-BackPlan plan_back(const osiv_handle* h, int VS, int batch) {
+BackPlan plan_back(const osiv_handle* h, int VS, int batch, bool stack = false) {
     BackPlan p;
     p.ns = pick_ns(h, VS);
     const int tx = p.ns == 4 ? h->geom.nx / 4 : (h->geom.nx + BK_TX - 1) / BK_TX;
@@ -248,7 +247,7 @@ BackPlan plan_back(const osiv_handle* h, int VS, int batch) {
     // shares per quarter turn (NS == 4) or in all: as many as fit, then the fewest that keep the same number of
     // views per share
     // several slices: pairs of slices share the chord weights in blocks of at most 448 threads, two blocks per SM (A8)
-    p.sb = pick_sb(h, VS, batch);
+    p.sb = pick_sb(h, VS, batch, stack);
     const int tmax = std::max(p.tpb * p.ns, p.sb == 2 ? BKB_MAX_THREADS : BK_MAX_THREADS);
     int sq = std::max(1, std::min(tmax / (p.tpb * p.ns), VSb));
     const int trips = (VSb + sq - 1) / sq;
@@ -278,7 +277,9 @@ cudaError_t launch_back(const BackPlan& p, int batch, const BackArgs& a, cudaStr
 int ensure_intervals(osiv_handle* h, const BackPlan& p, cudaStream_t st) {
     const int w = p.ns == 4 ? 1 : 0;
     if (h->d_itab[w] && h->itab_tiles[w] == p.ntiles) return OSIV_OK;
-    if (h->d_itab[w]) { OSIV_CUDA(cudaFree(h->d_itab[w])); h->d_itab[w] = nullptr; }
+    // one table at a time: the other orbit size's table (osiv_set_symmetry toggled, or a subset without whole orbits) goes
+    for (int k = 0; k < 2; ++k)
+        if (h->d_itab[k]) { OSIV_CUDA(cudaFree(h->d_itab[k])); h->d_itab[k] = nullptr; h->itab_tiles[k] = 0; }
     OSIV_CUDA(cudaMalloc((void**)&h->d_itab[w], (size_t)h->geom.n_views * p.ntiles * sizeof(int)));
     k_build_intervals<<<dim3((p.ntiles + 255) / 256, h->geom.n_views), 256, 0, st>>>(h->dg, p.ns, p.ngx, p.ntiles, h->d_itab[w]);
     h->itab_tiles[w] = p.ntiles;
@@ -343,7 +344,9 @@ int osiv_default_params(osiv_params* p) {
 }
 
 static int check_geometry(const osiv_geometry& g) {
+    // n_views is a gridDim.y of the set-up kernels (k_build_intervals, k_scale_sino)
     if (g.nx <= 0 || g.ny <= 0 || g.n_views <= 0 || g.n_channels <= 0 || g.nx > 16384 || g.ny > 16384 ||
+        g.n_views > 65535 || g.n_channels >= (1 << 20) ||
         (g.model != 0 && g.model != 1) || g.reserved != 0)
         return OSIV_ERR_INVALID_ARG;
     if (!(g.pixel_mm > 0.0) || !(g.sad_mm > 0.0) || !std::isfinite(g.pixel_mm) || !std::isfinite(g.sad_mm) ||
@@ -523,7 +526,6 @@ int osiv_forward(osiv_handle* h, const float* d_img, float* d_sino, int32_t batc
     DeviceGuard guard(h->device);
     if (!guard.ok) { cudaGetLastError(); return OSIV_ERR_CUDA; }
     cudaStream_t st = (cudaStream_t)cuda_stream;
-    h->stack_mode = 0;
     const int VS = subset_views(h, subset, n_subsets);
     const FwdPlan p = plan_forward(h, VS, batch);
     int rc = ensure_images(h, batch, p.sb, st);
@@ -534,7 +536,7 @@ int osiv_forward(osiv_handle* h, const float* d_img, float* d_sino, int32_t batc
     FwdArgs a{};
     a.g = h->dg; a.img = h->d_imgA; a.imgT = h->d_imgTA;
     a.subset = subset; a.M = subset < 0 ? 1 : n_subsets; a.VS = VS; a.batch = batch; a.rpb = p.rpb; a.segs = p.segs; a.sino = d_sino;
-    launch_forward<0>(p, batch, a, st, false);
+    if (launch_forward<0>(p, batch, a, st, false) != cudaSuccess) { cudaGetLastError(); return OSIV_ERR_CUDA; }
     return launch_check(h, 2);
 }
 
@@ -545,7 +547,6 @@ int osiv_backward(osiv_handle* h, const float* d_sino, float* d_img, int32_t bat
     DeviceGuard guard(h->device);
     if (!guard.ok) { cudaGetLastError(); return OSIV_ERR_CUDA; }
     cudaStream_t st = (cudaStream_t)cuda_stream;
-    h->stack_mode = 0;
     const int VS = subset_views(h, subset, n_subsets), M = subset < 0 ? 1 : n_subsets;
     const BackPlan p = plan_back(h, VS, batch);
     int rc = ensure_res(h, VS, p.ns, batch, st);
@@ -557,13 +558,13 @@ int osiv_backward(osiv_handle* h, const float* d_sino, float* d_img, int32_t bat
     b.g = h->dg; b.res = h->d_res; b.Cp = Cp; b.subset = subset; b.M = M; b.VS = VS; b.batch = batch; b.out = d_img; b.tpb = p.tpb; b.shares = p.shares; b.ngx = p.ngx;
     if ((rc = ensure_intervals(h, p, st)) != OSIV_OK) return rc;
     b.itab = h->d_itab[p.ns == 4]; b.ntiles = p.ntiles;
-    launch_back<0>(p, batch, b, st, false);
+    if (launch_back<0>(p, batch, b, st, false) != cudaSuccess) { cudaGetLastError(); return OSIV_ERR_CUDA; }
     return launch_check(h, 2);
 }
 
 int osiv_tv_gradient(osiv_handle* h, const float* d_img, float* d_grad, int32_t batch, double tv_eps,
                      void* cuda_stream) {
-    if (!h || !d_img || !d_grad || batch <= 0 || batch > h->max_batch || !(tv_eps >= 0.0)) return OSIV_ERR_INVALID_ARG;
+    if (!h || !d_img || !d_grad || batch <= 0 || batch > h->max_batch || !(tv_eps > 0.0)) return OSIV_ERR_INVALID_ARG;
     DeviceGuard guard(h->device);
     if (!guard.ok) { cudaGetLastError(); return OSIV_ERR_CUDA; }
     cudaStream_t st = (cudaStream_t)cuda_stream;
@@ -582,24 +583,23 @@ int osiv_reconstruct(osiv_handle* h, const float* d_counts, const float* d_blank
     const int M = prm->n_subsets, N = prm->n_iters;
     if (M <= 0 || N < 0 || h->geom.n_views % M != 0 || (prm->monitor_mode != 0 && prm->monitor_mode != 1)) return OSIV_ERR_INVALID_ARG;
     if (!d_blank && !(blank_scalar > 0.f)) return OSIV_ERR_INVALID_ARG;
-    if (!(prm->tv_eps >= 0.0) || !std::isfinite(prm->beta) || !std::isfinite(prm->mu0) || !(prm->kappa > 0.0))
+    if (!(prm->tv_eps > 0.0) || !std::isfinite(prm->beta) || !std::isfinite(prm->mu0) || !(prm->kappa > 0.0))
         return OSIV_ERR_INVALID_ARG;
     const bool stack = prm->view_shift != 0 || prm->tv_z > 0.0;
     if (prm->reserved != 0 || !(prm->tv_z >= 0.0) || !std::isfinite(prm->tv_z) ||
         (stack && (prm->return_best || prm->forced_lambda)))
         return OSIV_ERR_INVALID_ARG;
     if ((long long)h->geom.n_views * batch >= (1ll << 31)) return OSIV_ERR_INVALID_ARG;     // view_shift * slice stays in 32 bits
-    h->stack_mode = stack ? 1 : 0;
     const int vshift = (int)(((long long)prm->view_shift % h->geom.n_views + h->geom.n_views) % h->geom.n_views);
     DeviceGuard guard(h->device);
     if (!guard.ok) { cudaGetLastError(); return OSIV_ERR_CUDA; }
     cudaStream_t st = (cudaStream_t)cuda_stream;
 
     const int VS = h->geom.n_views / M, C = h->geom.n_channels;
-    const FwdPlan fp = plan_forward(h, VS, batch);
+    const FwdPlan fp = plan_forward(h, VS, batch, stack);
     int rc = ensure_images(h, batch, fp.sb, st);
     if (rc != OSIV_OK) return rc;
-    const BackPlan bp = plan_back(h, VS, batch);
+    const BackPlan bp = plan_back(h, VS, batch, stack);
     if ((rc = ensure_res(h, VS, fp.ns, batch, st)) != OSIV_OK) return rc;
     const int Cp = C + h->res_pad;
     if ((rc = ensure_forward_ws(h, fp, batch)) != OSIV_OK) return rc;
@@ -648,17 +648,17 @@ int osiv_reconstruct(osiv_handle* h, const float* d_counts, const float* d_blank
     for (int n = 0; n < N; ++n) {
         const int m = n % M;                               // PAPER.md:118, C11
         f.img = cur; f.imgT = curT; f.subset = m;
-        launch_forward<1>(fp, batch, f, st, pdl);
+        if (launch_forward<1>(fp, batch, f, st, pdl) != cudaSuccess) { cudaGetLastError(); return OSIV_ERR_CUDA; }
         if (prof) cudaEventRecord(h->events[2 * n + 1], st);
         b.img = cur; b.img_new = nxt; b.imgT_new = nxtT; b.subset = m;
         b.state_in = state[n & 1]; b.state_out = state[(n + 1) & 1];
-        launch_back<1>(bp, batch, b, st, pdl);
+        if (launch_back<1>(bp, batch, b, st, pdl) != cudaSuccess) { cudaGetLastError(); return OSIV_ERR_CUDA; }
         if (prof) cudaEventRecord(h->events[2 * n + 2], st);
+        h->launches += 2;
         float* t;
         t = cur; cur = nxt; nxt = t;
         t = curT; curT = nxtT; nxtT = t;
     }
-    h->launches += 2 * (int64_t)N;
     if (prof) {
         OSIV_CUDA(cudaStreamSynchronize(st));
         for (int n = 0; n < N; ++n) {
@@ -673,7 +673,7 @@ int osiv_reconstruct(osiv_handle* h, const float* d_counts, const float* d_blank
     if (prm->return_best) {
         // the final iterate competes too, judged on the subset that would come next (C12)
         f.img = cur; f.imgT = curT; f.subset = N % M;
-        launch_forward<1>(fp, batch, f, st, false);
+        if (launch_forward<1>(fp, batch, f, st, false) != cudaSuccess) { cudaGetLastError(); return OSIV_ERR_CUDA; }
         k_final_monitor<<<batch, 32, 0, st>>>(h->d_dparts, fp.nparts, fin, h->d_not_finite);
         h->launches += 2;
     }
@@ -709,8 +709,12 @@ int osiv_reconstruct_host(osiv_handle* h, const float* h_counts, const float* h_
         OSIV_CUDA(cudaMemcpyAsync(h->d_hblank, h_blank, (size_t)h->geom.n_channels * sizeof(float), cudaMemcpyHostToDevice, st));
     rc = osiv_reconstruct(h, h->d_hcounts, h_blank ? h->d_hblank : nullptr, blank_scalar, prm, batch, h->d_himg, h_trace, st);
     if (rc != OSIV_OK && rc != OSIV_ERR_NOT_FINITE) return rc;
+    // this call synchronises anyway: the sticky non-finite flags come back with the image, trace or not
+    std::vector<int> nf(batch, 0);
     OSIV_CUDA(cudaMemcpyAsync(h_img_out, h->d_himg, ni * sizeof(float), cudaMemcpyDeviceToHost, st));
+    OSIV_CUDA(cudaMemcpyAsync(nf.data(), h->d_not_finite, (size_t)batch * sizeof(int), cudaMemcpyDeviceToHost, st));
     OSIV_CUDA(cudaStreamSynchronize(st));
+    for (int s = 0; s < batch; ++s) if (nf[s]) return OSIV_ERR_NOT_FINITE;
     return rc;
 }
 

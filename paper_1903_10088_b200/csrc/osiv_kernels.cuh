@@ -38,9 +38,6 @@ constexpr int PAD = 4;                     // zero columns left and right of eve
 constexpr int PADR = 1;                    // zero rows above and below a padded image
 constexpr int FWD_MAX_THREADS = 1024;      // K1: one block per SM, threads = rays per block x line segments per ray
 constexpr int FWD_MIN_LINES = 8;           // K1: a segment is at least this many image lines
-#ifndef OSIV_PDL_LATE
-#define OSIV_PDL_LATE 0                    // 1: release the next launch after the main loop instead of right after the wait
-#endif
 constexpr int BK_TX = 2, BK_TY = 2;        // pixels per thread in the backprojector
 constexpr int BK_WX = 8, BK_WY = 4;        // tiles per warp: a warp covers 16 x 8 pixels
 constexpr int BKB_MAX_THREADS = 448;       // K2 serving two slices per block (SB == 2): two such blocks per SM

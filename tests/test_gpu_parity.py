@@ -549,7 +549,121 @@ def test_reconstruct_config3_full(osiv):
 
 
 @pytest.mark.parametrize("beta", [0.001, 0.02])
-def test_reconstruct_config3_other_betas_short(osiv, beta):
+def test_reconstruct_config3_other_betas_full(osiv, beta):
+    """BASELINE.json configs[2]: "beta swept over {0.001, 0.005, 0.02}", each for the full 500 iterations (the oracle
+    needs well under a minute per run on the GPU box's host cores); lambda peaks near 0.025 and decays."""
     cfg = si.scan_config("3")
-    got, tr, ref, tr_ref, st = run_pair(osiv, cfg, dict(beta=beta, n_subsets=20, n_iters=60))
+    got, tr, ref, tr_ref, st = run_pair(osiv, cfg, dict(beta=beta, n_subsets=20, n_iters=500))
+    assert st == 0
     check_run(got, tr, ref, tr_ref)
+    assert 0.02 < tr[:, 1].max() < 0.03 and tr[-1, 1] < tr[:, 1].max()
+
+
+def test_pairs_of_slices_path_at_config4_size(osiv):
+    """A8 where the clock runs (BASELINE.json configs[3]: slices of 512x512, 800 x 738, 20 subsets): the launch plan of the
+    pair-of-slices path at this size (K1 two 512-thread blocks per SM, K2 view shares of 56 tiles) is another regime
+    than the toy sizes of test_pairs_of_slices_path_matches_oracle.  An odd batch (7: the last pair half empty) and an
+    even batch (6) for 60 iterations (three passes over the 20 subsets), slice by slice against the oracle with equal
+    lambda traces; projector pair of the batch as well."""
+    cfg = si.scan_config("4")
+    og, gg = geoms(cfg)
+    B, N, M = 7, 60, cfg.n_subsets
+    counts = np.stack([si.make_case(cfg, slice_index=s)[2] for s in range(B)])
+    kw = dict(beta=cfg.betas[0], n_subsets=M, n_iters=N)
+    refs = [oracle.reconstruct(og, counts[s], cfg.i0, oracle.Params(**kw)) for s in range(B)]
+    rng = np.random.default_rng(cfg.seed + 9)
+    with osiv.Handle(gg, max_batch=B) as h:
+        plan = h.plan(M, B)
+        assert plan["k1_orbit"] == 4 and plan["k2_threads"] <= 448      # the pair path, quarter-turn kernels
+        for batch in (B, B - 1):
+            got, tr = h.reconstruct(dev(counts[:batch]), cfg.i0, osiv.Params(**kw), trace=True)
+            for s in range(batch):
+                ref, tr_ref, st = refs[s]
+                assert st == 0
+                assert np.array_equal(tr[s, :, 1], tr_ref[:, 1]), (batch, s)
+                assert np.all(np.abs(tr[s, :, 0] - tr_ref[:, 0]) <= 1e-5 * tr_ref[:, 0])
+                assert rel(host(got)[s], ref) < IMG_TOL
+            if batch == B:
+                first = host(got)
+        # one slice alone agrees with the same slice inside the batch up to the rounding order of the sums
+        one, tr1 = h.reconstruct(dev(counts[2:3]), cfg.i0, osiv.Params(**kw), trace=True)
+        assert rel(host(one)[0], first[2].astype(np.float64)) < 2e-6 and np.array_equal(tr1[0, :, 1], refs[2][1][:, 1])
+        # the batch's projector pair on one subset
+        img = rng.uniform(0.0, 0.013, size=(B, cfg.ny, cfg.nx)).astype(np.float32)
+        sino = rng.uniform(0.0, 1.0, size=(B, cfg.n_views // M, cfg.n_channels)).astype(np.float32)
+        f, b = host(h.forward(dev(img), 3, M)), host(h.backward(dev(sino), 3, M))
+        for s in (0, 3, B - 1):
+            assert rel(f[s], oracle.forward(og, img[s], 3, M)) < PROJ_TOL
+            assert rel(b[s], oracle.backward(og, sino[s], 3, M)) < PROJ_TOL
+
+
+def test_projector_pair_max_size_config5b_all_views(osiv):
+    """1024x1024, 1600 x 1476, all views (BASELINE.json configs[4], the launch bench.py --workload 5b times): forward
+    and back in full against the oracle (about 2.9e9 weights per pass: some tens of seconds on the host cores)."""
+    cfg = si.scan_config("5b")
+    og, gg = geoms(cfg)
+    img, sino = si.uniform_image(cfg), si.uniform_sinogram(cfg)
+    with osiv.Handle(gg, max_batch=1) as h:
+        got = host(h.forward(dev(img)[None]))[0]
+        gotb = host(h.backward(dev(sino)[None]))[0]
+    assert rel(got, oracle.forward(og, img)) < PROJ_TOL
+    assert rel(gotb, oracle.backward(og, sino)) < PROJ_TOL
+    lhs = np.dot(got.astype(np.float64).ravel(), sino.astype(np.float64).ravel())
+    rhs = np.dot(img.astype(np.float64).ravel(), gotb.astype(np.float64).ravel())
+    assert abs(lhs - rhs) / abs(lhs) < 2e-6
+
+
+def test_stack_of_slices_at_256(osiv):
+    """8(f)-3 beyond toy sizes: config 2's geometry (256x256, 400 x 384, 10 subsets, quarter-turn kernels) as a stack of
+    5 slices with the gantry advanced 7 views per slice and the 3-D TV on, 30 iterations."""
+    cfg = si.scan_config("2")
+    og, gg = geoms(cfg)
+    S, k, tvz = 5, 7, 0.8
+    counts = np.stack([si.make_case(cfg, slice_index=s)[2] for s in range(S)])
+    kw = dict(beta=0.01, n_subsets=cfg.n_subsets, n_iters=30)
+    ref, tr_ref, status = oracle.reconstruct_stack(og, counts, cfg.i0, oracle.Params(**kw), view_shift=k, tv_z=tvz)
+    assert status == 0
+    with osiv.Handle(gg, max_batch=S) as h:
+        got, tr = h.reconstruct(dev(counts), cfg.i0, osiv.Params(view_shift=k, tv_z=tvz, **kw), trace=True)
+        free = h.reconstruct(dev(counts), cfg.i0, osiv.Params(view_shift=k, **kw))
+    for s in range(S):
+        assert np.array_equal(tr[s, :, 1], tr_ref[s, :, 1])
+        assert np.all(np.abs(tr[s, :, 0] - tr_ref[s, :, 0]) <= 1e-5 * tr_ref[s, :, 0])
+        assert rel(host(got)[s], ref[s]) < IMG_TOL
+    assert rel(host(free)[2], ref[2]) > 10 * rel(host(got)[2], ref[2])          # the coupling is really on
+
+
+def test_forced_lambda_ramp_up_to_the_oracles_stability_limit(osiv):
+    """G12: arithmetic parity under a forced step is defined while the iteration is stable.  Where that ends is taken from
+    the oracle, not assumed: under the steep ramp lambda(n) = 0.01 + 0.002 n the oracle's monitor falls until the step
+    crosses the stability limit and then grows; the CUDA path must agree with the oracle up to two iterations before that
+    turn (beyond it rounding noise is amplified on both sides and the trajectories separate)."""
+    cfg = si.scan_config("1")
+    og, gg = geoms(cfg)
+    counts = si.make_case(cfg)[2]
+    lam = 0.01 + 0.002 * np.arange(40)
+    kw = dict(beta=0.01, n_subsets=2)
+    _, tr_all, _ = oracle.reconstruct(og, counts, cfg.i0, oracle.Params(n_iters=40, forced_lambda=lam, **kw))
+    D = tr_all[:, 0]
+    per = D[0::2]                                            # subset 0's visits
+    turn = 2 * (int(np.argmax(np.diff(per) > 0)) + 1) if (np.diff(per) > 0).any() else 40
+    n_ok = max(turn - 2, 1)
+    assert 10 <= n_ok <= 40, turn                            # the ramp does reach the limit inside the window
+    ref, tr_ref, _ = oracle.reconstruct(og, counts, cfg.i0, oracle.Params(n_iters=n_ok, forced_lambda=lam[:n_ok].copy(), **kw))
+    with osiv.Handle(gg, max_batch=1) as h:
+        got, tr = h.reconstruct(dev(counts)[None], cfg.i0, osiv.Params(n_iters=n_ok, forced_lambda=lam[:n_ok].copy(), **kw), trace=True)
+    check_run(host(got)[0], tr[0], ref, tr_ref)
+
+
+def test_not_finite_is_reported_by_the_host_call_without_a_trace(osiv):
+    cfg = si.scan_config("1")
+    _, gg = geoms(cfg)
+    counts = si.make_case(cfg)[2][None].copy()
+    counts[0, 0, 0] = np.inf
+    with osiv.Handle(gg, max_batch=1) as h:
+        with pytest.raises(osiv.OsivError) as e:
+            h.reconstruct_host(counts, cfg.i0, osiv.Params(n_iters=2))
+        assert e.value.status == osiv.OSIV_ERR_NOT_FINITE
+        with pytest.raises(osiv.OsivError) as e:
+            h.reconstruct(dev(counts), cfg.i0, osiv.Params(n_iters=2, tv_eps=0.0))
+        assert e.value.status == osiv.OSIV_ERR_INVALID_ARG
