@@ -350,7 +350,12 @@ def main():
     ap.add_argument("--slices", type=int, default=0, help="slices per GPU (default 1; 64 for workload 4)")
     ap.add_argument("--beta", type=float, default=None)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--probe", action="store_true", help="print the measured FP32 / issue / L2 / shared-memory / L1 peaks and exit")
     args = ap.parse_args()
+    if args.probe:
+        import paper_1903_10088_b200 as osiv
+        print(json.dumps({"probe_peaks": osiv.probe_peaks(0), "how": "csrc/osiv_probes.cu: saturating loops, CUDA events, best of 5"}))
+        return 0
     cfg = si.scan_config(args.workload)
     beta = args.beta if args.beta is not None else (0.005 if args.workload == "3" else (cfg.betas[0] if cfg.betas else 0.0))
     if args.workload in ("5a", "5b"):

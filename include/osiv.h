@@ -204,6 +204,15 @@ int osiv_get_plan(const osiv_handle* h, int32_t n_subsets, int32_t batch, int32_
 int osiv_set_profiling(osiv_handle* h, int32_t enable);
 int osiv_get_profile(const osiv_handle* h, double* ms_forward, int64_t* n_forward, double* ms_back, int64_t* n_back);
 
+/* Micro-probes of the units that bound the two hot kernels (csrc/osiv_probes.cu): saturating loops
+ * of one instruction kind at full occupancy on `device`, CUDA-event timed, best of 5 (takes about 0.1 s).
+ * out8 = { FP32 TFLOP/s with FFMA (three register operands), FP32 TFLOP/s with FFMA2 (fma.rn.f32x2),
+ *          G warp-instructions/s issued (FMA-pipe and ALU-pipe instructions alternating),
+ *          GB/s read out of L2 (ld.global.cg over a 64 MiB buffer, every block streaming all of it),
+ *          GB/s shared-memory reads (conflict-free LDS.128), GB/s L1-hit reads with LDG.128, GB/s L1-hit reads with
+ *          LDG.32 (one 128-byte wavefront per warp instruction), number of SMs }.  Synchronises the device. */
+int osiv_probe_peaks(int32_t device, double* out8);
+
 #ifdef __cplusplus
 }
 #endif

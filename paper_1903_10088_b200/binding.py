@@ -18,7 +18,7 @@ OSIV_OK, OSIV_ERR_INVALID_ARG, OSIV_ERR_CUDA, OSIV_ERR_NOT_FINITE = 0, -1, -2, -
 EXPORTED_SYMBOLS = (
     "osiv_version", "osiv_strerror", "osiv_default_params", "osiv_create", "osiv_destroy", "osiv_ray_table", "osiv_get_dgamma",
     "osiv_get_tau", "osiv_launch_count", "osiv_set_symmetry", "osiv_set_overlap", "osiv_get_plan", "osiv_set_profiling", "osiv_get_profile", "osiv_forward", "osiv_backward", "osiv_tv_gradient", "osiv_reconstruct",
-    "osiv_reconstruct_host",
+    "osiv_reconstruct_host", "osiv_probe_peaks",
 )
 
 
@@ -116,12 +116,24 @@ def lib():
         L.osiv_tv_gradient.argtypes = [vp, vp, vp, ip, C.c_double, vp]
         L.osiv_reconstruct.argtypes = [vp, vp, vp, C.c_float, C.POINTER(_CParams), ip, vp, vp, vp]
         L.osiv_reconstruct_host.argtypes = [vp, vp, vp, C.c_float, C.POINTER(_CParams), ip, vp, vp, vp]
+        L.osiv_probe_peaks.argtypes = [ip, C.POINTER(C.c_double)]
         _lib = L
     return _lib
 
 
 def version() -> int:
     return lib().osiv_version()
+
+
+PROBE_FIELDS = ("ffma_tflops", "ffma2_tflops", "issue_ginst_per_s", "l2_read_gbs", "smem_read_gbs", "l1_read_gbs",
+                "l1_read_b32_gbs", "sms")
+
+
+def probe_peaks(device: int = 0) -> dict:
+    """osiv_probe_peaks: measured FP32 / issue / L2 / shared-memory / L1 peaks of `device` (diagnostics)."""
+    out = (C.c_double * 8)()
+    _check(lib().osiv_probe_peaks(int(device), out), "osiv_probe_peaks")
+    return dict(zip(PROBE_FIELDS, (float(v) for v in out)))
 
 
 def strerror(status: int) -> str:

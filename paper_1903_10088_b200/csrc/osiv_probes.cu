@@ -1,0 +1,215 @@
+// osiv_probes.cu -- micro-probes of the units that bound the OS-TV kernels ("run three micro-probes in
+// the same session: FP32 FMA issue rate, L2-resident read bandwidth, shared-memory read bandwidth"), plus the L1-hit
+// read bandwidth that K1's gathers live on.  DIAGNOSTICS: not part of the method; bench.py --probe and the bench line's
+// roofline fractions use them as measured denominators (MEASURED_PEAKS.json holds only the HBM copy and bf16 GEMM peaks).
+// Every probe is a saturating loop of one instruction kind at full occupancy, timed with CUDA events, best of 5.
+#include "../../include/osiv.h"
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace {
+
+constexpr int PT = 1024;             // threads per block, two blocks per SM: 64 warps resident
+constexpr int ACC = 8;               // independent dependency chains per thread
+
+// ---- FP32 FMA, three register operands (FFMA R, R, R, R) ----
+__global__ void __launch_bounds__(PT, 2) p_ffma(float b, float c, int iters, float* sink) {
+    float a[ACC];
+#pragma unroll
+    for (int k = 0; k < ACC; ++k) a[k] = (float)(threadIdx.x + k);
+    for (int i = 0; i < iters; ++i) {
+#pragma unroll
+        for (int u = 0; u < 4; ++u)
+#pragma unroll
+            for (int k = 0; k < ACC; ++k) a[k] = fmaf(a[k], b, c);
+    }
+    float s = 0.f;
+#pragma unroll
+    for (int k = 0; k < ACC; ++k) s += a[k];
+    if (s == 12345.678f) sink[0] = s;
+}
+
+// ---- packed FP32 pairs (FFMA2: fma.rn.f32x2), the form K1/K2 accumulate with ----
+__global__ void __launch_bounds__(PT, 2) p_ffma2(float b, float c, int iters, float* sink) {
+    uint64_t a[ACC], bb, cc;
+    asm("mov.b64 %0, {%1, %1};" : "=l"(bb) : "f"(b));
+    asm("mov.b64 %0, {%1, %1};" : "=l"(cc) : "f"(c));
+#pragma unroll
+    for (int k = 0; k < ACC; ++k) { const float v = (float)(threadIdx.x + k); asm("mov.b64 %0, {%1, %1};" : "=l"(a[k]) : "f"(v)); }
+    for (int i = 0; i < iters; ++i) {
+#pragma unroll
+        for (int u = 0; u < 4; ++u)
+#pragma unroll
+            for (int k = 0; k < ACC; ++k) asm volatile("fma.rn.f32x2 %0, %0, %1, %2;" : "+l"(a[k]) : "l"(bb), "l"(cc));
+    }
+    uint64_t s = 0;
+#pragma unroll
+    for (int k = 0; k < ACC; ++k) s ^= a[k];
+    if (s == 0x123456789abcdefull) sink[0] = 1.f;
+}
+
+// ---- instruction issue: FMA-pipe and ALU-pipe instructions alternating, so that neither pipe's own rate is the limit ----
+__global__ void __launch_bounds__(PT, 2) p_issue(float b, float c, int k0, int iters, float* sink) {
+    float a[4];
+    int x[4];
+#pragma unroll
+    for (int k = 0; k < 4; ++k) { a[k] = (float)(threadIdx.x + k); x[k] = threadIdx.x * 7 + k; }
+    for (int i = 0; i < iters; ++i) {
+#pragma unroll
+        for (int u = 0; u < 8; ++u)
+#pragma unroll
+            for (int k = 0; k < 4; ++k) {
+                a[k] = fmaf(a[k], b, c);                         // fma pipe
+                x[k] = __byte_perm(x[k], k0, 0x4321);            // alu pipe: one PRMT (a chain ptxas cannot fold)
+            }
+    }
+    float s = 0.f;
+    int t = 0;
+#pragma unroll
+    for (int k = 0; k < 4; ++k) { s += a[k]; t ^= x[k]; }
+    if (s == 12345.678f || t == 0x7fffffff) sink[0] = s + (float)t;
+}
+
+// ---- L2-resident reads: every block streams the whole buffer (L2-sized, far above the L1s) with ld.global.cg ----
+__global__ void __launch_bounds__(PT, 2) p_l2(const float4* __restrict__ buf, size_t n_vec, int reps, float* sink) {
+    float s = 0.f;
+    const size_t start = ((size_t)blockIdx.x * 7919u * PT) % n_vec;
+    for (int r = 0; r < reps; ++r) {
+        for (size_t i0 = 0; i0 < n_vec; i0 += (size_t)PT * 4) {
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                size_t i = start + i0 + (size_t)u * PT + threadIdx.x;
+                if (i >= n_vec) i -= n_vec;
+                const float4 v = __ldcg(buf + i);
+                s += v.x + v.y + v.z + v.w;
+            }
+        }
+    }
+    if (s == 12345.678f) sink[0] = s;
+}
+
+// ---- L1 hits: every block re-reads its own 32 KiB window of global memory with 16-byte loads ----
+__global__ void __launch_bounds__(PT, 2) p_l1(const float4* __restrict__ buf, int iters, float* sink) {
+    const float4* w = buf + (size_t)blockIdx.x * 2048;          // 2048 float4 = 32 KiB per block
+    float s = 0.f;
+    for (int i = 0; i < iters; ++i) {
+#pragma unroll
+        for (int u = 0; u < 8; ++u) {
+            const float4 v = __ldg(w + ((threadIdx.x + (u + i) * 64) & 2047));
+            s += v.x + v.w;
+        }
+    }
+    if (s == 12345.678f) sink[0] = s;
+}
+
+// ---- the same with scalar loads: one 128-byte wavefront per warp instruction (K1's gather width) ----
+__global__ void __launch_bounds__(PT, 2) p_l1_b32(const float* __restrict__ buf, int iters, float* sink) {
+    const float* w = buf + (size_t)blockIdx.x * 8192;
+    float s = 0.f;
+    for (int i = 0; i < iters; ++i) {
+#pragma unroll
+        for (int u = 0; u < 8; ++u) s += __ldg(w + ((threadIdx.x + (u + i) * 128) & 8191));
+    }
+    if (s == 12345.678f) sink[0] = s;
+}
+
+// ---- shared memory: conflict-free 16-byte loads ----
+__global__ void __launch_bounds__(PT, 2) p_smem(int iters, float* sink) {
+    __shared__ float4 sm[2048];                                  // 32 KiB
+    for (int i = threadIdx.x; i < 2048; i += PT) sm[i] = make_float4((float)i, 1.f, 2.f, 3.f);
+    __syncthreads();
+    float s = 0.f;
+    for (int i = 0; i < iters; ++i) {
+#pragma unroll
+        for (int u = 0; u < 8; ++u) {
+            const float4 v = sm[(threadIdx.x + (u + i) * 64) & 2047];
+            s += v.x + v.w;
+        }
+    }
+    if (s == 12345.678f) sink[0] = s;
+}
+
+template <class F>
+int best_ms(F launch, double* ms) {
+    cudaEvent_t e0, e1;
+    if (cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) return OSIV_ERR_CUDA;
+    double best = 1e30;
+    for (int r = 0; r < 6; ++r) {                                // first pass is the warm-up
+        cudaEventRecord(e0);
+        launch();
+        cudaEventRecord(e1);
+        if (cudaEventSynchronize(e1) != cudaSuccess) { cudaEventDestroy(e0); cudaEventDestroy(e1); return OSIV_ERR_CUDA; }
+        float t = 0.f;
+        cudaEventElapsedTime(&t, e0, e1);
+        if (r > 0 && t < best) best = t;
+    }
+    cudaEventDestroy(e0); cudaEventDestroy(e1);
+    *ms = best;
+    return cudaGetLastError() == cudaSuccess ? OSIV_OK : OSIV_ERR_CUDA;
+}
+
+}  // namespace
+
+extern "C" int osiv_probe_peaks(int32_t device, double* out8) {
+    if (!out8 || device < 0) return OSIV_ERR_INVALID_ARG;
+    int prev = -1, sms = 0;
+    if (cudaGetDevice(&prev) != cudaSuccess || cudaSetDevice(device) != cudaSuccess ||
+        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, device) != cudaSuccess) {
+        cudaGetLastError();
+        return OSIV_ERR_CUDA;
+    }
+    const int grid = 2 * sms;
+    const size_t l2_bytes = (size_t)64 << 20;                    // 64 MiB: inside the 126 MB L2, twice the sum of all L1s
+    float* sink = nullptr;
+    float4* buf = nullptr;
+    int rc = OSIV_OK;
+    if (cudaMalloc((void**)&sink, 256) != cudaSuccess || cudaMalloc((void**)&buf, l2_bytes) != cudaSuccess ||
+        cudaMemset(buf, 0, l2_bytes) != cudaSuccess) {
+        rc = OSIV_ERR_CUDA;
+    }
+    double ms = 0.0;
+    const double threads = (double)grid * PT;
+    if (rc == OSIV_OK) {
+        const int it = 4096;
+        rc = best_ms([&] { p_ffma<<<grid, PT>>>(1.0001f, 0.5f, it, sink); }, &ms);
+        out8[0] = threads * it * 4 * ACC * 2 / (ms * 1e-3) / 1e12;                 // TFLOP/s, FFMA
+    }
+    if (rc == OSIV_OK) {
+        const int it = 4096;
+        rc = best_ms([&] { p_ffma2<<<grid, PT>>>(1.0001f, 0.5f, it, sink); }, &ms);
+        out8[1] = threads * it * 4 * ACC * 4 / (ms * 1e-3) / 1e12;                 // TFLOP/s, FFMA2
+    }
+    if (rc == OSIV_OK) {
+        const int it = 2048;
+        rc = best_ms([&] { p_issue<<<grid, PT>>>(1.0001f, 0.5f, 0x5a5a, it, sink); }, &ms);
+        // per inner step one FFMA and one PRMT (checked in the SASS: 32 + 32 per loop body, the loop's own 3 not counted)
+        out8[2] = threads / 32.0 * it * 8 * 4 * 2 / (ms * 1e-3) / 1e9;             // G warp-instructions/s
+    }
+    if (rc == OSIV_OK) {
+        const int reps = 2;
+        rc = best_ms([&] { p_l2<<<grid, PT>>>(buf, l2_bytes / 16, reps, sink); }, &ms);
+        out8[3] = (double)grid * reps * (double)l2_bytes / (ms * 1e-3) / 1e9;      // GB/s out of L2
+    }
+    if (rc == OSIV_OK) {
+        const int it = 4096;
+        rc = best_ms([&] { p_smem<<<grid, PT>>>(it, sink); }, &ms);
+        out8[4] = threads * it * 8 * 16 / (ms * 1e-3) / 1e9;                       // GB/s, LDS.128
+    }
+    if (rc == OSIV_OK) {
+        const int it = 4096;
+        rc = best_ms([&] { p_l1<<<grid, PT>>>(buf, it, sink); }, &ms);
+        out8[5] = threads * it * 8 * 16 / (ms * 1e-3) / 1e9;                       // GB/s, LDG.128 hitting L1
+    }
+    if (rc == OSIV_OK) {
+        const int it = 4096;
+        rc = best_ms([&] { p_l1_b32<<<grid, PT>>>(reinterpret_cast<const float*>(buf), it, sink); }, &ms);
+        out8[6] = threads * it * 8 * 4 / (ms * 1e-3) / 1e9;                        // GB/s, LDG.32 hitting L1
+    }
+    out8[7] = (double)sms;
+    if (sink) cudaFree(sink);
+    if (buf) cudaFree(buf);
+    cudaGetLastError();
+    if (prev >= 0) cudaSetDevice(prev);
+    return rc;
+}
