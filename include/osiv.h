@@ -204,6 +204,16 @@ int osiv_get_plan(const osiv_handle* h, int32_t n_subsets, int32_t batch, int32_
 int osiv_set_profiling(osiv_handle* h, int32_t enable);
 int osiv_get_profile(const osiv_handle* h, double* ms_forward, int64_t* n_forward, double* ms_back, int64_t* n_back);
 
+/* Phase timeline of the two hot kernels (only in the build made with -DOSIV_TRACE, `python -m
+ * paper_1903_10088_b200.build --trace` -> libosiv_trace.so; the regular library returns OSIV_ERR_INVALID_ARG).
+ * Every block of slice group 0 stamps its SM's cycle counter at its phase boundaries; h_out receives
+ * [4][256][12] uint64: first index = (iteration & 1) * 2 + kernel (0 = K1, 1 = K2) of the last two iterations run on
+ * the current device, second = block, third = {block start, before the dependent-launch wait, after it, end of the
+ * main loop (latest warp), after the block barrier, block end (latest warp) -- all in SM cycles --, SM id, a mark
+ * inside the prologue [cycles], the GPU's global nanosecond timer read at block start, unused...}.  n_entries must be
+ * 4*256*12.  Synchronises the device.  Driver: `python -m paper_1903_10088_b200.timeline`. */
+int osiv_debug_timeline(uint64_t* h_out, int32_t n_entries);
+
 /* Micro-probes of the units that bound the two hot kernels (csrc/osiv_probes.cu): saturating loops
  * of one instruction kind at full occupancy on `device`, CUDA-event timed, best of 5 (takes about 0.1 s).
  * out8 = { FP32 TFLOP/s with FFMA (three register operands), FP32 TFLOP/s with FFMA2 (fma.rn.f32x2),

@@ -18,7 +18,7 @@ OSIV_OK, OSIV_ERR_INVALID_ARG, OSIV_ERR_CUDA, OSIV_ERR_NOT_FINITE = 0, -1, -2, -
 EXPORTED_SYMBOLS = (
     "osiv_version", "osiv_strerror", "osiv_default_params", "osiv_create", "osiv_destroy", "osiv_ray_table", "osiv_get_dgamma",
     "osiv_get_tau", "osiv_launch_count", "osiv_set_symmetry", "osiv_set_overlap", "osiv_get_plan", "osiv_set_profiling", "osiv_get_profile", "osiv_forward", "osiv_backward", "osiv_tv_gradient", "osiv_reconstruct",
-    "osiv_reconstruct_host", "osiv_probe_peaks",
+    "osiv_reconstruct_host", "osiv_probe_peaks", "osiv_debug_timeline",
 )
 
 
@@ -91,7 +91,8 @@ def lib():
     """Load libosiv.so (building it with nvcc if the sources are newer).  Raises if it cannot be had."""
     global _lib
     if _lib is None:
-        path = _build.build()
+        # OSIV_TRACE_BUILD=1 selects the timeline build of the same sources (diagnostics; see timeline.py)
+        path = _build.build(trace=os.environ.get("OSIV_TRACE_BUILD", "") == "1")
         L = C.CDLL(path)
         vp, ip = C.c_void_p, C.c_int32
         L.osiv_version.restype = C.c_int
@@ -117,6 +118,7 @@ def lib():
         L.osiv_reconstruct.argtypes = [vp, vp, vp, C.c_float, C.POINTER(_CParams), ip, vp, vp, vp]
         L.osiv_reconstruct_host.argtypes = [vp, vp, vp, C.c_float, C.POINTER(_CParams), ip, vp, vp, vp]
         L.osiv_probe_peaks.argtypes = [ip, C.POINTER(C.c_double)]
+        L.osiv_debug_timeline.argtypes = [vp, ip]
         _lib = L
     return _lib
 

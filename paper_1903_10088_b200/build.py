@@ -36,16 +36,27 @@ def needs_build() -> bool:
     return any(os.path.getmtime(d) > t for d in DEPS)
 
 
-def build(force: bool = False, verbose: bool = False) -> str:
-    if force or needs_build():
-        cmd = [nvcc_path()] + NVCC_FLAGS + ["-I", INCLUDE, "-o", SO] + SOURCES
+SO_TRACE = os.path.join(_HERE, "libosiv_trace.so")      # the same sources with -DOSIV_TRACE (phase timeline, diagnostics)
+
+
+def _stale(so: str) -> bool:
+    if not os.path.exists(so):
+        return True
+    t = os.path.getmtime(so)
+    return any(os.path.getmtime(d) > t for d in DEPS)
+
+
+def build(force: bool = False, verbose: bool = False, trace: bool = False) -> str:
+    so = SO_TRACE if trace else SO
+    if force or _stale(so):
+        cmd = [nvcc_path()] + NVCC_FLAGS + (["-DOSIV_TRACE"] if trace else []) + ["-I", INCLUDE, "-o", so] + SOURCES
         res = subprocess.run(cmd, capture_output=True, text=True)
         if verbose or res.returncode != 0:
             sys.stderr.write(res.stdout + res.stderr)
         if res.returncode != 0:
-            raise RuntimeError("nvcc failed building libosiv.so")
-    return SO
+            raise RuntimeError("nvcc failed building " + os.path.basename(so))
+    return so
 
 
 if __name__ == "__main__":
-    print(build(force="--force" in sys.argv, verbose=True))
+    print(build(force="--force" in sys.argv, verbose=True, trace="--trace" in sys.argv))

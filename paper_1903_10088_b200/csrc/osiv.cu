@@ -24,7 +24,8 @@ struct osiv_handle {
     float2* d_views = nullptr;
     float* d_hs = nullptr;
     // per-slice workspace, grown lazily
-    int ws_batch = 0, ws_sb = 1;        // slices the image buffers hold, and their interleave (DevGeom::sb)
+    int ws_batch = 0, ws_sb = 1, ws_ns = 1;   // slices the image buffers hold, their interleave (DevGeom::sb) and layout (1: one
+                                              // float per pixel, 4: the orbit float4 per pixel of the quarter-turn path)
     float *d_imgA = nullptr, *d_imgB = nullptr, *d_imgTA = nullptr, *d_imgTB = nullptr;
     float* d_best = nullptr;
     size_t res_elems = 0;       float* d_res = nullptr;
@@ -146,14 +147,17 @@ int check_subset(const osiv_handle* h, int subset, int n_subsets) {
     return OSIV_OK;
 }
 
-// padded image buffers for `batch` slices in the layout DevGeom::sb = sb (slices interleaved per pixel in groups of
-// sb); the pads are zeroed when the buffers are made or the layout changes and never written again
-int ensure_images(osiv_handle* h, int batch, int sb, cudaStream_t st) {
+// padded image buffers for `batch` slices in the layout (sb, ns): slices interleaved per pixel in groups of sb; ns = 1:
+// one float per pixel, ns = 4: the orbit float4 per pixel (header of osiv_kernels.cuh).  The buffers are sized for the
+// float4 layout when the geometry admits it; the pads are zeroed when the buffers are made or the layout changes and
+// never written again.
+int ensure_images(osiv_handle* h, int batch, int sb, int ns, cudaStream_t st) {
     const int slices = (batch + sb - 1) / sb * sb;
     h->dg.sb = sb;
-    if (h->ws_batch >= slices && h->ws_sb == sb) return OSIV_OK;
+    if (h->ws_batch >= slices && h->ws_sb == sb && h->ws_ns == ns) return OSIV_OK;
     const int n = std::max(slices, h->ws_batch);
-    const size_t ne = (size_t)h->dg.img_elems * n, nt = (size_t)h->dg.imgT_elems * n;
+    const size_t per = h->dg.sym4 ? 4 : 1;
+    const size_t ne = (size_t)h->dg.img_elems * n * per, nt = (size_t)h->dg.imgT_elems * n * per;
     if (h->ws_batch < slices) {
         float** bufs[4] = {&h->d_imgA, &h->d_imgB, &h->d_imgTA, &h->d_imgTB};
         for (auto b : bufs) if (*b) { OSIV_CUDA(cudaFree(*b)); *b = nullptr; }
@@ -171,13 +175,15 @@ int ensure_images(osiv_handle* h, int batch, int sb, cudaStream_t st) {
     OSIV_CUDA(cudaMemsetAsync(h->d_imgTB, 0, nt * sizeof(float), st));
     h->ws_batch = n;
     h->ws_sb = sb;
+    h->ws_ns = ns;
     return OSIV_OK;
 }
 
 // ---- launch plans -------------------------------------------------------------------------------------
 // NS = 4 (quarter-turn orbits share one weight) needs a square grid with nx % 4 == 0, V % 4 == 0 and a subset
 // made of whole orbits (V_S % 4 == 0); everything else takes the general NS = 1 kernels.
-int pick_ns(const osiv_handle* h, int VS) { return (h->dg.sym4 && !h->force_ns1 && VS % 4 == 0) ? 4 : 1; }
+// A stack of slices (view_shift / tv_z) always takes the general kernels.
+int pick_ns(const osiv_handle* h, int VS, bool stack = false) { return (h->dg.sym4 && !h->force_ns1 && !stack && VS % 4 == 0) ? 4 : 1; }
 
 constexpr int BATCH_THREADS = 512;      // K1 block size cap when a launch carries several slices: two blocks per SM
 constexpr int BATCH_MIN_SLICES = 4;     // fewer slices than this run one after the other in full-size blocks
@@ -186,15 +192,18 @@ constexpr int BATCH_MIN_SLICES = 4;     // fewer slices than this run one after 
 // K2's tiles per block leave room for at least one view share in its 448-thread blocks.
 int pick_sb(const osiv_handle* h, int VS, int batch, bool stack) {
     if (batch < BATCH_MIN_SLICES || stack) return 1;      // a stack's slices differ in their views: no pairs
-    const int ns = pick_ns(h, VS);
+    const int ns = pick_ns(h, VS, stack);
     const int tx = ns == 4 ? h->geom.nx / 4 : (h->geom.nx + BK_TX - 1) / BK_TX;
     const int ty = ns == 4 ? h->geom.ny / 4 : (h->geom.ny + BK_TY - 1) / BK_TY;
     const long long tiles = (long long)(((tx + BK_WX - 1) / BK_WX + 1) / 2) * (((ty + BK_WY - 1) / BK_WY + 1) / 2) * 4 * 32;
-    const long long tpb = std::max<long long>(1, (tiles + h->num_sms - 1) / h->num_sms);
+    const long long tpb = (std::max<long long>(1, (tiles + h->num_sms - 1) / h->num_sms) + 7) / 8 * 8;
     return tpb * ns <= BKB_MAX_THREADS ? 2 : 1;
 }
 
 struct FwdPlan { int threads, rpb, segs, nparts, ns, sb; size_t smem; };
+
+// magic of osiv::fastdiv: n / d == umulhi(n, ceil(2^32 / d)) for 0 <= n < 2^32 / d (every use here stays below 2^21)
+unsigned div_magic(int d) { return d <= 1 ? 0u : (unsigned)(((1ull << 32) + (unsigned)d - 1) / (unsigned)d); }
 struct BackPlan { int nblk, threads, tpb, shares, ngx, ns, sb, ntiles; size_t smem; };
 
 // K1: the subset's base rays are dealt out in runs of rpb consecutive rays, one run per block and one block per SM
@@ -202,7 +211,7 @@ struct BackPlan { int nblk, threads, tpb, shares, ngx, ns, sb, ntiles; size_t sm
 // threads while a segment keeps at least FWD_MIN_LINES image lines.
 FwdPlan plan_forward(const osiv_handle* h, int VS, int batch, bool stack = false) {
     FwdPlan p;
-    p.ns = pick_ns(h, VS);
+    p.ns = pick_ns(h, VS, stack);
     const long long R = (long long)(VS / p.ns) * h->geom.n_channels;
     p.rpb = (int)std::min<long long>(FWD_MAX_THREADS, std::max<long long>(1, (R + h->num_sms - 1) / h->num_sms));
     const int nmax = std::max(h->geom.nx, h->geom.ny);
@@ -234,7 +243,7 @@ cudaError_t launch_forward(FwdPlan p, int batch, const FwdArgs& a, cudaStream_t 
 // consecutive tiles, one run per block and one block per SM (per slice); a block is tpb tiles x `shares` view shares.
 BackPlan plan_back(const osiv_handle* h, int VS, int batch, bool stack = false) {
     BackPlan p;
-    p.ns = pick_ns(h, VS);
+    p.ns = pick_ns(h, VS, stack);
     const int tx = p.ns == 4 ? h->geom.nx / 4 : (h->geom.nx + BK_TX - 1) / BK_TX;
     const int ty = p.ns == 4 ? h->geom.ny / 4 : (h->geom.ny + BK_TY - 1) / BK_TY;
     p.ngx = ((tx + BK_WX - 1) / BK_WX + 1) / 2;
@@ -242,6 +251,9 @@ BackPlan plan_back(const osiv_handle* h, int VS, int batch, bool stack = false) 
     const long long tiles = (long long)p.ngx * ngy * 4 * 32;
     p.ntiles = (int)tiles;
     p.tpb = (int)std::min<long long>(BK_MAX_THREADS / p.ns, std::max<long long>(1, (tiles + h->num_sms - 1) / h->num_sms));
+    // whole units of 8 tiles (4 x 2, the lanes of a quarter-warp: tile_origin) per block, so that every 16-byte load of the
+    // candidate loop is served for 8 neighbouring tiles
+    p.tpb = std::min((p.tpb + 7) / 8 * 8, BK_MAX_THREADS / p.ns / 8 * 8);
     p.nblk = (int)((tiles + p.tpb - 1) / p.tpb);
     const int VSb = VS / p.ns;
     // shares per quarter turn (NS == 4) or in all: as many as fit, then the fewest that keep the same number of
@@ -268,8 +280,7 @@ cudaError_t launch_back(const BackPlan& p, int batch, const BackArgs& a, cudaStr
     attr[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = attr; cfg.numAttrs = pdl ? 1 : 0;
     if (p.sb == 2) return p.ns == 4 ? cudaLaunchKernelEx(&cfg, k_back<MODE, 4, 2, 0>, a) : cudaLaunchKernelEx(&cfg, k_back<MODE, 1, 2, 0>, a);
-    if (MODE == 1 && (a.view_shift != 0 || a.tv_z > 0.f))
-        return p.ns == 4 ? cudaLaunchKernelEx(&cfg, k_back<1, 4, 1, 1>, a) : cudaLaunchKernelEx(&cfg, k_back<1, 1, 1, 1>, a);
+    if (MODE == 1 && (a.view_shift != 0 || a.tv_z > 0.f)) return cudaLaunchKernelEx(&cfg, k_back<1, 1, 1, 1>, a);      // a stack: ns == 1
     return p.ns == 4 ? cudaLaunchKernelEx(&cfg, k_back<MODE, 4, 1, 0>, a) : cudaLaunchKernelEx(&cfg, k_back<MODE, 1, 1, 0>, a);
 }
 
@@ -281,7 +292,7 @@ int ensure_intervals(osiv_handle* h, const BackPlan& p, cudaStream_t st) {
     for (int k = 0; k < 2; ++k)
         if (h->d_itab[k]) { OSIV_CUDA(cudaFree(h->d_itab[k])); h->d_itab[k] = nullptr; h->itab_tiles[k] = 0; }
     OSIV_CUDA(cudaMalloc((void**)&h->d_itab[w], (size_t)h->geom.n_views * p.ntiles * sizeof(int)));
-    k_build_intervals<<<dim3((p.ntiles + 255) / 256, h->geom.n_views), 256, 0, st>>>(h->dg, p.ns, p.ngx, p.ntiles, h->d_itab[w]);
+    k_build_intervals<<<dim3((p.ntiles + 255) / 256, h->geom.n_views), 256, 0, st>>>(h->dg, p.ns, p.ngx, div_magic(p.ngx), p.ntiles, h->d_itab[w]);
     h->itab_tiles[w] = p.ntiles;
     h->launches += 1;
     OSIV_CUDA(cudaGetLastError());
@@ -417,7 +428,6 @@ int osiv_create(const osiv_geometry* geom, int32_t max_batch, int32_t device, os
         // K2's shared-memory reduction buffer: up to 1024 threads x 16 floats
         cudaFuncSetAttribute(k_back<0, 4, 1, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024) != cudaSuccess ||
         cudaFuncSetAttribute(k_back<1, 4, 1, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024) != cudaSuccess ||
-        cudaFuncSetAttribute(k_back<1, 4, 1, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024) != cudaSuccess ||
         cudaFuncSetAttribute(k_back<0, 4, 2, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024) != cudaSuccess ||
         cudaFuncSetAttribute(k_back<1, 4, 2, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024) != cudaSuccess) {
         cudaGetLastError();
@@ -480,6 +490,18 @@ int osiv_get_tau(const osiv_handle* h, int32_t n_subsets, double kappa, double* 
 
 int64_t osiv_launch_count(const osiv_handle* h) { return h ? h->launches : 0; }
 
+int osiv_debug_timeline(uint64_t* h_out, int32_t n_entries) {
+#ifdef OSIV_TRACE
+    if (!h_out || n_entries != 4 * TL_BLOCKS * TL_SLOTS) return OSIV_ERR_INVALID_ARG;
+    OSIV_CUDA(cudaDeviceSynchronize());
+    OSIV_CUDA(cudaMemcpyFromSymbol(h_out, g_timeline, sizeof(unsigned long long) * 4 * TL_BLOCKS * TL_SLOTS));
+    return OSIV_OK;
+#else
+    (void)h_out; (void)n_entries;
+    return OSIV_ERR_INVALID_ARG;                          // not the timeline build
+#endif
+}
+
 int osiv_set_symmetry(osiv_handle* h, int32_t enable) {
     if (!h) return OSIV_ERR_INVALID_ARG;
     h->force_ns1 = enable ? 0 : 1;
@@ -528,14 +550,13 @@ int osiv_forward(osiv_handle* h, const float* d_img, float* d_sino, int32_t batc
     cudaStream_t st = (cudaStream_t)cuda_stream;
     const int VS = subset_views(h, subset, n_subsets);
     const FwdPlan p = plan_forward(h, VS, batch);
-    int rc = ensure_images(h, batch, p.sb, st);
+    int rc = ensure_images(h, batch, p.sb, p.ns, st);
     if (rc != OSIV_OK) return rc;
     if ((rc = ensure_forward_ws(h, p, batch)) != OSIV_OK) return rc;
-    k_pad_transpose<<<dim3((h->geom.nx + 31) / 32, (h->geom.ny + 31) / 32, batch), 256, 0, st>>>(h->dg, d_img, h->d_imgA,
-                                                                                             h->d_imgTA);
+    k_pad_transpose<<<px_grid(h, batch), 256, 0, st>>>(h->dg, p.ns, d_img, h->d_imgA, h->d_imgTA);
     FwdArgs a{};
     a.g = h->dg; a.img = h->d_imgA; a.imgT = h->d_imgTA;
-    a.subset = subset; a.M = subset < 0 ? 1 : n_subsets; a.VS = VS; a.batch = batch; a.rpb = p.rpb; a.segs = p.segs; a.sino = d_sino;
+    a.subset = subset; a.M = subset < 0 ? 1 : n_subsets; a.VS = VS; a.batch = batch; a.rpb = p.rpb; a.segs = p.segs; a.rpb_magic = div_magic(p.rpb); a.C_magic = div_magic(h->geom.n_channels); a.sino = d_sino;
     if (launch_forward<0>(p, batch, a, st, false) != cudaSuccess) { cudaGetLastError(); return OSIV_ERR_CUDA; }
     return launch_check(h, 2);
 }
@@ -555,7 +576,7 @@ int osiv_backward(osiv_handle* h, const float* d_sino, float* d_img, int32_t bat
     k_scale_sino<<<dim3((h->geom.n_channels + 255) / 256, VS, batch), 256, 0, st>>>(h->dg, d_sino, h->d_res, subset, M, VS,
                                                                                     p.ns, Cp);
     BackArgs b{};
-    b.g = h->dg; b.res = h->d_res; b.Cp = Cp; b.subset = subset; b.M = M; b.VS = VS; b.batch = batch; b.out = d_img; b.tpb = p.tpb; b.shares = p.shares; b.ngx = p.ngx;
+    b.g = h->dg; b.res = h->d_res; b.Cp = Cp; b.subset = subset; b.M = M; b.VS = VS; b.batch = batch; b.out = d_img; b.tpb = p.tpb; b.shares = p.shares; b.ngx = p.ngx; b.tpb_magic = div_magic(p.tpb); b.ngx_magic = div_magic(p.ngx);
     if ((rc = ensure_intervals(h, p, st)) != OSIV_OK) return rc;
     b.itab = h->d_itab[p.ns == 4]; b.ntiles = p.ntiles;
     if (launch_back<0>(p, batch, b, st, false) != cudaSuccess) { cudaGetLastError(); return OSIV_ERR_CUDA; }
@@ -568,10 +589,9 @@ int osiv_tv_gradient(osiv_handle* h, const float* d_img, float* d_grad, int32_t 
     DeviceGuard guard(h->device);
     if (!guard.ok) { cudaGetLastError(); return OSIV_ERR_CUDA; }
     cudaStream_t st = (cudaStream_t)cuda_stream;
-    int rc = ensure_images(h, batch, 1, st);
+    int rc = ensure_images(h, batch, 1, 1, st);
     if (rc != OSIV_OK) return rc;
-    k_pad_transpose<<<dim3((h->geom.nx + 31) / 32, (h->geom.ny + 31) / 32, batch), 256, 0, st>>>(h->dg, d_img, h->d_imgA,
-                                                                                             h->d_imgTA);
+    k_pad_transpose<<<px_grid(h, batch), 256, 0, st>>>(h->dg, 1, d_img, h->d_imgA, h->d_imgTA);
     k_tv<<<dim3((h->geom.nx + 31) / 32, (h->geom.ny + 15) / 16, batch), 128, 0, st>>>(h->dg, h->d_imgA,
                                                                                      (float)(tv_eps * tv_eps), d_grad);
     return launch_check(h, 2);
@@ -597,7 +617,7 @@ int osiv_reconstruct(osiv_handle* h, const float* d_counts, const float* d_blank
 
     const int VS = h->geom.n_views / M, C = h->geom.n_channels;
     const FwdPlan fp = plan_forward(h, VS, batch, stack);
-    int rc = ensure_images(h, batch, fp.sb, st);
+    int rc = ensure_images(h, batch, fp.sb, fp.ns, st);
     if (rc != OSIV_OK) return rc;
     const BackPlan bp = plan_back(h, VS, batch, stack);
     if ((rc = ensure_res(h, VS, fp.ns, batch, st)) != OSIV_OK) return rc;
@@ -615,15 +635,15 @@ int osiv_reconstruct(osiv_handle* h, const float* d_counts, const float* d_blank
     float* best = prm->return_best ? h->d_best : nullptr;
     SliceState* state[2] = {h->d_state, h->d_state + h->max_batch};
     k_init_state<<<1, 32, 0, st>>>(state[0], h->d_not_finite, batch, prm->lambda0, d_blank, blank_scalar, C, h->d_inv_bref);
-    k_fill<<<px_grid(h, batch), 256, 0, st>>>(h->dg, (float)prm->mu0, h->d_imgA, h->d_imgTA, best);
+    k_fill<<<px_grid(h, batch), 256, 0, st>>>(h->dg, fp.ns, (float)prm->mu0, h->d_imgA, h->d_imgTA, best);
     h->launches += 2;
 
     FwdArgs f{};
-    f.g = h->dg; f.M = M; f.VS = VS; f.batch = batch; f.view_shift = vshift; f.rpb = fp.rpb; f.segs = fp.segs;
+    f.g = h->dg; f.M = M; f.VS = VS; f.batch = batch; f.view_shift = vshift; f.rpb = fp.rpb; f.segs = fp.segs; f.rpb_magic = div_magic(fp.rpb); f.C_magic = div_magic(C);
     f.counts = d_counts; f.blank = d_blank; f.blank_scalar = blank_scalar; f.inv_bref = h->d_inv_bref;
     f.res = h->d_res; f.Cp = Cp; f.dparts = h->d_dparts;
     BackArgs b{};
-    b.g = h->dg; b.res = h->d_res; b.Cp = Cp; b.M = M; b.VS = VS; b.batch = batch; b.view_shift = vshift; b.tv_z = (float)prm->tv_z; b.best = best; b.tpb = bp.tpb; b.shares = bp.shares; b.ngx = bp.ngx;
+    b.g = h->dg; b.res = h->d_res; b.Cp = Cp; b.M = M; b.VS = VS; b.batch = batch; b.view_shift = vshift; b.tv_z = (float)prm->tv_z; b.best = best; b.tpb = bp.tpb; b.shares = bp.shares; b.ngx = bp.ngx; b.tpb_magic = div_magic(bp.tpb); b.ngx_magic = div_magic(bp.ngx);
     if ((rc = ensure_intervals(h, bp, st)) != OSIV_OK) return rc;
     b.itab = h->d_itab[bp.ns == 4]; b.ntiles = bp.ntiles;
     b.dparts = h->d_dparts; b.nparts = fp.nparts; b.not_finite = h->d_not_finite;
@@ -647,7 +667,7 @@ int osiv_reconstruct(osiv_handle* h, const float* d_counts, const float* d_blank
     }
     for (int n = 0; n < N; ++n) {
         const int m = n % M;                               // PAPER.md:118, C11
-        f.img = cur; f.imgT = curT; f.subset = m;
+        f.img = cur; f.imgT = curT; f.subset = m; f.iter = n; b.iter = n;
         if (launch_forward<1>(fp, batch, f, st, pdl) != cudaSuccess) { cudaGetLastError(); return OSIV_ERR_CUDA; }
         if (prof) cudaEventRecord(h->events[2 * n + 1], st);
         b.img = cur; b.img_new = nxt; b.imgT_new = nxtT; b.subset = m;
@@ -677,7 +697,7 @@ int osiv_reconstruct(osiv_handle* h, const float* d_counts, const float* d_blank
         k_final_monitor<<<batch, 32, 0, st>>>(h->d_dparts, fp.nparts, fin, h->d_not_finite);
         h->launches += 2;
     }
-    k_unpad<<<px_grid(h, batch), 256, 0, st>>>(h->dg, cur, best, fin, d_img_out);
+    k_unpad<<<px_grid(h, batch), 256, 0, st>>>(h->dg, fp.ns, cur, best, fin, d_img_out);
     rc = launch_check(h, 1);
     if (rc != OSIV_OK) return rc;
 

@@ -22,10 +22,13 @@
 // Quarter-turn symmetry (NS = 4).  When the grid is square with nx % 4 == 0, V % 4 == 0 and the subset
 // holds whole orbits {v, v+V/4, v+V/2, v+3V/4}, the scan is invariant under the rotation
 // R: (xc,yc) -> (-yc,xc), i.e. pixel (ix,iy) -> (N-1-iy, ix):  a(v + kV/4, c; R^k P) = a(v, c; P).
-// Every chord weight is then evaluated once and used for the four rotated (ray, pixel) pairs: K1 walks
-// ray (v,c) and gathers mu at P, RP, R^2P, R^3P (row-major and transposed image copies make all four
-// walks contiguous); K2 evaluates a(v,c;T) for its base tile T and feeds the accumulators of T, RT, R^2T,
-// R^3T with the residuals of views v, v+V/4, v+V/2, v+3V/4.  The ray table is built with exactly
+// Every chord weight is then evaluated once and used for the four rotated (ray, pixel) pairs.  The image of this path
+// is stored ORBIT-INTERLEAVED: one float4 per pixel P holding {mu(P), mu(RP), mu(R^2P), mu(R^3P)} (array Q, row-major,
+// plus its transpose QT so that rays of either orientation walk contiguous lines), so K1 walks ray (v,c) with ONE
+// 16-byte gather per touched pixel for all four rays of the orbit (the load/store unit issues one warp load per ~1.8
+// cycles whatever its width, and the four scalar gathers of the earlier layout were K1's bound); K2 evaluates a(v,c;T)
+// for its base tile T and feeds the accumulators of T, RT, R^2T, R^3T with the residuals of views v, v+V/4, v+V/2,
+// v+3V/4, and its epilogue finishes one base pixel in all four rotations from the 3x3 neighbourhood of float4s.  The ray table is built with exactly
 // rotated coefficients (alpha,beta,g0,h) -> (-beta,alpha,g0,h), so both kernels still use one weight per
 // (ray, pixel) pair.  NS = 1 is the general path (any geometry).
 #pragma once
@@ -33,6 +36,35 @@
 #include <stdint.h>
 
 namespace osiv {
+
+// ---- phase timeline (diagnostics; only in the build with -DOSIV_TRACE, `python -m paper_1903_10088_b200.build --trace`):
+// every block of the two hot kernels of slice group 0 stamps its SM's cycle counter (clock64: a few cycles per stamp) at
+// its phase boundaries into g_timeline[(iteration & 1) * 2 + kernel][block][slot]; slots: 0 block start, 1 before the
+// dependent-launch wait, 2 after it, 3 end of the main loop (latest warp), 4 after the block barrier, 5 block end (latest
+// warp), 6 = SM id, 7 = a mark inside the prologue (K1: own ray loaded and clipped, before the first barrier; K2: tile
+// origin known), 8 = %globaltimer [ns] read right after slot 0 (ties the SM's cycle counter to the device-wide clock).
+constexpr int TL_BLOCKS = 256, TL_SLOTS = 12;
+#ifdef OSIV_TRACE
+__device__ unsigned long long g_timeline[4][TL_BLOCKS][TL_SLOTS];
+__device__ __forceinline__ void tl_stamp(int iter, int kernel, int slot, bool latest) {
+    if (blockIdx.z != 0 || blockIdx.x >= TL_BLOCKS) return;
+    unsigned long long* row = g_timeline[(iter & 1) * 2 + kernel][blockIdx.x];
+    if (latest) { if ((threadIdx.x & 31) == 0) atomicMax(&row[slot], (unsigned long long)clock64()); }
+    else if (threadIdx.x == 0) {
+        row[slot] = (unsigned long long)clock64();
+        if (slot == 0) {
+            unsigned sm; unsigned long long gt;
+            asm volatile("mov.u32 %0, %%smid;" : "=r"(sm));
+            asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(gt));
+            row[6] = sm; row[8] = gt;
+            row[3] = 0; row[5] = 0;                      // the "latest warp" slots restart for this launch
+        }
+    }
+}
+#define OSIV_TL(iter, kernel, slot, latest) tl_stamp(iter, kernel, slot, latest)
+#else
+#define OSIV_TL(iter, kernel, slot, latest) do {} while (0)
+#endif
 
 constexpr int PAD = 4;                     // zero columns left and right of every padded image line
 constexpr int PADR = 1;                    // zero rows above and below a padded image
@@ -84,6 +116,8 @@ struct FwdArgs {
     int batch;                             // slices in this launch (SB == 2: the last pair may be half empty)
     int view_shift;                        // stack of slices (H1): slice s uses the table's view (v + view_shift*s) mod V
     int rpb, segs;                         // rays per block, line segments per ray (block = rpb * segs threads, rounded up to warps)
+    unsigned rpb_magic, C_magic;           // fastdiv by rpb and by g.C
+    int iter;                              // iteration number (timeline build only)
     float* sino;                           // MODE 0: [batch][VS][C]
     const float* counts;                   // MODE 1: [batch][V][C]
     const float* blank;                    // [C] or null
@@ -104,6 +138,8 @@ struct BackArgs {
     int view_shift;                        // stack of slices (H1), as in FwdArgs
     float tv_z;                            // stack of slices (H2): > 0 adds the z term of the 3-D TV (SB == 1 only)
     int tpb, shares, ngx;                  // tiles per block, view shares, 2x2 patch groups per row of groups
+    unsigned tpb_magic, ngx_magic;         // fastdiv by tpb and by ngx
+    int iter;                              // iteration number (timeline build only)
     const int* itab;                       // [V][ntiles] candidate intervals (k_build_intervals)
     int ntiles;
     float* out;                            // MODE 0: [batch][ny][nx]
@@ -120,6 +156,10 @@ struct BackArgs {
     double tau;
     float beta_over_M, eps2;
 };
+
+// n / d for 0 <= n < 2^32 / d with the host's magic = ceil(2^32 / d) (0 for d = 1): one multiply instead of the division
+// sequence (the start-up path of both hot kernels lies on the iteration's critical path)
+__device__ __forceinline__ int fastdiv(int n, unsigned magic) { return magic ? (int)__umulhi((unsigned)n, magic) : n; }
 
 __device__ __forceinline__ size_t pad_off(const DevGeom& g, int iy, int ix) {
     return (size_t)(iy + PADR) * g.pitch + PAD + ix;
@@ -138,6 +178,11 @@ __device__ __forceinline__ size_t slice_base(const DevGeom& g, long long elems, 
 // predecessor has completed and its writes are visible, and pdl_launch_next() -- placed AFTER the wait, so that at
 // most one successor is ever resident early -- lets the successor's blocks move into the SM slots this grid frees.
 __device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+// Pins a value of the prologue in front of the wait.  ptxas treats griddepcontrol.wait (ACQBULK) like a long-latency
+// operation and hoists it to the top of its basic block -- above the constant-memory loads and the arithmetic of a
+// straight-line prologue, which then runs only after the predecessor has completed (seen in the SASS); it does not move
+// it across a warp barrier, so the value is made an operand of one.
+__device__ __forceinline__ void pdl_before_wait(int x) { asm volatile("bar.warp.sync 0xffffffff;" ::"r"(x) : "memory"); }
 __device__ __forceinline__ void pdl_launch_next() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
 
 // Packed FP32 pairs (Blackwell FFMA2: two IEEE fp32 FMAs per instruction, the scalar operand broadcast): halves the
@@ -176,24 +221,25 @@ __global__ void __launch_bounds__(FWD_MAX_THREADS, 1) k_forward(const FwdArgs a)
     typedef typename Px<SB>::T PX;
     const DevGeom& g = a.g;
     const int t = threadIdx.x, s0 = blockIdx.z * SB;             // slices s0 .. s0 + SB - 1
+    OSIV_TL(a.iter, 0, 0, false);
     const int rpb = a.rpb, segs = a.segs;
-    const int seg = t / rpb, i = t - seg * rpb;
+    const int seg = fastdiv(t, a.rpb_magic), i = t - seg * rpb;
     const int VSb = a.VS / NS, Vq = g.V / NS;
     const int R = VSb * g.C;
     const int r = blockIdx.x * rpb + i;
     const bool walker = seg < segs && r < R;
     const int rr = min(r, R - 1);
-    const int jb = rr / g.C, c = rr - jb * g.C;
+    const int jb = fastdiv(rr, a.C_magic), c = rr - jb * g.C;
     const int v = a.subset < 0 ? jb : a.subset + jb * a.M;          // base view of the orbit
     extern __shared__ float part[];                                 // [segs][NS][SB][rpb]
     __shared__ double dred[2][FWD_MAX_THREADS / 32];
     __shared__ int rng[4];                                          // line ranges of the block's row- / column-major rays
 
-    float acc[NS];                                                  // SB == 1, NS == 1
-    uint64_t acc01 = 0ull, acc23 = 0ull;                            // SB == 1, NS == 4: pairs of patterns
-    uint64_t acc2[NS];                                              // SB == 2: per pattern, the pair of slices
+    float acc[1] = {0.f};                                           // NS == 1, SB == 1
+    uint64_t acc2[1] = {0ull};                                      // NS == 1, SB == 2: the pair of slices
+    uint64_t acc4[SB][2];                                           // NS == 4: per slice, orbit rays (0, 1) and (2, 3)
 #pragma unroll
-    for (int k = 0; k < NS; ++k) { acc[k] = 0.f; acc2[k] = 0ull; }
+    for (int sl = 0; sl < SB; ++sl) { acc4[sl][0] = 0ull; acc4[sl][1] = 0ull; }
     // H1: a slice of a stack sees the gantry view_shift views further on per slice; the counts keep the acquisition index
     int vt = v;                                                     // (a real branch: the default path must not pay for the modulo)
     if (a.view_shift) { vt = v + (int)(((unsigned)a.view_shift * (unsigned)s0) % (unsigned)g.V); if (vt >= g.V) vt -= g.V; }
@@ -203,7 +249,8 @@ __global__ void __launch_bounds__(FWD_MAX_THREADS, 1) k_forward(const FwdArgs a)
         const float kk = rowmaj ? ray.x : ray.y;          // coefficient of the in-line coordinate, |kk| >= 1 (Joseph: +-1)
         const float uu = rowmaj ? ray.y : ray.x;          // coefficient of the marching coordinate (+-1; Joseph: +-1/|k|)
         const PX* bufA = rowmaj ? reinterpret_cast<const PX*>(a.img) + (size_t)blockIdx.z * g.img_elems : reinterpret_cast<const PX*>(a.imgT) + (size_t)blockIdx.z * g.imgT_elems;
-        const PX* bufB = rowmaj ? reinterpret_cast<const PX*>(a.imgT) + (size_t)blockIdx.z * g.imgT_elems : reinterpret_cast<const PX*>(a.img) + (size_t)blockIdx.z * g.img_elems;
+        // NS == 4: the orbit-interleaved image Q (rays crossing rows) or its transpose QT (rays crossing columns), SB float4 per pixel
+        const float4* qA = reinterpret_cast<const float4*>(rowmaj ? a.img : a.imgT) + (size_t)blockIdx.z * (rowmaj ? g.img_elems : g.imgT_elems) * SB;
         const int pitch = rowmaj ? g.pitch : g.pitchT;    // NS == 4: square grid, both pitches are equal
         const int na = rowmaj ? g.nx : g.ny, nb = rowmaj ? g.ny : g.nx;
         const float ca = rowmaj ? g.cx : g.cy, cb = rowmaj ? g.cy : g.cx;
@@ -221,6 +268,7 @@ __global__ void __launch_bounds__(FWD_MAX_THREADS, 1) k_forward(const FwdArgs a)
         // pixel outside the image: the clamped index lands in the zero padding and the term vanishes.
         // (Row-major and column-major rays of one block form two such unions: their lines are different things.)
         if (t < 4) rng[t] = (t & 1) ? -1 : (1 << 30);
+        OSIV_TL(a.iter, 0, 7, false);
         __syncthreads();
         {
             const int big = 1 << 30;
@@ -241,73 +289,88 @@ __global__ void __launch_bounds__(FWD_MAX_THREADS, 1) k_forward(const FwdArgs a)
         const int j1 = min(j0 + len, wlo + nsteps);
         const int imax = na + PAD - 2;
         int offP = (j0 + PADR) * pitch + PAD;                 // line j, walking up
-        int offM = (nb - 1 - j0 + PADR) * pitch + PAD;        // line nb-1-j, walking down
         float bf = (float)j0 - cb;
+        OSIV_TL(a.iter, 0, 1, false);
         pdl_wait();                                           // mu(n) is the previous launch's output
         pdl_launch_next();
-        // Two lines per trip, written so that all 2 x 2 x NS gathers of a trip are in flight together: the walk is
-        // bound by load latency.  The odd line past j1 (only in the last trip) gets zero weights; its addresses stay
-        // inside the padded buffers because j1 <= nb.
-        for (int jj = j0; jj < j1; jj += 2, offP += 2 * pitch, offM -= 2 * pitch, bf += 2.f) {
+        OSIV_TL(a.iter, 0, 2, false);
+        // Two lines per trip, written so that all gathers of a trip are in flight together: the walk is bound by the
+        // load path.  The odd line past j1 (only in the last trip) gets zero weights; its addresses stay inside the
+        // padded buffers because j1 <= nb.
+        // floor() by the add-a-big-number trick (|t| < 2^22; FRND/F2I run at a quarter of the FP32 rate): r = t - 1/2 +
+        // 1.5 * 2^23 rounds to the nearest integer, which is floor(t) unless t is an integer n, where it may be n - 1:
+        // then pixels n - 1 and n are taken instead of n and n + 1, and both left-out pixels are a whole pixel away
+        // from the crossing (weight 0 in either model).
+        constexpr float BIG = 12582912.f;
+        for (int jj = j0; jj < j1; jj += 2, offP += 2 * pitch, bf += 2.f) {
             float w[2][2];
             int i0[2];
 #pragma unroll
             for (int u = 0; u < 2; ++u) {
                 const float bg = fmaf(uu, bf + (float)u, ray.z);
-                const float fa = floorf(fmaf(-bg, invk, ca));     // index of the pixel left of the crossing
+                const float r = (fmaf(-bg, invk, ca) - 0.5f) + BIG;
+                const float fa = r - BIG;                         // index of the pixel left of the crossing
                 const float q0 = fmaf(kk, fa - ca, bg);
                 const float q1 = q0 + kk;
                 w[u][0] = __saturatef(hk - fabsf(q0));
                 w[u][1] = __saturatef(hk - fabsf(q1));
-                i0[u] = min(max((int)fa, -PAD), imax);
+                i0[u] = min(max(__float_as_int(r) - 0x4B400000, -PAD), imax);
             }
             if (jj + 1 >= j1) { w[1][0] = 0.f; w[1][1] = 0.f; }
-            PX x[2][NS][2];
+            if constexpr (NS == 4) {
+                // one float4 per pixel and slice = the pixel in the four rotated positions: component k belongs to ray
+                // (v + k V/4, c) of the orbit, with the same weight
+                float4 x[2][2][SB];
 #pragma unroll
-            for (int u = 0; u < 2; ++u) {
-                const int oP = offP + u * pitch, oM = offM - u * pitch;
-                const PX* p0 = bufA + (oP + i0[u]);
-                x[u][0][0] = __ldg(p0); x[u][0][1] = __ldg(p0 + 1);
-                if (NS == 4) {
-                    const int ir = na - 2 - i0[u];                // mirrored index of pixel i0+1
-                    const PX* p1 = bufB + (oM + i0[u]);        // pattern 1: other copy, line nb-1-j, same order
-                    const PX* p2 = bufA + (oM + ir);           // pattern 2: same copy, line nb-1-j, mirrored
-                    const PX* p3 = bufB + (oP + ir);           // pattern 3: other copy, line j, mirrored
-                    x[u][1 % NS][0] = __ldg(p1); x[u][1 % NS][1] = __ldg(p1 + 1);
-                    x[u][2 % NS][0] = __ldg(p2); x[u][2 % NS][1] = __ldg(p2 + 1);
-                    x[u][3 % NS][0] = __ldg(p3); x[u][3 % NS][1] = __ldg(p3 + 1);
+                for (int u = 0; u < 2; ++u) {
+                    const float4* p0 = qA + (size_t)(offP + u * pitch + i0[u]) * SB;
+#pragma unroll
+                    for (int e = 0; e < 2; ++e)
+#pragma unroll
+                        for (int sl = 0; sl < SB; ++sl) x[u][e][sl] = __ldg(p0 + e * SB + sl);
                 }
-            }
 #pragma unroll
-            for (int u = 0; u < 2; ++u) {
-                if constexpr (SB == 2) {                          // per pattern, the two slices as an FFMA2 pair
+                for (int u = 0; u < 2; ++u)
 #pragma unroll
-                    for (int k = 0; k < NS; ++k) {
-                        const float wa = k < 2 ? w[u][0] : w[u][1], wb = k < 2 ? w[u][1] : w[u][0];   // patterns 2, 3 walk mirrored
-                        ffma2(acc2[k], pack2(x[u][k][0].x, x[u][k][0].y), wa);
-                        ffma2(acc2[k], pack2(x[u][k][1].x, x[u][k][1].y), wb);
+                    for (int e = 0; e < 2; ++e)
+#pragma unroll
+                        for (int sl = 0; sl < SB; ++sl) {
+                            ffma2(acc4[sl][0], pack2(x[u][e][sl].x, x[u][e][sl].y), w[u][e]);
+                            ffma2(acc4[sl][1], pack2(x[u][e][sl].z, x[u][e][sl].w), w[u][e]);
+                        }
+            } else {
+                PX x[2][2];
+#pragma unroll
+                for (int u = 0; u < 2; ++u) {
+                    const PX* p0 = bufA + (offP + u * pitch + i0[u]);
+                    x[u][0] = __ldg(p0); x[u][1] = __ldg(p0 + 1);
+                }
+#pragma unroll
+                for (int u = 0; u < 2; ++u) {
+                    if constexpr (SB == 2) {                      // the two slices as an FFMA2 pair
+                        ffma2(acc2[0], pack2(x[u][0].x, x[u][0].y), w[u][0]);
+                        ffma2(acc2[0], pack2(x[u][1].x, x[u][1].y), w[u][1]);
+                    } else {
+                        acc[0] = fmaf(w[u][0], x[u][0], acc[0]);
+                        acc[0] = fmaf(w[u][1], x[u][1], acc[0]);
                     }
-                } else if constexpr (NS == 4) {                   // (acc0, acc1) and (acc2, acc3) as FFMA2 pairs
-                    ffma2(acc01, pack2(x[u][0][0], x[u][1 % NS][0]), w[u][0]);
-                    ffma2(acc01, pack2(x[u][0][1], x[u][1 % NS][1]), w[u][1]);
-                    ffma2(acc23, pack2(x[u][2 % NS][0], x[u][3 % NS][0]), w[u][1]);
-                    ffma2(acc23, pack2(x[u][2 % NS][1], x[u][3 % NS][1]), w[u][0]);
-                } else {
-                    acc[0] = fmaf(w[u][0], x[u][0][0], acc[0]);
-                    acc[0] = fmaf(w[u][1], x[u][0][1], acc[0]);
                 }
             }
         }
     }
-    // this thread's sums: fin[pattern][slice of the block]
+    OSIV_TL(a.iter, 0, 3, true);
+    // this thread's sums: fin[ray of the orbit][slice of the block]
     float fin[NS][SB];
-    if constexpr (SB == 2) {
+    if constexpr (NS == 4) {
 #pragma unroll
-        for (int k = 0; k < NS; ++k) unpack2(acc2[k], fin[k][0], fin[k][SB - 1]);
+        for (int sl = 0; sl < SB; ++sl) {
+            unpack2(acc4[sl][0], fin[0][sl], fin[1 % NS][sl]);
+            unpack2(acc4[sl][1], fin[2 % NS][sl], fin[3 % NS][sl]);
+        }
+    } else if constexpr (SB == 2) {
+        unpack2(acc2[0], fin[0][0], fin[0][SB - 1]);
     } else {
-        if (NS == 4) { unpack2(acc01, acc[0], acc[1 % NS]); unpack2(acc23, acc[2 % NS], acc[3 % NS]); }
-#pragma unroll
-        for (int k = 0; k < NS; ++k) fin[k][0] = acc[k];
+        fin[0][0] = acc[0];
     }
     if (seg < segs) {
 #pragma unroll
@@ -327,6 +390,7 @@ __global__ void __launch_bounds__(FWD_MAX_THREADS, 1) k_forward(const FwdArgs a)
         ib = __ldg(a.inv_bref);
     }
     __syncthreads();
+    OSIV_TL(a.iter, 0, 4, false);
     const int nw = (ne * rpb + 31) / 32;                      // epilogue warps
     if (t >= 32 * nw) return;
 
@@ -335,16 +399,23 @@ __global__ void __launch_bounds__(FWD_MAX_THREADS, 1) k_forward(const FwdArgs a)
     for (int sl = 0; sl < SB; ++sl) d2[sl] = 0.0;
     if (epi) {
         for (int ko = seg; ko < NS; ko += ne) {
-            // pattern -> rotation (patterns 1 and 3 swap for a column-major base ray: R maps its walk onto the other
-            // copy with the mirrored index first)
-            const int pk = (NS == 4 && !rowmaj && (ko & 1)) ? 4 - ko : ko;
+            const int pk = ko;
 #pragma unroll
             for (int sl = 0; sl < SB; ++sl) {
                 const int s = s0 + sl;
                 if (s >= a.batch) break;
-                float x = 0.f;                                    // sum over the ray's segments in a fixed order
-                for (int q = 0; q < segs; ++q) x += part[((q * NS + pk) * SB + sl) * rpb + i];
-                const float l = h * x;
+                // sum over the ray's segments in a fixed order: four interleaved partial sums, so that the loads do not
+                // wait for one another
+                float xs[4] = {0.f, 0.f, 0.f, 0.f};
+                const float* pp = part + (pk * SB + sl) * rpb + i;
+                const int stride = NS * SB * rpb;
+                int q = 0;
+                for (; q + 4 <= segs; q += 4) {
+#pragma unroll
+                    for (int e = 0; e < 4; ++e) xs[e] += pp[(q + e) * stride];
+                }
+                for (; q < segs; ++q) xs[0] += pp[q * stride];
+                const float l = h * ((xs[0] + xs[1]) + (xs[2] + xs[3]));
                 if (MODE == 0) {
                     a.sino[((size_t)s * a.VS + jb + ko * VSb) * g.C + c] = l;
                 } else {
@@ -370,12 +441,17 @@ __global__ void __launch_bounds__(FWD_MAX_THREADS, 1) k_forward(const FwdArgs a)
             if ((t & 31) == 0) dred[sl][t >> 5] = d2[sl];
         }
         asm volatile("bar.sync 1, %0;" ::"r"(32 * nw) : "memory");     // only the epilogue warps meet here
-        if (t < SB && s0 + t < a.batch) {
-            double D = 0.0;
-            for (int w = 0; w < nw; ++w) D += dred[t][w];
-            a.dparts[(size_t)(s0 + t) * gridDim.x + blockIdx.x] = D;
+        if (t < 32) {                                                  // warp 0: the warp sums in a fixed (butterfly) order
+#pragma unroll
+            for (int sl = 0; sl < SB; ++sl) {
+                double D = t < nw ? dred[sl][t] : 0.0;
+#pragma unroll
+                for (int off = 16; off > 0; off >>= 1) D += __shfl_xor_sync(0xffffffffu, D, off);
+                if (t == 0 && s0 + sl < a.batch) a.dparts[(size_t)(s0 + sl) * gridDim.x + blockIdx.x] = D;
+            }
         }
     }
+    OSIV_TL(a.iter, 0, 5, true);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -505,6 +581,36 @@ __device__ __forceinline__ void tv_grad_tile3(const float (&m)[4][4], const floa
         }
 }
 
+// Quarter-turn path: value and TV gradient (C8) of pixel R^K P from the 3x3 neighbourhood E of orbit float4s around the
+// base pixel P = (px, py):  E[1+dy][1+dx] = {mu(P'), mu(RP'), mu(R^2P'), mu(R^3P')}, P' = P + (dx, dy).  The neighbour of
+// R^K P at image offset (a, b) is R^K (P + R^-K (a, b)), i.e. component K of the entry at base offset R^-K (a, b).
+template <int K> __device__ __forceinline__ float orbit_comp(const float4& v) { return K == 0 ? v.x : K == 1 ? v.y : K == 2 ? v.z : v.w; }
+template <int K> __device__ __forceinline__ float orbit_nb(const float4 (&E)[3][3], int a, int b) {
+    const int dx = K == 0 ? a : K == 1 ? b : K == 2 ? -a : -b;
+    const int dy = K == 0 ? b : K == 1 ? -a : K == 2 ? -b : a;
+    return orbit_comp<K>(E[1 + dy][1 + dx]);
+}
+template <int K>
+__device__ __forceinline__ void orbit_tv(const float4 (&E)[3][3], int px, int py, int N, float eps2, float& cur, float& grad) {
+    const int x = K == 0 ? px : K == 1 ? N - 1 - py : K == 2 ? N - 1 - px : py;        // R^K P
+    const int y = K == 0 ? py : K == 1 ? px : K == 2 ? N - 1 - py : N - 1 - px;
+    const bool hx1 = x + 1 < N, hy1 = y + 1 < N;
+    const float c = orbit_nb<K>(E, 0, 0);
+    const float dxc = hx1 ? orbit_nb<K>(E, 1, 0) - c : 0.f, dyc = hy1 ? orbit_nb<K>(E, 0, 1) - c : 0.f;
+    float sgrad = 0.f;
+    if (x > 0) {                                                     // cell (x-1, y)
+        const float l = orbit_nb<K>(E, -1, 0), dxl = c - l, dyl = hy1 ? orbit_nb<K>(E, -1, 1) - l : 0.f;
+        sgrad += dxl * rsqrtf(eps2 + dxl * dxl + dyl * dyl);
+    }
+    if (y > 0) {                                                     // cell (x, y-1)
+        const float d = orbit_nb<K>(E, 0, -1), dyb = c - d, dxb = hx1 ? orbit_nb<K>(E, 1, -1) - d : 0.f;
+        sgrad += dyb * rsqrtf(eps2 + dxb * dxb + dyb * dyb);
+    }
+    sgrad -= (dxc + dyc) * rsqrtf(eps2 + dxc * dxc + dyc * dyc);
+    cur = c;
+    grad = sgrad;
+}
+
 __device__ __forceinline__ void load_nbhd(const DevGeom& g, const float* img, int x0, int y0, float (&m)[4][4]) {
 #pragma unroll
     for (int r = 0; r < 4; ++r) {
@@ -615,12 +721,15 @@ __device__ __forceinline__ void back_load(const float* const (&sp)[SB], int u, f
 // k of the tile (TV gradient, update, stores).  The host sizes the grid to one block per SM (plan_back).
 // ------------------------------------------------------------------------------------------------
 // tile number -> patch (8 x 4 tiles; patches grouped 2 x 2, groups row-major) -> origin (x0, y0) of the 2x2-pixel tile
-__device__ __forceinline__ void tile_origin(int T, int ngx, int& x0, int& y0) {
+__device__ __forceinline__ void tile_origin(int T, int ngx, unsigned ngx_magic, int& x0, int& y0) {
     const int patch = T >> 5, w = T & 31;
     const int grp = patch >> 2, sub = patch & 3;
-    const int gy = grp / ngx, gx = grp - gy * ngx;
-    x0 = (((gx << 1) + (sub & 1)) * BK_WX + (w & (BK_WX - 1))) * BK_TX;
-    y0 = (((gy << 1) + (sub >> 1)) * BK_WY + (w / BK_WX)) * BK_TY;
+    const int gy = fastdiv(grp, ngx_magic), gx = grp - gy * ngx;
+    // inside the patch a quarter-warp (8 lanes: the unit in which a 16-byte load is served) covers 4 x 2 tiles, the four
+    // quarter-warps 2 x 2 such blocks: its lanes' candidate windows then lie closer together than along a row of 8 tiles
+    const int wx = (w & 3) + ((w >> 3) & 1) * 4, wy = ((w >> 2) & 1) + (w >> 4) * 2;
+    x0 = (((gx << 1) + (sub & 1)) * BK_WX + wx) * BK_TX;
+    y0 = (((gy << 1) + (sub >> 1)) * BK_WY + wy) * BK_TY;
 }
 
 // Candidate interval of the tile at (x0, y0) in table view v: the channels whose ray can cross the tile form the interval
@@ -645,13 +754,30 @@ __device__ __forceinline__ int tile_interval(const DevGeom& g, int x0, int y0, i
 
 // A0 for K2: the intervals of every (view, tile) once per handle and orbit size -- they depend on the geometry only, and
 // worked out inside K2 they were a sixth of its instructions and most of its start-up path.  tab [V][ntiles].
-__global__ void __launch_bounds__(256) k_build_intervals(DevGeom g, int ns, int ngx, int ntiles, int* __restrict__ tab) {
+// The bound of tile_interval is then narrowed to the tile's exact support: the first and last channel of it for which
+// K2's own weight expression (back_weights, the same float operations on the same table entry) gives a non-zero weight
+// to one of the tile's pixels; every candidate outside contributes exactly 0, so leaving it out changes no bit, and
+// the candidate loop -- bound by the load path, two 16-byte loads per candidate -- gets about a fifth shorter.
+__global__ void __launch_bounds__(256) k_build_intervals(DevGeom g, int ns, int ngx, unsigned ngx_magic, int ntiles, int* __restrict__ tab) {
     const int T = blockIdx.x * 256 + threadIdx.x, v = blockIdx.y;
     if (T >= ntiles) return;
     int x0, y0;
-    tile_origin(T, ngx, x0, y0);
+    tile_origin(T, ngx, ngx_magic, x0, y0);
     const int xlim = ns == 4 ? (g.nx >> 1) : g.nx, ylim = ns == 4 ? (g.ny >> 1) : g.ny;
-    tab[(size_t)v * ntiles + T] = (x0 < xlim && y0 < ylim) ? tile_interval(g, x0, y0, v) : g.C;
+    int packed = g.C;
+    if (x0 < xlim && y0 < ylim) {
+        const int loose = tile_interval(g, x0, y0, v);
+        const int c_lo = loose & 0xfffff, n = loose >> 20;
+        const float xc0 = (float)x0 - g.cx, yc0 = (float)y0 - g.cy;
+        int first = -1, last = -1;
+        for (int u = 0; u < n; ++u) {
+            float w[4];
+            back_weights(__ldg(&g.rays[(size_t)v * g.C + c_lo + u]), xc0, yc0, w);
+            if (w[0] > 0.f || w[1] > 0.f || w[2] > 0.f || w[3] > 0.f) { if (first < 0) first = u; last = u; }
+        }
+        if (first >= 0) packed = (c_lo + first) | ((last - first + 1) << 20);
+    }
+    tab[(size_t)v * ntiles + T] = packed;
 }
 
 // STACK == 1 (SB == 1 only): the slices of the launch form a volume (readings H1-H3) -- per-slice view shift and the z
@@ -660,14 +786,15 @@ template <int MODE, int NS, int SB, int STACK>
 __global__ void __launch_bounds__(SB == 1 ? BK_MAX_THREADS : BKB_MAX_THREADS, SB == 1 ? 1 : 2) k_back(const BackArgs a) {
     const DevGeom& g = a.g;
     const int t = threadIdx.x, lane = t & 31, s0 = blockIdx.z * SB;       // slices s0 .. s0 + SB - 1
+    OSIV_TL(a.iter, 1, 0, false);
     const int tpb = a.tpb, shares = a.shares;
-    const int q = t / tpb, i = t - q * tpb;
-    extern __shared__ float red[];                        // [SB][shares][NS * 4][tpb]
+    const int q = fastdiv(t, a.tpb_magic), i = t - q * tpb;
+    extern __shared__ float red[];                        // NS == 4: [SB][4 pixels][shares][tpb] float4 (the 4 rotations); NS == 1: [SB][shares][4][tpb]
 
     const int xlim = NS == 4 ? (g.nx >> 1) : g.nx, ylim = NS == 4 ? (g.ny >> 1) : g.ny;
     int x0, y0;
     const int T = blockIdx.x * tpb + i;
-    tile_origin(T, a.ngx, x0, y0);
+    tile_origin(T, a.ngx, a.ngx_magic, x0, y0);
     const bool active = q < shares && x0 < xlim && y0 < ylim;
 
     // acc[m][ty*2+tx]: NS == 4: m = component of the orbit's residual float4 (this thread's views all lie in quarter
@@ -676,6 +803,7 @@ __global__ void __launch_bounds__(SB == 1 ? BK_MAX_THREADS : BKB_MAX_THREADS, SB
 #pragma unroll
     for (int j = 0; j < SB; ++j) acc[j].clear();
 
+    OSIV_TL(a.iter, 1, 7, false);
     const int VSb = a.VS / NS;
     const int vshift = STACK ? (int)(((unsigned)a.view_shift * (unsigned)s0) % (unsigned)g.V) : 0;
     const int quarter = NS == 4 ? (q & 3) : 0;
@@ -691,32 +819,51 @@ __global__ void __launch_bounds__(SB == 1 ? BK_MAX_THREADS : BKB_MAX_THREADS, SB
         // candidate in the ray table and in the residual rows, and the warp's candidate count.  The warp runs
         // max-over-lanes candidates in lock step (no remainder code); a lane's extra candidates have zero weight (the
         // ray misses its tile) or read the zero columns C..Cp-1 of res, and a lane that is off reads only those.
-        auto interval = [&](int it, int& offR, int& offS) -> int {
-            const int jbr = jfirst + it * jstep;
-            const bool on = active && jbr < VSb;
-            const int jb = min(jbr, VSb - 1);
+        // Trips are taken four at a time.  Their packed intervals are plain loads from the table (unconditional, index
+        // clamped: four loads in flight, nothing from K1 needed, so the first four are fetched and decoded before the
+        // wait, and the next four while the current ones are walked); the candidates of two trips are then walked
+        // together, which keeps 2 x 2 x 2 sixteen-byte loads in flight per thread.
+        const int Tc = min(T, a.ntiles - 1);
+        auto trip_view = [&](int it, int& jb) -> int {           // table view of trip `it` of this thread's share
+            jb = min(jfirst + it * jstep, VSb - 1);
             const int jj = jb + quarter * VSb;
             int v = a.subset < 0 ? jj : a.subset + jj * a.M;
-            if (STACK) { v += vshift; if (v >= g.V) v -= g.V; }      // H1: the table's view
-            const int packed = on ? __ldg(&a.itab[(size_t)v * a.ntiles + T]) : g.C;      // k_build_intervals
-            const int c_lo = packed & 0xfffff;
+            if (STACK) { v += vshift; if (v >= g.V) v -= g.V; }      // H1
+            return v;
+        };
+        auto fetch = [&](int it) -> int {                        // k_build_intervals' entry, or "empty" (first channel C, count 0)
+            int jb;
+            const int v = trip_view(it, jb);
+            const int pk = __ldg(&a.itab[(size_t)v * a.ntiles + Tc]);
+            return (active && jfirst + it * jstep < VSb) ? pk : g.C;
+        };
+        auto decode = [&](int it, int pk, int& offR, int& offS) -> int {
+            int jb;
+            const int v = trip_view(it, jb);
+            const int c_lo = pk & 0xfffff;
             offR = v * g.C + c_lo;
             offS = jb * a.Cp + c_lo;
-            return __reduce_max_sync(0xffffffffu, packed >> 20);
+            return __reduce_max_sync(0xffffffffu, pk >> 20);
         };
-        // Trips are taken four at a time: the four intervals are independent chains of arithmetic, and the first four
-        // need nothing from K1, so they are worked out before the wait; the candidates of two trips are then walked
-        // together, which keeps 2 x 2 x 2 sixteen-byte loads in flight per thread.
         constexpr int CH = 4;
-        int offR[CH], offS[CH], ncw[CH];
+        int offR[CH], offS[CH], ncw[CH], pk[CH];
+#pragma unroll
+        for (int e = 0; e < CH; ++e) pk[e] = e < ntrips ? fetch(e) : g.C;
 #pragma unroll
         for (int e = 0; e < CH; ++e) {
-            offR[e] = offS[e] = 0; ncw[e] = 0;
-            if (e < ntrips) ncw[e] = interval(e, offR[e], offS[e]);
+            ncw[e] = decode(e, pk[e], offR[e], offS[e]);
+            pdl_before_wait(ncw[e]);
         }
+        OSIV_TL(a.iter, 1, 1, false);
         pdl_wait();                                              // the residuals are the previous launch's output
         pdl_launch_next();
+        OSIV_TL(a.iter, 1, 2, false);
         for (int it0 = 0;;) {
+            const bool more = it0 + CH < ntrips;                 // warp-uniform
+            if (more) {
+#pragma unroll
+                for (int e = 0; e < CH; ++e) pk[e] = it0 + CH + e < ntrips ? fetch(it0 + CH + e) : g.C;
+            }
 #pragma unroll
             for (int e = 0; e < CH; e += 2) {
                 const float4* rpA = g.rays + offR[e];
@@ -785,228 +932,234 @@ __global__ void __launch_bounds__(SB == 1 ? BK_MAX_THREADS : BKB_MAX_THREADS, SB
                     }
                 }
             }
+            if (!more) break;
             it0 += CH;
-            if (it0 >= ntrips) break;
 #pragma unroll
-            for (int e = 0; e < CH; ++e) {
-                ncw[e] = 0;
-                if (it0 + e < ntrips) ncw[e] = interval(it0 + e, offR[e], offS[e]);
+            for (int e = 0; e < CH; ++e) ncw[e] = decode(it0 + e, pk[e], offR[e], offS[e]);
+        }
+    }
+    OSIV_TL(a.iter, 1, 3, true);
+    // The shares' sums meet in shared memory: red[slice j][share q][rotation k][pixel p][tile i]; rotation k of the tile
+    // collects component (quarter + k) % 4 of the orbit's residuals  <=>  component m feeds rotation (m - quarter) % 4.
+    if (q < shares) {
+#pragma unroll
+        for (int j = 0; j < SB; ++j) {
+            if constexpr (NS == 4) {
+                float4* red4 = reinterpret_cast<float4*>(red);
+#pragma unroll
+                for (int p = 0; p < 4; ++p) {
+                    float r4[4];
+#pragma unroll
+                    for (int m = 0; m < 4; ++m) r4[(m - quarter) & 3] = acc[j].get(m, p);
+                    red4[((j * 4 + p) * shares + q) * tpb + i] = make_float4(r4[0], r4[1], r4[2], r4[3]);
+                }
+            } else {
+#pragma unroll
+                for (int p = 0; p < 4; ++p) red[((j * shares + q) * 4 + p) * tpb + i] = acc[j].get(0, p);
             }
         }
     }
-    if constexpr (SB == 1) {                               // one slice per block: scalars (the register budget is tight)
-        const int s = s0;
-        // rotation k of the tile = orbit component (quarter + k) % 4  <=>  component m feeds rotation (m - quarter) % 4
-        if (q < shares) {
-#pragma unroll
-            for (int m = 0; m < NS; ++m)
-#pragma unroll
-                for (int p = 0; p < 4; ++p) red[(q * (NS * 4) + ((m - quarter) & (NS - 1)) * 4 + p) * tpb + i] = acc[0].get(m, p);
-        }
+    const bool tile_ok = x0 < xlim && y0 < ylim;
 
-        // thread (tile i, k = q < NS) finishes rotation k of the base tile: origin (xk, yk) and, below, where base pixel
-        // (tx,ty) lands.  Everything that does not depend on the other shares' sums -- monitor, step rule, neighbourhood
-        // of mu(n), TV gradient -- is done before the barrier, so that its loads overlap the wait for the slowest warp.
-        const bool fin = q < NS;
-        const bool fin_active = fin && x0 < xlim && y0 < ylim;
-        const int k = q;
-        int xk = x0, yk = y0;
-        if (NS == 4) {
-            const int N = g.nx;
-            if (k == 1)      { xk = N - 2 - y0; yk = x0; }
-            else if (k == 2) { xk = N - 2 - x0; yk = N - 2 - y0; }
-            else if (k == 3) { xk = y0;         yk = N - 2 - x0; }
+    if constexpr (NS == 4) {
+        // ---- quarter-turn path: thread (tile i, p = q < 4) finishes base pixel p of the tile in all four rotations.
+        // Everything that does not depend on the other shares' sums -- monitor, step rule, the 3x3 neighbourhood of
+        // float4s of mu(n) (= the neighbourhoods of all four rotated pixels), TV gradient -- is done before the
+        // barrier, so that its loads overlap the wait for the slowest warp.
+        const bool fin_active = q < 4 && tile_ok;
+        const int N = g.nx;
+        const int px = x0 + (q & 1), py = y0 + ((q >> 1) & 1);      // base pixel P (q < 4)
+        StepInfo si[SB];
+        float step[SB], cur[SB][4], tv[SB][4];
+        if (MODE == 1 && t < 32 * ((4 * tpb + 31) / 32)) {           // whole warps: step_rule shuffles
+            const bool writer = blockIdx.x == 0 && t < 32;
+#pragma unroll
+            for (int j = 0; j < SB; ++j) {
+                const int s = s0 + j;
+                if (s >= a.batch) break;
+                float4 E[3][3];
+                if (fin_active) {
+                    const float4* Q = reinterpret_cast<const float4*>(a.img) + (size_t)blockIdx.z * g.img_elems * SB + j;
+#pragma unroll
+                    for (int dy = 0; dy < 3; ++dy)
+#pragma unroll
+                        for (int dx = 0; dx < 3; ++dx) E[dy][dx] = __ldg(Q + (size_t)((py + dy - 1 + PADR) * g.pitch + PAD + px + dx - 1) * SB);
+                }
+                si[j] = step_rule(a, s, lane, writer);
+                step[j] = (float)(si[j].lambda * a.tau);
+                if (fin_active) {                                    // A5 for R^k P, k = 0..3
+                    orbit_tv<0>(E, px, py, N, a.eps2, cur[j][0], tv[j][0]);
+                    orbit_tv<1>(E, px, py, N, a.eps2, cur[j][1], tv[j][1]);
+                    orbit_tv<2>(E, px, py, N, a.eps2, cur[j][2], tv[j][2]);
+                    orbit_tv<3>(E, px, py, N, a.eps2, cur[j][3], tv[j][3]);
+                }
+            }
         }
+        __syncthreads();
+        OSIV_TL(a.iter, 1, 4, false);
+        if (!fin_active) return;
+        // the four rotated positions of P: R^k P
+        const int rx[4] = {px, N - 1 - py, N - 1 - px, py}, ry[4] = {py, px, N - 1 - py, N - 1 - px};
+#pragma unroll
+        for (int j = 0; j < SB; ++j) {
+            const int s = s0 + j;
+            if (s >= a.batch) break;
+            float gsum[4] = {0.f, 0.f, 0.f, 0.f};                    // g at R^k P: sums over the view shares, fixed order
+            const float4* rp = reinterpret_cast<const float4*>(red) + (size_t)(j * 4 + q) * shares * tpb + i;
+#pragma unroll 4
+            for (int qq = 0; qq < shares; ++qq, rp += tpb) {
+                const float4 v = *rp;
+                gsum[0] += v.x; gsum[1] += v.y; gsum[2] += v.z; gsum[3] += v.w;
+            }
+            if constexpr (MODE == 0) {
+                float* out = a.out + (size_t)s * N * N;
+#pragma unroll
+                for (int k = 0; k < 4; ++k) out[(size_t)ry[k] * N + rx[k]] = gsum[k];
+            } else {
+            // ---- A6 update (Eq. 3) with mu > 0; the new float4 of R^k P is the orbit read from k on
+            float un[4];
+#pragma unroll
+            for (int k = 0; k < 4; ++k) un[k] = fmaxf(fmaf(step[j], gsum[k] - a.beta_over_M * tv[j][k], cur[j][k]), 0.f);
+            float4* Qn = reinterpret_cast<float4*>(a.img_new) + (size_t)blockIdx.z * g.img_elems * SB + j;
+            float4* QTn = reinterpret_cast<float4*>(a.imgT_new) + (size_t)blockIdx.z * g.imgT_elems * SB + j;
+#pragma unroll
+            for (int k = 0; k < 4; ++k) {
+                const float4 v = make_float4(un[k], un[(k + 1) & 3], un[(k + 2) & 3], un[(k + 3) & 3]);
+                Qn[pad_off(g, ry[k], rx[k]) * SB] = v;
+                QTn[padT_off(g, rx[k], ry[k]) * SB] = v;
+            }
+            if (a.best && si[j].improved) {                          // A7: mu(n) had the smallest monitor so far
+                float* best = a.best + (size_t)s * N * N;
+#pragma unroll
+                for (int k = 0; k < 4; ++k) best[(size_t)ry[k] * N + rx[k]] = cur[j][k];
+            }
+            }
+        }
+        OSIV_TL(a.iter, 1, 5, true);
+    } else if constexpr (SB == 1) {                        // general path, one slice per block: scalars (the register budget is tight)
+        const int s = s0;
+        // thread (tile i, share 0) finishes the tile.  Everything that does not depend on the other shares' sums --
+        // monitor, step rule, neighbourhood of mu(n), TV gradient -- is done before the barrier, so that its loads
+        // overlap the wait for the slowest warp.
+        const bool fin_active = q == 0 && tile_ok;
         StepInfo si;
         float step = 0.f;
         float m[4][4], tv[2][2];
-        if (MODE == 1 && t < 32 * ((NS * tpb + 31) / 32)) {           // whole warps: step_rule shuffles
+        if (MODE == 1 && t < 32 * ((tpb + 31) / 32)) {               // whole warps: step_rule shuffles
             const bool writer = blockIdx.x == 0 && t < 32;
-            if (fin_active) load_nbhd(g, a.img + (size_t)s * g.img_elems, xk, yk, m);
+            if (fin_active) load_nbhd(g, a.img + (size_t)s * g.img_elems, x0, y0, m);
             si = step_rule(a, s, lane, writer);
             step = (float)(si.lambda * a.tau);
             if (fin_active) {
                 if (STACK && a.tv_z > 0.f) {                        // stack of slices: the z term needs slices s-1 and s+1
                     const bool has_up = s + 1 < a.batch, has_dn = s > 0;
                     float up[4][4], dn[4][4];
-                    load_nbhd(g, a.img + (size_t)(has_up ? s + 1 : s) * g.img_elems, xk, yk, up);
-                    load_nbhd(g, a.img + (size_t)(has_dn ? s - 1 : s) * g.img_elems, xk, yk, dn);
-                    tv_grad_tile3(m, up, dn, has_up, has_dn, a.tv_z, xk, yk, g.nx, g.ny, a.eps2, tv);
+                    load_nbhd(g, a.img + (size_t)(has_up ? s + 1 : s) * g.img_elems, x0, y0, up);
+                    load_nbhd(g, a.img + (size_t)(has_dn ? s - 1 : s) * g.img_elems, x0, y0, dn);
+                    tv_grad_tile3(m, up, dn, has_up, has_dn, a.tv_z, x0, y0, g.nx, g.ny, a.eps2, tv);
                 } else {
-                    tv_grad_tile(m, xk, yk, g.nx, g.ny, a.eps2, tv);
+                    tv_grad_tile(m, x0, y0, g.nx, g.ny, a.eps2, tv);
                 }
             }
         }
         __syncthreads();
         if (!fin_active) return;
-
-        {
-            // sums over the view shares, fixed order
-            float b[4];
+        float b[4];                                                  // sums over the view shares, fixed order
 #pragma unroll
-            for (int p = 0; p < 4; ++p) {
-                float x = 0.f;
-                for (int qq = 0; qq < shares; ++qq) x += red[(qq * (NS * 4) + k * 4 + p) * tpb + i];
-                b[p] = x;
-            }
-            float o00 = b[0], o01 = b[1], o10 = b[2], o11 = b[3];
-            if (NS == 4) {
-                if (k == 1)      { o00 = b[2]; o01 = b[0]; o10 = b[3]; o11 = b[1]; }
-                else if (k == 2) { o00 = b[3]; o01 = b[2]; o10 = b[1]; o11 = b[0]; }
-                else if (k == 3) { o00 = b[1]; o01 = b[3]; o10 = b[0]; o11 = b[2]; }
-            }
-            const bool vx1 = xk + 1 < g.nx, vy1 = yk + 1 < g.ny;
-            if (MODE == 0) {
-                float* out = a.out + (size_t)s * g.nx * g.ny;
-                out[(size_t)yk * g.nx + xk] = o00;
-                if (vx1) out[(size_t)yk * g.nx + xk + 1] = o01;
-                if (vy1) out[(size_t)(yk + 1) * g.nx + xk] = o10;
-                if (vx1 && vy1) out[(size_t)(yk + 1) * g.nx + xk + 1] = o11;
-                return;
-            }
-
-            // ---- A5 TV gradient of mu(n), A6 update (Eq. 3) with mu > 0, A7 best copy ----
-            const float u00 = fmaxf(fmaf(step, o00 - a.beta_over_M * tv[0][0], m[1][1]), 0.f);
-            const float u01 = fmaxf(fmaf(step, o01 - a.beta_over_M * tv[0][1], m[1][2]), 0.f);
-            const float u10 = fmaxf(fmaf(step, o10 - a.beta_over_M * tv[1][0], m[2][1]), 0.f);
-            const float u11 = fmaxf(fmaf(step, o11 - a.beta_over_M * tv[1][1], m[2][2]), 0.f);
-
-            float* nimg = a.img_new + (size_t)s * g.img_elems;
-            float* nimgT = a.imgT_new + (size_t)s * g.imgT_elems;
-            nimg[pad_off(g, yk, xk)] = u00;
-            nimgT[padT_off(g, xk, yk)] = u00;
-            if (vx1) { nimg[pad_off(g, yk, xk + 1)] = u01; nimgT[padT_off(g, xk + 1, yk)] = u01; }
-            if (vy1) { nimg[pad_off(g, yk + 1, xk)] = u10; nimgT[padT_off(g, xk, yk + 1)] = u10; }
-            if (vx1 && vy1) { nimg[pad_off(g, yk + 1, xk + 1)] = u11; nimgT[padT_off(g, xk + 1, yk + 1)] = u11; }
-
-            if (a.best && si.improved) {
-                float* best = a.best + (size_t)s * g.nx * g.ny;
-                best[(size_t)yk * g.nx + xk] = m[1][1];
-                if (vx1) best[(size_t)yk * g.nx + xk + 1] = m[1][2];
-                if (vy1) best[(size_t)(yk + 1) * g.nx + xk] = m[2][1];
-                if (vx1 && vy1) best[(size_t)(yk + 1) * g.nx + xk + 1] = m[2][2];
-            }
+        for (int p = 0; p < 4; ++p) {
+            float x = 0.f;
+            for (int qq = 0; qq < shares; ++qq) x += red[(qq * 4 + p) * tpb + i];
+            b[p] = x;
         }
-    } else {                                               // a pair of slices per block
-        // rotation k of the tile = orbit component (quarter + k) % 4  <=>  component m feeds rotation (m - quarter) % 4
-        if (q < shares) {
-#pragma unroll
-            for (int j = 0; j < SB; ++j)
-#pragma unroll
-                for (int m = 0; m < NS; ++m)
-#pragma unroll
-                    for (int p = 0; p < 4; ++p)
-                        red[((j * shares + q) * (NS * 4) + ((m - quarter) & (NS - 1)) * 4 + p) * tpb + i] = acc[j].get(m, p);
+        const bool vx1 = x0 + 1 < g.nx, vy1 = y0 + 1 < g.ny;
+        if (MODE == 0) {
+            float* out = a.out + (size_t)s * g.nx * g.ny;
+            out[(size_t)y0 * g.nx + x0] = b[0];
+            if (vx1) out[(size_t)y0 * g.nx + x0 + 1] = b[1];
+            if (vy1) out[(size_t)(y0 + 1) * g.nx + x0] = b[2];
+            if (vx1 && vy1) out[(size_t)(y0 + 1) * g.nx + x0 + 1] = b[3];
+            return;
         }
-
-        // thread (tile i, k = q < NS) finishes rotation k of the base tile: origin (xk, yk) and, below, where base pixel
-        // (tx,ty) lands.  Everything that does not depend on the other shares' sums -- monitor, step rule, neighbourhood
-        // of mu(n), TV gradient -- is done before the barrier, so that its loads overlap the wait for the slowest warp.
-        const bool fin = q < NS;
-        const bool fin_active = fin && x0 < xlim && y0 < ylim;
-        const int k = q;
-        int xk = x0, yk = y0;
-        if (NS == 4) {
-            const int N = g.nx;
-            if (k == 1)      { xk = N - 2 - y0; yk = x0; }
-            else if (k == 2) { xk = N - 2 - x0; yk = N - 2 - y0; }
-            else if (k == 3) { xk = y0;         yk = N - 2 - x0; }
+        // ---- A5 TV gradient of mu(n), A6 update (Eq. 3) with mu > 0, A7 best copy ----
+        const float u00 = fmaxf(fmaf(step, b[0] - a.beta_over_M * tv[0][0], m[1][1]), 0.f);
+        const float u01 = fmaxf(fmaf(step, b[1] - a.beta_over_M * tv[0][1], m[1][2]), 0.f);
+        const float u10 = fmaxf(fmaf(step, b[2] - a.beta_over_M * tv[1][0], m[2][1]), 0.f);
+        const float u11 = fmaxf(fmaf(step, b[3] - a.beta_over_M * tv[1][1], m[2][2]), 0.f);
+        float* nimg = a.img_new + (size_t)s * g.img_elems;
+        float* nimgT = a.imgT_new + (size_t)s * g.imgT_elems;
+        nimg[pad_off(g, y0, x0)] = u00;
+        nimgT[padT_off(g, x0, y0)] = u00;
+        if (vx1) { nimg[pad_off(g, y0, x0 + 1)] = u01; nimgT[padT_off(g, x0 + 1, y0)] = u01; }
+        if (vy1) { nimg[pad_off(g, y0 + 1, x0)] = u10; nimgT[padT_off(g, x0, y0 + 1)] = u10; }
+        if (vx1 && vy1) { nimg[pad_off(g, y0 + 1, x0 + 1)] = u11; nimgT[padT_off(g, x0 + 1, y0 + 1)] = u11; }
+        if (a.best && si.improved) {
+            float* best = a.best + (size_t)s * g.nx * g.ny;
+            best[(size_t)y0 * g.nx + x0] = m[1][1];
+            if (vx1) best[(size_t)y0 * g.nx + x0 + 1] = m[1][2];
+            if (vy1) best[(size_t)(y0 + 1) * g.nx + x0] = m[2][1];
+            if (vx1 && vy1) best[(size_t)(y0 + 1) * g.nx + x0 + 1] = m[2][2];
         }
+    } else {                                               // general path, a pair of slices per block (images interleaved per pixel)
+        const bool fin_active = q == 0 && tile_ok;
         StepInfo si[SB];
         float step[SB], m[SB][4][4], tv[SB][2][2];
-        if (MODE == 1 && t < 32 * ((NS * tpb + 31) / 32)) {           // whole warps: step_rule shuffles
+        if (MODE == 1 && t < 32 * ((tpb + 31) / 32)) {               // whole warps: step_rule shuffles
             const bool writer = blockIdx.x == 0 && t < 32;
-            if constexpr (SB == 2) {
-                if (fin_active) load_nbhd2(g, reinterpret_cast<const float2*>(a.img) + (size_t)blockIdx.z * g.img_elems, xk, yk, m[0], m[SB - 1]);
-            }
+            if (fin_active) load_nbhd2(g, reinterpret_cast<const float2*>(a.img) + (size_t)blockIdx.z * g.img_elems, x0, y0, m[0], m[SB - 1]);
 #pragma unroll
             for (int j = 0; j < SB; ++j) {
                 const int s = s0 + j;
                 if (s >= a.batch) break;
-                if (SB == 1 && fin_active) load_nbhd(g, a.img + (size_t)s * g.img_elems, xk, yk, m[j]);
                 si[j] = step_rule(a, s, lane, writer);
                 step[j] = (float)(si[j].lambda * a.tau);
-                if (fin_active) {
-                    if (STACK && a.tv_z > 0.f) {                    // stack of slices: the z term needs slices s-1 and s+1
-                        const bool has_up = s + 1 < a.batch, has_dn = s > 0;
-                        float up[4][4], dn[4][4];
-                        load_nbhd(g, a.img + (size_t)(has_up ? s + 1 : s) * g.img_elems, xk, yk, up);
-                        load_nbhd(g, a.img + (size_t)(has_dn ? s - 1 : s) * g.img_elems, xk, yk, dn);
-                        tv_grad_tile3(m[j], up, dn, has_up, has_dn, a.tv_z, xk, yk, g.nx, g.ny, a.eps2, tv[j]);
-                    } else {
-                        tv_grad_tile(m[j], xk, yk, g.nx, g.ny, a.eps2, tv[j]);
-                    }
-                }
+                if (fin_active) tv_grad_tile(m[j], x0, y0, g.nx, g.ny, a.eps2, tv[j]);
             }
         }
         __syncthreads();
         if (!fin_active) return;
-
-        float un[SB][4] = {};                                     // SB == 2: mu(n+1) of the tile in both slices (0 in an empty one)
+        float un[SB][4] = {};                                     // mu(n+1) of the tile in both slices (0 in an empty one)
+        const bool vx1 = x0 + 1 < g.nx, vy1 = y0 + 1 < g.ny;
 #pragma unroll
         for (int j = 0; j < SB; ++j) {
             const int s = s0 + j;
             if (s >= a.batch) break;
-            // sums over the view shares, fixed order
-            float b[4];
+            float b[4];                                           // sums over the view shares, fixed order
 #pragma unroll
             for (int p = 0; p < 4; ++p) {
                 float x = 0.f;
-                for (int qq = 0; qq < shares; ++qq) x += red[((j * shares + qq) * (NS * 4) + k * 4 + p) * tpb + i];
+                for (int qq = 0; qq < shares; ++qq) x += red[((j * shares + qq) * 4 + p) * tpb + i];
                 b[p] = x;
             }
-            float o00 = b[0], o01 = b[1], o10 = b[2], o11 = b[3];
-            if (NS == 4) {
-                if (k == 1)      { o00 = b[2]; o01 = b[0]; o10 = b[3]; o11 = b[1]; }
-                else if (k == 2) { o00 = b[3]; o01 = b[2]; o10 = b[1]; o11 = b[0]; }
-                else if (k == 3) { o00 = b[1]; o01 = b[3]; o10 = b[0]; o11 = b[2]; }
-            }
-            const bool vx1 = xk + 1 < g.nx, vy1 = yk + 1 < g.ny;
             if (MODE == 0) {
                 float* out = a.out + (size_t)s * g.nx * g.ny;
-                out[(size_t)yk * g.nx + xk] = o00;
-                if (vx1) out[(size_t)yk * g.nx + xk + 1] = o01;
-                if (vy1) out[(size_t)(yk + 1) * g.nx + xk] = o10;
-                if (vx1 && vy1) out[(size_t)(yk + 1) * g.nx + xk + 1] = o11;
+                out[(size_t)y0 * g.nx + x0] = b[0];
+                if (vx1) out[(size_t)y0 * g.nx + x0 + 1] = b[1];
+                if (vy1) out[(size_t)(y0 + 1) * g.nx + x0] = b[2];
+                if (vx1 && vy1) out[(size_t)(y0 + 1) * g.nx + x0 + 1] = b[3];
                 continue;
             }
-
-            // ---- A5 TV gradient of mu(n), A6 update (Eq. 3) with mu > 0, A7 best copy ----
-            const float u00 = fmaxf(fmaf(step[j], o00 - a.beta_over_M * tv[j][0][0], m[j][1][1]), 0.f);
-            const float u01 = fmaxf(fmaf(step[j], o01 - a.beta_over_M * tv[j][0][1], m[j][1][2]), 0.f);
-            const float u10 = fmaxf(fmaf(step[j], o10 - a.beta_over_M * tv[j][1][0], m[j][2][1]), 0.f);
-            const float u11 = fmaxf(fmaf(step[j], o11 - a.beta_over_M * tv[j][1][1], m[j][2][2]), 0.f);
-            if constexpr (SB == 2) {
-                un[j][0] = u00; un[j][1] = u01; un[j][2] = u10; un[j][3] = u11;      // stored below, both slices at once
-            } else {
-                float* nimg = a.img_new + (size_t)s * g.img_elems;
-                float* nimgT = a.imgT_new + (size_t)s * g.imgT_elems;
-                nimg[pad_off(g, yk, xk)] = u00;
-                nimgT[padT_off(g, xk, yk)] = u00;
-                if (vx1) { nimg[pad_off(g, yk, xk + 1)] = u01; nimgT[padT_off(g, xk + 1, yk)] = u01; }
-                if (vy1) { nimg[pad_off(g, yk + 1, xk)] = u10; nimgT[padT_off(g, xk, yk + 1)] = u10; }
-                if (vx1 && vy1) { nimg[pad_off(g, yk + 1, xk + 1)] = u11; nimgT[padT_off(g, xk + 1, yk + 1)] = u11; }
-            }
-
+            un[j][0] = fmaxf(fmaf(step[j], b[0] - a.beta_over_M * tv[j][0][0], m[j][1][1]), 0.f);
+            un[j][1] = fmaxf(fmaf(step[j], b[1] - a.beta_over_M * tv[j][0][1], m[j][1][2]), 0.f);
+            un[j][2] = fmaxf(fmaf(step[j], b[2] - a.beta_over_M * tv[j][1][0], m[j][2][1]), 0.f);
+            un[j][3] = fmaxf(fmaf(step[j], b[3] - a.beta_over_M * tv[j][1][1], m[j][2][2]), 0.f);
             if (a.best && si[j].improved) {
                 float* best = a.best + (size_t)s * g.nx * g.ny;
-                best[(size_t)yk * g.nx + xk] = m[j][1][1];
-                if (vx1) best[(size_t)yk * g.nx + xk + 1] = m[j][1][2];
-                if (vy1) best[(size_t)(yk + 1) * g.nx + xk] = m[j][2][1];
-                if (vx1 && vy1) best[(size_t)(yk + 1) * g.nx + xk + 1] = m[j][2][2];
+                best[(size_t)y0 * g.nx + x0] = m[j][1][1];
+                if (vx1) best[(size_t)y0 * g.nx + x0 + 1] = m[j][1][2];
+                if (vy1) best[(size_t)(y0 + 1) * g.nx + x0] = m[j][2][1];
+                if (vx1 && vy1) best[(size_t)(y0 + 1) * g.nx + x0 + 1] = m[j][2][2];
             }
         }
-        if constexpr (SB == 2 && MODE == 1) {
+        if constexpr (MODE == 1) {
             float2* nimg = reinterpret_cast<float2*>(a.img_new) + (size_t)blockIdx.z * g.img_elems;
             float2* nimgT = reinterpret_cast<float2*>(a.imgT_new) + (size_t)blockIdx.z * g.imgT_elems;
-            const bool vx1 = xk + 1 < g.nx, vy1 = yk + 1 < g.ny;
             const float2 u00 = make_float2(un[0][0], un[SB - 1][0]), u01 = make_float2(un[0][1], un[SB - 1][1]);
             const float2 u10 = make_float2(un[0][2], un[SB - 1][2]), u11 = make_float2(un[0][3], un[SB - 1][3]);
-            nimg[pad_off(g, yk, xk)] = u00;
-            nimgT[padT_off(g, xk, yk)] = u00;
-            if (vx1) { nimg[pad_off(g, yk, xk + 1)] = u01; nimgT[padT_off(g, xk + 1, yk)] = u01; }
-            if (vy1) { nimg[pad_off(g, yk + 1, xk)] = u10; nimgT[padT_off(g, xk, yk + 1)] = u10; }
-            if (vx1 && vy1) { nimg[pad_off(g, yk + 1, xk + 1)] = u11; nimgT[padT_off(g, xk + 1, yk + 1)] = u11; }
+            nimg[pad_off(g, y0, x0)] = u00;
+            nimgT[padT_off(g, x0, y0)] = u00;
+            if (vx1) { nimg[pad_off(g, y0, x0 + 1)] = u01; nimgT[padT_off(g, x0 + 1, y0)] = u01; }
+            if (vy1) { nimg[pad_off(g, y0 + 1, x0)] = u10; nimgT[padT_off(g, x0, y0 + 1)] = u10; }
+            if (vx1 && vy1) { nimg[pad_off(g, y0 + 1, x0 + 1)] = u11; nimgT[padT_off(g, x0 + 1, y0 + 1)] = u11; }
         }
     }
 }
@@ -1015,34 +1168,39 @@ __global__ void __launch_bounds__(SB == 1 ? BK_MAX_THREADS : BKB_MAX_THREADS, SB
 // Small helpers around the two hot kernels
 // ------------------------------------------------------------------------------------------------
 
-// [batch][ny][nx] -> padded img and padded transpose imgT (32x32 tiles through shared memory)
-__global__ void __launch_bounds__(256) k_pad_transpose(DevGeom g, const float* __restrict__ src,
+// Image layouts of the padded working buffers (per group of g.sb slices, slices interleaved per pixel):
+//   NS == 1: one float per pixel and slice:   img[((iy+PADR)*pitch + PAD+ix) * sb + sl],  imgT the transpose;
+//   NS == 4: one float4 per pixel and slice:  Q  [((iy+PADR)*pitch + PAD+ix) * sb + sl] = {mu(P), mu(RP), mu(R^2P), mu(R^3P)},
+//            R: (ix,iy) -> (N-1-iy, ix);  QT the transpose.
+__device__ __forceinline__ void orbit_pos(int N, int ix, int iy, int k, int& x, int& y) {
+    x = k == 0 ? ix : k == 1 ? N - 1 - iy : k == 2 ? N - 1 - ix : iy;
+    y = k == 0 ? iy : k == 1 ? ix : k == 2 ? N - 1 - iy : N - 1 - ix;
+}
+
+// [batch][ny][nx] -> the padded working layout and its transpose
+__global__ void __launch_bounds__(256) k_pad_transpose(DevGeom g, int ns, const float* __restrict__ src,
                                                        float* __restrict__ img, float* __restrict__ imgT) {
-    __shared__ float tile[32][33];
     const int s = blockIdx.z;
-    const int bx = blockIdx.x * 32, by = blockIdx.y * 32;
-    const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;       // 32 x 8
+    const int x = blockIdx.x * 32 + (threadIdx.x & 31);
+    const int y = blockIdx.y * 8 + (threadIdx.x >> 5);
+    if (x >= g.nx || y >= g.ny) return;
     src += (size_t)s * g.nx * g.ny;
-    img += slice_base(g, g.img_elems, s);
-    imgT += slice_base(g, g.imgT_elems, s);
-    for (int r = ty; r < 32; r += 8) {
-        const int x = bx + tx, y = by + r;
-        float v = 0.f;
-        if (x < g.nx && y < g.ny) {
-            v = src[(size_t)y * g.nx + x];
-            img[pad_off(g, y, x) * g.sb] = v;
-        }
-        tile[r][tx] = v;
-    }
-    __syncthreads();
-    for (int r = ty; r < 32; r += 8) {
-        const int x = bx + r, y = by + tx;
-        if (x < g.nx && y < g.ny) imgT[padT_off(g, x, y) * g.sb] = tile[tx][r];
+    if (ns == 4) {
+        float v[4];
+#pragma unroll
+        for (int k = 0; k < 4; ++k) { int xx, yy; orbit_pos(g.nx, x, y, k, xx, yy); v[k] = src[(size_t)yy * g.nx + xx]; }
+        const float4 q = make_float4(v[0], v[1], v[2], v[3]);
+        reinterpret_cast<float4*>(img)[(size_t)(s / g.sb) * g.img_elems * g.sb + pad_off(g, y, x) * g.sb + s % g.sb] = q;
+        reinterpret_cast<float4*>(imgT)[(size_t)(s / g.sb) * g.imgT_elems * g.sb + padT_off(g, x, y) * g.sb + s % g.sb] = q;
+    } else {
+        const float v = src[(size_t)y * g.nx + x];
+        img[slice_base(g, g.img_elems, s) + pad_off(g, y, x) * g.sb] = v;
+        imgT[slice_base(g, g.imgT_elems, s) + padT_off(g, x, y) * g.sb] = v;
     }
 }
 
-// padded img -> [batch][ny][nx]; with best != null picks per slice: improved ? img : best   (C12)
-__global__ void __launch_bounds__(256) k_unpad(DevGeom g, const float* __restrict__ img,
+// working layout -> [batch][ny][nx]; with best != null picks per slice: improved ? img : best   (C12)
+__global__ void __launch_bounds__(256) k_unpad(DevGeom g, int ns, const float* __restrict__ img,
                                                const float* __restrict__ best, const SliceState* __restrict__ state,
                                                float* __restrict__ out) {
     const int s = blockIdx.z;
@@ -1051,18 +1209,25 @@ __global__ void __launch_bounds__(256) k_unpad(DevGeom g, const float* __restric
     if (x >= g.nx || y >= g.ny) return;
     const size_t o = (size_t)s * g.nx * g.ny + (size_t)y * g.nx + x;
     if (best && !state[s].improved) out[o] = best[o];
+    else if (ns == 4) out[o] = reinterpret_cast<const float4*>(img)[(size_t)(s / g.sb) * g.img_elems * g.sb + pad_off(g, y, x) * g.sb + s % g.sb].x;
     else out[o] = img[slice_base(g, g.img_elems, s) + pad_off(g, y, x) * g.sb];
 }
 
-// homogeneous initial image into both padded layouts, and into best
-__global__ void __launch_bounds__(256) k_fill(DevGeom g, float mu0, float* __restrict__ img,
+// homogeneous initial image into both working layouts, and into best
+__global__ void __launch_bounds__(256) k_fill(DevGeom g, int ns, float mu0, float* __restrict__ img,
                                               float* __restrict__ imgT, float* __restrict__ best) {
     const int s = blockIdx.z;
     const int x = blockIdx.x * 32 + (threadIdx.x & 31);
     const int y = blockIdx.y * 8 + (threadIdx.x >> 5);
     if (x >= g.nx || y >= g.ny) return;
-    img[slice_base(g, g.img_elems, s) + pad_off(g, y, x) * g.sb] = mu0;
-    imgT[slice_base(g, g.imgT_elems, s) + padT_off(g, x, y) * g.sb] = mu0;
+    if (ns == 4) {
+        const float4 q = make_float4(mu0, mu0, mu0, mu0);
+        reinterpret_cast<float4*>(img)[(size_t)(s / g.sb) * g.img_elems * g.sb + pad_off(g, y, x) * g.sb + s % g.sb] = q;
+        reinterpret_cast<float4*>(imgT)[(size_t)(s / g.sb) * g.imgT_elems * g.sb + padT_off(g, x, y) * g.sb + s % g.sb] = q;
+    } else {
+        img[slice_base(g, g.img_elems, s) + pad_off(g, y, x) * g.sb] = mu0;
+        imgT[slice_base(g, g.imgT_elems, s) + padT_off(g, x, y) * g.sb] = mu0;
+    }
     if (best) best[(size_t)s * g.nx * g.ny + (size_t)y * g.nx + x] = mu0;
 }
 

@@ -96,8 +96,8 @@ __global__ void __launch_bounds__(PT, 2) p_l1(const float4* __restrict__ buf, in
     for (int i = 0; i < iters; ++i) {
 #pragma unroll
         for (int u = 0; u < 8; ++u) {
-            const float4 v = __ldg(w + ((threadIdx.x + (u + i) * 64) & 2047));
-            s += v.x + v.w;
+            const float4 v = __ldg(w + ((threadIdx.x + (u + i * 8) * 64) & 2047));
+            s += (v.x + v.y) + (v.z + v.w);
         }
     }
     if (s == 12345.678f) sink[0] = s;
@@ -109,7 +109,7 @@ __global__ void __launch_bounds__(PT, 2) p_l1_b32(const float* __restrict__ buf,
     float s = 0.f;
     for (int i = 0; i < iters; ++i) {
 #pragma unroll
-        for (int u = 0; u < 8; ++u) s += __ldg(w + ((threadIdx.x + (u + i) * 128) & 8191));
+        for (int u = 0; u < 8; ++u) s += __ldg(w + ((threadIdx.x + (u + i * 8) * 128) & 8191));
     }
     if (s == 12345.678f) sink[0] = s;
 }
@@ -123,11 +123,20 @@ __global__ void __launch_bounds__(PT, 2) p_smem(int iters, float* sink) {
     for (int i = 0; i < iters; ++i) {
 #pragma unroll
         for (int u = 0; u < 8; ++u) {
-            const float4 v = sm[(threadIdx.x + (u + i) * 64) & 2047];
-            s += v.x + v.w;
+            const float4 v = sm[(threadIdx.x + (u + i * 8) * 64) & 2047];
+            s += (v.x + v.y) + (v.z + v.w);
         }
     }
     if (s == 12345.678f) sink[0] = s;
+}
+
+// non-trivial contents for the read probes (an all-zero buffer could be served by zero-line shortcuts)
+__global__ void p_fill(uint32_t* buf, size_t n) {
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
+        uint32_t x = (uint32_t)i * 2654435761u + 12345u;
+        x ^= x >> 15; x *= 2246822519u; x ^= x >> 13;
+        buf[i] = 0x3f000000u | (x & 0x007fffffu);                 // floats in [0.5, 1)
+    }
 }
 
 template <class F>
@@ -167,6 +176,8 @@ extern "C" int osiv_probe_peaks(int32_t device, double* out8) {
     if (cudaMalloc((void**)&sink, 256) != cudaSuccess || cudaMalloc((void**)&buf, l2_bytes) != cudaSuccess ||
         cudaMemset(buf, 0, l2_bytes) != cudaSuccess) {
         rc = OSIV_ERR_CUDA;
+    } else {
+        p_fill<<<4 * sms, 256>>>(reinterpret_cast<uint32_t*>(buf), l2_bytes / 4);
     }
     double ms = 0.0;
     const double threads = (double)grid * PT;
