@@ -189,6 +189,15 @@ int osiv_set_symmetry(osiv_handle* h, int32_t enable);
  * plain stream order (same results bit for bit; used by the tests and for A/B timing). */
 int osiv_set_overlap(osiv_handle* h, int32_t enable);
 
+/* Which K2 runs.  On the quarter-turn path with one slice per block (batch < 4, no stack), grids whose side is a multiple
+ * of 8 and fans below 90 degrees, K2 is the kernel that stages each block's ray-table, residual and interval windows in
+ * shared memory with bulk copies (csrc/osiv_back_staged.cuh); general_only = 1 forces the general gather kernel instead
+ * (used by the tests to compare the two).  Results differ only by rounding order. */
+int osiv_set_back_kernel(osiv_handle* h, int32_t general_only);
+/* *staged = 1 if osiv_reconstruct / osiv_backward with `n_subsets` subsets (<= 0: all views) and `batch` slices would
+ * run the staged K2, else 0.  Host only. */
+int osiv_get_back_kernel(const osiv_handle* h, int32_t n_subsets, int32_t batch, int32_t* staged);
+
 /* Launch plan osiv_reconstruct would use for `n_subsets` subsets (<= 0: all views) and `batch` slices:
  * (independent slices: a stack with view_shift or tv_z never pairs slices)
  * out8 = {K1 orbit size (1 or 4), K1 line segments per ray, K1 blocks, K1 threads per block,
@@ -207,11 +216,11 @@ int osiv_get_profile(const osiv_handle* h, double* ms_forward, int64_t* n_forwar
 /* Phase timeline of the two hot kernels (only in the build made with -DOSIV_TRACE, `python -m
  * paper_1903_10088_b200.build --trace` -> libosiv_trace.so; the regular library returns OSIV_ERR_INVALID_ARG).
  * Every block of slice group 0 stamps its SM's cycle counter at its phase boundaries; h_out receives
- * [4][256][12] uint64: first index = (iteration & 1) * 2 + kernel (0 = K1, 1 = K2) of the last two iterations run on
+ * [4][256][16] uint64: first index = (iteration & 1) * 2 + kernel (0 = K1, 1 = K2) of the last two iterations run on
  * the current device, second = block, third = {block start, before the dependent-launch wait, after it, end of the
  * main loop (latest warp), after the block barrier, block end (latest warp) -- all in SM cycles --, SM id, a mark
  * inside the prologue [cycles], the GPU's global nanosecond timer read at block start, unused...}.  n_entries must be
- * 4*256*12.  Synchronises the device.  Driver: `python -m paper_1903_10088_b200.timeline`. */
+ * 4*256*16.  Synchronises the device.  Driver: `python -m paper_1903_10088_b200.timeline`. */
 int osiv_debug_timeline(uint64_t* h_out, int32_t n_entries);
 
 /* Micro-probes of the units that bound the two hot kernels (csrc/osiv_probes.cu): saturating loops

@@ -17,7 +17,7 @@ OSIV_OK, OSIV_ERR_INVALID_ARG, OSIV_ERR_CUDA, OSIV_ERR_NOT_FINITE = 0, -1, -2, -
 
 EXPORTED_SYMBOLS = (
     "osiv_version", "osiv_strerror", "osiv_default_params", "osiv_create", "osiv_destroy", "osiv_ray_table", "osiv_get_dgamma",
-    "osiv_get_tau", "osiv_launch_count", "osiv_set_symmetry", "osiv_set_overlap", "osiv_get_plan", "osiv_set_profiling", "osiv_get_profile", "osiv_forward", "osiv_backward", "osiv_tv_gradient", "osiv_reconstruct",
+    "osiv_get_tau", "osiv_launch_count", "osiv_set_symmetry", "osiv_set_overlap", "osiv_set_back_kernel", "osiv_get_back_kernel", "osiv_get_plan", "osiv_set_profiling", "osiv_get_profile", "osiv_forward", "osiv_backward", "osiv_tv_gradient", "osiv_reconstruct",
     "osiv_reconstruct_host", "osiv_probe_peaks", "osiv_debug_timeline",
 )
 
@@ -108,6 +108,8 @@ def lib():
         L.osiv_launch_count.argtypes = [vp]
         L.osiv_set_symmetry.argtypes = [vp, ip]
         L.osiv_set_overlap.argtypes = [vp, ip]
+        L.osiv_set_back_kernel.argtypes = [vp, ip]
+        L.osiv_get_back_kernel.argtypes = [vp, ip, ip, C.POINTER(C.c_int32)]
         L.osiv_get_plan.argtypes = [vp, ip, ip, C.POINTER(C.c_int32)]
         L.osiv_set_profiling.argtypes = [vp, ip]
         L.osiv_get_profile.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_int64), C.POINTER(C.c_double),
@@ -241,6 +243,16 @@ class Handle:
     def set_overlap(self, enable: bool) -> None:
         """enable=False chains K1 and K2 in plain stream order instead of programmatic dependent launches"""
         _check(lib().osiv_set_overlap(self._h, 1 if enable else 0), "osiv_set_overlap")
+
+    def set_back_kernel(self, general_only: bool) -> None:
+        """general_only=True forces the general gather K2 where the shared-memory-staged K2 would run"""
+        _check(lib().osiv_set_back_kernel(self._h, 1 if general_only else 0), "osiv_set_back_kernel")
+
+    def back_kernel(self, n_subsets: int = 0, batch: int = 1) -> str:
+        """'staged' or 'general': the K2 that reconstruct / backward would run"""
+        out = C.c_int32()
+        _check(lib().osiv_get_back_kernel(self._h, n_subsets, batch, C.byref(out)), "osiv_get_back_kernel")
+        return "staged" if out.value else "general"
 
     def plan(self, n_subsets: int = 0, batch: int = 1) -> dict:
         out = (C.c_int32 * 8)()

@@ -17,7 +17,7 @@ CSRC = os.path.join(_HERE, "csrc")
 INCLUDE = os.path.join(os.path.dirname(_HERE), "include")
 SO = os.path.join(_HERE, "libosiv.so")
 SOURCES = [os.path.join(CSRC, "osiv.cu"), os.path.join(CSRC, "osiv_probes.cu")]
-DEPS = SOURCES + [os.path.join(CSRC, "osiv_kernels.cuh"), os.path.join(INCLUDE, "osiv.h")]
+DEPS = SOURCES + [os.path.join(CSRC, "osiv_kernels.cuh"), os.path.join(CSRC, "osiv_back_staged.cuh"), os.path.join(INCLUDE, "osiv.h")]
 NVCC_FLAGS = ["-O3", "-std=c++17", "-lineinfo", "-gencode", "arch=compute_100a,code=sm_100a",
               "-shared", "-Xcompiler", "-fPIC", "-Xptxas", "-v"]
 

@@ -4,9 +4,11 @@
 // compute entry point returns OSIV_ERR_CUDA.
 #include "../../include/osiv.h"
 #include "osiv_kernels.cuh"
+#include "osiv_back_staged.cuh"
 
 #include <algorithm>
 #include <cmath>
+#include <cstdio>
 #include <cstdlib>
 #include <cstring>
 #include <new>
@@ -47,6 +49,16 @@ struct osiv_handle {
     size_t hi_elems = 0;        float* d_himg = nullptr;
     int64_t launches = 0;
     int force_ns1 = 0;                  // osiv_set_symmetry(h, 0): always take the general path
+    // staged K2 (osiv_back_staged.cuh): regions of the base quadrant, per-(view, block) windows, per-tile intervals
+    int st_ready = 0;                   // 1: tables built and usable; 0: this geometry does not take the staged kernel
+    int st_off = 0;                     // osiv_set_back_kernel(h, 1): always the general K2
+    int st_nblk = 0, st_tpbp = 0, st_W = 0;
+    int4* d_regions = nullptr;
+    unsigned short* d_itab2 = nullptr;
+    int* d_bwin = nullptr;
+    unsigned char* d_blob = nullptr;    // per-subset constants of the staged K2 for blob_M subsets (k_build_blob)
+    size_t blob_bytes = 0;
+    int blob_M = 0;
     int use_pdl = 1;                    // osiv_set_overlap(h, 0): plain stream order between K1 and K2
     // per-kernel event timing (osiv_set_profiling)
     bool profiling = false;
@@ -67,7 +79,14 @@ struct DeviceGuard {
     ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
 };
 
-#define OSIV_CUDA(call) do { if ((call) != cudaSuccess) { cudaGetLastError(); return OSIV_ERR_CUDA; } } while (0)
+// OSIV_DEBUG=1 in the environment names the failing CUDA call on stderr (diagnostics; the library is otherwise silent)
+inline bool cuda_failed(cudaError_t e, const char* what) {
+    if (e == cudaSuccess) return false;
+    if (std::getenv("OSIV_DEBUG")) std::fprintf(stderr, "libosiv: %s: %s\n", what, cudaGetErrorString(e));
+    cudaGetLastError();
+    return true;
+}
+#define OSIV_CUDA(call) do { if (cuda_failed((call), #call)) return OSIV_ERR_CUDA; } while (0)
 
 template <class T>
 int grow(T** p, size_t* have, size_t want) {
@@ -284,6 +303,168 @@ cudaError_t launch_back(const BackPlan& p, int batch, const BackArgs& a, cudaStr
     return p.ns == 4 ? cudaLaunchKernelEx(&cfg, k_back<MODE, 4, 1, 0>, a) : cudaLaunchKernelEx(&cfg, k_back<MODE, 1, 1, 0>, a);
 }
 
+// ---- staged K2 (osiv_back_staged.cuh) ------------------------------------------------------------------
+constexpr size_t SMEM_OPTIN = 227 * 1024;       // shared memory one block may ask for on sm_100
+
+// The base quadrant in tiles of 4 x 2 pixels (TX x TY) is cut into nblk rectangles of about equal area: rows of blocks,
+// each row cut into nb_r columns; every rectangle must hold at most BS_MAX_TPB tiles.  Returns {} when that fails.
+std::vector<int4> staged_regions(int TX, int TY, int nblk, int* tpb_out) {
+    std::vector<int4> out;
+    int nrows = std::max(1, (int)std::lround(std::sqrt((double)nblk * (TY * (double)BS_TY) / (TX * (double)BS_TX))));
+    nrows = std::min(std::min(nrows, TY), nblk);
+    if ((nblk + nrows - 1) / nrows > TX) return out;
+    std::vector<int> nb(nrows), hgt(nrows), wmax(nrows);
+    int cum = 0, y_prev = 0;
+    for (int r = 0; r < nrows; ++r) {
+        nb[r] = nblk / nrows + (r < nblk % nrows ? 1 : 0);
+        cum += nb[r];
+        int y = (int)std::floor((double)TY * cum / nblk + 0.5);
+        y = std::max(y, y_prev + 1);
+        y = std::min(y, TY - (nrows - 1 - r));
+        hgt[r] = y - y_prev;
+        y_prev = y;
+        wmax[r] = (TX + nb[r] - 1) / nb[r];
+    }
+    // move tile rows from block rows whose widest rectangle is too large to the block row with the most room
+    for (int guard = 0; guard < 4 * TY; ++guard) {
+        int bad = -1;
+        for (int r = 0; r < nrows; ++r) if (wmax[r] * hgt[r] > BS_MAX_TPB && (bad < 0 || wmax[r] * hgt[r] > wmax[bad] * hgt[bad])) bad = r;
+        if (bad < 0) break;
+        int to = -1;
+        for (int r = 0; r < nrows; ++r)
+            if (r != bad && wmax[r] * (hgt[r] + 1) <= BS_MAX_TPB && (to < 0 || wmax[r] * (hgt[r] + 1) < wmax[to] * (hgt[to] + 1))) to = r;
+        if (to < 0 || hgt[bad] <= 1) return out;
+        hgt[bad] -= 1; hgt[to] += 1;
+    }
+    int tpb = 0, y0 = 0;
+    for (int r = 0; r < nrows; ++r) {
+        if (wmax[r] * hgt[r] > BS_MAX_TPB) { out.clear(); return out; }
+        for (int k = 0; k < nb[r]; ++k) {
+            const int x0 = (int)((long long)TX * k / nb[r]), x1 = (int)((long long)TX * (k + 1) / nb[r]);
+            const int w = x1 - x0;
+            out.push_back(make_int4(x0 | (y0 << 16), w | (hgt[r] << 16), (int)div_magic(w), 0));
+            tpb = std::max(tpb, w * hgt[r]);
+        }
+        y0 += hgt[r];
+    }
+    *tpb_out = tpb;
+    return out;
+}
+
+// A0 for the staged K2, at osiv_create: regions, per-(view, block) windows and per-tile candidate intervals.  Leaves
+// h->st_ready = 0 (the general K2 serves) when the geometry does not qualify; an error only for CUDA failures.
+int build_staged(osiv_handle* h, double tile_hw_staged) {
+    const osiv_geometry& g = h->geom;
+    h->st_ready = 0;
+    if (!h->dg.sym4 || g.nx % (2 * BS_TX) != 0 || h->dgamma * g.n_channels >= 0.5 * M_PI) return OSIV_OK;
+    const int TX = g.nx / 2 / BS_TX, TY = g.ny / 2 / BS_TY;
+    const long long tiles = (long long)TX * TY;
+    // whole multiples of the SM count, about 56 tiles per block; small grids: at least 8 tiles per block
+    const long long tgt = 60;           // (30 or 20 tiles per block, two or three blocks per SM, measured 9 and 24 % slower)
+    int nblk = (int)std::min<long long>((long long)h->num_sms * ((tiles + tgt * h->num_sms - 1) / (tgt * h->num_sms)),
+                                        std::max<long long>(1, tiles / 8));
+    std::vector<int4> regions;
+    int tpb = 0;
+    for (int tries = 0; tries < 8 && regions.empty(); ++tries, nblk += h->num_sms)
+        if (nblk <= BS_MAX_REGIONS) regions = staged_regions(TX, TY, nblk, &tpb);
+    if (regions.empty()) return OSIV_OK;
+    nblk = (int)regions.size();
+    const int tpbp = (tpb + 31) / 32 * 32;
+    const size_t n_itab = (size_t)g.n_views * nblk * tpbp;
+    int* d_max = nullptr;
+    int hmax[2] = {0, 0};
+    if (cudaMalloc((void**)&h->d_regions, regions.size() * sizeof(int4)) != cudaSuccess ||
+        cudaMalloc((void**)&h->d_itab2, n_itab * sizeof(unsigned short)) != cudaSuccess ||
+        cudaMalloc((void**)&h->d_bwin, (size_t)g.n_views * nblk * sizeof(int)) != cudaSuccess ||
+        cudaMalloc((void**)&d_max, 2 * sizeof(int)) != cudaSuccess ||
+        cudaMemset(d_max, 0, 2 * sizeof(int)) != cudaSuccess ||
+        cudaMemcpy(h->d_regions, regions.data(), regions.size() * sizeof(int4), cudaMemcpyHostToDevice) != cudaSuccess) {
+        if (d_max) cudaFree(d_max);
+        cudaGetLastError();
+        return OSIV_ERR_CUDA;
+    }
+    k_build_staged<<<dim3(nblk, g.n_views), tpbp>>>(h->dg, (float)tile_hw_staged, g.model == 1 ? 0.f : 0.5f, g.model == 1 ? 1.f : 0.5f,
+                                                    h->d_regions, nblk, tpbp, h->d_itab2, h->d_bwin, d_max);
+    h->launches += 1;
+    const bool ok = cudaMemcpy(hmax, d_max, sizeof(hmax), cudaMemcpyDeviceToHost) == cudaSuccess;
+    cudaFree(d_max);
+    if (!ok) { cudaGetLastError(); return OSIV_ERR_CUDA; }
+    // a lane walks up to the warp's largest count, rounded up to even, from its own first candidate
+    const int W = (hmax[0] + hmax[1] + 2 + 1) / 2 * 2;
+    if (hmax[0] >= 256 || hmax[1] >= 255 || W > 512) return OSIV_OK;
+    const size_t slot = 16 + (size_t)W * 8 + (size_t)tpbp * 2 + (size_t)W * 16;       // constants + residual window
+    const size_t fixed = BS_HDR_BYTES + (size_t)BS_SHARES * tpbp * BS_RED_PITCH * sizeof(float4);
+    if (fixed + 4 * slot > SMEM_OPTIN || 4 > BS_RCH * ((BS_SHARES * tpbp) / W)) return OSIV_OK;
+    if (cudaFuncSetAttribute(k_back_staged<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_OPTIN) != cudaSuccess ||
+        cudaFuncSetAttribute(k_back_staged<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_OPTIN) != cudaSuccess) {
+        cudaGetLastError();
+        return OSIV_ERR_CUDA;
+    }
+    h->st_nblk = nblk; h->st_tpbp = tpbp; h->st_W = W;
+    h->st_ready = 1;
+    return OSIV_OK;
+}
+
+struct StagedPlan { int nblk, tpbp, threads, W, JR, nrounds, slot_c; size_t smem; };
+
+// the blob of the staged K2 for M subsets (M = 1: all views in one), rebuilt when M changes
+int ensure_blob(osiv_handle* h, int M, cudaStream_t st) {
+    if (h->d_blob && h->blob_M == M) return OSIV_OK;
+    const int V = h->geom.n_views, VS = V / M;
+    const int slot_c = 16 + h->st_W * 8 + h->st_tpbp * 2;
+    const size_t want = (size_t)V * h->st_nblk * slot_c;
+    h->blob_M = 0;
+    int rc = grow(&h->d_blob, &h->blob_bytes, want);
+    if (rc != OSIV_OK) return rc;
+    k_build_blob<<<dim3(h->st_nblk, VS, M), 128, 0, st>>>(h->dg, M, VS, h->st_nblk, h->st_tpbp, h->st_W, slot_c, h->d_itab2, h->d_bwin, h->d_blob);
+    h->launches += 1;
+    OSIV_CUDA(cudaGetLastError());
+    h->blob_M = M;
+    return OSIV_OK;
+}
+
+// the staged K2 serves one slice per block on the quarter-turn path when the subset has at least two base views
+bool use_staged(const osiv_handle* h, const BackPlan& p, bool stack) {
+    return h->st_ready && !h->st_off && p.ns == 4 && p.sb == 1 && !stack;
+}
+// ... and K1's monitor partials per slice fit the step-rule warp's registers
+bool use_staged(const osiv_handle* h, const BackPlan& p, bool stack, const FwdPlan& f) {
+    return use_staged(h, p, stack) && f.nparts <= 32 * BS_DPK;
+}
+
+StagedPlan plan_staged(const osiv_handle* h, int VS) {
+    StagedPlan p;
+    p.nblk = h->st_nblk; p.tpbp = h->st_tpbp; p.W = h->st_W;
+    p.threads = BS_SHARES * p.tpbp;
+    p.slot_c = 16 + p.W * 8 + p.tpbp * 2;
+    const size_t per_view = 4 * ((size_t)p.slot_c + (size_t)p.W * 16);
+    const size_t fixed = BS_HDR_BYTES + (size_t)BS_SHARES * p.tpbp * BS_RED_PITCH * sizeof(float4);
+    const int VSb = VS / 4;
+    p.JR = (int)std::min<size_t>(std::min(VSb, BS_MAX_JR), (SMEM_OPTIN - fixed) / per_view);
+    p.JR = std::max(1, std::min(p.JR, BS_RCH * (p.threads / p.W) / 4));       // a thread fetches at most BS_RCH residual chunks per round
+    p.nrounds = (VSb + p.JR - 1) / p.JR;
+    p.smem = fixed + (size_t)p.JR * per_view;
+    return p;
+}
+
+template <int MODE>
+cudaError_t launch_back_staged(const osiv_handle* h, const StagedPlan& p, int batch, const BackArgs& a, cudaStream_t st, bool pdl) {
+    BackSArgs sa;
+    sa.b = a;
+    sa.regions = h->d_regions; sa.blob = h->d_blob;
+    sa.nblk = p.nblk; sa.tpbp = p.tpbp; sa.tpbp_magic = div_magic(p.tpbp); sa.W = p.W; sa.W_magic = div_magic(p.W); sa.SP = p.threads / p.W; sa.JR = p.JR; sa.nrounds = p.nrounds;
+    sa.slot_c = p.slot_c;
+    sa.hka = h->geom.model == 1 ? 0.f : 0.5f; sa.hkb = h->geom.model == 1 ? 1.f : 0.5f;
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = dim3(p.nblk, 1, batch); cfg.blockDim = dim3(p.threads); cfg.stream = st;
+    cfg.dynamicSmemBytes = p.smem;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr; cfg.numAttrs = pdl ? 1 : 0;
+    return cudaLaunchKernelEx(&cfg, k_back_staged<MODE>, sa);
+}
+
 // K2's candidate intervals for this orbit size: one pass of k_build_intervals over all views, on first use
 int ensure_intervals(osiv_handle* h, const BackPlan& p, cudaStream_t st) {
     const int w = p.ns == 4 ? 1 : 0;
@@ -414,7 +595,9 @@ int osiv_create(const osiv_geometry* geom, int32_t max_batch, int32_t device, os
         hs[i] = rays[i].w;
         rays[i].w = g.model == 1 ? 1.f : 0.5f * (std::fabs(rays[i].x) + std::fabs(rays[i].y));
     }
-    rays.resize(rays.size() + h->res_pad + 4, make_float4(0.f, 0.f, 0.f, 0.f));
+    // zero slack after the last view: K2 reads past a view's last channel (general kernel: res_pad entries; staged
+    // kernel: up to one window of at most 512 entries)
+    rays.resize(rays.size() + h->res_pad + 4 + 512, make_float4(0.f, 0.f, 0.f, 0.f));
     if (cudaMalloc((void**)&h->d_rays, rays.size() * sizeof(float4)) != cudaSuccess ||
         cudaMalloc((void**)&h->d_hs, hs.size() * sizeof(float)) != cudaSuccess ||
         cudaMemcpy(h->d_hs, hs.data(), hs.size() * sizeof(float), cudaMemcpyHostToDevice) != cudaSuccess ||
@@ -453,6 +636,17 @@ int osiv_create(const osiv_geometry* geom, int32_t max_batch, int32_t device, os
     d.sym4 = (g.nx == g.ny && g.nx % 4 == 0 && g.n_views % 4 == 0) ? 1 : 0;
     d.sb = 1;
     d.rays = h->d_rays; d.views = h->d_views; d.hs = h->d_hs;
+    {
+        // staged K2: its tiles are 4 x 2 pixels (same bound as tile_hw with that tile's radius)
+        const double tr = g.model == 1
+            ? 0.5 * g.pixel_mm * std::sqrt((double)((BS_TX - 1) * (BS_TX - 1) + (BS_TY - 1) * (BS_TY - 1))) + g.pixel_mm
+            : 0.5 * g.pixel_mm * std::sqrt((double)(BS_TX * BS_TX + BS_TY * BS_TY));
+        const double xs = std::min(tr / (g.sad_mm - rmax), 1.0);
+        const int rc = build_staged(h, std::asin(xs) / xs * tr / dgamma * 1.0005);
+        if (rc != OSIV_OK) { osiv_destroy(h); return rc; }
+        // the staged kernel copies whole windows of a residual row: the row's zero columns must cover one window
+        if (h->st_ready) h->res_pad = std::max(h->res_pad, (h->st_W + 3) / 4 * 4);
+    }
     *out = h;
     return OSIV_OK;
 }
@@ -464,7 +658,8 @@ int osiv_destroy(osiv_handle* h) {
         cudaDeviceSynchronize();
         void* ptrs[] = {h->d_rays, h->d_views, h->d_hs, h->d_imgA, h->d_imgB, h->d_imgTA, h->d_imgTB, h->d_best, h->d_res,
                         h->d_dparts, h->d_state, h->d_not_finite, h->d_inv_bref, h->d_trace,
-                        h->d_forced, h->d_dhist, h->d_itab[0], h->d_itab[1], h->d_hcounts, h->d_hblank, h->d_himg};
+                        h->d_forced, h->d_dhist, h->d_itab[0], h->d_itab[1], h->d_hcounts, h->d_hblank, h->d_himg,
+                        h->d_regions, h->d_itab2, h->d_bwin, h->d_blob};
         for (void* p : ptrs) if (p) cudaFree(p);
         for (cudaEvent_t e : h->events) cudaEventDestroy(e);
         cudaGetLastError();
@@ -508,6 +703,19 @@ int osiv_set_symmetry(osiv_handle* h, int32_t enable) {
     return OSIV_OK;
 }
 
+int osiv_set_back_kernel(osiv_handle* h, int32_t general_only) {
+    if (!h) return OSIV_ERR_INVALID_ARG;
+    h->st_off = general_only ? 1 : 0;
+    return OSIV_OK;
+}
+
+int osiv_get_back_kernel(const osiv_handle* h, int32_t n_subsets, int32_t batch, int32_t* staged) {
+    if (!h || !staged || batch <= 0 || (n_subsets > 0 && h->geom.n_views % n_subsets != 0)) return OSIV_ERR_INVALID_ARG;
+    const int VS = n_subsets > 0 ? h->geom.n_views / n_subsets : h->geom.n_views;
+    *staged = use_staged(h, plan_back(h, VS, batch), false, plan_forward(h, VS, batch)) ? 1 : 0;
+    return OSIV_OK;
+}
+
 int osiv_set_overlap(osiv_handle* h, int32_t enable) {
     if (!h) return OSIV_ERR_INVALID_ARG;
     h->use_pdl = enable ? 1 : 0;
@@ -521,6 +729,10 @@ int osiv_get_plan(const osiv_handle* h, int32_t n_subsets, int32_t batch, int32_
     const BackPlan b = plan_back(h, VS, batch);
     out8[0] = f.ns; out8[1] = f.segs; out8[2] = f.nparts * ((batch + f.sb - 1) / f.sb); out8[3] = f.threads;
     out8[4] = b.ns; out8[5] = b.shares; out8[6] = b.nblk * ((batch + b.sb - 1) / b.sb); out8[7] = b.threads;
+    if (use_staged(h, b, false)) {
+        const StagedPlan sp = plan_staged(h, VS);
+        out8[5] = BS_SHARES; out8[6] = sp.nblk * batch; out8[7] = sp.threads;
+    }
     return OSIV_OK;
 }
 
@@ -577,6 +789,11 @@ int osiv_backward(osiv_handle* h, const float* d_sino, float* d_img, int32_t bat
                                                                                     p.ns, Cp);
     BackArgs b{};
     b.g = h->dg; b.res = h->d_res; b.Cp = Cp; b.subset = subset; b.M = M; b.VS = VS; b.batch = batch; b.out = d_img; b.tpb = p.tpb; b.shares = p.shares; b.ngx = p.ngx; b.tpb_magic = div_magic(p.tpb); b.ngx_magic = div_magic(p.ngx);
+    if (use_staged(h, p, false)) {
+        if ((rc = ensure_blob(h, M, st)) != OSIV_OK) return rc;
+        if (launch_back_staged<0>(h, plan_staged(h, VS), batch, b, st, false) != cudaSuccess) { cudaGetLastError(); return OSIV_ERR_CUDA; }
+        return launch_check(h, 2);
+    }
     if ((rc = ensure_intervals(h, p, st)) != OSIV_OK) return rc;
     b.itab = h->d_itab[p.ns == 4]; b.ntiles = p.ntiles;
     if (launch_back<0>(p, batch, b, st, false) != cudaSuccess) { cudaGetLastError(); return OSIV_ERR_CUDA; }
@@ -644,8 +861,14 @@ int osiv_reconstruct(osiv_handle* h, const float* d_counts, const float* d_blank
     f.res = h->d_res; f.Cp = Cp; f.dparts = h->d_dparts;
     BackArgs b{};
     b.g = h->dg; b.res = h->d_res; b.Cp = Cp; b.M = M; b.VS = VS; b.batch = batch; b.view_shift = vshift; b.tv_z = (float)prm->tv_z; b.best = best; b.tpb = bp.tpb; b.shares = bp.shares; b.ngx = bp.ngx; b.tpb_magic = div_magic(bp.tpb); b.ngx_magic = div_magic(bp.ngx);
-    if ((rc = ensure_intervals(h, bp, st)) != OSIV_OK) return rc;
-    b.itab = h->d_itab[bp.ns == 4]; b.ntiles = bp.ntiles;
+    const bool staged = use_staged(h, bp, stack, fp);
+    const StagedPlan sp = staged ? plan_staged(h, VS) : StagedPlan{};
+    if (staged) {
+        if ((rc = ensure_blob(h, M, st)) != OSIV_OK) return rc;
+    } else {
+        if ((rc = ensure_intervals(h, bp, st)) != OSIV_OK) return rc;
+        b.itab = h->d_itab[bp.ns == 4]; b.ntiles = bp.ntiles;
+    }
     b.dparts = h->d_dparts; b.nparts = fp.nparts; b.not_finite = h->d_not_finite;
     b.ip.lambda0 = prm->lambda0; b.ip.up = prm->lambda_up; b.ip.down = prm->lambda_down; b.ip.lmin = prm->lambda_min;
     b.ip.forced = (prm->forced_lambda && N > 0) ? h->d_forced : nullptr;
@@ -668,11 +891,11 @@ int osiv_reconstruct(osiv_handle* h, const float* d_counts, const float* d_blank
     for (int n = 0; n < N; ++n) {
         const int m = n % M;                               // PAPER.md:118, C11
         f.img = cur; f.imgT = curT; f.subset = m; f.iter = n; b.iter = n;
-        if (launch_forward<1>(fp, batch, f, st, pdl) != cudaSuccess) { cudaGetLastError(); return OSIV_ERR_CUDA; }
+        OSIV_CUDA(launch_forward<1>(fp, batch, f, st, pdl));
         if (prof) cudaEventRecord(h->events[2 * n + 1], st);
         b.img = cur; b.img_new = nxt; b.imgT_new = nxtT; b.subset = m;
         b.state_in = state[n & 1]; b.state_out = state[(n + 1) & 1];
-        if (launch_back<1>(bp, batch, b, st, pdl) != cudaSuccess) { cudaGetLastError(); return OSIV_ERR_CUDA; }
+        OSIV_CUDA(staged ? launch_back_staged<1>(h, sp, batch, b, st, pdl) : launch_back<1>(bp, batch, b, st, pdl));
         if (prof) cudaEventRecord(h->events[2 * n + 2], st);
         h->launches += 2;
         float* t;

@@ -43,7 +43,7 @@ namespace osiv {
 // dependent-launch wait, 2 after it, 3 end of the main loop (latest warp), 4 after the block barrier, 5 block end (latest
 // warp), 6 = SM id, 7 = a mark inside the prologue (K1: own ray loaded and clipped, before the first barrier; K2: tile
 // origin known), 8 = %globaltimer [ns] read right after slot 0 (ties the SM's cycle counter to the device-wide clock).
-constexpr int TL_BLOCKS = 256, TL_SLOTS = 12;
+constexpr int TL_BLOCKS = 256, TL_SLOTS = 16;
 #ifdef OSIV_TRACE
 __device__ unsigned long long g_timeline[4][TL_BLOCKS][TL_SLOTS];
 __device__ __forceinline__ void tl_stamp(int iter, int kernel, int slot, bool latest) {
@@ -57,7 +57,7 @@ __device__ __forceinline__ void tl_stamp(int iter, int kernel, int slot, bool la
             asm volatile("mov.u32 %0, %%smid;" : "=r"(sm));
             asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(gt));
             row[6] = sm; row[8] = gt;
-            row[3] = 0; row[5] = 0;                      // the "latest warp" slots restart for this launch
+            row[3] = 0; row[5] = 0; for (int k = 9; k < TL_SLOTS; ++k) row[k] = 0;     // the "latest warp" slots restart for this launch
         }
     }
 }
@@ -468,10 +468,10 @@ __device__ __forceinline__ double sum_partials(const double* p, int n, int lane)
     return D;
 }
 
-__device__ __forceinline__ StepInfo step_rule(const BackArgs& a, int s, int lane, bool writer) {
+// A3 from the monitor value D(n) and the state after iteration n-1 (every lane of the calling warp holds both)
+__device__ __forceinline__ StepInfo step_decide(const BackArgs& a, int s, double D, const SliceState& st, int lane, bool writer) {
     StepInfo si;
-    si.D = sum_partials(a.dparts + (size_t)s * a.nparts, a.nparts, lane);
-    const SliceState st = a.state_in[s];
+    si.D = D;
     const int n = st.n;
     double lam;
     if (a.ip.forced)          lam = a.ip.forced[n];
@@ -495,6 +495,12 @@ __device__ __forceinline__ StepInfo step_rule(const BackArgs& a, int s, int lane
         }
     }
     return si;
+}
+
+__device__ __forceinline__ StepInfo step_rule(const BackArgs& a, int s, int lane, bool writer) {
+    const double D = sum_partials(a.dparts + (size_t)s * a.nparts, a.nparts, lane);
+    const SliceState st = a.state_in[s];
+    return step_decide(a, s, D, st, lane, writer);
 }
 
 // final iterate's monitor (return_best): one warp per slice

@@ -23,7 +23,7 @@ ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
-TL_BLOCKS, TL_SLOTS = 256, 12
+TL_BLOCKS, TL_SLOTS = 256, 16
 SLOTS = ("start", "before wait", "after wait", "loop end", "after barrier", "end")
 
 
@@ -39,7 +39,7 @@ def fetch():
 def to_ns(t, sm_mhz):
     """slots 0-5 and 7 are SM cycle counts; slot 8 is the global nanosecond timer at slot 0: every stamp in global ns"""
     out = t.astype(np.float64).copy()
-    for j in (0, 1, 2, 3, 4, 5, 7):
+    for j in (0, 1, 2, 3, 4, 5, 7, 9, 10, 11, 12, 13, 14, 15):
         out[:, j] = t[:, 8] + (t[:, j] - t[:, 0]) * (1e3 / sm_mhz)
     return out
 
@@ -56,7 +56,7 @@ def summarise(buf, n_last, sm_mhz):
     t0 = float(np.min(tabs[0][:, 2]))                    # first block of the first kernel released
     out = []
     for name, t in zip(names, tabs):
-        rel = (t[:, :8] - t0) * 1e-3
+        rel = (t[:, :16] - t0) * 1e-3
         out.append((name, t.shape[0], rel))
     return out
 
@@ -106,6 +106,12 @@ def main():
     for name, nb, rel in rows:
         d = rel[:, 7] - rel[:, 0]
         print(f"  {name}: {np.median(d):.2f} [{d.max():.2f}]")
+    print("staged K2 only, us after the dependent-launch wait returned, median [max] over blocks (latest warp of a block): "
+          "TV gradients done / warp 0 has issued its loads / residual windows stored / block barrier passed / blob landed / first trip walked / loop end")
+    for name, nb, rel in rows:
+        if name.startswith("K2") and rel[:, 11].max() > rel[:, 0].min():
+            d = [rel[:, j] - rel[:, 2] for j in (9, 10, 12, 11, 13, 14, 3)]
+            print(f"  {name}: " + " / ".join(f"{np.median(x):.2f} [{x.max():.2f}]" for x in d))
     ends = [rel[:, 5].max() for _, _, rel in rows]
     rels = [rel[:, 2].min() for _, _, rel in rows]
     print()

@@ -109,6 +109,60 @@ def test_quarter_turn_path_is_taken_and_agrees_with_the_general_path(osiv):
         assert h.plan(1, 1)["k1_orbit"] == 1
 
 
+SYM8 = si.ScanConfig("sym8", 40, 40, 1.3, 24, 45, sad_mm=120.0, theta0_rad=0.3, channel_offset=0.25, seed=12)   # side % 8 == 0: staged K2
+SYM64 = si.ScanConfig("sym64", 64, 64, 1.0, 88, 97, theta0_rad=0.05, seed=13)
+
+
+@pytest.mark.parametrize("cfg,subsets,model", [
+    (SYM8, [(-1, 1), (1, 2), (2, 3)], 0),                 # V_S = 24, 12, 8
+    (SYM64, [(-1, 1), (3, 11), (1, 2)], 0),               # V_S = 88 (several staging rounds), 8, 44
+    (si.scan_config("2"), [(-1, 1), (7, 10)], 0),         # all 400 views: 100 base views in rounds; 40 views: one round
+    (SYM64, [(-1, 1), (0, 2)], 1),                        # Joseph's matrix through the same kernel
+], ids=["sym8", "sym64", "config2", "sym64-joseph"])
+def test_staged_back_kernel_matches_oracle_and_general_kernel(osiv, cfg, subsets, model):
+    """K2 with its windows staged in shared memory (csrc/osiv_back_staged.cuh: 4 x 2 tiles, 8-byte ray entries with a
+    per-window orientation flag, bulk-copied constants) against the oracle's A^T and against the general gather K2."""
+    og = oracle.Geometry(cfg.nx, cfg.ny, cfg.pixel_mm, cfg.n_views, cfg.n_channels, cfg.sad_mm, cfg.dgamma_rad,
+                         cfg.channel_offset, cfg.theta0_rad, model=model)
+    gg = osiv.Geometry(cfg.nx, cfg.ny, cfg.pixel_mm, cfg.n_views, cfg.n_channels, cfg.sad_mm, cfg.sdd_mm,
+                       cfg.dgamma_rad, cfg.channel_offset, cfg.theta0_rad, model=model)
+    rng = np.random.default_rng(cfg.seed + 5)
+    with osiv.Handle(gg, max_batch=3) as h:
+        for sub, M in subsets:
+            vs = cfg.n_views if sub < 0 else cfg.n_views // M
+            sino = rng.uniform(0.0, 1.0, size=(3, vs, cfg.n_channels)).astype(np.float32)
+            assert h.back_kernel(M if sub >= 0 else 0, 3) == "staged"
+            got = host(h.backward(dev(sino), sub, M))
+            h.set_back_kernel(general_only=True)
+            assert h.back_kernel(M if sub >= 0 else 0, 3) == "general"
+            gen = host(h.backward(dev(sino), sub, M))
+            h.set_back_kernel(general_only=False)
+            for s in range(3):
+                assert rel(got[s], oracle.backward(og, sino[s], sub, M)) < PROJ_TOL, (cfg.name, sub, M, s)
+            assert rel(got, gen) < 2e-6
+            again = host(h.backward(dev(sino), sub, M))
+            assert np.array_equal(got, again)                     # no atomics on data, fixed-order sums
+
+
+def test_staged_back_kernel_in_the_iteration(osiv):
+    """The whole iteration with the staged K2 against the general K2 (same K1): equal lambda traces, images equal to
+    rounding order; with return_best, a per-channel blank scan and three slices per launch."""
+    cfg = si.scan_config("2")
+    _, gg = geoms(cfg)
+    counts = np.stack([si.make_case(cfg, slice_index=s)[2] for s in range(3)])
+    blank = (cfg.i0 * (1.0 + 0.05 * np.cos(np.arange(cfg.n_channels)))).astype(np.float32)
+    prm = osiv.Params(beta=0.005, n_subsets=10, n_iters=40, return_best=1)
+    with osiv.Handle(gg, max_batch=3) as h:
+        assert h.back_kernel(10, 3) == "staged"
+        a, ta = h.reconstruct(dev(counts), dev(blank), prm, trace=True)
+        h.set_back_kernel(general_only=True)
+        b, tb = h.reconstruct(dev(counts), dev(blank), prm, trace=True)
+    a, b = host(a), host(b)
+    assert np.array_equal(ta[:, :, 1], tb[:, :, 1])
+    assert np.allclose(ta[:, :, 0], tb[:, :, 0], rtol=1e-5)
+    assert rel(a, b) < 5e-6
+
+
 def test_projector_near_axis_rays(osiv):
     """G10 stress: theta0 = 1e-7 puts the central ray of views 0 and V/2 (and, with V = 4k, V/4 and 3V/4) within
     1e-7 rad of a pixel edge.  The chord of such a ray is a ramp 1e-7 pixel wide, which float32 positions
