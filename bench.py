@@ -36,9 +36,27 @@ UNIT = "iterations/s"
 FP32_FLOP_PER_NNZ = 6          # q (FMA, 2) + half-width minus |q| (1) + clamp (1) + accumulate (FMA, 2)
 NNZ_PER_RAY_PER_N = 1.193      # measured non-zeros per ray / N when the fan spans the inscribed circle
 SM_COUNT, FP32_LANES_PER_SM = 148, 128
-# dram__bytes_read.sum + dram__bytes_write.sum per launch at config 3 from the committed full-set ncu capture
-# (profiles/r1g_ncu_config3.md; ncu flushes the caches before every replay, so this is the cold-cache figure)
-NCU_DRAM_BYTES_PER_LAUNCH = {"3": {"k_forward<1>": 2431744, "k_back<1>": 4125184}}
+# per-launch instruction / wavefront / sector / DRAM-byte counts of the two hot kernels at config 3: read from the
+# committed ncu capture of this code (profiles/<NCU_COUNTS>.csv, written by `python -m paper_1903_10088_b200.ncu_summary`
+# from ncu's raw page; the .md beside it names the ncu command).  Counts do not depend on timing; the times they are
+# divided by are measured live in this run.
+NCU_COUNTS = {"3": "r2_ncu_config3_counts.csv"}
+
+
+def load_ncu_counts(workload):
+    """{'k_forward': {...}, 'k_back': {...}} from the committed capture, or {} when there is none for this workload"""
+    import csv
+    name = NCU_COUNTS.get(workload)
+    path = os.path.join(ROOT, "profiles", name) if name else None
+    if not path or not os.path.exists(path):
+        return {}, None
+    out = {}
+    for row in csv.DictReader(open(path)):
+        key = "k_forward" if row["kernel"].startswith("k_forward") else "k_back" if row["kernel"].startswith("k_back") else None
+        if key and key not in out:
+            out[key] = {k: float(v) for k, v in row.items() if k != "kernel"}
+            out[key]["name"] = row["kernel"]
+    return out, "profiles/" + name
 
 
 def load_peaks():
@@ -239,7 +257,11 @@ def run_ours(args, cfg, beta):
 
     peaks, peak_kind = load_peaks()
     sm_mhz_peak = float(peaks.get("sm_max_mhz", 1965.0))
-    alu_peak_tflops = SM_COUNT * FP32_LANES_PER_SM * 2 * sm_mhz_peak * 1e6 / 1e12
+    alu_peak_derived = SM_COUNT * FP32_LANES_PER_SM * 2 * sm_mhz_peak * 1e6 / 1e12
+    # the binding units' peaks, measured in this process (csrc/osiv_probes.cu; MEASURED_PEAKS.json has HBM and bf16 only)
+    probe = osiv.probe_peaks(local)
+    alu_peak_tflops = float(probe["ffma_tflops"])
+    ncu, ncu_file = load_ncu_counts(cfg.name if batch == 1 else "")
     vs = cfg.n_views // cfg.n_subsets
     nnz = NNZ_PER_RAY_PER_N * max(cfg.nx, cfg.ny) * vs * cfg.n_channels * batch       # per launch, fwd = back
     kernels = {}
@@ -248,23 +270,47 @@ def run_ours(args, cfg, beta):
         tf = nnz * FP32_FLOP_PER_NNZ / (us * 1e-6) / 1e12
         kernels[name] = {"avg_us": us, "achieved_tflops": tf, "frac": tf / alu_peak_tflops, "launches": n}
     dom = max(kernels, key=lambda k: kernels[k]["avg_us"])
+    # issue / L1 / L2 / DRAM fractions: counts per launch from the committed ncu capture of this code over the live time
+    for name in kernels:
+        c = ncu.get("k_forward" if name.startswith("k_forward") else "k_back")
+        if not c:
+            continue
+        t = kernels[name]["avg_us"] * 1e-6
+        l1_bytes = c["l1_wavefronts_per_sm"] * 128.0 * SM_COUNT
+        kernels[name].update({
+            "ncu_kernel": c["name"],
+            "issue": {"warp_instructions": c["warp_instructions"], "achieved_ginst_s": c["warp_instructions"] / t / 1e9,
+                      "peak_ginst_s": probe["issue_ginst_per_s"], "frac": c["warp_instructions"] / t / 1e9 / probe["issue_ginst_per_s"]},
+            "l1": {"wavefronts_per_sm": c["l1_wavefronts_per_sm"], "achieved_gbs": l1_bytes / t / 1e9,
+                   "peak_gbs": probe["l1_read_gbs"], "frac": l1_bytes / t / 1e9 / probe["l1_read_gbs"],
+                   "note": "data-pipe wavefronts x 128 B (global and shared memory share the pipe)"},
+            "l2": {"sectors": c["l2_sectors"], "achieved_gbs": c["l2_sectors"] * 32.0 / t / 1e9,
+                   "peak_gbs": probe["l2_read_gbs"], "frac": c["l2_sectors"] * 32.0 / t / 1e9 / probe["l2_read_gbs"]},
+            "dram_bytes": c["dram_bytes"]})
     # compulsory HBM bytes per launch: everything is L2-resident, so this is a floor
     hbm_bytes = {"k_forward<1>": (cfg.nx * cfg.ny * 4 + 2 * vs * cfg.n_channels * 4 + vs * cfg.n_channels * 32) * batch,
                  # + K2's candidate-interval table: one int per (view of the subset, 2x2 tile of the base quadrant)
                  "k_back<1>": (cfg.nx * cfg.ny * 4 * 3 + vs * cfg.n_channels * 16) * batch + vs * (cfg.nx // 4) * (cfg.ny // 4) * 4}
+    chain_t = t_dev / args.steps / (2 * cfg.n_iters)
     roof = {"bound": "alu", "kernel": dom, "achieved": kernels[dom]["achieved_tflops"], "peak": alu_peak_tflops,
             "unit": "TFLOP/s", "frac": kernels[dom]["frac"],
-            "traffic": NCU_DRAM_BYTES_PER_LAUNCH.get(cfg.name, {}).get(dom),
-            "peak_source": f"148 SMs x 128 FP32 lanes x 2 flop x {sm_mhz_peak:.0f} MHz ({peak_kind} sm_max_mhz)",
+            "traffic": kernels[dom].get("dram_bytes"),
+            "traffic_source": (ncu_file + ": dram__bytes_read.sum + dram__bytes_write.sum per launch, cold caches") if ncu_file else None,
+            "peak_source": f"FP32 FFMA probe run in this process (csrc/osiv_probes.cu); derived 148 SMs x 128 lanes x 2 flop x "
+                           f"{sm_mhz_peak:.0f} MHz = {alu_peak_derived:.1f} TFLOP/s",
+            "probe_peaks": probe,
+            "issue": kernels[dom].get("issue"), "l1": kernels[dom].get("l1"), "l2": kernels[dom].get("l2"),
+            "counts_source": ncu_file,
             "algorithmic_flop_per_launch": nnz * FP32_FLOP_PER_NNZ, "nnz_per_launch": nnz,
             "timing": "CUDA events around every launch on the launching stream, 2 extra steps after the timed region; "
                       "an event between two launches serialises them, so these are stand-alone kernel durations "
                       "(in the timed region K1 and K2 overlap their prologues through programmatic dependent launch)",
             "kernels": kernels,
             # in the timed region K1 and K2 are chained by dependent launches: the step's time over its hot launches
-            "chain": {"us_per_launch": 1e6 * t_dev / args.steps / (2 * cfg.n_iters),
-                      "achieved_tflops": nnz * FP32_FLOP_PER_NNZ / (t_dev / args.steps / (2 * cfg.n_iters)) / 1e12,
-                      "frac": nnz * FP32_FLOP_PER_NNZ / (t_dev / args.steps / (2 * cfg.n_iters)) / 1e12 / alu_peak_tflops},
+            "chain": {"us_per_launch": 1e6 * chain_t,
+                      "achieved_tflops": nnz * FP32_FLOP_PER_NNZ / chain_t / 1e12,
+                      "frac": nnz * FP32_FLOP_PER_NNZ / chain_t / 1e12 / alu_peak_tflops,
+                      "issue_frac": (sum(c["warp_instructions"] for c in ncu.values()) / 2.0 / chain_t / 1e9 / probe["issue_ginst_per_s"]) if len(ncu) == 2 else None},
             "hbm": {"compulsory_bytes_per_launch": hbm_bytes[dom],
                     "achieved_gbs": hbm_bytes[dom] / (kernels[dom]["avg_us"] * 1e-6) / 1e9,
                     "peak_gbs": float(peaks["hbm_gbs"]), "peak_kind": peak_kind,
@@ -286,19 +332,33 @@ def run_ours(args, cfg, beta):
             "gpu_launches": int(launches),
             "roofline": roof}
 
+    # the other workloads of BASELINE.json inside the same JSON line (one line per run; these are not the headline)
+    if world == 1 and args.workload == "3" and batch == 1 and not args.no_extra:
+        del h, counts, out, flush
+        torch.cuda.empty_cache()
+        extra = {}
+        extra["config4"] = batch_throughput(osiv, si.scan_config("4"), 0.005, 64, 2, 1, dev)
+        for name in ("5a", "5b"):
+            pa = argparse.Namespace(steps=5, warmup=3)
+            extra["config" + name] = projector_pair(pa, si.scan_config(name))
+        for b2 in (0.001, 0.02):                    # config 3's beta sweep: same launches, other data
+            extra[f"config3_beta{b2}"] = batch_throughput(osiv, cfg, b2, 1, 3, 1, dev)
+        line["extra"] = extra
     if not args.no_cpu_baseline:
-        n_sample = min(cfg.n_iters, 5 * cfg.n_subsets)
+        n_sample = min(cfg.n_iters, 10 * cfg.n_subsets)
         dt, cores, _ = oracle_sample(cfg, beta, counts_np[0], n_sample)
         line["cpu_baseline"] = {"value": n_sample / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
                                 "sample": f"first {n_sample} of {cfg.n_iters} subset iterations of slice 0 "
                                           f"({dt:.1f} s, float64 oracle with OpenMP)"}
+        if args.cpu_plan != "none":
+            line["cpu_baseline"]["plan"] = cpu_plan(args, args.cpu_plan == "full")
     print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()
     return 0
 
 
-def run_projector_pair(args, cfg):
+def projector_pair(args, cfg):
     """Config 5 (BASELINE.json): forward A and adjoint A^T alone, all views, on a uniform-random image / sinogram.
     Not the headline metric: one extra JSON line with ms per pass, nnz/s ("rays.pixels/s" = ray-pixel intersections),
     algorithmic GB/s against the measured HBM peak and the adjoint-identity error of the fp32 outputs."""
@@ -336,8 +396,71 @@ def run_projector_pair(args, cfg):
                       "hbm_frac": bytes_alg / (ms * 1e-3) / 1e9 / float(peaks["hbm_gbs"]), "hbm_peak_kind": kind,
                       "alu_frac": nnz * FP32_FLOP_PER_NNZ / (ms * 1e-3) / 1e12 /
                                   (SM_COUNT * FP32_LANES_PER_SM * 2 * float(peaks.get("sm_max_mhz", 1965.0)) * 1e6 / 1e12)}
-    print(json.dumps(line))
+    return line
+
+
+def run_projector_pair(args, cfg):
+    print(json.dumps(projector_pair(args, cfg)))
     return 0
+
+
+def batch_throughput(osiv, cfg, beta, batch, steps, warmup, dev):
+    """slices/s of `batch` slices per launch (config 4): CUDA events around whole reconstructions, L2 flushed in between"""
+    import torch
+    geom = osiv.Geometry(cfg.nx, cfg.ny, cfg.pixel_mm, cfg.n_views, cfg.n_channels, cfg.sad_mm, cfg.sdd_mm,
+                         cfg.dgamma_rad, cfg.channel_offset, cfg.theta0_rad)
+    counts = torch.from_numpy(np.stack([si.make_case(cfg, slice_index=s)[2] for s in range(batch)])).to(dev)
+    prm = osiv.Params(beta=beta, n_subsets=cfg.n_subsets, n_iters=cfg.n_iters)
+    out = torch.empty((batch, cfg.ny, cfg.nx), dtype=torch.float32, device=dev)
+    flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device=dev)
+    with osiv.Handle(geom, max_batch=batch, device=dev.index or 0) as h:
+        for _ in range(warmup):
+            h.reconstruct(counts, cfg.i0, prm, out=out)
+        ts = []
+        for _ in range(steps):
+            flush.zero_()
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(); h.reconstruct(counts, cfg.i0, prm, out=out); b.record()
+            torch.cuda.synchronize()
+            ts.append(a.elapsed_time(b))
+        plan = h.plan(cfg.n_subsets, batch)
+    ms = float(np.mean(ts))
+    vs = cfg.n_views // cfg.n_subsets
+    nnz = NNZ_PER_RAY_PER_N * max(cfg.nx, cfg.ny) * vs * cfg.n_channels * batch
+    us_launch = 1e3 * ms / (2 * cfg.n_iters)
+    return {"workload": f"config{cfg.name}: {batch} slices of {cfg.nx}x{cfg.ny}, {cfg.n_views}x{cfg.n_channels}, {cfg.n_subsets} subsets, "
+                        f"{cfg.n_iters} iterations, beta={beta}", "steps": steps, "warmup": warmup, "ms_per_step": ms,
+            "slices_per_s": batch / (ms * 1e-3), "iterations_per_s": batch * cfg.n_iters / (ms * 1e-3),
+            "us_per_slice_iteration": 1e3 * ms / (batch * cfg.n_iters), "plan": plan,
+            "achieved_tflops": nnz * FP32_FLOP_PER_NNZ / (us_launch * 1e-6) / 1e12}
+
+
+def cpu_plan(args, full):
+    """the float64 oracle, as it stands, on the host cores (never inside a timed GPU region):
+    configs 1 and 2 in full, one projector pass of 5a; with --cpu-plan full also config 3's 500 iterations, 5b and two slices
+    of config 4 (scaled to 64 and labelled so)."""
+    import oracle
+    out = {"cores": oracle.num_threads(), "kind": "oracle"}
+    for name in ("1", "2") + (("3",) if full else ()):
+        c = si.scan_config(name)
+        _, _, cnt = si.make_case(c)
+        beta = 0.005 if name == "3" else c.betas[0]
+        dt, _, _ = oracle_sample(c, beta, cnt, c.n_iters)
+        out["config" + name] = {"seconds": dt, "iterations": c.n_iters, "iterations_per_s": c.n_iters / dt, "sample": "full reconstruction"}
+    if full:
+        c = si.scan_config("4")
+        dts = [oracle_sample(c, 0.005, si.make_case(c, slice_index=s)[2], c.n_iters)[0] for s in range(2)]
+        out["config4"] = {"seconds_64_slices_scaled": 32.0 * sum(dts), "seconds_2_slices": sum(dts),
+                          "slices_per_s": 2.0 / sum(dts), "sample": "2 slices x 500 iterations, scaled x32 (labelled as scaled)"}
+    for name in ("5a",) + (("5b",) if full else ()):
+        c = si.scan_config(name)
+        og = oracle.Geometry(c.nx, c.ny, c.pixel_mm, c.n_views, c.n_channels, c.sad_mm)
+        img, sino = si.uniform_image(c), si.uniform_sinogram(c)
+        t0 = time.perf_counter(); oracle.forward(og, img); t1 = time.perf_counter(); oracle.backward(og, sino); t2 = time.perf_counter()
+        nnz = NNZ_PER_RAY_PER_N * max(c.nx, c.ny) * c.n_views * c.n_channels
+        out["config" + name] = {"forward_s": t1 - t0, "back_s": t2 - t1, "forward_nnz_per_s": nnz / (t1 - t0), "back_nnz_per_s": nnz / (t2 - t1),
+                                "sample": "one forward and one back pass over all views"}
+    return out
 
 
 def main():
@@ -350,6 +473,9 @@ def main():
     ap.add_argument("--slices", type=int, default=0, help="slices per GPU (default 1; 64 for workload 4)")
     ap.add_argument("--beta", type=float, default=None)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-extra", action="store_true", help="skip the config 4 / 5a / 5b / beta-sweep figures inside the line")
+    ap.add_argument("--cpu-plan", default="short", choices=["none", "short", "full"],
+                    help="BASELINE.md section 3 oracle timings next to cpu_baseline: short = configs 1, 2, 5a; full = + 3, 4, 5b (minutes)")
     ap.add_argument("--probe", action="store_true", help="print the measured FP32 / issue / L2 / shared-memory / L1 peaks and exit")
     args = ap.parse_args()
     if args.probe:

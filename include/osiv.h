@@ -223,6 +223,12 @@ int osiv_get_profile(const osiv_handle* h, double* ms_forward, int64_t* n_forwar
  * 4*256*16.  Synchronises the device.  Driver: `python -m paper_1903_10088_b200.timeline`. */
 int osiv_debug_timeline(uint64_t* h_out, int32_t n_entries);
 
+/* Index checks of the two hot kernels (only in the build made with -DOSIV_CHECKED, `python -m paper_1903_10088_b200.build
+ * --check` -> libosiv_check.so; the regular library returns OSIV_ERR_INVALID_ARG).  Every gather index that relies on
+ * clamping, zero padding or slack behind a row is compared with its buffer's extent on the device; h_out3 receives
+ * {violations since the library was loaded, site number of the first one, warp-level checks made}.  Synchronises the device. */
+int osiv_debug_checks(uint64_t* h_out3);
+
 /* Micro-probes of the units that bound the two hot kernels (csrc/osiv_probes.cu): saturating loops
  * of one instruction kind at full occupancy on `device`, CUDA-event timed, best of 5 (takes about 0.1 s).
  * out8 = { FP32 TFLOP/s with FFMA (three register operands), FP32 TFLOP/s with FFMA2 (fma.rn.f32x2),

@@ -6,6 +6,6 @@ CPU fallback: importing works anywhere, but every compute call raises ``OsivErro
 device, and loading raises if the library has not been built (``python -m paper_1903_10088_b200.build``).
 """
 from .binding import (  # noqa: F401
-    Geometry, Params, Handle, OsivError, lib, lib_path, version, strerror, default_params, ray_table, probe_peaks,
+    Geometry, Params, Handle, OsivError, lib, lib_path, version, strerror, default_params, ray_table, probe_peaks, debug_checks,
     OSIV_OK, OSIV_ERR_INVALID_ARG, OSIV_ERR_CUDA, OSIV_ERR_NOT_FINITE, EXPORTED_SYMBOLS,
 )

@@ -17,7 +17,7 @@ OSIV_OK, OSIV_ERR_INVALID_ARG, OSIV_ERR_CUDA, OSIV_ERR_NOT_FINITE = 0, -1, -2, -
 
 EXPORTED_SYMBOLS = (
     "osiv_version", "osiv_strerror", "osiv_default_params", "osiv_create", "osiv_destroy", "osiv_ray_table", "osiv_get_dgamma",
-    "osiv_get_tau", "osiv_launch_count", "osiv_set_symmetry", "osiv_set_overlap", "osiv_set_back_kernel", "osiv_get_back_kernel", "osiv_get_plan", "osiv_set_profiling", "osiv_get_profile", "osiv_forward", "osiv_backward", "osiv_tv_gradient", "osiv_reconstruct",
+    "osiv_get_tau", "osiv_launch_count", "osiv_set_symmetry", "osiv_set_overlap", "osiv_set_back_kernel", "osiv_get_back_kernel", "osiv_debug_checks", "osiv_get_plan", "osiv_set_profiling", "osiv_get_profile", "osiv_forward", "osiv_backward", "osiv_tv_gradient", "osiv_reconstruct",
     "osiv_reconstruct_host", "osiv_probe_peaks", "osiv_debug_timeline",
 )
 
@@ -92,7 +92,8 @@ def lib():
     global _lib
     if _lib is None:
         # OSIV_TRACE_BUILD=1 selects the timeline build of the same sources (diagnostics; see timeline.py)
-        path = _build.build(trace=os.environ.get("OSIV_TRACE_BUILD", "") == "1")
+        # OSIV_CHECK_BUILD=1 selects the build with device-side index checks (diagnostics; osiv_debug_checks)
+        path = _build.build(trace=os.environ.get("OSIV_TRACE_BUILD", "") == "1", check=os.environ.get("OSIV_CHECK_BUILD", "") == "1")
         L = C.CDLL(path)
         vp, ip = C.c_void_p, C.c_int32
         L.osiv_version.restype = C.c_int
@@ -121,6 +122,7 @@ def lib():
         L.osiv_reconstruct_host.argtypes = [vp, vp, vp, C.c_float, C.POINTER(_CParams), ip, vp, vp, vp]
         L.osiv_probe_peaks.argtypes = [ip, C.POINTER(C.c_double)]
         L.osiv_debug_timeline.argtypes = [vp, ip]
+        L.osiv_debug_checks.argtypes = [vp]
         _lib = L
     return _lib
 
@@ -131,6 +133,13 @@ def version() -> int:
 
 PROBE_FIELDS = ("ffma_tflops", "ffma2_tflops", "issue_ginst_per_s", "l2_read_gbs", "smem_read_gbs", "l1_read_gbs",
                 "l1_read_b32_gbs", "sms")
+
+
+def debug_checks() -> dict:
+    """osiv_debug_checks: {violations, first_site, checks} of the checked build (raises OsivError in the regular build)"""
+    out = (C.c_uint64 * 3)()
+    _check(lib().osiv_debug_checks(out), "osiv_debug_checks")
+    return {"violations": int(out[0]), "first_site": int(out[1]), "checks": int(out[2])}
 
 
 def probe_peaks(device: int = 0) -> dict:

@@ -46,10 +46,13 @@ def _stale(so: str) -> bool:
     return any(os.path.getmtime(d) > t for d in DEPS)
 
 
-def build(force: bool = False, verbose: bool = False, trace: bool = False) -> str:
-    so = SO_TRACE if trace else SO
+SO_CHECK = os.path.join(_HERE, "libosiv_check.so")      # the same sources with -DOSIV_CHECKED (index checks, diagnostics)
+
+
+def build(force: bool = False, verbose: bool = False, trace: bool = False, check: bool = False) -> str:
+    so = SO_TRACE if trace else SO_CHECK if check else SO
     if force or _stale(so):
-        cmd = [nvcc_path()] + NVCC_FLAGS + (["-DOSIV_TRACE"] if trace else []) + ["-I", INCLUDE, "-o", so] + SOURCES
+        cmd = [nvcc_path()] + NVCC_FLAGS + (["-DOSIV_TRACE"] if trace else ["-DOSIV_CHECKED"] if check else []) + ["-I", INCLUDE, "-o", so] + SOURCES
         res = subprocess.run(cmd, capture_output=True, text=True)
         if verbose or res.returncode != 0:
             sys.stderr.write(res.stdout + res.stderr)
@@ -59,4 +62,4 @@ def build(force: bool = False, verbose: bool = False, trace: bool = False) -> st
 
 
 if __name__ == "__main__":
-    print(build(force="--force" in sys.argv, verbose=True, trace="--trace" in sys.argv))
+    print(build(force="--force" in sys.argv, verbose=True, trace="--trace" in sys.argv, check="--check" in sys.argv))

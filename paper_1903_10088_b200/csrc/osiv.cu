@@ -49,6 +49,7 @@ struct osiv_handle {
     size_t hi_elems = 0;        float* d_himg = nullptr;
     int64_t launches = 0;
     int force_ns1 = 0;                  // osiv_set_symmetry(h, 0): always take the general path
+    long long ray_entries = 0;          // float4 entries behind d_rays (table + zero slack)
     // staged K2 (osiv_back_staged.cuh): regions of the base quadrant, per-(view, block) windows, per-tile intervals
     int st_ready = 0;                   // 1: tables built and usable; 0: this geometry does not take the staged kernel
     int st_off = 0;                     // osiv_set_back_kernel(h, 1): always the general K2
@@ -389,8 +390,8 @@ int build_staged(osiv_handle* h, double tile_hw_staged) {
     const bool ok = cudaMemcpy(hmax, d_max, sizeof(hmax), cudaMemcpyDeviceToHost) == cudaSuccess;
     cudaFree(d_max);
     if (!ok) { cudaGetLastError(); return OSIV_ERR_CUDA; }
-    // a lane walks up to the warp's largest count, rounded up to even, from its own first candidate
-    const int W = (hmax[0] + hmax[1] + 2 + 1) / 2 * 2;
+    // a lane walks up to the warp's largest count from its own first candidate
+    const int W = (hmax[0] + hmax[1] + 1) / 2 * 2;
     if (hmax[0] >= 256 || hmax[1] >= 255 || W > 512) return OSIV_OK;
     const size_t slot = 16 + (size_t)W * 8 + (size_t)tpbp * 2 + (size_t)W * 16;       // constants + residual window
     const size_t fixed = BS_HDR_BYTES + (size_t)BS_SHARES * tpbp * BS_RED_PITCH * sizeof(float4);
@@ -598,6 +599,7 @@ int osiv_create(const osiv_geometry* geom, int32_t max_batch, int32_t device, os
     // zero slack after the last view: K2 reads past a view's last channel (general kernel: res_pad entries; staged
     // kernel: up to one window of at most 512 entries)
     rays.resize(rays.size() + h->res_pad + 4 + 512, make_float4(0.f, 0.f, 0.f, 0.f));
+    h->ray_entries = (long long)rays.size();
     if (cudaMalloc((void**)&h->d_rays, rays.size() * sizeof(float4)) != cudaSuccess ||
         cudaMalloc((void**)&h->d_hs, hs.size() * sizeof(float)) != cudaSuccess ||
         cudaMemcpy(h->d_hs, hs.data(), hs.size() * sizeof(float), cudaMemcpyHostToDevice) != cudaSuccess ||
@@ -684,6 +686,18 @@ int osiv_get_tau(const osiv_handle* h, int32_t n_subsets, double kappa, double* 
 }
 
 int64_t osiv_launch_count(const osiv_handle* h) { return h ? h->launches : 0; }
+
+int osiv_debug_checks(uint64_t* h_out3) {
+#ifdef OSIV_CHECKED
+    if (!h_out3) return OSIV_ERR_INVALID_ARG;
+    OSIV_CUDA(cudaDeviceSynchronize());
+    OSIV_CUDA(cudaMemcpyFromSymbol(h_out3, g_check, 3 * sizeof(unsigned long long)));
+    return OSIV_OK;
+#else
+    (void)h_out3;
+    return OSIV_ERR_INVALID_ARG;                          // not the checked build
+#endif
+}
 
 int osiv_debug_timeline(uint64_t* h_out, int32_t n_entries) {
 #ifdef OSIV_TRACE
@@ -788,6 +802,7 @@ int osiv_backward(osiv_handle* h, const float* d_sino, float* d_img, int32_t bat
     k_scale_sino<<<dim3((h->geom.n_channels + 255) / 256, VS, batch), 256, 0, st>>>(h->dg, d_sino, h->d_res, subset, M, VS,
                                                                                     p.ns, Cp);
     BackArgs b{};
+    b.res_floats = (long long)h->res_elems; b.ray_entries = h->ray_entries;
     b.g = h->dg; b.res = h->d_res; b.Cp = Cp; b.subset = subset; b.M = M; b.VS = VS; b.batch = batch; b.out = d_img; b.tpb = p.tpb; b.shares = p.shares; b.ngx = p.ngx; b.tpb_magic = div_magic(p.tpb); b.ngx_magic = div_magic(p.ngx);
     if (use_staged(h, p, false)) {
         if ((rc = ensure_blob(h, M, st)) != OSIV_OK) return rc;
@@ -858,8 +873,9 @@ int osiv_reconstruct(osiv_handle* h, const float* d_counts, const float* d_blank
     FwdArgs f{};
     f.g = h->dg; f.M = M; f.VS = VS; f.batch = batch; f.view_shift = vshift; f.rpb = fp.rpb; f.segs = fp.segs; f.rpb_magic = div_magic(fp.rpb); f.C_magic = div_magic(C);
     f.counts = d_counts; f.blank = d_blank; f.blank_scalar = blank_scalar; f.inv_bref = h->d_inv_bref;
-    f.res = h->d_res; f.Cp = Cp; f.dparts = h->d_dparts;
+    f.res = h->d_res; f.Cp = Cp; f.dparts = h->d_dparts; f.res_floats = (long long)h->res_elems;
     BackArgs b{};
+    b.res_floats = (long long)h->res_elems; b.ray_entries = h->ray_entries;
     b.g = h->dg; b.res = h->d_res; b.Cp = Cp; b.M = M; b.VS = VS; b.batch = batch; b.view_shift = vshift; b.tv_z = (float)prm->tv_z; b.best = best; b.tpb = bp.tpb; b.shares = bp.shares; b.ngx = bp.ngx; b.tpb_magic = div_magic(bp.tpb); b.ngx_magic = div_magic(bp.ngx);
     const bool staged = use_staged(h, bp, stack, fp);
     const StagedPlan sp = staged ? plan_staged(h, VS) : StagedPlan{};

@@ -213,12 +213,13 @@ __global__ void __launch_bounds__(128) k_build_blob(DevGeom g, int M, int VS, in
     }
 }
 
-// the candidates [rel, rel + n) of one trip against the thread's tile; two per step
+// the candidates [rel, rel + n) of one trip against the thread's tile; two per step, then the odd one
 template <int ORI>
 __device__ __forceinline__ void bs_walk(const float2* __restrict__ rp, const float4* __restrict__ vp, int n, int rel, int sw, bool o_first_x,
                                         float xc0, float yc0, float hka, float hkb, uint64_t (&acc)[2][BS_PX]) {
+    int u = 0;
 #pragma unroll 1
-    for (int u = 0; u < n; u += 2) {
+    for (; u + 1 < n; u += 2) {
         const float2 e0 = rp[u], e1 = rp[u + 1];
         const float4 v0 = vp[u], v1 = vp[u + 1];
         float w0[BS_PX], w1[BS_PX];
@@ -230,6 +231,15 @@ __device__ __forceinline__ void bs_walk(const float2* __restrict__ rp, const flo
             ffma2(acc[0][p], a0, w0[p]); ffma2(acc[1][p], b0, w0[p]);
             ffma2(acc[0][p], a1, w1[p]); ffma2(acc[1][p], b1, w1[p]);
         }
+    }
+    if (u < n) {
+        const float2 e0 = rp[u];
+        const float4 v0 = vp[u];
+        float w0[BS_PX];
+        bs_weights<ORI>(e0, (rel + u < sw) == o_first_x, xc0, yc0, hka, hkb, w0);
+        const uint64_t a0 = pack2(v0.x, v0.y), b0 = pack2(v0.z, v0.w);
+#pragma unroll
+        for (int p = 0; p < BS_PX; ++p) { ffma2(acc[0][p], a0, w0[p]); ffma2(acc[1][p], b0, w0[p]); }
     }
 }
 
@@ -286,6 +296,7 @@ __global__ void __launch_bounds__(BS_SHARES * BS_MAX_TPB, 1) k_back_staged(const
             const bool ok = s0 < SP && slot < nj * 4;
             const int c0 = __ldg(reinterpret_cast<const int*>(blob + (size_t)(j0 * 4 + (ok ? slot : 0)) * sa.slot_c));
             roff[n] = ok ? (j0 + (slot >> 2)) * a.Cp + c0 + r0 : -1;
+            OSIV_CHECK(!ok || (c0 >= 0 && c0 + W <= a.Cp && (long long)(roff[n] + 1) * 4 <= (long long)a.VS * a.Cp), 6);
         }
     };
     auto load_res = [&](float4 (&rv)[BS_RCH]) {
@@ -382,9 +393,10 @@ __global__ void __launch_bounds__(BS_SHARES * BS_MAX_TPB, 1) k_back_staged(const
                 const unsigned e = reinterpret_cast<const unsigned short*>(sp + 16 + W * 8)[i];
                 const int cnt = active ? (int)(e >> 8) : 0, rel = e & 0xff;
                 const int n = __reduce_max_sync(0xffffffffu, cnt);
+                OSIV_CHECK(e != 0xffffu && rel + n <= W && slot < JR * 4, 7);
                 const float2* rp = reinterpret_cast<const float2*>(sp + 16) + rel;
                 const float4* vp = rst + (size_t)slot * W + rel;
-                // the warp walks max-over-lanes candidates in lock step, two per step; a lane's extra candidates lie outside
+                // the warp walks max-over-lanes candidates in lock step; a lane's extra candidates lie outside
                 // its tile's support (weight exactly 0) or read the zero columns of the residual row
                 if (ori == 0)      bs_walk<0>(rp, vp, n, 0, 0, true, xc0, yc0, sa.hka, sa.hkb, acc);
                 else if (ori == 1) bs_walk<1>(rp, vp, n, 0, 0, true, xc0, yc0, sa.hka, sa.hkb, acc);

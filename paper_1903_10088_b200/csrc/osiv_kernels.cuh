@@ -66,6 +66,21 @@ __device__ __forceinline__ void tl_stamp(int iter, int kernel, int slot, bool la
 #define OSIV_TL(iter, kernel, slot, latest) do {} while (0)
 #endif
 
+// ---- index checks (diagnostics; only in the build with -DOSIV_CHECKED, `python -m paper_1903_10088_b200.build --check`;
+// compute-sanitizer is closed on the pool this was developed on): the gathers of both hot kernels rely on clamped indices
+// landing in zero padding and on reads past a row's last channel staying inside the buffers; every such index is
+// compared with its buffer's extent, g_check = {violations, site of the first one, checks made}.
+#ifdef OSIV_CHECKED
+__device__ unsigned long long g_check[4];
+__device__ __forceinline__ void osiv_check(bool ok, int site) {
+    if (!ok) { if (atomicAdd(&g_check[0], 1ull) == 0ull) g_check[1] = (unsigned long long)site; }
+    else if ((threadIdx.x & 31) == 0) atomicAdd(&g_check[2], 1ull);
+}
+#define OSIV_CHECK(cond, site) osiv_check((cond), (site))
+#else
+#define OSIV_CHECK(cond, site) do {} while (0)
+#endif
+
 constexpr int PAD = 4;                     // zero columns left and right of every padded image line
 constexpr int PADR = 1;                    // zero rows above and below a padded image
 constexpr int FWD_MAX_THREADS = 1024;      // K1: one block per SM, threads = rays per block x line segments per ray
@@ -127,6 +142,7 @@ struct FwdArgs {
                                            // holding the orbit {j, j+VS/4, j+VS/2, j+3VS/4}; columns C..Cp-1 stay zero
     int Cp;
     double* dparts;                        // MODE 1: [batch][gridDim.x] partial sums of D
+    long long res_floats;                  // floats in `res` (checked build)
 };
 
 struct BackArgs {
@@ -155,6 +171,7 @@ struct BackArgs {
     IterParams ip;
     double tau;
     float beta_over_M, eps2;
+    long long res_floats, ray_entries;     // floats in `res`, float4 entries behind g.rays (checked build)
 };
 
 // n / d for 0 <= n < 2^32 / d with the host's magic = ceil(2^32 / d) (0 for d = 1): one multiply instead of the division
@@ -323,6 +340,7 @@ __global__ void __launch_bounds__(FWD_MAX_THREADS, 1) k_forward(const FwdArgs a)
                 float4 x[2][2][SB];
 #pragma unroll
                 for (int u = 0; u < 2; ++u) {
+                    OSIV_CHECK(offP + u * pitch + i0[u] >= 0 && offP + u * pitch + i0[u] + 1 < (rowmaj ? g.img_elems : g.imgT_elems), 1);
                     const float4* p0 = qA + (size_t)(offP + u * pitch + i0[u]) * SB;
 #pragma unroll
                     for (int e = 0; e < 2; ++e)
@@ -342,6 +360,7 @@ __global__ void __launch_bounds__(FWD_MAX_THREADS, 1) k_forward(const FwdArgs a)
                 PX x[2][2];
 #pragma unroll
                 for (int u = 0; u < 2; ++u) {
+                    OSIV_CHECK(offP + u * pitch + i0[u] >= 0 && offP + u * pitch + i0[u] + 1 < (rowmaj ? g.img_elems : g.imgT_elems), 2);
                     const PX* p0 = bufA + (offP + u * pitch + i0[u]);
                     x[u][0] = __ldg(p0); x[u][1] = __ldg(p0 + 1);
                 }
@@ -427,6 +446,7 @@ __global__ void __launch_bounds__(FWD_MAX_THREADS, 1) k_forward(const FwdArgs a)
                     const double d = (double)l - (double)p;
                     d2[sl] += d * d;
                     // NS == 4: the orbit's four residuals share one float4 (K2 reads them with one load per candidate ray)
+                    OSIV_CHECK((long long)((((size_t)s * VSb + jb) * a.Cp + c) * NS + ko) < a.res_floats, 3);
                     a.res[(((size_t)s * VSb + jb) * a.Cp + c) * NS + ko] = hr;
                 }
             }
@@ -892,6 +912,8 @@ __global__ void __launch_bounds__(SB == 1 ? BK_MAX_THREADS : BKB_MAX_THREADS, SB
                         const int n = max(ncw[e], ncw[e + 1]);
 #pragma unroll 2
                         for (int u = 0; u < n; ++u) {
+                            OSIV_CHECK(offR[e] + u < a.ray_entries && offR[e + 1] + u < a.ray_entries, 4);
+                            OSIV_CHECK((long long)(offS[e] + u + 1) * NS <= (long long)a.VS * a.Cp && (long long)(offS[e + 1] + u + 1) * NS <= (long long)a.VS * a.Cp, 5);
                             const float4 rA = __ldg(rpA + u), rB = __ldg(rpB + u);
                             const float4 sA = NS == 4 ? __ldg(spA + u) : make_float4(__ldg(tpA + u), 0.f, 0.f, 0.f);
                             const float4 sB = NS == 4 ? __ldg(spB + u) : make_float4(__ldg(tpB + u), 0.f, 0.f, 0.f);

@@ -96,7 +96,9 @@ __global__ void __launch_bounds__(PT, 2) p_l1(const float4* __restrict__ buf, in
     for (int i = 0; i < iters; ++i) {
 #pragma unroll
         for (int u = 0; u < 8; ++u) {
-            const float4 v = __ldg(w + ((threadIdx.x + (u + i * 8) * 64) & 2047));
+            float4 v;
+            asm volatile("ld.global.nc.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w)
+                         : "l"(w + ((threadIdx.x + (u + i * 8) * 64) & 2047)));
             s += (v.x + v.y) + (v.z + v.w);
         }
     }
@@ -109,7 +111,11 @@ __global__ void __launch_bounds__(PT, 2) p_l1_b32(const float* __restrict__ buf,
     float s = 0.f;
     for (int i = 0; i < iters; ++i) {
 #pragma unroll
-        for (int u = 0; u < 8; ++u) s += __ldg(w + ((threadIdx.x + (u + i * 8) * 128) & 8191));
+        for (int u = 0; u < 8; ++u) {
+            float v;
+            asm volatile("ld.global.nc.f32 %0, [%1];" : "=f"(v) : "l"(w + ((threadIdx.x + (u + i * 8) * 128) & 8191)));
+            s += v;
+        }
     }
     if (s == 12345.678f) sink[0] = s;
 }
@@ -120,10 +126,15 @@ __global__ void __launch_bounds__(PT, 2) p_smem(int iters, float* sink) {
     for (int i = threadIdx.x; i < 2048; i += PT) sm[i] = make_float4((float)i, 1.f, 2.f, 3.f);
     __syncthreads();
     float s = 0.f;
+    const uint32_t base = (uint32_t)__cvta_generic_to_shared(sm);
     for (int i = 0; i < iters; ++i) {
 #pragma unroll
         for (int u = 0; u < 8; ++u) {
-            const float4 v = sm[(threadIdx.x + (u + i * 8) * 64) & 2047];
+            // volatile: the contents never change, and a plain load of a loop-invariant address is hoisted out of the loop
+            // (the first version of this probe "measured" 129 TB/s, 3.5 times what 128 B/clk/SM allow)
+            float4 v;
+            asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w)
+                         : "r"(base + 16u * ((threadIdx.x + (u + i * 8) * 64) & 2047)));
             s += (v.x + v.y) + (v.z + v.w);
         }
     }

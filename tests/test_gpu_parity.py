@@ -721,3 +721,43 @@ def test_not_finite_is_reported_by_the_host_call_without_a_trace(osiv):
         with pytest.raises(osiv.OsivError) as e:
             h.reconstruct(dev(counts), cfg.i0, osiv.Params(n_iters=2, tv_eps=0.0))
         assert e.value.status == osiv.OSIV_ERR_INVALID_ARG
+
+
+def test_checked_build_finds_no_out_of_range_index():
+    """compute-sanitizer is closed on the development pool, so the gathers that rely on clamped indices, zero padding and
+    slack behind a row are checked by the library itself: the same sources built with -DOSIV_CHECKED compare every such
+    index with its buffer's extent on the device (include/osiv.h `osiv_debug_checks`).  Runs in a child process because
+    the build is chosen when the library is loaded."""
+    import os
+    import subprocess
+    import sys
+    code = r'''
+import numpy as np, torch
+import synth_inputs as si
+import paper_1903_10088_b200 as osiv
+def geom(c, **kw):
+    return osiv.Geometry(c.nx, c.ny, c.pixel_mm, c.n_views, c.n_channels, c.sad_mm, c.sdd_mm, c.dgamma_rad, c.channel_offset, c.theta0_rad, **kw)
+cases = [(si.scan_config("1"), 1, 1), (si.scan_config("2"), 10, 1), (si.scan_config("2"), 10, 5),
+         (si.ScanConfig("sym8", 40, 40, 1.3, 24, 45, sad_mm=120.0, theta0_rad=0.3, channel_offset=0.25, seed=12), 2, 3),
+         (si.ScanConfig("odd", 37, 29, 1.3, 24, 45, sad_mm=120.0, theta0_rad=0.3, channel_offset=0.25, seed=7), 2, 4)]
+for c, M, B in cases:
+    counts = torch.from_numpy(np.stack([si.make_case(c, slice_index=s)[2] for s in range(B)])).cuda()
+    with osiv.Handle(geom(c), max_batch=B) as h:
+        h.reconstruct(counts, c.i0, osiv.Params(beta=0.005, n_subsets=M, n_iters=12, return_best=1))
+        img = torch.rand((B, c.ny, c.nx), device="cuda") * 0.013
+        sino = h.forward(img)
+        h.backward(sino)
+        if B >= 3:
+            h.reconstruct(counts, c.i0, osiv.Params(beta=0.005, n_subsets=M, n_iters=6, view_shift=1, tv_z=0.5))
+        h.set_back_kernel(True)
+        h.reconstruct(counts, c.i0, osiv.Params(beta=0.005, n_subsets=M, n_iters=6))
+    torch.cuda.synchronize()
+r = osiv.debug_checks()
+print("CHECKS", r)
+assert r["violations"] == 0 and r["checks"] > 100000, r
+'''
+    env = dict(os.environ, OSIV_CHECK_BUILD="1")
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    res = subprocess.run([sys.executable, "-c", code], cwd=root, env=env, capture_output=True, text=True, timeout=900)
+    assert res.returncode == 0, res.stdout[-2000:] + res.stderr[-2000:]
+    assert "CHECKS" in res.stdout
