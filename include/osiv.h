@@ -189,6 +189,15 @@ int osiv_set_symmetry(osiv_handle* h, int32_t enable);
  * plain stream order (same results bit for bit; used by the tests and for A/B timing). */
 int osiv_set_overlap(osiv_handle* h, int32_t enable);
 
+/* One CUDA graph per call.  By default (enable = 1) osiv_reconstruct captures its launch sequence (set-up, n_iters x
+ * (K1, K2) with their programmatic dependent edges, result) into a CUDA graph when a call repeats the previous call's
+ * arguments (pointers, parameters, batch) and replays it with a single cudaGraphLaunch while they keep repeating (SURVEY.md section 7 step
+ * 7); calls with forced_lambda or with per-kernel profiling, and drivers that cannot capture the sequence, enqueue launch
+ * by launch.  enable = 0 always enqueues launch by launch (same results bit for bit; used by the tests).
+ * osiv_graph_replays counts the graph launches made so far. */
+int osiv_set_graph(osiv_handle* h, int32_t enable);
+int64_t osiv_graph_replays(const osiv_handle* h);
+
 /* Which K2 runs.  On the quarter-turn path with one slice per block (batch < 4, no stack), grids whose side is a multiple
  * of 8 and fans below 90 degrees, K2 is the kernel that stages each block's ray-table, residual and interval windows in
  * shared memory with bulk copies (csrc/osiv_back_staged.cuh); general_only = 1 forces the general gather kernel instead

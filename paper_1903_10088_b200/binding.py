@@ -17,7 +17,7 @@ OSIV_OK, OSIV_ERR_INVALID_ARG, OSIV_ERR_CUDA, OSIV_ERR_NOT_FINITE = 0, -1, -2, -
 
 EXPORTED_SYMBOLS = (
     "osiv_version", "osiv_strerror", "osiv_default_params", "osiv_create", "osiv_destroy", "osiv_ray_table", "osiv_get_dgamma",
-    "osiv_get_tau", "osiv_launch_count", "osiv_set_symmetry", "osiv_set_overlap", "osiv_set_back_kernel", "osiv_get_back_kernel", "osiv_debug_checks", "osiv_get_plan", "osiv_set_profiling", "osiv_get_profile", "osiv_forward", "osiv_backward", "osiv_tv_gradient", "osiv_reconstruct",
+    "osiv_get_tau", "osiv_launch_count", "osiv_set_symmetry", "osiv_set_overlap", "osiv_set_back_kernel", "osiv_get_back_kernel", "osiv_set_graph", "osiv_graph_replays", "osiv_debug_checks", "osiv_get_plan", "osiv_set_profiling", "osiv_get_profile", "osiv_forward", "osiv_backward", "osiv_tv_gradient", "osiv_reconstruct",
     "osiv_reconstruct_host", "osiv_probe_peaks", "osiv_debug_timeline",
 )
 
@@ -110,6 +110,9 @@ def lib():
         L.osiv_set_symmetry.argtypes = [vp, ip]
         L.osiv_set_overlap.argtypes = [vp, ip]
         L.osiv_set_back_kernel.argtypes = [vp, ip]
+        L.osiv_set_graph.argtypes = [vp, ip]
+        L.osiv_graph_replays.argtypes = [vp]
+        L.osiv_graph_replays.restype = C.c_int64
         L.osiv_get_back_kernel.argtypes = [vp, ip, ip, C.POINTER(C.c_int32)]
         L.osiv_get_plan.argtypes = [vp, ip, ip, C.POINTER(C.c_int32)]
         L.osiv_set_profiling.argtypes = [vp, ip]
@@ -252,6 +255,13 @@ class Handle:
     def set_overlap(self, enable: bool) -> None:
         """enable=False chains K1 and K2 in plain stream order instead of programmatic dependent launches"""
         _check(lib().osiv_set_overlap(self._h, 1 if enable else 0), "osiv_set_overlap")
+
+    def set_graph(self, enable: bool) -> None:
+        """enable=False enqueues every launch of reconstruct from the host instead of replaying a captured CUDA graph"""
+        _check(lib().osiv_set_graph(self._h, 1 if enable else 0), "osiv_set_graph")
+
+    def graph_replays(self) -> int:
+        return int(lib().osiv_graph_replays(self._h))
 
     def set_back_kernel(self, general_only: bool) -> None:
         """general_only=True forces the general gather K2 where the shared-memory-staged K2 would run"""

@@ -61,6 +61,14 @@ struct osiv_handle {
     size_t blob_bytes = 0;
     int blob_M = 0;
     int use_pdl = 1;                    // osiv_set_overlap(h, 0): plain stream order between K1 and K2
+    // the launch sequence of one osiv_reconstruct call as a CUDA graph, replayed while the call's arguments repeat
+    int use_graph = 1;                  // osiv_set_graph(h, 0): enqueue every launch from the host
+    cudaStream_t cap_stream = nullptr;  // capture happens here (the caller's stream may be the legacy default stream)
+    cudaGraphExec_t graph_exec = nullptr, graph_exec2 = nullptr;   // two instances, used alternately: the upload of one launch
+                                                                    // overlaps the run of the previous one
+    std::vector<unsigned char> graph_key;
+    int64_t graph_launches = 0;         // kernels in the captured sequence
+    int64_t graph_replays = 0;
     // per-kernel event timing (osiv_set_profiling)
     bool profiling = false;
     std::vector<cudaEvent_t> events;
@@ -89,9 +97,13 @@ inline bool cuda_failed(cudaError_t e, const char* what) {
 }
 #define OSIV_CUDA(call) do { if (cuda_failed((call), #call)) return OSIV_ERR_CUDA; } while (0)
 
+// bumped whenever a workspace buffer is (re)allocated: a captured graph holds device pointers and is dropped when this moves
+long long g_alloc_gen = 0;
+
 template <class T>
 int grow(T** p, size_t* have, size_t want) {
     if (*have >= want && *p) return OSIV_OK;
+    ++g_alloc_gen;
     if (*p) { OSIV_CUDA(cudaFree(*p)); *p = nullptr; *have = 0; }
     OSIV_CUDA(cudaMalloc((void**)p, want * sizeof(T)));
     *have = want;
@@ -183,6 +195,7 @@ int ensure_images(osiv_handle* h, int batch, int sb, int ns, cudaStream_t st) {
         for (auto b : bufs) if (*b) { OSIV_CUDA(cudaFree(*b)); *b = nullptr; }
         if (h->d_best) { OSIV_CUDA(cudaFree(h->d_best)); h->d_best = nullptr; }
         h->ws_batch = 0;
+        ++g_alloc_gen;
         OSIV_CUDA(cudaMalloc((void**)&h->d_imgA, ne * sizeof(float)));
         OSIV_CUDA(cudaMalloc((void**)&h->d_imgB, ne * sizeof(float)));
         OSIV_CUDA(cudaMalloc((void**)&h->d_imgTA, nt * sizeof(float)));
@@ -473,6 +486,7 @@ int ensure_intervals(osiv_handle* h, const BackPlan& p, cudaStream_t st) {
     // one table at a time: the other orbit size's table (osiv_set_symmetry toggled, or a subset without whole orbits) goes
     for (int k = 0; k < 2; ++k)
         if (h->d_itab[k]) { OSIV_CUDA(cudaFree(h->d_itab[k])); h->d_itab[k] = nullptr; h->itab_tiles[k] = 0; }
+    ++g_alloc_gen;
     OSIV_CUDA(cudaMalloc((void**)&h->d_itab[w], (size_t)h->geom.n_views * p.ntiles * sizeof(int)));
     k_build_intervals<<<dim3((p.ntiles + 255) / 256, h->geom.n_views), 256, 0, st>>>(h->dg, p.ns, p.ngx, div_magic(p.ngx), p.ntiles, h->d_itab[w]);
     h->itab_tiles[w] = p.ntiles;
@@ -664,6 +678,9 @@ int osiv_destroy(osiv_handle* h) {
                         h->d_regions, h->d_itab2, h->d_bwin, h->d_blob};
         for (void* p : ptrs) if (p) cudaFree(p);
         for (cudaEvent_t e : h->events) cudaEventDestroy(e);
+        if (h->graph_exec) cudaGraphExecDestroy(h->graph_exec);
+        if (h->graph_exec2) cudaGraphExecDestroy(h->graph_exec2);
+        if (h->cap_stream) cudaStreamDestroy(h->cap_stream);
         cudaGetLastError();
     }
     delete h;
@@ -722,6 +739,14 @@ int osiv_set_back_kernel(osiv_handle* h, int32_t general_only) {
     h->st_off = general_only ? 1 : 0;
     return OSIV_OK;
 }
+
+int osiv_set_graph(osiv_handle* h, int32_t enable) {
+    if (!h) return OSIV_ERR_INVALID_ARG;
+    h->use_graph = enable ? 1 : 0;
+    return OSIV_OK;
+}
+
+int64_t osiv_graph_replays(const osiv_handle* h) { return h ? h->graph_replays : 0; }
 
 int osiv_get_back_kernel(const osiv_handle* h, int32_t n_subsets, int32_t batch, int32_t* staged) {
     if (!h || !staged || batch <= 0 || (n_subsets > 0 && h->geom.n_views % n_subsets != 0)) return OSIV_ERR_INVALID_ARG;
@@ -866,9 +891,6 @@ int osiv_reconstruct(osiv_handle* h, const float* d_counts, const float* d_blank
 
     float* best = prm->return_best ? h->d_best : nullptr;
     SliceState* state[2] = {h->d_state, h->d_state + h->max_batch};
-    k_init_state<<<1, 32, 0, st>>>(state[0], h->d_not_finite, batch, prm->lambda0, d_blank, blank_scalar, C, h->d_inv_bref);
-    k_fill<<<px_grid(h, batch), 256, 0, st>>>(h->dg, fp.ns, (float)prm->mu0, h->d_imgA, h->d_imgTA, best);
-    h->launches += 2;
 
     FwdArgs f{};
     f.g = h->dg; f.M = M; f.VS = VS; f.batch = batch; f.view_shift = vshift; f.rpb = fp.rpb; f.segs = fp.segs; f.rpb_magic = div_magic(fp.rpb); f.C_magic = div_magic(C);
@@ -893,9 +915,16 @@ int osiv_reconstruct(osiv_handle* h, const float* d_counts, const float* d_blank
     b.ip.monitor_mode = prm->monitor_mode; b.ip.M = M; b.ip.dhist = h->d_dhist;
     b.tau = tau; b.beta_over_M = (float)(prm->beta / M); b.eps2 = (float)(prm->tv_eps * prm->tv_eps);
 
-    float *cur = h->d_imgA, *curT = h->d_imgTA, *nxt = h->d_imgB, *nxtT = h->d_imgTB;
     const bool prof = h->profiling && N > 0;
     const bool pdl = h->use_pdl != 0;
+    // ---- the launch sequence of the call: set-up, N x (K1, K2), the final monitor, the result.  Either enqueued on the
+    // caller's stream launch by launch, or captured once into a CUDA graph (on the handle's own stream; programmatic
+    // dependent launches become programmatic graph edges) and replayed with one cudaGraphLaunch while the arguments repeat.
+    auto enqueue = [&](cudaStream_t st, bool prof) -> int {
+    float *cur = h->d_imgA, *curT = h->d_imgTA, *nxt = h->d_imgB, *nxtT = h->d_imgTB;
+    k_init_state<<<1, 32, 0, st>>>(state[0], h->d_not_finite, batch, prm->lambda0, d_blank, blank_scalar, C, h->d_inv_bref);
+    k_fill<<<px_grid(h, batch), 256, 0, st>>>(h->dg, fp.ns, (float)prm->mu0, h->d_imgA, h->d_imgTA, best);
+    h->launches += 2;
     if (prof) {
         while (h->events.size() < (size_t)2 * N + 1) {
             cudaEvent_t e;
@@ -937,8 +966,59 @@ int osiv_reconstruct(osiv_handle* h, const float* d_counts, const float* d_blank
         h->launches += 2;
     }
     k_unpad<<<px_grid(h, batch), 256, 0, st>>>(h->dg, fp.ns, cur, best, fin, d_img_out);
-    rc = launch_check(h, 1);
-    if (rc != OSIV_OK) return rc;
+    return launch_check(h, 1);
+    };  // enqueue
+
+    // the graph's key: everything the captured launches depend on
+    struct Key {
+        const void *counts, *blank, *out;
+        float blank_scalar;
+        int batch, has_trace, pdl, st_off, ns1;
+        long long gen;
+        osiv_params prm;
+    } key;
+    std::memset(&key, 0, sizeof(key));
+    key.counts = d_counts; key.blank = d_blank; key.out = d_img_out; key.blank_scalar = blank_scalar; key.batch = batch;
+    key.has_trace = h_trace != nullptr; key.pdl = h->use_pdl; key.st_off = h->st_off; key.ns1 = h->force_ns1; key.gen = g_alloc_gen;
+    std::memcpy(&key.prm, prm, sizeof(osiv_params));
+    const bool graphable = h->use_graph && !prof && N > 0 && !prm->forced_lambda;
+    const bool same_key = h->graph_key.size() == sizeof(key) && std::memcmp(h->graph_key.data(), &key, sizeof(key)) == 0;
+    if (!graphable || !same_key) {
+        // a first call with these arguments (or one that cannot be captured) is enqueued launch by launch: capturing and
+        // instantiating a thousand nodes costs more than one enqueue, so the graph is built only when the arguments repeat
+        if (h->graph_exec) { cudaGraphExecDestroy(h->graph_exec); h->graph_exec = nullptr; }
+        if (h->graph_exec2) { cudaGraphExecDestroy(h->graph_exec2); h->graph_exec2 = nullptr; }
+        h->graph_key.clear();
+        if (graphable) h->graph_key.assign(reinterpret_cast<unsigned char*>(&key), reinterpret_cast<unsigned char*>(&key) + sizeof(key));
+        if ((rc = enqueue(st, prof)) != OSIV_OK) return rc;
+    } else {
+        if (!h->graph_exec) {
+            if (!h->cap_stream) OSIV_CUDA(cudaStreamCreateWithFlags(&h->cap_stream, cudaStreamNonBlocking));
+            const int64_t before = h->launches;
+            cudaGraph_t graph = nullptr;
+            bool ok = cudaStreamBeginCapture(h->cap_stream, cudaStreamCaptureModeThreadLocal) == cudaSuccess;
+            if (ok) {
+                const int erc = enqueue(h->cap_stream, false);
+                ok = cudaStreamEndCapture(h->cap_stream, &graph) == cudaSuccess && erc == OSIV_OK && graph;
+            }
+            h->graph_launches = h->launches - before;
+            h->launches = before;
+            if (ok) ok = cudaGraphInstantiate(&h->graph_exec, graph, 0) == cudaSuccess && cudaGraphInstantiate(&h->graph_exec2, graph, 0) == cudaSuccess;
+            if (graph) cudaGraphDestroy(graph);
+            if (!ok) {                                    // this driver cannot capture the sequence: launch by launch from now on
+                cudaGetLastError();
+                if (h->graph_exec) cudaGraphExecDestroy(h->graph_exec);
+                h->graph_exec = h->graph_exec2 = nullptr;
+                h->use_graph = 0;
+                if ((rc = enqueue(st, false)) != OSIV_OK) return rc;
+            }
+        }
+        if (h->graph_exec) {
+            OSIV_CUDA(cudaGraphLaunch((h->graph_replays & 1) ? h->graph_exec2 : h->graph_exec, st));
+            h->launches += h->graph_launches;
+            h->graph_replays += 1;
+        }
+    }
 
     if (h_trace) {
         std::vector<int> nf(batch);

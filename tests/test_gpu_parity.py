@@ -761,3 +761,34 @@ assert r["violations"] == 0 and r["checks"] > 100000, r
     res = subprocess.run([sys.executable, "-c", code], cwd=root, env=env, capture_output=True, text=True, timeout=900)
     assert res.returncode == 0, res.stdout[-2000:] + res.stderr[-2000:]
     assert "CHECKS" in res.stdout
+
+
+def test_graph_replay_gives_the_same_bits_as_launch_by_launch(osiv):
+    """osiv_reconstruct as one CUDA graph (captured when a call repeats the previous call's arguments, with the dependent
+    launches as programmatic edges) against the same call enqueued launch by launch: identical images and traces, on the
+    staged-K2 path (config 2), the general path (config 1), with return_best and with several slices."""
+    for cfg, M, B, rb in [(si.scan_config("2"), 10, 1, 0), (si.scan_config("1"), 1, 2, 1), (si.scan_config("2"), 10, 5, 1)]:
+        _, gg = geoms(cfg)
+        counts = dev(np.stack([si.make_case(cfg, slice_index=s)[2] for s in range(B)]))
+        prm = osiv.Params(beta=0.005, n_subsets=M, n_iters=30, return_best=rb)
+        out = torch.empty((B, cfg.ny, cfg.nx), dtype=torch.float32, device="cuda")
+        with osiv.Handle(gg, max_batch=B) as h:
+            h.set_graph(False)
+            ref, tr_ref = h.reconstruct(counts, cfg.i0, prm, out=out, trace=True)
+            ref = host(ref).copy()
+            assert h.graph_replays() == 0
+            h.set_graph(True)
+            n0 = h.launch_count()
+            imgs = []
+            for _ in range(3):                         # first call: launch by launch; second: capture + replay; third: replay
+                got, tr = h.reconstruct(counts, cfg.i0, prm, out=out, trace=True)
+                imgs.append(host(got).copy())
+                assert np.array_equal(tr, tr_ref)
+            assert h.graph_replays() == 2
+            assert (h.launch_count() - n0) % 3 == 0      # replays account for the same launches
+            for im in imgs:
+                assert np.array_equal(im, ref)
+            # other arguments: back to launch by launch, and still the same arithmetic
+            prm2 = osiv.Params(beta=0.005, n_subsets=M, n_iters=29, return_best=rb)
+            h.reconstruct(counts, cfg.i0, prm2, out=out)
+            assert h.graph_replays() == 2
