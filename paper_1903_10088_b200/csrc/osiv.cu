@@ -57,6 +57,10 @@ struct osiv_handle {
     int4* d_regions = nullptr;
     unsigned short* d_itab2 = nullptr;
     int* d_bwin = nullptr;
+    float* d_invk = nullptr;            // [V][C] 1 / (in-line coefficient) of every ray (K1's start-up path)
+    int4* d_k1rng = nullptr;            // K1's block line ranges for (k1rng_M subsets, orbit size, rays per block), k_build_fwd_ranges
+    size_t k1rng_elems = 0;
+    long long k1rng_key = -1;
     unsigned char* d_blob = nullptr;    // per-subset constants of the staged K2 for blob_M subsets (k_build_blob)
     size_t blob_bytes = 0;
     int blob_M = 0;
@@ -499,6 +503,20 @@ int ensure_forward_ws(osiv_handle* h, const FwdPlan& p, int batch) {
     return grow(&h->d_dparts, &h->dpart_elems, (size_t)batch * p.nparts);
 }
 
+// K1's block line ranges for M subsets (M = 1: all views), rebuilt when M or the block shape changes
+int ensure_fwd_ranges(osiv_handle* h, const FwdPlan& p, int M, cudaStream_t st) {
+    const long long key = (((long long)M * 8 + p.ns) * 4096 + p.rpb) * 65536 + p.nparts;
+    if (h->d_k1rng && h->k1rng_key == key) return OSIV_OK;
+    h->k1rng_key = -1;
+    int rc = grow(&h->d_k1rng, &h->k1rng_elems, (size_t)M * p.nparts);
+    if (rc != OSIV_OK) return rc;
+    k_build_fwd_ranges<<<dim3(p.nparts, M), (p.rpb + 31) / 32 * 32, 0, st>>>(h->dg, M, h->geom.n_views / M, p.ns, p.rpb, h->d_k1rng);
+    h->launches += 1;
+    OSIV_CUDA(cudaGetLastError());
+    h->k1rng_key = key;
+    return OSIV_OK;
+}
+
 // residual buffer [batch][V_S][Cp] floats (NS == 4: [batch][V_S/4][Cp] float4); columns C..Cp-1 must be zero, and they
 // move when the layout changes, so the buffer is cleared whenever (V_S, orbit size, batch) differs from the last call
 int ensure_res(osiv_handle* h, int VS, int ns, int batch, cudaStream_t st) {
@@ -612,11 +630,15 @@ int osiv_create(const osiv_geometry* geom, int32_t max_batch, int32_t device, os
     }
     // zero slack after the last view: K2 reads past a view's last channel (general kernel: res_pad entries; staged
     // kernel: up to one window of at most 512 entries)
+    std::vector<float> invk(rays.size());
+    for (size_t i = 0; i < rays.size(); ++i) invk[i] = 1.0f / (std::fabs(rays[i].x) >= std::fabs(rays[i].y) ? rays[i].x : rays[i].y);
     rays.resize(rays.size() + h->res_pad + 4 + 512, make_float4(0.f, 0.f, 0.f, 0.f));
     h->ray_entries = (long long)rays.size();
     if (cudaMalloc((void**)&h->d_rays, rays.size() * sizeof(float4)) != cudaSuccess ||
         cudaMalloc((void**)&h->d_hs, hs.size() * sizeof(float)) != cudaSuccess ||
         cudaMemcpy(h->d_hs, hs.data(), hs.size() * sizeof(float), cudaMemcpyHostToDevice) != cudaSuccess ||
+        cudaMalloc((void**)&h->d_invk, invk.size() * sizeof(float)) != cudaSuccess ||
+        cudaMemcpy(h->d_invk, invk.data(), invk.size() * sizeof(float), cudaMemcpyHostToDevice) != cudaSuccess ||
         cudaMalloc((void**)&h->d_views, views.size() * sizeof(float2)) != cudaSuccess ||
         cudaMalloc((void**)&h->d_state, (size_t)2 * max_batch * sizeof(SliceState)) != cudaSuccess ||
         cudaMalloc((void**)&h->d_not_finite, (size_t)max_batch * sizeof(int)) != cudaSuccess ||
@@ -675,7 +697,7 @@ int osiv_destroy(osiv_handle* h) {
         void* ptrs[] = {h->d_rays, h->d_views, h->d_hs, h->d_imgA, h->d_imgB, h->d_imgTA, h->d_imgTB, h->d_best, h->d_res,
                         h->d_dparts, h->d_state, h->d_not_finite, h->d_inv_bref, h->d_trace,
                         h->d_forced, h->d_dhist, h->d_itab[0], h->d_itab[1], h->d_hcounts, h->d_hblank, h->d_himg,
-                        h->d_regions, h->d_itab2, h->d_bwin, h->d_blob};
+                        h->d_regions, h->d_itab2, h->d_bwin, h->d_blob, h->d_invk, h->d_k1rng};
         for (void* p : ptrs) if (p) cudaFree(p);
         for (cudaEvent_t e : h->events) cudaEventDestroy(e);
         if (h->graph_exec) cudaGraphExecDestroy(h->graph_exec);
@@ -808,6 +830,8 @@ int osiv_forward(osiv_handle* h, const float* d_img, float* d_sino, int32_t batc
     FwdArgs a{};
     a.g = h->dg; a.img = h->d_imgA; a.imgT = h->d_imgTA;
     a.subset = subset; a.M = subset < 0 ? 1 : n_subsets; a.VS = VS; a.batch = batch; a.rpb = p.rpb; a.segs = p.segs; a.rpb_magic = div_magic(p.rpb); a.C_magic = div_magic(h->geom.n_channels); a.sino = d_sino;
+    if ((rc = ensure_fwd_ranges(h, p, a.M, st)) != OSIV_OK) return rc;
+    a.rng_tab = h->d_k1rng; a.invk = h->d_invk; a.segs_magic = div_magic(p.segs);
     if (launch_forward<0>(p, batch, a, st, false) != cudaSuccess) { cudaGetLastError(); return OSIV_ERR_CUDA; }
     return launch_check(h, 2);
 }
@@ -896,6 +920,11 @@ int osiv_reconstruct(osiv_handle* h, const float* d_counts, const float* d_blank
     f.g = h->dg; f.M = M; f.VS = VS; f.batch = batch; f.view_shift = vshift; f.rpb = fp.rpb; f.segs = fp.segs; f.rpb_magic = div_magic(fp.rpb); f.C_magic = div_magic(C);
     f.counts = d_counts; f.blank = d_blank; f.blank_scalar = blank_scalar; f.inv_bref = h->d_inv_bref;
     f.res = h->d_res; f.Cp = Cp; f.dparts = h->d_dparts; f.res_floats = (long long)h->res_elems;
+    f.segs_magic = div_magic(fp.segs); f.invk = h->d_invk;
+    if (!stack) {                                        // a stack's slices see shifted views: its blocks work their ranges out
+        if ((rc = ensure_fwd_ranges(h, fp, M, st)) != OSIV_OK) return rc;
+        f.rng_tab = h->d_k1rng;
+    }
     BackArgs b{};
     b.res_floats = (long long)h->res_elems; b.ray_entries = h->ray_entries;
     b.g = h->dg; b.res = h->d_res; b.Cp = Cp; b.M = M; b.VS = VS; b.batch = batch; b.view_shift = vshift; b.tv_z = (float)prm->tv_z; b.best = best; b.tpb = bp.tpb; b.shares = bp.shares; b.ngx = bp.ngx; b.tpb_magic = div_magic(bp.tpb); b.ngx_magic = div_magic(bp.ngx);

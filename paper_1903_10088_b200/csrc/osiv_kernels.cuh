@@ -133,6 +133,10 @@ struct FwdArgs {
     int rpb, segs;                         // rays per block, line segments per ray (block = rpb * segs threads, rounded up to warps)
     unsigned rpb_magic, C_magic;           // fastdiv by rpb and by g.C
     int iter;                              // iteration number (timeline build only)
+    const int4* rng_tab;                   // [M][gridDim.x] line ranges of every block's row- / column-major rays {lo, hi, lo, hi}
+                                           // (k_build_fwd_ranges), or null: the block works them out itself (stacks)
+    const float* invk;                     // [V][C] 1 / (in-line coefficient) of every ray, or null
+    unsigned segs_magic;
     float* sino;                           // MODE 0: [batch][VS][C]
     const float* counts;                   // MODE 1: [batch][V][C]
     const float* blank;                    // [C] or null
@@ -229,6 +233,43 @@ __device__ __forceinline__ void ffma2(uint64_t& c, uint64_t a, float b) {       
 // SB == 2 (launches with several slices, A8): a block serves a pair of slices whose padded images are interleaved per
 // pixel (DevGeom::sb == 2), so every gather is one float2 = the pixel in both slices, the chord weights -- the bulk of
 // K1's instructions -- are worked out once per pair, and the FFMA2 pairs run over the two slices.
+// image lines [flo, fhi] of the ray's major axis on which its crossing lies within half a pixel of the image:
+// |uu*b + g0| < |kk|*(na/2 + 1/2)
+__device__ __forceinline__ void ray_lines(const DevGeom& g, const float4 ray, int& flo, int& fhi) {
+    const bool rowmaj = fabsf(ray.x) >= fabsf(ray.y);
+    const float kk = rowmaj ? ray.x : ray.y, uu = rowmaj ? ray.y : ray.x;
+    const int na = rowmaj ? g.nx : g.ny, nb = rowmaj ? g.ny : g.nx;
+    const float cb = rowmaj ? g.cy : g.cx;
+    const float A = fabsf(kk) * (0.5f * na + 0.5f);
+    const float iu = 1.0f / uu;                           // exact chord: uu = +-1; Joseph: |uu| <= 1
+    const float b1 = iu * (-ray.z - A), b2 = iu * (-ray.z + A);
+    flo = (int)fminf(fmaxf(ceilf(fminf(b1, b2) + cb) - 1.f, 0.f), (float)nb);
+    fhi = (int)fminf(fmaxf(floorf(fmaxf(b1, b2) + cb) + 1.f, -1.f), (float)(nb - 1));
+}
+
+// A0 for K1, once per handle, subset count and block shape: the union of line ranges of every block's row-major and
+// column-major rays (what k_forward otherwise works out with two block barriers at every launch).  grid (blocks, M).
+__global__ void __launch_bounds__(1024) k_build_fwd_ranges(DevGeom g, int M, int VS, int ns, int rpb, int4* __restrict__ tab) {
+    __shared__ int rng[4];
+    const int i = threadIdx.x, m = blockIdx.y;
+    if (i < 4) rng[i] = (i & 1) ? -1 : (1 << 30);
+    __syncthreads();
+    const int VSb = VS / ns, R = VSb * g.C, r = blockIdx.x * rpb + i;
+    if (i < rpb && r < R) {
+        const int jb = r / g.C, c = r - jb * g.C;
+        const int v = m + jb * M;
+        const float4 ray = __ldg(&g.rays[(size_t)v * g.C + c]);
+        int flo, fhi;
+        ray_lines(g, ray, flo, fhi);
+        if (fhi >= flo) {
+            const int o = fabsf(ray.x) >= fabsf(ray.y) ? 0 : 2;
+            atomicMin(&rng[o], flo); atomicMax(&rng[o + 1], fhi);
+        }
+    }
+    __syncthreads();
+    if (i == 0) tab[(size_t)m * gridDim.x + blockIdx.x] = make_int4(rng[0], rng[1], rng[2], rng[3]);
+}
+
 template <int SB> struct Px;
 template <> struct Px<1> { typedef float T; };
 template <> struct Px<2> { typedef float2 T; };
@@ -269,23 +310,24 @@ __global__ void __launch_bounds__(FWD_MAX_THREADS, 1) k_forward(const FwdArgs a)
         // NS == 4: the orbit-interleaved image Q (rays crossing rows) or its transpose QT (rays crossing columns), SB float4 per pixel
         const float4* qA = reinterpret_cast<const float4*>(rowmaj ? a.img : a.imgT) + (size_t)blockIdx.z * (rowmaj ? g.img_elems : g.imgT_elems) * SB;
         const int pitch = rowmaj ? g.pitch : g.pitchT;    // NS == 4: square grid, both pitches are equal
-        const int na = rowmaj ? g.nx : g.ny, nb = rowmaj ? g.ny : g.nx;
+        const int na = rowmaj ? g.nx : g.ny;
         const float ca = rowmaj ? g.cx : g.cy, cb = rowmaj ? g.cy : g.cx;
-        const float invk = 1.0f / kk;
+        const float invk = a.invk ? __ldg(&a.invk[(size_t)vt * g.C + c]) : 1.0f / kk;
         const float hk = ray.w;
-        // lines where the crossing lies within half a pixel of the image: |uu*b + g0| < |kk|*(na/2 + 1/2)
-        const float A = fabsf(kk) * (0.5f * na + 0.5f);
-        const float iu = 1.0f / uu;                       // exact chord: uu = +-1; Joseph: |uu| <= 1
-        const float b1 = iu * (-ray.z - A), b2 = iu * (-ray.z + A);
-        const int flo = (int)fminf(fmaxf(ceilf(fminf(b1, b2) + cb) - 1.f, 0.f), (float)nb);
-        const int fhi = (int)fminf(fmaxf(floorf(fmaxf(b1, b2) + cb) + 1.f, -1.f), (float)(nb - 1));
         // The block walks the union of its rays' line ranges in lock step, so that at every step the lanes of a warp
         // read neighbouring pixels of ONE image line (1-2 cache lines per load instead of up to 32; rays clipped by an
         // image corner start many lines apart).  On a line outside a ray's own range the crossing is more than half a
         // pixel outside the image: the clamped index lands in the zero padding and the term vanishes.
         // (Row-major and column-major rays of one block form two such unions: their lines are different things.)
-        if (t < 4) rng[t] = (t & 1) ? -1 : (1 << 30);
+        int wlo, whi;
         OSIV_TL(a.iter, 0, 7, false);
+        if (a.rng_tab) {                                      // tabulated (A0): no barrier in the start-up path
+            const int4 rg = __ldg(&a.rng_tab[(size_t)(a.subset < 0 ? 0 : a.subset) * gridDim.x + blockIdx.x]);
+            wlo = rowmaj ? rg.x : rg.z; whi = rowmaj ? rg.y : rg.w;
+        } else {
+        int flo, fhi;
+        ray_lines(g, ray, flo, fhi);
+        if (t < 4) rng[t] = (t & 1) ? -1 : (1 << 30);
         __syncthreads();
         {
             const int big = 1 << 30;
@@ -299,9 +341,10 @@ __global__ void __launch_bounds__(FWD_MAX_THREADS, 1) k_forward(const FwdArgs a)
             }
         }
         __syncthreads();
-        const int wlo = rowmaj ? rng[0] : rng[2], whi = rowmaj ? rng[1] : rng[3];
-        const int nsteps = walker ? whi - wlo + 1 : 0;
-        const int len = (nsteps + segs - 1) / segs;
+        wlo = rowmaj ? rng[0] : rng[2]; whi = rowmaj ? rng[1] : rng[3];
+        }
+        const int nsteps = walker ? max(whi - wlo + 1, 0) : 0;
+        const int len = fastdiv(nsteps + segs - 1, a.segs_magic);
         const int j0 = wlo + seg * len;
         const int j1 = min(j0 + len, wlo + nsteps);
         const int imax = na + PAD - 2;
