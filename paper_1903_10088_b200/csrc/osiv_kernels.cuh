@@ -504,14 +504,10 @@ __global__ void __launch_bounds__(FWD_MAX_THREADS, 1) k_forward(const FwdArgs a)
             if ((t & 31) == 0) dred[sl][t >> 5] = d2[sl];
         }
         asm volatile("bar.sync 1, %0;" ::"r"(32 * nw) : "memory");     // only the epilogue warps meet here
-        if (t < 32) {                                                  // warp 0: the warp sums in a fixed (butterfly) order
-#pragma unroll
-            for (int sl = 0; sl < SB; ++sl) {
-                double D = t < nw ? dred[sl][t] : 0.0;
-#pragma unroll
-                for (int off = 16; off > 0; off >>= 1) D += __shfl_xor_sync(0xffffffffu, D, off);
-                if (t == 0 && s0 + sl < a.batch) a.dparts[(size_t)(s0 + sl) * gridDim.x + blockIdx.x] = D;
-            }
+        if (t < SB) {                                                  // one thread per slice: the warp sums in a fixed order
+            double D = 0.0;
+            for (int w = 0; w < nw; ++w) D += dred[t][w];
+            if (s0 + t < a.batch) a.dparts[(size_t)(s0 + t) * gridDim.x + blockIdx.x] = D;
         }
     }
     OSIV_TL(a.iter, 0, 5, true);
@@ -659,6 +655,12 @@ template <int K> __device__ __forceinline__ float orbit_nb(const float4 (&E)[3][
     const int dy = K == 0 ? b : K == 1 ? -a : K == 2 ? -b : a;
     return orbit_comp<K>(E[1 + dy][1 + dx]);
 }
+// 1/sqrt(x) for x >= eps^2 > 0: the bare MUFU.RSQ (rsqrtf adds two scalings for denormal inputs that cannot occur here)
+__device__ __forceinline__ float rsqrt_fast(float x) {
+    float y;
+    asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
 template <int K>
 __device__ __forceinline__ void orbit_tv(const float4 (&E)[3][3], int px, int py, int N, float eps2, float& cur, float& grad) {
     const int x = K == 0 ? px : K == 1 ? N - 1 - py : K == 2 ? N - 1 - px : py;        // R^K P
@@ -669,13 +671,13 @@ __device__ __forceinline__ void orbit_tv(const float4 (&E)[3][3], int px, int py
     float sgrad = 0.f;
     if (x > 0) {                                                     // cell (x-1, y)
         const float l = orbit_nb<K>(E, -1, 0), dxl = c - l, dyl = hy1 ? orbit_nb<K>(E, -1, 1) - l : 0.f;
-        sgrad += dxl * rsqrtf(eps2 + dxl * dxl + dyl * dyl);
+        sgrad += dxl * rsqrt_fast(eps2 + dxl * dxl + dyl * dyl);
     }
     if (y > 0) {                                                     // cell (x, y-1)
         const float d = orbit_nb<K>(E, 0, -1), dyb = c - d, dxb = hx1 ? orbit_nb<K>(E, 1, -1) - d : 0.f;
-        sgrad += dyb * rsqrtf(eps2 + dxb * dxb + dyb * dyb);
+        sgrad += dyb * rsqrt_fast(eps2 + dxb * dxb + dyb * dyb);
     }
-    sgrad -= (dxc + dyc) * rsqrtf(eps2 + dxc * dxc + dyc * dyc);
+    sgrad -= (dxc + dyc) * rsqrt_fast(eps2 + dxc * dxc + dyc * dyc);
     cur = c;
     grad = sgrad;
 }
