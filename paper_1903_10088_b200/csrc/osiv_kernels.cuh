@@ -308,7 +308,10 @@ __global__ void __launch_bounds__(FWD_MAX_THREADS, 1) k_forward(const FwdArgs a)
         const float uu = rowmaj ? ray.y : ray.x;          // coefficient of the marching coordinate (+-1; Joseph: +-1/|k|)
         const PX* bufA = rowmaj ? reinterpret_cast<const PX*>(a.img) + (size_t)blockIdx.z * g.img_elems : reinterpret_cast<const PX*>(a.imgT) + (size_t)blockIdx.z * g.imgT_elems;
         // NS == 4: the orbit-interleaved image Q (rays crossing rows) or its transpose QT (rays crossing columns), SB float4 per pixel
-        const float4* qA = reinterpret_cast<const float4*>(rowmaj ? a.img : a.imgT) + (size_t)blockIdx.z * (rowmaj ? g.img_elems : g.imgT_elems) * SB;
+        // (slice-major, NOT interleaved per pixel: with two slices' float4s side by side a warp's 16-byte gathers are strided by 32
+        // bytes and every L1 wavefront carries half its width -- 12.9 k instead of 8.5 k wavefronts per slice and SM, ncu)
+        const long long q_plane = rowmaj ? g.img_elems : g.imgT_elems;
+        const float4* qA = reinterpret_cast<const float4*>(rowmaj ? a.img : a.imgT) + (size_t)blockIdx.z * q_plane * SB;
         const int pitch = rowmaj ? g.pitch : g.pitchT;    // NS == 4: square grid, both pitches are equal
         const int na = rowmaj ? g.nx : g.ny;
         const float ca = rowmaj ? g.cx : g.cy, cb = rowmaj ? g.cy : g.cx;
@@ -384,11 +387,11 @@ __global__ void __launch_bounds__(FWD_MAX_THREADS, 1) k_forward(const FwdArgs a)
 #pragma unroll
                 for (int u = 0; u < 2; ++u) {
                     OSIV_CHECK(offP + u * pitch + i0[u] >= 0 && offP + u * pitch + i0[u] + 1 < (rowmaj ? g.img_elems : g.imgT_elems), 1);
-                    const float4* p0 = qA + (size_t)(offP + u * pitch + i0[u]) * SB;
+                    const float4* p0 = qA + (offP + u * pitch + i0[u]);
 #pragma unroll
                     for (int e = 0; e < 2; ++e)
 #pragma unroll
-                        for (int sl = 0; sl < SB; ++sl) x[u][e][sl] = __ldg(p0 + e * SB + sl);
+                        for (int sl = 0; sl < SB; ++sl) x[u][e][sl] = __ldg(p0 + sl * q_plane + e);
                 }
 #pragma unroll
                 for (int u = 0; u < 2; ++u)
@@ -1052,11 +1055,11 @@ __global__ void __launch_bounds__(SB == 1 ? BK_MAX_THREADS : BKB_MAX_THREADS, SB
                 if (s >= a.batch) break;
                 float4 E[3][3];
                 if (fin_active) {
-                    const float4* Q = reinterpret_cast<const float4*>(a.img) + (size_t)blockIdx.z * g.img_elems * SB + j;
+                    const float4* Q = reinterpret_cast<const float4*>(a.img) + (size_t)(blockIdx.z * SB + j) * g.img_elems;
 #pragma unroll
                     for (int dy = 0; dy < 3; ++dy)
 #pragma unroll
-                        for (int dx = 0; dx < 3; ++dx) E[dy][dx] = __ldg(Q + (size_t)((py + dy - 1 + PADR) * g.pitch + PAD + px + dx - 1) * SB);
+                        for (int dx = 0; dx < 3; ++dx) E[dy][dx] = __ldg(Q + (size_t)((py + dy - 1 + PADR) * g.pitch + PAD + px + dx - 1));
                 }
                 si[j] = step_rule(a, s, lane, writer);
                 step[j] = (float)(si[j].lambda * a.tau);
@@ -1093,13 +1096,13 @@ __global__ void __launch_bounds__(SB == 1 ? BK_MAX_THREADS : BKB_MAX_THREADS, SB
             float un[4];
 #pragma unroll
             for (int k = 0; k < 4; ++k) un[k] = fmaxf(fmaf(step[j], gsum[k] - a.beta_over_M * tv[j][k], cur[j][k]), 0.f);
-            float4* Qn = reinterpret_cast<float4*>(a.img_new) + (size_t)blockIdx.z * g.img_elems * SB + j;
-            float4* QTn = reinterpret_cast<float4*>(a.imgT_new) + (size_t)blockIdx.z * g.imgT_elems * SB + j;
+            float4* Qn = reinterpret_cast<float4*>(a.img_new) + (size_t)(blockIdx.z * SB + j) * g.img_elems;
+            float4* QTn = reinterpret_cast<float4*>(a.imgT_new) + (size_t)(blockIdx.z * SB + j) * g.imgT_elems;
 #pragma unroll
             for (int k = 0; k < 4; ++k) {
                 const float4 v = make_float4(un[k], un[(k + 1) & 3], un[(k + 2) & 3], un[(k + 3) & 3]);
-                Qn[pad_off(g, ry[k], rx[k]) * SB] = v;
-                QTn[padT_off(g, rx[k], ry[k]) * SB] = v;
+                Qn[pad_off(g, ry[k], rx[k])] = v;
+                QTn[padT_off(g, rx[k], ry[k])] = v;
             }
             if (a.best && si[j].improved) {                          // A7: mu(n) had the smallest monitor so far
                 float* best = a.best + (size_t)s * N * N;
@@ -1241,9 +1244,9 @@ __global__ void __launch_bounds__(SB == 1 ? BK_MAX_THREADS : BKB_MAX_THREADS, SB
 // Small helpers around the two hot kernels
 // ------------------------------------------------------------------------------------------------
 
-// Image layouts of the padded working buffers (per group of g.sb slices, slices interleaved per pixel):
+// Image layouts of the padded working buffers (NS == 1: per group of g.sb slices, slices interleaved per pixel; NS == 4: slice-major):
 //   NS == 1: one float per pixel and slice:   img[((iy+PADR)*pitch + PAD+ix) * sb + sl],  imgT the transpose;
-//   NS == 4: one float4 per pixel and slice:  Q  [((iy+PADR)*pitch + PAD+ix) * sb + sl] = {mu(P), mu(RP), mu(R^2P), mu(R^3P)},
+//   NS == 4: one float4 per pixel and slice:  Q  [sl][(iy+PADR)*pitch + PAD+ix] = {mu(P), mu(RP), mu(R^2P), mu(R^3P)},
 //            R: (ix,iy) -> (N-1-iy, ix);  QT the transpose.
 __device__ __forceinline__ void orbit_pos(int N, int ix, int iy, int k, int& x, int& y) {
     x = k == 0 ? ix : k == 1 ? N - 1 - iy : k == 2 ? N - 1 - ix : iy;
@@ -1263,8 +1266,8 @@ __global__ void __launch_bounds__(256) k_pad_transpose(DevGeom g, int ns, const 
 #pragma unroll
         for (int k = 0; k < 4; ++k) { int xx, yy; orbit_pos(g.nx, x, y, k, xx, yy); v[k] = src[(size_t)yy * g.nx + xx]; }
         const float4 q = make_float4(v[0], v[1], v[2], v[3]);
-        reinterpret_cast<float4*>(img)[(size_t)(s / g.sb) * g.img_elems * g.sb + pad_off(g, y, x) * g.sb + s % g.sb] = q;
-        reinterpret_cast<float4*>(imgT)[(size_t)(s / g.sb) * g.imgT_elems * g.sb + padT_off(g, x, y) * g.sb + s % g.sb] = q;
+        reinterpret_cast<float4*>(img)[(size_t)s * g.img_elems + pad_off(g, y, x)] = q;
+        reinterpret_cast<float4*>(imgT)[(size_t)s * g.imgT_elems + padT_off(g, x, y)] = q;
     } else {
         const float v = src[(size_t)y * g.nx + x];
         img[slice_base(g, g.img_elems, s) + pad_off(g, y, x) * g.sb] = v;
@@ -1282,7 +1285,7 @@ __global__ void __launch_bounds__(256) k_unpad(DevGeom g, int ns, const float* _
     if (x >= g.nx || y >= g.ny) return;
     const size_t o = (size_t)s * g.nx * g.ny + (size_t)y * g.nx + x;
     if (best && !state[s].improved) out[o] = best[o];
-    else if (ns == 4) out[o] = reinterpret_cast<const float4*>(img)[(size_t)(s / g.sb) * g.img_elems * g.sb + pad_off(g, y, x) * g.sb + s % g.sb].x;
+    else if (ns == 4) out[o] = reinterpret_cast<const float4*>(img)[(size_t)s * g.img_elems + pad_off(g, y, x)].x;
     else out[o] = img[slice_base(g, g.img_elems, s) + pad_off(g, y, x) * g.sb];
 }
 
@@ -1295,8 +1298,8 @@ __global__ void __launch_bounds__(256) k_fill(DevGeom g, int ns, float mu0, floa
     if (x >= g.nx || y >= g.ny) return;
     if (ns == 4) {
         const float4 q = make_float4(mu0, mu0, mu0, mu0);
-        reinterpret_cast<float4*>(img)[(size_t)(s / g.sb) * g.img_elems * g.sb + pad_off(g, y, x) * g.sb + s % g.sb] = q;
-        reinterpret_cast<float4*>(imgT)[(size_t)(s / g.sb) * g.imgT_elems * g.sb + padT_off(g, x, y) * g.sb + s % g.sb] = q;
+        reinterpret_cast<float4*>(img)[(size_t)s * g.img_elems + pad_off(g, y, x)] = q;
+        reinterpret_cast<float4*>(imgT)[(size_t)s * g.imgT_elems + padT_off(g, x, y)] = q;
     } else {
         img[slice_base(g, g.img_elems, s) + pad_off(g, y, x) * g.sb] = mu0;
         imgT[slice_base(g, g.imgT_elems, s) + padT_off(g, x, y) * g.sb] = mu0;
