@@ -102,6 +102,11 @@ def main():
         print(f"| {name} | {d(0, 1):.2f} | {d(1, 2):.2f} | {d(2, 3):.2f} (max {mx(2, 3):.2f}) | {d(3, 4):.2f} | {d(4, 5):.2f} (max {mx(4, 5):.2f}) | "
               f"{rel[:, 5].max() - rel[:, 2].min():.2f} |")
     print()
+    print("work balance over blocks, main loop (after wait -> loop end): mean / median / max / min us; mean = what a perfectly balanced grid would take")
+    for name, nb, rel in rows:
+        d = rel[:, 3] - rel[:, 2]
+        print(f"  {name}: {d.mean():.2f} / {np.median(d):.2f} / {d.max():.2f} / {d.min():.2f}")
+    print()
     print("prologue mark (slot 7: K1 own ray loaded and clipped; K2 tile origin known), us after block start, median [max]:")
     for name, nb, rel in rows:
         d = rel[:, 7] - rel[:, 0]
