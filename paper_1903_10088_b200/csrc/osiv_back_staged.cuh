@@ -334,7 +334,8 @@ __global__ void __launch_bounds__(BS_SHARES * BS_MAX_TPB, 1) k_back_staged(const
 #pragma unroll
             for (int dx = 0; dx < 3; ++dx) E[dy][dx] = __ldg(Q + (size_t)((py + dy - 1 + PADR) * g.pitch + PAD + px + dx - 1));
     }
-    __syncthreads();                                      // mbarriers initialised
+    // (no block barrier here: the mbarrier thread 0 has initialised is first touched by the others behind the barrier that
+    // follows the residual stores, and a barrier in the start-up path would make every warp wait for thread 0's set-up)
     OSIV_TL(a.iter, 1, 1, false);
     pdl_wait();                                           // the residuals and the monitor partials are the previous launch's output
     pdl_launch_next();
@@ -450,6 +451,11 @@ __global__ void __launch_bounds__(BS_SHARES * BS_MAX_TPB, 1) k_back_staged(const
         for (int k = 0; k < 4; ++k) gsum[k] += c[(k + qq) & 3];
     }
     const int rx[4] = {px, N - 1 - py, N - 1 - px, py}, ry[4] = {py, px, N - 1 - py, N - 1 - px};      // R^k P
+    // padded offsets of R^k P in Q and of its transposed position in QT (square grid: one pitch): with A = (px+1) pitch,
+    // B = (py+1) pitch and (N - x) pitch = (N+1) pitch - (x+1) pitch the eight offsets are sums of two products
+    const int pA = (px + PADR) * g.pitch, pB = (py + PADR) * g.pitch, pN = (N - 1 + 2 * PADR) * g.pitch, n1 = N - 1;
+    const int oq[4] = {pB + PAD + px, pA + PAD + n1 - py, pN - pB + PAD + n1 - px, pN - pA + PAD + py};
+    const int ot[4] = {pA + PAD + py, pN - pB + PAD + px, pN - pA + PAD + n1 - py, pB + PAD + n1 - px};
     if constexpr (MODE == 0) {
         float* out = a.out + (size_t)s * N * N;
 #pragma unroll
@@ -465,8 +471,8 @@ __global__ void __launch_bounds__(BS_SHARES * BS_MAX_TPB, 1) k_back_staged(const
 #pragma unroll
         for (int k = 0; k < 4; ++k) {
             const float4 v = make_float4(un[k], un[(k + 1) & 3], un[(k + 2) & 3], un[(k + 3) & 3]);
-            Qn[pad_off(g, ry[k], rx[k])] = v;
-            QTn[padT_off(g, rx[k], ry[k])] = v;
+            Qn[oq[k]] = v;
+            QTn[ot[k]] = v;
         }
         if (a.best && reinterpret_cast<const int*>(s_step)[1]) {             // A7: mu(n) had the smallest monitor so far
             float* best = a.best + (size_t)s * N * N;
