@@ -524,7 +524,14 @@ struct StepInfo { double lambda; double D; int improved; };
 
 __device__ __forceinline__ double sum_partials(const double* p, int n, int lane) {
     double D = 0.0;
-    for (int i = lane; i < n; i += 32) D += __ldg(&p[i]);
+    // lane l adds p[l], p[l + 32], ... in that order; eight loads in flight (a slot past the end adds an exact 0)
+    for (int i0 = 0; i0 < n; i0 += 256) {
+        double v[8];
+#pragma unroll
+        for (int k = 0; k < 8; ++k) v[k] = i0 + lane + 32 * k < n ? __ldg(&p[i0 + lane + 32 * k]) : 0.0;
+#pragma unroll
+        for (int k = 0; k < 8; ++k) D += v[k];
+    }
 #pragma unroll
     for (int off = 16; off > 0; off >>= 1) D += __shfl_xor_sync(0xffffffffu, D, off);
     return D;
