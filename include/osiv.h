@@ -191,7 +191,8 @@ int osiv_set_overlap(osiv_handle* h, int32_t enable);
 
 /* One CUDA graph per call.  By default (enable = 1) osiv_reconstruct captures its launch sequence (set-up, n_iters x
  * (K1, K2) with their programmatic dependent edges, result) into a CUDA graph when a call repeats the previous call's
- * arguments (pointers, parameters, batch) and replays it with a single cudaGraphLaunch while they keep repeating (SURVEY.md section 7 step
+ * arguments (pointers, parameters, batch) and replays it with a single cudaGraphLaunch while they keep repeating (the
+ * graphs of the two most recent argument sets are kept) (SURVEY.md section 7 step
  * 7); calls with forced_lambda or with per-kernel profiling, and drivers that cannot capture the sequence, enqueue launch
  * by launch.  enable = 0 always enqueues launch by launch (same results bit for bit; used by the tests).
  * osiv_graph_replays counts the graph launches made so far. */

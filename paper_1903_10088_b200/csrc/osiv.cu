@@ -68,10 +68,13 @@ struct osiv_handle {
     // the launch sequence of one osiv_reconstruct call as a CUDA graph, replayed while the call's arguments repeat
     int use_graph = 1;                  // osiv_set_graph(h, 0): enqueue every launch from the host
     cudaStream_t cap_stream = nullptr;  // capture happens here (the caller's stream may be the legacy default stream)
-    cudaGraphExec_t graph_exec = nullptr, graph_exec2 = nullptr;   // two instances, used alternately: the upload of one launch
-                                                                    // overlaps the run of the previous one
-    std::vector<unsigned char> graph_key;
-    int64_t graph_launches = 0;         // kernels in the captured sequence
+    struct GraphSlot {                  // two argument sets are remembered (a caller alternating between the device-pointer and
+        std::vector<unsigned char> key; //  the host-buffer entry point keeps both graphs)
+        cudaGraphExec_t exec = nullptr;
+        int64_t launches = 0;           // kernels in the captured sequence
+        long long last_use = 0;
+    } gslot[2];
+    long long gclock = 0;
     int64_t graph_replays = 0;
     // per-kernel event timing (osiv_set_profiling)
     bool profiling = false;
@@ -700,8 +703,7 @@ int osiv_destroy(osiv_handle* h) {
                         h->d_regions, h->d_itab2, h->d_bwin, h->d_blob, h->d_invk, h->d_k1rng};
         for (void* p : ptrs) if (p) cudaFree(p);
         for (cudaEvent_t e : h->events) cudaEventDestroy(e);
-        if (h->graph_exec) cudaGraphExecDestroy(h->graph_exec);
-        if (h->graph_exec2) cudaGraphExecDestroy(h->graph_exec2);
+        for (auto& gs : h->gslot) if (gs.exec) cudaGraphExecDestroy(gs.exec);
         if (h->cap_stream) cudaStreamDestroy(h->cap_stream);
         cudaGetLastError();
     }
@@ -1011,17 +1013,22 @@ int osiv_reconstruct(osiv_handle* h, const float* d_counts, const float* d_blank
     key.has_trace = h_trace != nullptr; key.pdl = h->use_pdl; key.st_off = h->st_off; key.ns1 = h->force_ns1; key.gen = g_alloc_gen;
     std::memcpy(&key.prm, prm, sizeof(osiv_params));
     const bool graphable = h->use_graph && !prof && N > 0 && !prm->forced_lambda;
-    const bool same_key = h->graph_key.size() == sizeof(key) && std::memcmp(h->graph_key.data(), &key, sizeof(key)) == 0;
-    if (!graphable || !same_key) {
-        // a first call with these arguments (or one that cannot be captured) is enqueued launch by launch: capturing and
-        // instantiating a thousand nodes costs more than one enqueue, so the graph is built only when the arguments repeat
-        if (h->graph_exec) { cudaGraphExecDestroy(h->graph_exec); h->graph_exec = nullptr; }
-        if (h->graph_exec2) { cudaGraphExecDestroy(h->graph_exec2); h->graph_exec2 = nullptr; }
-        h->graph_key.clear();
-        if (graphable) h->graph_key.assign(reinterpret_cast<unsigned char*>(&key), reinterpret_cast<unsigned char*>(&key) + sizeof(key));
+    osiv_handle::GraphSlot* slot = nullptr;
+    for (auto& gs : h->gslot)
+        if (gs.key.size() == sizeof(key) && std::memcmp(gs.key.data(), &key, sizeof(key)) == 0) slot = &gs;
+    if (!graphable) {
         if ((rc = enqueue(st, prof)) != OSIV_OK) return rc;
+    } else if (!slot) {
+        // a first call with these arguments is enqueued launch by launch: capturing and instantiating a thousand nodes costs
+        // more than one enqueue, so the graph is built only when the arguments repeat; they take the older slot
+        osiv_handle::GraphSlot& v = h->gslot[0].last_use <= h->gslot[1].last_use ? h->gslot[0] : h->gslot[1];
+        if (v.exec) { cudaGraphExecDestroy(v.exec); v.exec = nullptr; }
+        v.key.assign(reinterpret_cast<unsigned char*>(&key), reinterpret_cast<unsigned char*>(&key) + sizeof(key));
+        v.last_use = ++h->gclock;
+        if ((rc = enqueue(st, false)) != OSIV_OK) return rc;
     } else {
-        if (!h->graph_exec) {
+        slot->last_use = ++h->gclock;
+        if (!slot->exec) {
             if (!h->cap_stream) OSIV_CUDA(cudaStreamCreateWithFlags(&h->cap_stream, cudaStreamNonBlocking));
             const int64_t before = h->launches;
             cudaGraph_t graph = nullptr;
@@ -1030,21 +1037,20 @@ int osiv_reconstruct(osiv_handle* h, const float* d_counts, const float* d_blank
                 const int erc = enqueue(h->cap_stream, false);
                 ok = cudaStreamEndCapture(h->cap_stream, &graph) == cudaSuccess && erc == OSIV_OK && graph;
             }
-            h->graph_launches = h->launches - before;
+            slot->launches = h->launches - before;
             h->launches = before;
-            if (ok) ok = cudaGraphInstantiate(&h->graph_exec, graph, 0) == cudaSuccess && cudaGraphInstantiate(&h->graph_exec2, graph, 0) == cudaSuccess;
+            if (ok) ok = cudaGraphInstantiate(&slot->exec, graph, 0) == cudaSuccess;
             if (graph) cudaGraphDestroy(graph);
             if (!ok) {                                    // this driver cannot capture the sequence: launch by launch from now on
                 cudaGetLastError();
-                if (h->graph_exec) cudaGraphExecDestroy(h->graph_exec);
-                h->graph_exec = h->graph_exec2 = nullptr;
+                slot->exec = nullptr;
                 h->use_graph = 0;
                 if ((rc = enqueue(st, false)) != OSIV_OK) return rc;
             }
         }
-        if (h->graph_exec) {
-            OSIV_CUDA(cudaGraphLaunch((h->graph_replays & 1) ? h->graph_exec2 : h->graph_exec, st));
-            h->launches += h->graph_launches;
+        if (slot->exec) {
+            OSIV_CUDA(cudaGraphLaunch(slot->exec, st));
+            h->launches += slot->launches;
             h->graph_replays += 1;
         }
     }
