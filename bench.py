@@ -105,7 +105,7 @@ class ClockSampler:
             fd, self.path = tempfile.mkstemp(suffix=".csv")
             os.close(fd)
             self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.gpu), f"--query-gpu={self.Q}",
-                                          "--format=csv,noheader,nounits", "-lms", "50"],
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
                                          stdout=open(self.path, "w"), stderr=subprocess.DEVNULL)
         except Exception:
             self.proc = None
@@ -340,6 +340,8 @@ def run_ours(args, cfg, beta):
             "seconds_per_500_iter_recon": (t_dev / args.steps) * 500.0 / cfg.n_iters,
             "slices_per_s": world * batch * args.steps / t_dev,
             "wall_ms_per_step_incl_flush": 1e3 * wall / args.steps,
+            "wall_note": "host clock around the timed region: includes the L2 flushes and whatever the nvidia-smi clock sampler "
+                         "(one query per 100 ms) stalls; a loop without sampler and flush runs at the device time (DESIGN.md section 6)",
             "paper_context": {"gtx1080ti_s_per_slice_thinning_1_20": 3.71, "iterations_per_s": 134.8,
                               "source": "PAPER.md:156,164 Table I (other hardware, real data; context only)"},
             "clocks": clocks,
