@@ -687,6 +687,25 @@ def test_stack_of_slices_at_256(osiv):
     assert rel(host(free)[2], ref[2]) > 10 * rel(host(got)[2], ref[2])          # the coupling is really on
 
 
+def test_stack_of_slices_at_512(osiv):
+    """8(f)-3 at the size the clock runs at (PAPER.md:51 helical acquisition): config 3's geometry (512x512, 800 x 738, 20
+    subsets) as a stack of 3 slices, the gantry advanced 11 views per slice, 3-D TV on, 20 iterations (one pass over the
+    subsets) against the oracle's stack."""
+    cfg = si.scan_config("3")
+    og, gg = geoms(cfg)
+    S, k, tvz = 3, 11, 0.6
+    counts = np.stack([si.make_case(cfg, slice_index=s)[2] for s in range(S)])
+    kw = dict(beta=0.005, n_subsets=cfg.n_subsets, n_iters=20)
+    ref, tr_ref, status = oracle.reconstruct_stack(og, counts, cfg.i0, oracle.Params(**kw), view_shift=k, tv_z=tvz)
+    assert status == 0
+    with osiv.Handle(gg, max_batch=S) as h:
+        got, tr = h.reconstruct(dev(counts), cfg.i0, osiv.Params(view_shift=k, tv_z=tvz, **kw), trace=True)
+    for s in range(S):
+        assert np.array_equal(tr[s, :, 1], tr_ref[s, :, 1])
+        assert np.all(np.abs(tr[s, :, 0] - tr_ref[s, :, 0]) <= 1e-5 * tr_ref[s, :, 0])
+        assert rel(host(got)[s], ref[s]) < IMG_TOL
+
+
 def test_forced_lambda_ramp_up_to_the_oracles_stability_limit(osiv):
     """G12: arithmetic parity under a forced step is defined while the iteration is stable.  Where that ends is taken from
     the oracle, not assumed: under the steep ramp lambda(n) = 0.01 + 0.002 n the oracle's monitor falls until the step
