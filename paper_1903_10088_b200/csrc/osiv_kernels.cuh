@@ -357,19 +357,22 @@ __global__ void __launch_bounds__(FWD_MAX_THREADS, 1) k_forward(const FwdArgs a)
         pdl_wait();                                           // mu(n) is the previous launch's output
         pdl_launch_next();
         OSIV_TL(a.iter, 0, 2, false);
-        // Two lines per trip, written so that all gathers of a trip are in flight together: the walk is bound by the
-        // load path.  The odd line past j1 (only in the last trip) gets zero weights; its addresses stay inside the
-        // padded buffers because j1 <= nb.
+        // LPT lines per trip, written so that all gathers of a trip are in flight together: the walk is bound by the
+        // load path.  The lines past j1 (only in the last trip) get zero weights; with two lines per trip their addresses
+        // stay inside the padded buffers because j1 <= nb, with more the last valid line is read again.
         // floor() by the add-a-big-number trick (|t| < 2^22; FRND/F2I run at a quarter of the FP32 rate): r = t - 1/2 +
         // 1.5 * 2^23 rounds to the nearest integer, which is floor(t) unless t is an integer n, where it may be n - 1:
         // then pixels n - 1 and n are taken instead of n and n + 1, and both left-out pixels are a whole pixel away
         // from the crossing (weight 0 in either model).
         constexpr float BIG = 12582912.f;
-        for (int jj = j0; jj < j1; jj += 2, offP += 2 * pitch, bf += 2.f) {
-            float w[2][2];
-            int i0[2];
+        // image lines per trip: four on the one-slice quarter-turn path (eight 16-byte gathers in flight per thread; A/B at
+        // config 3: 2 lines 56.5 k, 3 55.9 k, 4 57.0 k, 5 55.8 k, 6 55.7 k, 7 56.4 k iterations/s), two elsewhere
+        constexpr int LPT = (NS == 4 && SB == 1) ? 4 : 2;
+        for (int jj = j0; jj < j1; jj += LPT, offP += LPT * pitch, bf += (float)LPT) {
+            float w[LPT][2];
+            int i0[LPT];
 #pragma unroll
-            for (int u = 0; u < 2; ++u) {
+            for (int u = 0; u < LPT; ++u) {
                 const float bg = fmaf(uu, bf + (float)u, ray.z);
                 const float r = (fmaf(-bg, invk, ca) - 0.5f) + BIG;
                 const float fa = r - BIG;                         // index of the pixel left of the crossing
@@ -379,22 +382,25 @@ __global__ void __launch_bounds__(FWD_MAX_THREADS, 1) k_forward(const FwdArgs a)
                 w[u][1] = __saturatef(hk - fabsf(q1));
                 i0[u] = min(max(__float_as_int(r) - 0x4B400000, -PAD), imax);
             }
-            if (jj + 1 >= j1) { w[1][0] = 0.f; w[1][1] = 0.f; }
+#pragma unroll
+            for (int u = 1; u < LPT; ++u)
+                if (jj + u >= j1) { w[u][0] = 0.f; w[u][1] = 0.f; }
             if constexpr (NS == 4) {
                 // one float4 per pixel and slice = the pixel in the four rotated positions: component k belongs to ray
                 // (v + k V/4, c) of the orbit, with the same weight
-                float4 x[2][2][SB];
+                float4 x[LPT][2][SB];
 #pragma unroll
-                for (int u = 0; u < 2; ++u) {
-                    OSIV_CHECK(offP + u * pitch + i0[u] >= 0 && offP + u * pitch + i0[u] + 1 < (rowmaj ? g.img_elems : g.imgT_elems), 1);
-                    const float4* p0 = qA + (offP + u * pitch + i0[u]);
+                for (int u = 0; u < LPT; ++u) {
+                    const int ul = LPT > 2 ? min(u, j1 - jj) : u;      // lines past the segment's end: any valid line (weights 0)
+                    OSIV_CHECK(offP + ul * pitch + i0[u] >= 0 && offP + ul * pitch + i0[u] + 1 < (rowmaj ? g.img_elems : g.imgT_elems), 1);
+                    const float4* p0 = qA + (offP + ul * pitch + i0[u]);
 #pragma unroll
                     for (int e = 0; e < 2; ++e)
 #pragma unroll
                         for (int sl = 0; sl < SB; ++sl) x[u][e][sl] = __ldg(p0 + sl * q_plane + e);
                 }
 #pragma unroll
-                for (int u = 0; u < 2; ++u)
+                for (int u = 0; u < LPT; ++u)
 #pragma unroll
                     for (int e = 0; e < 2; ++e)
 #pragma unroll
