@@ -144,6 +144,28 @@ def test_staged_back_kernel_matches_oracle_and_general_kernel(osiv, cfg, subsets
             assert np.array_equal(got, again)                     # no atomics on data, fixed-order sums
 
 
+@pytest.mark.parametrize("N,V,C", [(8, 8, 13), (16, 12, 25), (24, 16, 40), (72, 20, 101), (136, 24, 190)])
+def test_staged_back_kernel_region_partition_edge_sizes(osiv, N, V, C):
+    """The staged K2's block regions on small and awkward grids (one or two tiles in all, fewer regions than SMs, rows of
+    regions of unequal height): backprojection and a short reconstruction against the oracle."""
+    cfg = si.ScanConfig(f"edge{N}", N, N, 1.1, V, C, sad_mm=max(120.0, 2.0 * N), theta0_rad=0.11, channel_offset=-0.3, seed=100 + N,
+                        i0=5e4, n_subsets=1, n_iters=6, betas=(0.01,))
+    og, gg = geoms(cfg)
+    rng = np.random.default_rng(cfg.seed)
+    with osiv.Handle(gg, max_batch=2) as h:
+        assert h.back_kernel(0, 2) == "staged"
+        sino = rng.uniform(0.0, 1.0, size=(2, V, C)).astype(np.float32)
+        got = host(h.backward(dev(sino)))
+        for s in range(2):
+            assert rel(got[s], oracle.backward(og, sino[s])) < PROJ_TOL
+        _, _, counts = si.make_case(cfg)
+        prm = dict(beta=0.01, n_subsets=1, n_iters=6)
+        img, tr = h.reconstruct(dev(counts)[None], cfg.i0, osiv.Params(**prm), trace=True)
+        ref, tr_ref, _ = oracle.reconstruct(og, counts, cfg.i0, oracle.Params(**prm))
+        assert np.array_equal(tr[0, :, 1], tr_ref[:, 1])
+        assert rel(host(img)[0], ref) < IMG_TOL
+
+
 def test_staged_back_kernel_in_the_iteration(osiv):
     """The whole iteration with the staged K2 against the general K2 (same K1): equal lambda traces, images equal to
     rounding order; with return_best, a per-channel blank scan and three slices per launch."""
