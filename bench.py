@@ -327,7 +327,10 @@ def run_ours(args, cfg, beta):
             "chain": {"us_per_launch": 1e6 * chain_t,
                       "achieved_tflops": nnz * FP32_FLOP_PER_NNZ / chain_t / 1e12,
                       "frac": nnz * FP32_FLOP_PER_NNZ / chain_t / 1e12 / alu_peak_tflops,
-                      "issue_frac": (sum(c["warp_instructions"] for c in ncu.values()) / 2.0 / chain_t / 1e9 / probe["issue_ginst_per_s"]) if len(ncu) == 2 else None},
+                      "issue_frac": (sum(c["warp_instructions"] for c in ncu.values()) / 2.0 / chain_t / 1e9 / probe["issue_ginst_per_s"]) if len(ncu) == 2 else None,
+                      # the memory level that binds: L1 / shared-memory data-pipe wavefronts x 128 B of both kernels over the timed region
+                      "l1_gbs": (sum(c["l1_wavefronts_per_sm"] for c in ncu.values()) / 2.0 * 128.0 * SM_COUNT / chain_t / 1e9) if len(ncu) == 2 else None,
+                      "l1_frac": (sum(c["l1_wavefronts_per_sm"] for c in ncu.values()) / 2.0 * 128.0 * SM_COUNT / chain_t / 1e9 / probe["l1_read_gbs"]) if len(ncu) == 2 else None},
             "hbm": {"compulsory_bytes_per_launch": hbm_bytes[dom],
                     "achieved_gbs": hbm_bytes[dom] / (kernels[dom]["avg_us"] * 1e-6) / 1e9,
                     "peak_gbs": float(peaks["hbm_gbs"]), "peak_kind": peak_kind,
