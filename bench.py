@@ -40,7 +40,7 @@ SM_COUNT, FP32_LANES_PER_SM = 148, 128
 # committed ncu capture of this code (profiles/<NCU_COUNTS>.csv, written by `python -m paper_1903_10088_b200.ncu_summary`
 # from ncu's raw page; the .md beside it names the ncu command).  Counts do not depend on timing; the times they are
 # divided by are measured live in this run.
-NCU_COUNTS = {"3": "r2_ncu_config3_counts.csv"}
+NCU_COUNTS = {"3": "r2_ncu_config3_counts.csv", "5a": "r2_ncu_config5a_counts.csv", "5b": "r2_ncu_config5b_counts.csv"}
 
 
 def load_ncu_counts(workload):
@@ -412,12 +412,22 @@ def projector_pair(args, cfg):
     line = {"metric": "projector_pair", "workload": f"config{cfg.name}: {cfg.nx}x{cfg.ny}, {cfg.n_views}x{cfg.n_channels}, all views",
             "n_gpus": 1, "steps": args.steps, "dtype": "f32", "data": "synthetic", "nnz_per_pass": nnz,
             "adjoint_rel_error": abs(lhs - rhs) / abs(lhs), "l2": "flushed between passes"}
+    ncu, ncu_file = load_ncu_counts(cfg.name)
+    probe = osiv.probe_peaks(0)
     for name in ("forward", "back"):
         ms = out[name][0]
         line[name] = {"ms_per_pass": ms, "nnz_per_s": nnz / (ms * 1e-3), "algorithmic_gbs": bytes_alg / (ms * 1e-3) / 1e9,
                       "hbm_frac": bytes_alg / (ms * 1e-3) / 1e9 / float(peaks["hbm_gbs"]), "hbm_peak_kind": kind,
-                      "alu_frac": nnz * FP32_FLOP_PER_NNZ / (ms * 1e-3) / 1e12 /
-                                  (SM_COUNT * FP32_LANES_PER_SM * 2 * float(peaks.get("sm_max_mhz", 1965.0)) * 1e6 / 1e12)}
+                      "alu_frac": nnz * FP32_FLOP_PER_NNZ / (ms * 1e-3) / 1e12 / probe["ffma_tflops"]}
+        # the pass is two launches (layout kernel + projector); the projector's counts per launch from the committed capture
+        c = ncu.get("k_forward" if name == "forward" else "k_back")
+        if c:
+            t = ms * 1e-3
+            line[name].update({"issue_frac": c["warp_instructions"] / t / 1e9 / probe["issue_ginst_per_s"],
+                               "l1_gbs": c["l1_wavefronts_per_sm"] * 128.0 * SM_COUNT / t / 1e9,
+                               "l1_frac": c["l1_wavefronts_per_sm"] * 128.0 * SM_COUNT / t / 1e9 / probe["l1_read_gbs"],
+                               "l2_gbs": c["l2_sectors"] * 32.0 / t / 1e9, "l2_frac": c["l2_sectors"] * 32.0 / t / 1e9 / probe["l2_read_gbs"],
+                               "dram_gbs_cold": c["dram_bytes"] / t / 1e9, "counts_source": ncu_file})
     return line
 
 

@@ -201,9 +201,10 @@ int64_t osiv_graph_replays(const osiv_handle* h);
 
 /* Which K2 runs.  On the quarter-turn path with one slice per block (batch < 4, no stack), grids whose side is a multiple
  * of 8 and fans below 90 degrees, K2 is the kernel that stages each block's ray-table, residual and interval windows in
- * shared memory with bulk copies (csrc/osiv_back_staged.cuh); general_only = 1 forces the general gather kernel instead
- * (used by the tests to compare the two).  Results differ only by rounding order. */
-int osiv_set_back_kernel(osiv_handle* h, int32_t general_only);
+ * shared memory (csrc/osiv_back_staged.cuh) -- mode 0 (default): when one staging round holds the whole subset (otherwise
+ * the general gather kernel is the faster one); mode 1: never (used by the tests to compare the two kernels); mode 2:
+ * whenever the geometry allows, in as many rounds as it takes.  Results differ only by rounding order. */
+int osiv_set_back_kernel(osiv_handle* h, int32_t mode);
 /* *staged = 1 if osiv_reconstruct / osiv_backward with `n_subsets` subsets (<= 0: all views) and `batch` slices would
  * run the staged K2, else 0.  Host only. */
 int osiv_get_back_kernel(const osiv_handle* h, int32_t n_subsets, int32_t batch, int32_t* staged);

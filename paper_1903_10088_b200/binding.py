@@ -263,9 +263,10 @@ class Handle:
     def graph_replays(self) -> int:
         return int(lib().osiv_graph_replays(self._h))
 
-    def set_back_kernel(self, general_only: bool) -> None:
-        """general_only=True forces the general gather K2 where the shared-memory-staged K2 would run"""
-        _check(lib().osiv_set_back_kernel(self._h, 1 if general_only else 0), "osiv_set_back_kernel")
+    def set_back_kernel(self, general_only: bool = False, staged_rounds: bool = False) -> None:
+        """general_only=True forces the general gather K2 where the shared-memory-staged K2 would run; staged_rounds=True
+        lets the staged K2 also take subsets that need several staging rounds (by default the general kernel takes those)"""
+        _check(lib().osiv_set_back_kernel(self._h, 1 if general_only else 2 if staged_rounds else 0), "osiv_set_back_kernel")
 
     def back_kernel(self, n_subsets: int = 0, batch: int = 1) -> str:
         """'staged' or 'general': the K2 that reconstruct / backward would run"""

@@ -52,7 +52,8 @@ struct osiv_handle {
     long long ray_entries = 0;          // float4 entries behind d_rays (table + zero slack)
     // staged K2 (osiv_back_staged.cuh): regions of the base quadrant, per-(view, block) windows, per-tile intervals
     int st_ready = 0;                   // 1: tables built and usable; 0: this geometry does not take the staged kernel
-    int st_off = 0;                     // osiv_set_back_kernel(h, 1): always the general K2
+    int st_off = 0;                     // osiv_set_back_kernel: 0 = staged when one round suffices, 1 = always the general K2, 2 = staged
+                                        // whenever the geometry allows (several rounds)
     int st_nblk = 0, st_tpbp = 0, st_W = 0;
     int4* d_regions = nullptr;
     unsigned short* d_itab2 = nullptr;
@@ -444,15 +445,6 @@ int ensure_blob(osiv_handle* h, int M, cudaStream_t st) {
     return OSIV_OK;
 }
 
-// the staged K2 serves one slice per block on the quarter-turn path when the subset has at least two base views
-bool use_staged(const osiv_handle* h, const BackPlan& p, bool stack) {
-    return h->st_ready && !h->st_off && p.ns == 4 && p.sb == 1 && !stack;
-}
-// ... and K1's monitor partials per slice fit the step-rule warp's registers
-bool use_staged(const osiv_handle* h, const BackPlan& p, bool stack, const FwdPlan& f) {
-    return use_staged(h, p, stack) && f.nparts <= 32 * BS_DPK;
-}
-
 StagedPlan plan_staged(const osiv_handle* h, int VS) {
     StagedPlan p;
     p.nblk = h->st_nblk; p.tpbp = h->st_tpbp; p.W = h->st_W;
@@ -466,6 +458,19 @@ StagedPlan plan_staged(const osiv_handle* h, int VS) {
     p.nrounds = (VSb + p.JR - 1) / p.JR;
     p.smem = fixed + (size_t)p.JR * per_view;
     return p;
+}
+
+// The staged K2 serves one slice per block on the quarter-turn path when the subset's windows fit its shared memory in ONE
+// round (config 3: 10 base views).  With several rounds (all 800 views in osiv_backward: 13 rounds, each with its barriers
+// and a fresh fetch) the general kernel is faster -- 5a 0.118 against 0.144 ms, 5b 0.90 against 1.22 ms per pass -- and takes
+// those calls; osiv_set_back_kernel(h, 2) stages them anyway (tests of the round logic).
+bool use_staged(const osiv_handle* h, const BackPlan& p, bool stack, int VS) {
+    if (!(h->st_ready && h->st_off != 1 && p.ns == 4 && p.sb == 1 && !stack)) return false;
+    return h->st_off == 2 || plan_staged(h, VS).nrounds == 1;
+}
+// ... and K1's monitor partials per slice fit the step-rule warp's registers
+bool use_staged(const osiv_handle* h, const BackPlan& p, bool stack, int VS, const FwdPlan& f) {
+    return use_staged(h, p, stack, VS) && f.nparts <= 32 * BS_DPK;
 }
 
 template <int MODE>
@@ -758,9 +763,9 @@ int osiv_set_symmetry(osiv_handle* h, int32_t enable) {
     return OSIV_OK;
 }
 
-int osiv_set_back_kernel(osiv_handle* h, int32_t general_only) {
-    if (!h) return OSIV_ERR_INVALID_ARG;
-    h->st_off = general_only ? 1 : 0;
+int osiv_set_back_kernel(osiv_handle* h, int32_t mode) {
+    if (!h || mode < 0 || mode > 2) return OSIV_ERR_INVALID_ARG;
+    h->st_off = mode;
     return OSIV_OK;
 }
 
@@ -775,7 +780,7 @@ int64_t osiv_graph_replays(const osiv_handle* h) { return h ? h->graph_replays :
 int osiv_get_back_kernel(const osiv_handle* h, int32_t n_subsets, int32_t batch, int32_t* staged) {
     if (!h || !staged || batch <= 0 || (n_subsets > 0 && h->geom.n_views % n_subsets != 0)) return OSIV_ERR_INVALID_ARG;
     const int VS = n_subsets > 0 ? h->geom.n_views / n_subsets : h->geom.n_views;
-    *staged = use_staged(h, plan_back(h, VS, batch), false, plan_forward(h, VS, batch)) ? 1 : 0;
+    *staged = use_staged(h, plan_back(h, VS, batch), false, VS) ? 1 : 0;
     return OSIV_OK;
 }
 
@@ -792,7 +797,7 @@ int osiv_get_plan(const osiv_handle* h, int32_t n_subsets, int32_t batch, int32_
     const BackPlan b = plan_back(h, VS, batch);
     out8[0] = f.ns; out8[1] = f.segs; out8[2] = f.nparts * ((batch + f.sb - 1) / f.sb); out8[3] = f.threads;
     out8[4] = b.ns; out8[5] = b.shares; out8[6] = b.nblk * ((batch + b.sb - 1) / b.sb); out8[7] = b.threads;
-    if (use_staged(h, b, false)) {
+    if (use_staged(h, b, false, VS)) {
         const StagedPlan sp = plan_staged(h, VS);
         out8[5] = BS_SHARES; out8[6] = sp.nblk * batch; out8[7] = sp.threads;
     }
@@ -855,7 +860,7 @@ int osiv_backward(osiv_handle* h, const float* d_sino, float* d_img, int32_t bat
     BackArgs b{};
     b.res_floats = (long long)h->res_elems; b.ray_entries = h->ray_entries;
     b.g = h->dg; b.res = h->d_res; b.Cp = Cp; b.subset = subset; b.M = M; b.VS = VS; b.batch = batch; b.out = d_img; b.tpb = p.tpb; b.shares = p.shares; b.ngx = p.ngx; b.tpb_magic = div_magic(p.tpb); b.ngx_magic = div_magic(p.ngx);
-    if (use_staged(h, p, false)) {
+    if (use_staged(h, p, false, VS)) {
         if ((rc = ensure_blob(h, M, st)) != OSIV_OK) return rc;
         if (launch_back_staged<0>(h, plan_staged(h, VS), batch, b, st, false) != cudaSuccess) { cudaGetLastError(); return OSIV_ERR_CUDA; }
         return launch_check(h, 2);
@@ -930,7 +935,7 @@ int osiv_reconstruct(osiv_handle* h, const float* d_counts, const float* d_blank
     BackArgs b{};
     b.res_floats = (long long)h->res_elems; b.ray_entries = h->ray_entries;
     b.g = h->dg; b.res = h->d_res; b.Cp = Cp; b.M = M; b.VS = VS; b.batch = batch; b.view_shift = vshift; b.tv_z = (float)prm->tv_z; b.best = best; b.tpb = bp.tpb; b.shares = bp.shares; b.ngx = bp.ngx; b.tpb_magic = div_magic(bp.tpb); b.ngx_magic = div_magic(bp.ngx);
-    const bool staged = use_staged(h, bp, stack, fp);
+    const bool staged = use_staged(h, bp, stack, VS, fp);
     const StagedPlan sp = staged ? plan_staged(h, VS) : StagedPlan{};
     if (staged) {
         if ((rc = ensure_blob(h, M, st)) != OSIV_OK) return rc;

@@ -131,12 +131,13 @@ def test_staged_back_kernel_matches_oracle_and_general_kernel(osiv, cfg, subsets
         for sub, M in subsets:
             vs = cfg.n_views if sub < 0 else cfg.n_views // M
             sino = rng.uniform(0.0, 1.0, size=(3, vs, cfg.n_channels)).astype(np.float32)
+            h.set_back_kernel(staged_rounds=True)                 # also the subsets that take several staging rounds
             assert h.back_kernel(M if sub >= 0 else 0, 3) == "staged"
             got = host(h.backward(dev(sino), sub, M))
             h.set_back_kernel(general_only=True)
             assert h.back_kernel(M if sub >= 0 else 0, 3) == "general"
             gen = host(h.backward(dev(sino), sub, M))
-            h.set_back_kernel(general_only=False)
+            h.set_back_kernel(staged_rounds=True)
             for s in range(3):
                 assert rel(got[s], oracle.backward(og, sino[s], sub, M)) < PROJ_TOL, (cfg.name, sub, M, s)
             assert rel(got, gen) < 2e-6
@@ -153,6 +154,7 @@ def test_staged_back_kernel_region_partition_edge_sizes(osiv, N, V, C):
     og, gg = geoms(cfg)
     rng = np.random.default_rng(cfg.seed)
     with osiv.Handle(gg, max_batch=2) as h:
+        h.set_back_kernel(staged_rounds=True)
         assert h.back_kernel(0, 2) == "staged"
         sino = rng.uniform(0.0, 1.0, size=(2, V, C)).astype(np.float32)
         got = host(h.backward(dev(sino)))
