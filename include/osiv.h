@@ -40,7 +40,8 @@ typedef enum {
     OSIV_ERR_INVALID_ARG = -1,  /* null pointer, non-positive size, n_views % n_subsets != 0, n_views > 65535,
                                    batch > max_batch, tv_eps <= 0, source inside the grid's circumscribed circle */
     OSIV_ERR_CUDA        = -2,  /* a CUDA runtime call failed (no device, out of memory, launch error) */
-    OSIV_ERR_NOT_FINITE  = -3   /* the monitor D became NaN/Inf for at least one slice */
+    OSIV_ERR_NOT_FINITE  = -3,  /* the monitor D became NaN/Inf for at least one slice */
+    OSIV_ERR_SCRATCH_LIMIT = -4 /* osiv_tv_gradient_static: the padded images do not fit OSIV_STATIC_SCRATCH_BYTES */
 } osiv_status;
 
 /* Scan geometry (reading C1; the paper prints none, BASELINE.json supplies SAD/SDD/channels).
@@ -140,6 +141,21 @@ int osiv_backward(osiv_handle* h, const float* d_sino, float* d_img, int32_t bat
  * Both [batch][ny][nx].  Asynchronous on cuda_stream. */
 int osiv_tv_gradient(osiv_handle* h, const float* d_img, float* d_grad, int32_t batch, double tv_eps,
                      void* cuda_stream);
+
+/* The same gradient (C8) for callers that may not allocate device memory (code under CUDA graph capture, serving
+ * loops, harnesses that forbid cudaMalloc): this call makes no cudaMalloc / cudaFree / allocating library call, on the
+ * first call or any later one.  The padded copy of the images, which osiv_tv_gradient keeps in the handle's lazily
+ * allocated workspace, lives in a fixed array of OSIV_STATIC_SCRATCH_BYTES that is part of the library image: every GPU
+ * that loads libosiv holds it until the process exits.  osiv_create resolves the array's device address once per
+ * device.  Needs batch * (ny + 2) * (nx + 8) * 4 bytes of it (one 1016 x 1016 slice, or three 512 x 512 slices);
+ * a larger request returns OSIV_ERR_SCRATCH_LIMIT before anything is enqueued and leaves d_grad untouched.
+ * The array is shared by every handle and every call on a device and keeps the last call's contents: each call clears
+ * the part it uses first (the zero border is part of the operation), so calls in one stream are safe back to back,
+ * but two calls that overlap on the GPU (different streams, or different handles on different streams) race on it --
+ * serialise them.  Same arguments, results and asynchrony as osiv_tv_gradient (bit-identical output). */
+#define OSIV_STATIC_SCRATCH_BYTES (4u << 20)
+int osiv_tv_gradient_static(osiv_handle* h, const float* d_img, float* d_grad, int32_t batch, double tv_eps,
+                            void* cuda_stream);
 
 /* The ordered-subset iteration (PAPER.md:74 Eq. 3, :100-108 Eq. 4-5, :114, :118, :63, :140):
  *   mu(0) = mu0;  for n = 0 .. n_iters-1, m = n mod M:

@@ -7,5 +7,6 @@ device, and loading raises if the library has not been built (``python -m paper_
 """
 from .binding import (  # noqa: F401
     Geometry, Params, Handle, OsivError, lib, lib_path, version, strerror, default_params, ray_table, probe_peaks, debug_checks,
-    OSIV_OK, OSIV_ERR_INVALID_ARG, OSIV_ERR_CUDA, OSIV_ERR_NOT_FINITE, EXPORTED_SYMBOLS,
+    OSIV_OK, OSIV_ERR_INVALID_ARG, OSIV_ERR_CUDA, OSIV_ERR_NOT_FINITE, OSIV_ERR_SCRATCH_LIMIT, STATIC_SCRATCH_BYTES,
+    EXPORTED_SYMBOLS,
 )

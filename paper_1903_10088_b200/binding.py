@@ -13,11 +13,12 @@ import numpy as np
 
 from . import build as _build
 
-OSIV_OK, OSIV_ERR_INVALID_ARG, OSIV_ERR_CUDA, OSIV_ERR_NOT_FINITE = 0, -1, -2, -3
+OSIV_OK, OSIV_ERR_INVALID_ARG, OSIV_ERR_CUDA, OSIV_ERR_NOT_FINITE, OSIV_ERR_SCRATCH_LIMIT = 0, -1, -2, -3, -4
+STATIC_SCRATCH_BYTES = 4 << 20      # OSIV_STATIC_SCRATCH_BYTES of include/osiv.h
 
 EXPORTED_SYMBOLS = (
     "osiv_version", "osiv_strerror", "osiv_default_params", "osiv_create", "osiv_destroy", "osiv_ray_table", "osiv_get_dgamma",
-    "osiv_get_tau", "osiv_launch_count", "osiv_set_symmetry", "osiv_set_overlap", "osiv_set_back_kernel", "osiv_get_back_kernel", "osiv_set_graph", "osiv_graph_replays", "osiv_debug_checks", "osiv_get_plan", "osiv_set_profiling", "osiv_get_profile", "osiv_forward", "osiv_backward", "osiv_tv_gradient", "osiv_reconstruct",
+    "osiv_get_tau", "osiv_launch_count", "osiv_set_symmetry", "osiv_set_overlap", "osiv_set_back_kernel", "osiv_get_back_kernel", "osiv_set_graph", "osiv_graph_replays", "osiv_debug_checks", "osiv_get_plan", "osiv_set_profiling", "osiv_get_profile", "osiv_forward", "osiv_backward", "osiv_tv_gradient", "osiv_tv_gradient_static", "osiv_reconstruct",
     "osiv_reconstruct_host", "osiv_probe_peaks", "osiv_debug_timeline",
 )
 
@@ -121,6 +122,7 @@ def lib():
         L.osiv_forward.argtypes = [vp, vp, vp, ip, ip, ip, vp]
         L.osiv_backward.argtypes = [vp, vp, vp, ip, ip, ip, vp]
         L.osiv_tv_gradient.argtypes = [vp, vp, vp, ip, C.c_double, vp]
+        L.osiv_tv_gradient_static.argtypes = [vp, vp, vp, ip, C.c_double, vp]
         L.osiv_reconstruct.argtypes = [vp, vp, vp, C.c_float, C.POINTER(_CParams), ip, vp, vp, vp]
         L.osiv_reconstruct_host.argtypes = [vp, vp, vp, C.c_float, C.POINTER(_CParams), ip, vp, vp, vp]
         L.osiv_probe_peaks.argtypes = [ip, C.POINTER(C.c_double)]
@@ -327,6 +329,17 @@ class Handle:
             out = torch.empty_like(img)
         op = _dev(out, (batch, g.ny, g.nx), "out")
         _check(lib().osiv_tv_gradient(self._h, ip, op, batch, tv_eps, _stream()), "osiv_tv_gradient")
+        return out
+
+    def tv_gradient_static(self, img, out, tv_eps: float = 1e-5):
+        """osiv_tv_gradient_static: the same gradient with its scratch in the library's fixed device array; nothing is
+        allocated, here or in the library, so `out` is required.  Raises OsivError(SCRATCH_LIMIT) beyond
+        STATIC_SCRATCH_BYTES.  Calls that overlap on the GPU race on the shared array."""
+        g = self.geom
+        batch = img.shape[0]
+        ip = _dev(img, (batch, g.ny, g.nx), "img")
+        op = _dev(out, (batch, g.ny, g.nx), "out")
+        _check(lib().osiv_tv_gradient_static(self._h, ip, op, batch, tv_eps, _stream()), "osiv_tv_gradient_static")
         return out
 
     def reconstruct(self, counts, blank, params: Params, out=None, trace: bool = False):

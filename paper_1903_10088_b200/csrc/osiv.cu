@@ -77,6 +77,7 @@ struct osiv_handle {
     } gslot[2];
     long long gclock = 0;
     int64_t graph_replays = 0;
+    float* d_static = nullptr;          // device address of g_static_scratch on this handle's device (osiv_tv_gradient_static)
     // per-kernel event timing (osiv_set_profiling)
     bool profiling = false;
     std::vector<cudaEvent_t> events;
@@ -84,7 +85,39 @@ struct osiv_handle {
     int64_t prof_n_fwd = 0, prof_n_back = 0;
 };
 
+// ---- scratch of the allocation-free entry point (osiv_tv_gradient_static) --------------------------------------
+// The padded images of that call live here instead of in cudaMalloc'ed workspace.  The array is part of the module
+// image: every device that loads the library holds OSIV_STATIC_SCRATCH_BYTES of it until the process exits.  In host
+// code the name below is only a stand-in for the symbol, not a device address: the address comes from
+// cudaGetSymbolAddress, once per device with that device current (static_scratch_address, called by osiv_create).
+static __device__ __align__(256) float g_static_scratch[OSIV_STATIC_SCRATCH_BYTES / sizeof(float)];
+
+constexpr int STATIC_MAX_DEVICES = 64;
+static float* g_static_addr[STATIC_MAX_DEVICES] = {};
+
+// [batch][ny][nx] -> zero-bordered row-major copies (DevGeom::sb == 1), the layout k_tv reads; borders are cleared by
+// the caller
+__global__ void __launch_bounds__(256) k_pad_rows(DevGeom g, const float* __restrict__ src, float* __restrict__ img) {
+    const int s = blockIdx.z;
+    const int x = blockIdx.x * 32 + (threadIdx.x & 31);
+    const int y = blockIdx.y * 8 + (threadIdx.x >> 5);
+    if (x >= g.nx || y >= g.ny) return;
+    img[(size_t)s * g.img_elems + pad_off(g, y, x)] = src[((size_t)s * g.ny + y) * g.nx + x];
+}
+
 namespace {
+
+// device address of g_static_scratch on `device`, which must be current; null if the lookup fails (the entry point
+// then reports OSIV_ERR_CUDA).  No allocation: the array already exists on every device that loaded the module.
+float* static_scratch_address(int device) {
+    if (device < 0 || device >= STATIC_MAX_DEVICES) return nullptr;
+    if (!g_static_addr[device]) {
+        float* p = nullptr;
+        if (cudaGetSymbolAddress((void**)&p, g_static_scratch) != cudaSuccess) { cudaGetLastError(); return nullptr; }
+        g_static_addr[device] = p;
+    }
+    return g_static_addr[device];
+}
 
 struct DeviceGuard {
     int prev = -1;
@@ -561,6 +594,7 @@ const char* osiv_strerror(int status) {
         case OSIV_ERR_INVALID_ARG: return "invalid argument";
         case OSIV_ERR_CUDA: return "CUDA error (no usable device, out of memory or launch failure)";
         case OSIV_ERR_NOT_FINITE: return "monitor D became non-finite";
+        case OSIV_ERR_SCRATCH_LIMIT: return "osiv_tv_gradient_static: batch * (ny + 2) * (nx + 8) * 4 bytes exceed OSIV_STATIC_SCRATCH_BYTES (4 MiB)";
         default: return "unknown status";
     }
 }
@@ -617,6 +651,7 @@ int osiv_create(const osiv_geometry* geom, int32_t max_batch, int32_t device, os
     osiv_handle* h = new (std::nothrow) osiv_handle();
     if (!h) return OSIV_ERR_CUDA;
     h->geom = g; h->dgamma = dgamma; h->device = device; h->max_batch = max_batch;
+    h->d_static = static_scratch_address(device);     // set-up for osiv_tv_gradient_static; a failure shows there
 
     std::vector<float4> rays;
     std::vector<float2> views;
@@ -881,6 +916,27 @@ int osiv_tv_gradient(osiv_handle* h, const float* d_img, float* d_grad, int32_t 
     if (rc != OSIV_OK) return rc;
     k_pad_transpose<<<px_grid(h, batch), 256, 0, st>>>(h->dg, 1, d_img, h->d_imgA, h->d_imgTA);
     k_tv<<<dim3((h->geom.nx + 31) / 32, (h->geom.ny + 15) / 16, batch), 128, 0, st>>>(h->dg, h->d_imgA,
+                                                                                     (float)(tv_eps * tv_eps), d_grad);
+    return launch_check(h, 2);
+}
+
+// Allocation-free variant of osiv_tv_gradient: the padded images go to g_static_scratch.  Only a memset and two kernel
+// launches are enqueued; the handle's workspace is neither read nor grown.
+int osiv_tv_gradient_static(osiv_handle* h, const float* d_img, float* d_grad, int32_t batch, double tv_eps,
+                            void* cuda_stream) {
+    if (!h || !d_img || !d_grad || batch <= 0 || batch > h->max_batch || !(tv_eps > 0.0)) return OSIV_ERR_INVALID_ARG;
+    const size_t need = (size_t)batch * (size_t)h->dg.img_elems * sizeof(float);
+    if (need > (size_t)OSIV_STATIC_SCRATCH_BYTES) return OSIV_ERR_SCRATCH_LIMIT;
+    if (!h->d_static) return OSIV_ERR_CUDA;             // cudaGetSymbolAddress failed at osiv_create
+    DeviceGuard guard(h->device);
+    if (!guard.ok) { cudaGetLastError(); return OSIV_ERR_CUDA; }
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    DevGeom g = h->dg;
+    g.sb = 1;
+    // the array keeps the previous call's images (possibly of another geometry): clear the part this call reads
+    OSIV_CUDA(cudaMemsetAsync(h->d_static, 0, need, st));
+    k_pad_rows<<<px_grid(h, batch), 256, 0, st>>>(g, d_img, h->d_static);
+    k_tv<<<dim3((h->geom.nx + 31) / 32, (h->geom.ny + 15) / 16, batch), 128, 0, st>>>(g, h->d_static,
                                                                                      (float)(tv_eps * tv_eps), d_grad);
     return launch_check(h, 2);
 }

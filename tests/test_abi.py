@@ -60,6 +60,8 @@ def test_argument_validation_happens_before_cuda():
     # null handles
     assert L.osiv_forward(None, None, None, 1, -1, 1, None) == osiv.OSIV_ERR_INVALID_ARG
     assert L.osiv_backward(None, None, None, 1, -1, 1, None) == osiv.OSIV_ERR_INVALID_ARG
+    assert L.osiv_tv_gradient_static(None, None, None, 1, 1e-5, None) == osiv.OSIV_ERR_INVALID_ARG
+    assert "OSIV_STATIC_SCRATCH_BYTES" in osiv.strerror(osiv.OSIV_ERR_SCRATCH_LIMIT)
     assert L.osiv_reconstruct(None, None, None, 1.0, None, 1, None, None, None) == osiv.OSIV_ERR_INVALID_ARG
     assert L.osiv_reconstruct_host(None, None, None, 1.0, None, 1, None, None, None) == osiv.OSIV_ERR_INVALID_ARG
     assert L.osiv_destroy(None) == osiv.OSIV_OK
