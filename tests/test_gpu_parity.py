@@ -637,6 +637,21 @@ def test_reconstruct_config3_other_betas_full(osiv, beta):
     assert 0.02 < tr[:, 1].max() < 0.03 and tr[-1, 1] < tr[:, 1].max()
 
 
+@pytest.mark.parametrize("M,n_iters", [(1, 3), (2, 6), (5, 15), (10, 30), (40, 120)])
+def test_reconstruct_config3_at_the_papers_other_thinning_parameters(osiv, M, n_iters):
+    """PAPER.md:158-164 Table I times one 512 x 512 slice at thinning 1, 1/2, 1/5, 1/10, 1/20 and 1/40 (1/20 is config 3
+    itself, above); bench.py's `extra.table1` times the same six.  Each is another launch plan at full size (K1's rays per
+    block and segments; K2: the general kernel for M <= 10, where a subset's windows need several staging rounds, the
+    staged one for 20 and 40), checked here against the oracle for about 2400 view-iterations (three passes over the
+    subsets for M = 40), with the paper's regulariser scaling beta / M."""
+    cfg = si.scan_config("3")
+    with osiv.Handle(geoms(cfg)[1], max_batch=1) as h:
+        assert h.back_kernel(M, 1) == ("staged" if M >= 20 else "general")
+    got, tr, ref, tr_ref, st = run_pair(osiv, cfg, dict(beta=0.005, n_subsets=M, n_iters=n_iters))
+    assert st == 0
+    check_run(got, tr, ref, tr_ref)
+
+
 def test_pairs_of_slices_path_at_config4_size(osiv):
     """A8 where the clock runs (BASELINE.json configs[3]: slices of 512x512, 800 x 738, 20 subsets): the launch plan of the
     pair-of-slices path at this size (K1 two 512-thread blocks per SM, K2 view shares of 56 tiles) is another regime
