@@ -53,6 +53,7 @@ struct osiv_handle {
     // staged K2 (osiv_back_staged.cuh): regions of the base quadrant, per-(view, block) windows, per-tile intervals
     int st_ready = 0;                   // 1: tables built and usable; 0: this geometry does not take the staged kernel
     int st_off = 0;                     // osiv_set_back_kernel: 0 = staged when one round suffices, 1 = always the general K2, 2 = staged
+    std::vector<int4> st_regions;       // host copy of d_regions (passed in the kernel parameters when short enough)
                                         // whenever the geometry allows (several rounds)
     int st_nblk = 0, st_tpbp = 0, st_W = 0;
     int4* d_regions = nullptr;
@@ -456,6 +457,7 @@ int build_staged(osiv_handle* h, double tile_hw_staged) {
         return OSIV_ERR_CUDA;
     }
     h->st_nblk = nblk; h->st_tpbp = tpbp; h->st_W = W;
+    h->st_regions = regions;
     h->st_ready = 1;
     return OSIV_OK;
 }
@@ -514,6 +516,7 @@ cudaError_t launch_back_staged(const osiv_handle* h, const StagedPlan& p, int ba
     sa.nblk = p.nblk; sa.tpbp = p.tpbp; sa.tpbp_magic = div_magic(p.tpbp); sa.W = p.W; sa.W_magic = div_magic(p.W); sa.SP = p.threads / p.W; sa.JR = p.JR; sa.nrounds = p.nrounds;
     sa.slot_c = p.slot_c;
     sa.hka = h->geom.model == 1 ? 0.f : 0.5f; sa.hkb = h->geom.model == 1 ? 1.f : 0.5f;
+    if (p.nblk <= BS_PARAM_REGIONS) std::memcpy(sa.regions_c, h->st_regions.data(), (size_t)p.nblk * sizeof(int4));
     cudaLaunchConfig_t cfg{};
     cfg.gridDim = dim3(p.nblk, 1, batch); cfg.blockDim = dim3(p.threads); cfg.stream = st;
     cfg.dynamicSmemBytes = p.smem;

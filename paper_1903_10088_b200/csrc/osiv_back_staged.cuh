@@ -41,6 +41,7 @@ constexpr int BS_RED_PITCH = BS_PX + 1;              // float4 per (share, tile)
 constexpr int BS_RCH = 8;                            // residual chunks (16 bytes) a thread fetches per round: 4 * JR * W <= 8 * threads
 constexpr int BS_DPK = 8;                            // monitor partials per lane of the step-rule warp: K1 blocks per slice <= 256
 constexpr int BS_HDR_BYTES = 256;                    // mbarriers + step/improved words in front of the staging area
+constexpr int BS_PARAM_REGIONS = 160;                // regions that travel in the kernel parameters (constant bank) instead of a table
 
 struct BackSArgs {
     BackArgs b;                            // geometry, residuals, images, state, step-rule parameters (as for k_back)
@@ -55,6 +56,9 @@ struct BackSArgs {
     int SP;                                // residual slots fetched per pass = threads / W
     int slot_c;                            // 16 + W * 8 + tpbp * 2
     float hka, hkb;                        // half-width of a ray's trapezoid = |k| * hka + hkb (exact chord: 1/2, 1/2; Joseph: 0, 1)
+    // the same table in the kernel parameters when nblk <= BS_PARAM_REGIONS: a block learns its region from the constant
+    // bank instead of with an L2 round trip at the head of its start-up path (its neighbourhood loads depend on it)
+    int4 regions_c[BS_PARAM_REGIONS];
 };
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -310,7 +314,7 @@ __global__ void __launch_bounds__(BS_SHARES * BS_MAX_TPB, 1) k_back_staged(const
             if (roff[n] >= 0) rst[(n * SP + s0) * W + r0] = rv[n];
     };
     load_c0(0, min(JR, VSb));
-    const int4 reg = sa.regions[b];
+    const int4 reg = sa.nblk <= BS_PARAM_REGIONS ? sa.regions_c[b] : sa.regions[b];
     // walk role: tile slot i, share q
     const int q = fastdiv(t, sa.tpbp_magic), i = t - q * tpbp;
     int x0, y0;
