@@ -63,6 +63,7 @@ struct osiv_handle {
     int4* d_k1rng = nullptr;            // K1's block line ranges for (k1rng_M subsets, orbit size, rays per block), k_build_fwd_ranges
     size_t k1rng_elems = 0;
     long long k1rng_key = -1;
+    std::vector<unsigned short> k1order; // [M][blocks]: K1's runs of rays, longest walk first (FwdArgs::order), with d_k1rng
     unsigned char* d_blob = nullptr;    // per-subset constants of the staged K2 for blob_M subsets (k_build_blob)
     size_t blob_bytes = 0;
     int blob_M = 0;
@@ -557,6 +558,22 @@ int ensure_fwd_ranges(osiv_handle* h, const FwdPlan& p, int M, cudaStream_t st) 
     k_build_fwd_ranges<<<dim3(p.nparts, M), (p.rpb + 31) / 32 * 32, 0, st>>>(h->dg, M, h->geom.n_views / M, p.ns, p.rpb, h->d_k1rng);
     h->launches += 1;
     OSIV_CUDA(cudaGetLastError());
+    // the order in which K1's blocks take the runs: a block's walk is as long as the longer of its two line ranges
+    h->k1order.clear();
+    if (p.nparts <= FWD_ORDER_MAX) {
+        std::vector<int4> rng((size_t)M * p.nparts);
+        OSIV_CUDA(cudaMemcpyAsync(rng.data(), h->d_k1rng, rng.size() * sizeof(int4), cudaMemcpyDeviceToHost, st));
+        OSIV_CUDA(cudaStreamSynchronize(st));
+        h->k1order.resize(rng.size());
+        std::vector<int> idx(p.nparts);
+        for (int m = 0; m < M; ++m) {
+            const int4* r = rng.data() + (size_t)m * p.nparts;
+            for (int b = 0; b < p.nparts; ++b) idx[b] = b;
+            auto cost = [&](int b) { return std::max(std::max(r[b].y - r[b].x + 1, r[b].w - r[b].z + 1), 0); };
+            std::stable_sort(idx.begin(), idx.end(), [&](int x, int y) { return cost(x) > cost(y); });
+            for (int b = 0; b < p.nparts; ++b) h->k1order[(size_t)m * p.nparts + b] = (unsigned short)idx[b];
+        }
+    }
     h->k1rng_key = key;
     return OSIV_OK;
 }
@@ -1031,6 +1048,8 @@ int osiv_reconstruct(osiv_handle* h, const float* d_counts, const float* d_blank
     for (int n = 0; n < N; ++n) {
         const int m = n % M;                               // PAPER.md:118, C11
         f.img = cur; f.imgT = curT; f.subset = m; f.iter = n; b.iter = n;
+        f.use_order = (!stack && !h->k1order.empty()) ? 1 : 0;     // longest walks first: 58.16 -> 58.28 k iterations/s (shortest first: 57.95 k)
+        if (f.use_order) std::memcpy(f.order, &h->k1order[(size_t)m * fp.nparts], (size_t)fp.nparts * sizeof(unsigned short));
         OSIV_CUDA(launch_forward<1>(fp, batch, f, st, pdl));
         if (prof) cudaEventRecord(h->events[2 * n + 1], st);
         b.img = cur; b.img_new = nxt; b.imgT_new = nxtT; b.subset = m;
@@ -1055,7 +1074,7 @@ int osiv_reconstruct(osiv_handle* h, const float* d_counts, const float* d_blank
     SliceState* fin = state[N & 1];
     if (prm->return_best) {
         // the final iterate competes too, judged on the subset that would come next (C12)
-        f.img = cur; f.imgT = curT; f.subset = N % M;
+        f.img = cur; f.imgT = curT; f.subset = N % M; f.use_order = 0;
         if (launch_forward<1>(fp, batch, f, st, false) != cudaSuccess) { cudaGetLastError(); return OSIV_ERR_CUDA; }
         k_final_monitor<<<batch, 32, 0, st>>>(h->d_dparts, fp.nparts, fin, h->d_not_finite);
         h->launches += 2;

@@ -123,6 +123,8 @@ struct IterParams {
     double* dhist;                         // monitor_mode 1: [batch][2M] ring of the last 2M monitor values
 };
 
+constexpr int FWD_ORDER_MAX = 160;         // K1 blocks per slice whose order travels in the kernel parameters
+
 struct FwdArgs {
     DevGeom g;
     const float* img;                      // padded mu, slice stride g.img_elems
@@ -147,6 +149,12 @@ struct FwdArgs {
     int Cp;
     double* dparts;                        // MODE 1: [batch][gridDim.x] partial sums of D
     long long res_floats;                  // floats in `res` (checked build)
+    // Blocks are handed to the SMs in blockIdx order as the predecessor's blocks exit, about a microsecond between the
+    // first and the last: order[blockIdx.x] = the run of rays this block takes, the runs with the longest walks first
+    // (from the tabulated line ranges, per subset), so that the late starters are the short ones.  In the kernel
+    // parameters (constant bank): a table in memory would put a round trip at the head of the start-up path.
+    int use_order;
+    unsigned short order[FWD_ORDER_MAX];
 };
 
 struct BackArgs {
@@ -284,7 +292,8 @@ __global__ void __launch_bounds__(FWD_MAX_THREADS, 1) k_forward(const FwdArgs a)
     const int seg = fastdiv(t, a.rpb_magic), i = t - seg * rpb;
     const int VSb = a.VS / NS, Vq = g.V / NS;
     const int R = VSb * g.C;
-    const int r = blockIdx.x * rpb + i;
+    const int bx = a.use_order ? (int)a.order[blockIdx.x] : (int)blockIdx.x;      // the run of rays of this block
+    const int r = bx * rpb + i;
     const bool walker = seg < segs && r < R;
     const int rr = min(r, R - 1);
     const int jb = fastdiv(rr, a.C_magic), c = rr - jb * g.C;
@@ -325,7 +334,7 @@ __global__ void __launch_bounds__(FWD_MAX_THREADS, 1) k_forward(const FwdArgs a)
         int wlo, whi;
         OSIV_TL(a.iter, 0, 7, false);
         if (a.rng_tab) {                                      // tabulated (A0): no barrier in the start-up path
-            const int4 rg = __ldg(&a.rng_tab[(size_t)(a.subset < 0 ? 0 : a.subset) * gridDim.x + blockIdx.x]);
+            const int4 rg = __ldg(&a.rng_tab[(size_t)(a.subset < 0 ? 0 : a.subset) * gridDim.x + bx]);
             wlo = rowmaj ? rg.x : rg.z; whi = rowmaj ? rg.y : rg.w;
         } else {
         int flo, fhi;
@@ -516,7 +525,7 @@ __global__ void __launch_bounds__(FWD_MAX_THREADS, 1) k_forward(const FwdArgs a)
         if (t < SB) {                                                  // one thread per slice: the warp sums in a fixed order
             double D = 0.0;
             for (int w = 0; w < nw; ++w) D += dred[t][w];
-            if (s0 + t < a.batch) a.dparts[(size_t)(s0 + t) * gridDim.x + blockIdx.x] = D;
+            if (s0 + t < a.batch) a.dparts[(size_t)(s0 + t) * gridDim.x + bx] = D;
         }
     }
     OSIV_TL(a.iter, 0, 5, true);
