@@ -352,10 +352,17 @@ __global__ void __launch_bounds__(BS_SHARES * BS_MAX_TPB, 1) k_back_staged(const
     float cur[4] = {0.f, 0.f, 0.f, 0.f}, tv[4] = {0.f, 0.f, 0.f, 0.f};
     if (MODE == 1) {
         if (fin) {
-            orbit_tv<0>(E, px, py, N, a.eps2, cur[0], tv[0]);
-            orbit_tv<1>(E, px, py, N, a.eps2, cur[1], tv[1]);
-            orbit_tv<2>(E, px, py, N, a.eps2, cur[2], tv[2]);
-            orbit_tv<3>(E, px, py, N, a.eps2, cur[3], tv[3]);
+            if (px > 0 && py > 0) {                       // P lies in the base quadrant: off the image border
+                orbit_tv_inner<0>(E, a.eps2, cur[0], tv[0]);
+                orbit_tv_inner<1>(E, a.eps2, cur[1], tv[1]);
+                orbit_tv_inner<2>(E, a.eps2, cur[2], tv[2]);
+                orbit_tv_inner<3>(E, a.eps2, cur[3], tv[3]);
+            } else {
+                orbit_tv<0>(E, px, py, N, a.eps2, cur[0], tv[0]);
+                orbit_tv<1>(E, px, py, N, a.eps2, cur[1], tv[1]);
+                orbit_tv<2>(E, px, py, N, a.eps2, cur[2], tv[2]);
+                orbit_tv<3>(E, px, py, N, a.eps2, cur[3], tv[3]);
+            }
         }
     }
     OSIV_TL(a.iter, 1, 9, true);

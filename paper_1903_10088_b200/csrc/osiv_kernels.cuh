@@ -707,6 +707,26 @@ __device__ __forceinline__ void orbit_tv(const float4 (&E)[3][3], int px, int py
     grad = sgrad;
 }
 
+// The same for a pixel orbit off the image border (0 < px, py < N - 1; a quarter turn about the centre maps the border
+// ring onto itself, so one test serves the four rotations): no predicates, the same float operations in the same order.
+template <int K>
+__device__ __forceinline__ void orbit_tv_inner(const float4 (&E)[3][3], float eps2, float& cur, float& grad) {
+    const float c = orbit_nb<K>(E, 0, 0);
+    const float dxc = orbit_nb<K>(E, 1, 0) - c, dyc = orbit_nb<K>(E, 0, 1) - c;
+    float sgrad = 0.f;
+    {                                                                // cell (x-1, y)
+        const float l = orbit_nb<K>(E, -1, 0), dxl = c - l, dyl = orbit_nb<K>(E, -1, 1) - l;
+        sgrad += dxl * rsqrt_fast(eps2 + dxl * dxl + dyl * dyl);
+    }
+    {                                                                // cell (x, y-1)
+        const float d = orbit_nb<K>(E, 0, -1), dyb = c - d, dxb = orbit_nb<K>(E, 1, -1) - d;
+        sgrad += dyb * rsqrt_fast(eps2 + dxb * dxb + dyb * dyb);
+    }
+    sgrad -= (dxc + dyc) * rsqrt_fast(eps2 + dxc * dxc + dyc * dyc);
+    cur = c;
+    grad = sgrad;
+}
+
 __device__ __forceinline__ void load_nbhd(const DevGeom& g, const float* img, int x0, int y0, float (&m)[4][4]) {
 #pragma unroll
     for (int r = 0; r < 4; ++r) {
@@ -1086,10 +1106,17 @@ __global__ void __launch_bounds__(SB == 1 ? BK_MAX_THREADS : BKB_MAX_THREADS, SB
                 si[j] = step_rule(a, s, lane, writer);
                 step[j] = (float)(si[j].lambda * a.tau);
                 if (fin_active) {                                    // A5 for R^k P, k = 0..3
-                    orbit_tv<0>(E, px, py, N, a.eps2, cur[j][0], tv[j][0]);
-                    orbit_tv<1>(E, px, py, N, a.eps2, cur[j][1], tv[j][1]);
-                    orbit_tv<2>(E, px, py, N, a.eps2, cur[j][2], tv[j][2]);
-                    orbit_tv<3>(E, px, py, N, a.eps2, cur[j][3], tv[j][3]);
+                    if (px > 0 && py > 0) {                          // off the image border (P lies in the base quadrant)
+                        orbit_tv_inner<0>(E, a.eps2, cur[j][0], tv[j][0]);
+                        orbit_tv_inner<1>(E, a.eps2, cur[j][1], tv[j][1]);
+                        orbit_tv_inner<2>(E, a.eps2, cur[j][2], tv[j][2]);
+                        orbit_tv_inner<3>(E, a.eps2, cur[j][3], tv[j][3]);
+                    } else {
+                        orbit_tv<0>(E, px, py, N, a.eps2, cur[j][0], tv[j][0]);
+                        orbit_tv<1>(E, px, py, N, a.eps2, cur[j][1], tv[j][1]);
+                        orbit_tv<2>(E, px, py, N, a.eps2, cur[j][2], tv[j][2]);
+                        orbit_tv<3>(E, px, py, N, a.eps2, cur[j][3], tv[j][3]);
+                    }
                 }
             }
         }
