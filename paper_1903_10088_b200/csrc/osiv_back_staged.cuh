@@ -40,7 +40,8 @@ constexpr int BS_MAX_JR = 16;                        // base views staged per ro
 constexpr int BS_RED_PITCH = BS_PX + 1;              // float4 per (share, tile) row of the reduction buffer: odd, conflict-free
 constexpr int BS_RCH = 8;                            // residual chunks (16 bytes) a thread fetches per round: 4 * JR * W <= 8 * threads
 constexpr int BS_DPK = 8;                            // monitor partials per lane of the step-rule warp: K1 blocks per slice <= 256
-constexpr int BS_HDR_BYTES = 256;                    // mbarriers + step/improved words in front of the staging area
+constexpr int BS_HDR_BYTES = 2560;                   // mbarrier, step/improved words, ticket (first 256 bytes), then the slice's monitor
+                                                     // partials [32 * BS_DPK] doubles and its SliceState, in front of the staging area
 constexpr int BS_PARAM_REGIONS = 160;                // regions that travel in the kernel parameters (constant bank) instead of a table
 
 struct BackSArgs {
@@ -81,6 +82,13 @@ __device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, int byte
                  ::"r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
 }
 __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+
+// 8-byte asynchronous copy global -> shared (the monitor partials travel during the walk, no registers held)
+__device__ __forceinline__ void cp_async8(uint32_t dst, const void* src) {
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(dst), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
 
 __device__ __forceinline__ void bulk_prefetch_l2(const void* src, int bytes) {
     asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(src), "r"(bytes) : "memory");
@@ -346,6 +354,17 @@ __global__ void __launch_bounds__(BS_SHARES * BS_MAX_TPB, 1) k_back_staged(const
     OSIV_TL(a.iter, 1, 2, false);
     float4 rv[BS_RCH];
     load_res(rv);
+    // A3's inputs (K1's monitor partials of this slice, the state after the previous iteration) set out for shared memory
+    // now: the warp that evaluates the step rule after its walk then finds them there instead of behind a round trip
+    double* dp_s = reinterpret_cast<double*>(smem + 256);
+    double* st_s = dp_s + 32 * BS_DPK;
+    if (MODE == 1 && first_warp) {
+#pragma unroll
+        for (int k = 0; k < BS_DPK; ++k)
+            if (lane + 32 * k < a.nparts) cp_async8(smem_u32(dp_s + lane + 32 * k), &a.dparts[(size_t)s * a.nparts + lane + 32 * k]);
+        if (lane < (int)(sizeof(SliceState) / 8)) cp_async8(smem_u32(st_s + lane), reinterpret_cast<const double*>(&a.state_in[s]) + lane);
+        cp_async_commit();
+    }
     if (first_warp) OSIV_TL(a.iter, 1, 10, true);
 
     // ---- while the loads fly: A5 for R^k P, k = 0..3; then the windows go to shared memory; then A3 in warp 0
@@ -368,7 +387,8 @@ __global__ void __launch_bounds__(BS_SHARES * BS_MAX_TPB, 1) k_back_staged(const
     OSIV_TL(a.iter, 1, 9, true);
     store_res(rv);
     OSIV_TL(a.iter, 1, 12, true);
-    __syncthreads();                                      // residual windows in place
+    if (MODE == 1 && first_warp) cp_async_wait_all();
+    __syncthreads();                                      // residual windows (and the step rule's inputs) in place
     OSIV_TL(a.iter, 1, 11, true);
 
     uint64_t acc[2][BS_PX];                               // [h][p]: components (2h, 2h+1) of the orbit's residuals for pixel p
@@ -427,8 +447,8 @@ __global__ void __launch_bounds__(BS_SHARES * BS_MAX_TPB, 1) k_back_staged(const
         if (ticket == 0) {
             double dpv[BS_DPK];
 #pragma unroll
-            for (int k = 0; k < BS_DPK; ++k) dpv[k] = lane + 32 * k < a.nparts ? __ldcg(&a.dparts[(size_t)s * a.nparts + lane + 32 * k]) : 0.0;
-            const SliceState st_in = a.state_in[s];
+            for (int k = 0; k < BS_DPK; ++k) dpv[k] = lane + 32 * k < a.nparts ? dp_s[lane + 32 * k] : 0.0;
+            const SliceState st_in = *reinterpret_cast<const SliceState*>(st_s);
             double D = 0.0;
 #pragma unroll
             for (int k = 0; k < BS_DPK; ++k) if (lane + 32 * k < a.nparts) D += dpv[k];
