@@ -6,8 +6,9 @@
 // Why a second K2.  ncu on k_back at config 3 (profiles/r2a): 63 % of its executed instructions are start-up, interval
 // fetch/decode and epilogue, its candidate loop runs at the L1 data-pipe wavefront limit (two 16-byte gathers per
 // candidate and thread) and every trip waits for an L2 round trip.  Here
-//   * a block owns a compact rectangle of the base quadrant (about 20 x 22 pixels; table `BackSArgs::regions`), so the
-//     channels its tiles can see in one view form ONE short window of W channels;
+//   * a block owns a compact rectangle of the base quadrant (about 20 x 22 pixels; table `BackSArgs::regions`, which
+//     travels in the kernel parameters: a block reads its entry from the constant bank, not behind an L2 round trip),
+//     so the channels its tiles can see in one view form ONE short window of W channels;
 //   * everything constant a block needs for one subset -- per view the window of the ray table, compressed to 8 bytes
 //     per ray {k, g0} (one of alpha, beta is exactly 1 after a sign flip, which of them is a per-window flag; the
 //     half-width follows from k), and the block's row of candidate intervals -- lies CONTIGUOUSLY in a per-subset
@@ -21,9 +22,9 @@
 //     per pixel than 2 x 2 tiles; a candidate costs one 8-byte and one 16-byte shared-memory load (the walk is bound
 //     by shared-memory wavefronts), a trip one 16-bit load and a handful of integer instructions;
 //   * everything of the epilogue that does not need the sums (the 3 x 3 neighbourhood of orbit float4s, the TV gradient
-//     of all four rotated pixels) is done before the walk, while the copies are in flight; warp 0 evaluates
-//     the step rule; after the block barrier a thread only sums the eight view shares of one base pixel, updates its
-//     four rotations and stores.
+//     of all four rotated pixels) is done before the walk, while the copies are in flight; the first warp out of the
+//     walk evaluates the step rule from inputs that went to shared memory by cp.async during the walk; after the block
+//     barrier a thread only sums the eight view shares of one base pixel, updates its four rotations and stores.
 // The general kernel k_back stays the path for everything this one does not take (NS = 1, pairs of slices, stacks,
 // grids whose side is not a multiple of 8, fans of 90 degrees or more, windows that do not fit).
 #pragma once
